@@ -1,0 +1,260 @@
+"""Pins of the CPU oracle against what the paper and the mathematics fix (CPU only).
+
+The paper prints no worked numerical example of the layer, so the pins are:
+Eq. 1 closed form and round-trip bound, invariances, nibble bijection, brute force with
+python Fractions / pure-python integers, numpy int64 matmul for P (library routine on a
+special case), numpy FP64 matmul for the low-rank branch, r = 0 and R = 0 reductions,
+additivity, and the storage ratios PAPER.md L86 prints (tests/golden/).
+"""
+from fractions import Fraction
+import os
+
+import numpy as np
+import pytest
+
+from gen import inputs as gen
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+
+
+def bf16(x):
+    return gen.f32_to_bf16_bits(np.asarray(x, np.float32))
+
+
+def f32(b):
+    return gen.bf16_bits_to_f32(b)
+
+
+# --------------------------------------------------------------------------- quantizer (Eq. 1)
+def test_quantizer_closed_form_eq1(oracle):
+    """PAPER.md L43-47 Eq. 1 with q_max = 7 on a group whose amax is 7*2^p: s is exactly 2^p,
+    so Q = round(X / s) can be written down by hand."""
+    G = 64
+    x = np.zeros((1, G), np.float32)
+    vals = [7.0, -7.0, 3.0, -3.0, 0.5, 1.5, 2.5, -0.5, -1.5, -2.5, 6.5, 0.25, 0.75, -6.5, 1.0, 0.0]
+    x[0, :16] = vals
+    q, sx = oracle.quantize_act(bf16(x * 4.0), G)      # amax = 28 -> s = 4 exactly
+    assert sx[0, 0] == np.float32(4.0)
+    # round-half-even (reading R5): 0.5->0, 1.5->2, 2.5->2, 6.5->6, 0.25->0, 0.75->1
+    expect = [7, -7, 3, -3, 0, 2, 2, 0, -2, -2, 6, 0, 1, -6, 1, 0]
+    assert q[0, :16].tolist() == expect
+    assert (q[0, 16:] == 0).all()
+
+
+def test_quantizer_roundtrip_bound_and_range(oracle):
+    """|x~ - s*q| <= s/2 (+ slack 2^-18 for the reciprocal multiply); amax element -> +-7; codes in [-7,7]."""
+    L = gen.make_layer(32, 512, 16, 0, 128, seed=11)
+    q, sx = oracle.quantize_act(L.X, 128)
+    x = f32(L.X).astype(np.float64).reshape(32, 4, 128)
+    qq = q.reshape(32, 4, 128).astype(np.float64)
+    s = sx.astype(np.float64)[:, :, None]
+    assert q.min() >= -7 and q.max() <= 7
+    assert (np.abs(x - s * qq) <= 0.5 * s * (1 + 2.0 ** -18)).all()
+    amax_idx = np.abs(x).argmax(axis=2)
+    top = np.take_along_axis(qq, amax_idx[:, :, None], axis=2)
+    assert (np.abs(top) == 7).all()
+    # s = amax/7 in FP32
+    amax = np.abs(f32(L.X)).reshape(32, 4, 128).max(axis=2)
+    assert (sx == (amax / np.float32(7.0)).astype(np.float32)).all()
+
+
+def test_quantizer_invariances(oracle):
+    """Negation flips codes, keeps sx; 2^p scaling keeps codes, scales sx; rows are independent."""
+    L = gen.make_layer(8, 256, 16, 0, 64, seed=12)
+    q, sx = oracle.quantize_act(L.X, 64)
+    qn, sxn = oracle.quantize_act(L.X ^ np.uint16(0x8000), 64)
+    assert (qn == -q).all() and (sxn == sx).all()
+    x8 = bf16(f32(L.X) * np.float32(8.0))
+    q8, sx8 = oracle.quantize_act(x8, 64)
+    assert (q8 == q).all() and (sx8 == sx * np.float32(8.0)).all()
+    q1, sx1 = oracle.quantize_act(L.X[3:4], 64)
+    assert (q1 == q[3:4]).all() and (sx1 == sx[3:4]).all()
+
+
+def test_quantizer_zero_group_and_transform(oracle):
+    """R9: all-zero group -> codes 0, sx = 2^-30/7, finite.  tinv multiplies before the amax (L54-58)."""
+    x = np.zeros((2, 128), np.float32)
+    x[1, 64:] = np.linspace(-3, 3, 64)
+    q, sx = oracle.quantize_act(bf16(x), 64)
+    assert (q[0] == 0).all() and np.isfinite(sx).all()
+    assert sx[0, 0] == np.float32(2.0 ** -30) / np.float32(7.0)
+    tinv = np.full(128, 0.25, np.float32)            # power of two: x*tinv exact
+    qt, sxt = oracle.quantize_act(bf16(x), 64, tinv)
+    assert (qt[1] == q[1]).all() and sxt[1, 1] == sx[1, 1] * np.float32(0.25)
+    # a non-uniform tinv changes which element is the amax
+    tinv2 = np.ones(128, np.float32)
+    tinv2[64] = 0.0
+    q2, _ = oracle.quantize_act(bf16(x), 64, tinv2)
+    assert q2[1, 64] == 0 and abs(q2[1, 127]) == 7
+
+
+def test_quantizer_second_implementation_numpy(oracle):
+    """Independent numpy-float32 restatement of Eq. 1 in the op order of reading R8."""
+    L = gen.make_layer(16, 512, 16, 0, 128, seed=13, with_tinv=True)
+    q, sx = oracle.quantize_act(L.X, 128, L.tinv)
+    xt = (f32(L.X) * L.tinv[None, :]).astype(np.float32).reshape(16, 4, 128)
+    amax = np.maximum(np.abs(xt).max(axis=2), np.float32(2.0 ** -30))
+    s = (amax / np.float32(7.0)).astype(np.float32)
+    inv = (np.float32(1.0) / s).astype(np.float32)
+    qq = np.clip(np.rint((xt * inv[:, :, None]).astype(np.float32)), -7, 7).astype(np.int8)
+    assert (sx == s).all()
+    assert (q == qq.reshape(16, 512)).all()
+
+
+# --------------------------------------------------------------------------- pack / unpack
+def test_nibble_bijection_all_bytes(oracle):
+    allb = np.arange(256, dtype=np.uint8).reshape(1, 256)
+    q = oracle.unpack_nibbles(allb)
+    assert q.min() == -8 and q.max() == 7
+    assert (oracle.pack_nibbles(q) == allb).all()
+    # low nibble = even k (R10), two's complement: byte 0x8F -> (q0,q1) = (-1,-8)
+    assert oracle.unpack_nibbles(np.array([[0x8F]], np.uint8)).tolist() == [[-1, -8]]
+    assert oracle.pack_nibbles(np.array([[7, -8]], np.int8)).tolist() == [[0x87]]
+
+
+# --------------------------------------------------------------------------- residual P (Eq. 2)
+def test_residual_P_bruteforce_and_library(oracle):
+    rng = np.random.default_rng(5)
+    M, N, K, G = 3, 5, 128, 64
+    qx = rng.integers(-7, 8, (M, K), dtype=np.int8)
+    qw = rng.integers(-8, 8, (N, K), dtype=np.int8)
+    P = oracle.residual_P(oracle.pack_nibbles(qx), oracle.pack_nibbles(qw), G)
+    # pure python triple loop
+    for m in range(M):
+        for n in range(N):
+            for g in range(K // G):
+                acc = sum(int(qx[m, k]) * int(qw[n, k]) for k in range(g * G, (g + 1) * G))
+                assert P[m, g, n] == acc
+    # G = K: plain integer matmul (numpy int64 @)
+    P1 = oracle.residual_P(oracle.pack_nibbles(qx), oracle.pack_nibbles(qw), K)
+    assert (P1[:, 0, :] == qx.astype(np.int64) @ qw.astype(np.int64).T).all()
+    assert np.abs(P).max() <= 56 * G
+    # extreme codes hit the bound 7*8*G exactly
+    qx1 = np.full((1, K), -7, np.int8)
+    qw1 = np.full((1, K), -8, np.int8)
+    assert oracle.residual_P(oracle.pack_nibbles(qx1), oracle.pack_nibbles(qw1), G)[0, 0, 0] == 56 * G
+
+
+def test_residual_P_row_subset(oracle):
+    rng = np.random.default_rng(6)
+    qx = rng.integers(-7, 8, (6, 128), dtype=np.int8)
+    qw = rng.integers(-8, 8, (4, 128), dtype=np.int8)
+    Xq, R4 = oracle.pack_nibbles(qx), oracle.pack_nibbles(qw)
+    P = oracle.residual_P(Xq, R4, 64)
+    Ps = oracle.residual_P(Xq, R4, 64, rows=[4, 1])
+    assert (Ps[0] == P[4]).all() and (Ps[1] == P[1]).all()
+
+
+# --------------------------------------------------------------------------- whole forward
+def _fraction_forward(L, q, sx):
+    """Exact rational evaluation of steps 5-8 (tiny shapes only)."""
+    X = f32(L.X)
+    M, K, N, r, G = L.M, L.K, L.N, L.r, L.G
+    Y = [[None] * N for _ in range(M)]
+    for m in range(M):
+        H = [sum(Fraction(float(X[m, k])) * Fraction(float(L.L1[k, j])) for k in range(K)) for j in range(r)]
+        for n in range(N):
+            yres = Fraction(0)
+            for g in range(K // G):
+                acc = sum(int(q[m, k]) * int(L.Rq[n, k]) for k in range(g * G, (g + 1) * G))
+                yres += Fraction(float(sx[m, g])) * Fraction(float(L.sw[n, g])) * acc
+            ylr = sum(H[j] * Fraction(float(L.L2[j, n])) for j in range(r))
+            Y[m][n] = yres + ylr
+    return Y
+
+
+def test_forward_bruteforce_fractions(oracle):
+    L = gen.make_layer(2, 128, 16, 16, 64, seed=21, x_dist="normal", n_outlier=2, outlier_scale=20.0,
+                       lr_sigma=0.05)
+    out = oracle.forward(L.X, L.Rq, L.sw, L.L1, L.L2, L.G)
+    Yf = _fraction_forward(L, out["q"], out["sx"])
+    for m in range(L.M):
+        for n in range(L.N):
+            exact = float(Yf[m][n])
+            assert abs(out["Y"][m, n] - exact) <= 1e-12 * max(1.0, abs(exact))
+
+
+def test_forward_rank0_is_plain_w4a4(oracle):
+    """north_star: r = 0 reduces to plain W4A4 = Eq. 2 with group scales: sum_g sx*sw*(qx.qw)."""
+    L = gen.make_layer(4, 256, 32, 0, 64, seed=22)
+    out = oracle.forward(L.X, L.Rq, L.sw, None, None, L.G, want_P=True)
+    deqx = out["q"].astype(np.float64) * np.repeat(out["sx"].astype(np.float64), L.G, axis=1)
+    deqw = L.Rq.astype(np.float64) * np.repeat(L.sw.astype(np.float64), L.G, axis=1)
+    ref = deqx @ deqw.T                          # Q(X) Q(W) dequantized explicitly, FP64 BLAS
+    assert np.allclose(out["Y"], ref, rtol=1e-12, atol=1e-12)
+    assert out["P"].shape == (4, 4, 32)
+
+
+def test_forward_zero_residual_is_lowrank_gemm(oracle):
+    """north_star: zero residual reduces to the FP64 low-rank GEMM (X L1) L2, and = X (L1 L2)."""
+    L = gen.make_layer(4, 256, 32, 16, 64, seed=23)
+    Rq0 = np.zeros_like(L.Rq)
+    out = oracle.forward(L.X, Rq0, L.sw, L.L1, L.L2, L.G)
+    X = f32(L.X).astype(np.float64)
+    ref = (X @ L.L1.astype(np.float64)) @ L.L2.astype(np.float64)
+    assert np.allclose(out["Y"], ref, rtol=1e-12, atol=1e-12)
+    ref2 = X @ (L.L1.astype(np.float64) @ L.L2.astype(np.float64))
+    assert np.allclose(out["Y"], ref2, rtol=1e-10, atol=1e-10)
+
+
+def test_forward_additivity_and_transposition_sensitivity(oracle):
+    L = gen.make_layer(3, 256, 48, 16, 128, seed=24)
+    full = oracle.forward(L.X, L.Rq, L.sw, L.L1, L.L2, L.G)["Y"]
+    res = oracle.forward(L.X, L.Rq, L.sw, None, None, L.G)["Y"]
+    lr = oracle.forward(L.X, np.zeros_like(L.Rq), L.sw, L.L1, L.L2, L.G)["Y"]
+    assert np.allclose(full - res, lr, rtol=1e-10, atol=1e-10)
+    # non-square everything: a transposed operand anywhere would have failed the shape-specific refs above;
+    # here make sure the two branches are not tiny relative to each other (a dropped term would show)
+    assert np.abs(res).max() > 1e-3 and np.abs(lr).max() > 1e-3
+
+
+def test_scale_fold_constant_and_pow2_exact(oracle):
+    """Constant scales factor out; power-of-two scales and small integers make Y exactly representable."""
+    rng = np.random.default_rng(7)
+    M, N, K, G = 4, 8, 256, 64
+    qx = rng.integers(-7, 8, (M, K), dtype=np.int8)
+    qw = rng.integers(-8, 8, (N, K), dtype=np.int8)
+    a = np.array([0.5, 2.0, 1.0, 0.25], np.float32)
+    b = np.float16([2.0 ** -3] * 4 + [2.0 ** -5] * 4)
+    sx = np.repeat(a[:, None], K // G, axis=1)
+    sw = np.repeat(b[:, None], K // G, axis=1)
+    X = bf16(np.zeros((M, K), np.float32))
+    Y = oracle.forward_from_quantized(X, oracle.pack_nibbles(qx), sx, oracle.pack_nibbles(qw), sw, None, None, G)
+    ref = (a.astype(np.float64)[:, None] * b.astype(np.float64)[None, :]) * (qx.astype(np.int64) @ qw.astype(np.int64).T)
+    assert (Y == ref).all()
+
+
+def test_round_bf16(oracle):
+    v = np.array([1.0, 1.00390625, 1.01171875, -3.0, 0.0, 1e-40, 65504.0, 3.3895313892515355e38], np.float64)
+    got = oracle.round_bf16(v)
+    # 1 + 2^-8 is a tie -> even (1.0); 1 + 3*2^-8 is a tie -> even (1 + 4*2^-8 = 1.015625)
+    assert got[0] == 0x3F80 and got[1] == 0x3F80 and got[2] == 0x3F82 and got[3] == 0xC040 and got[4] == 0
+    rnd = np.random.default_rng(3).standard_normal(4096) * 37.0
+    assert (oracle.round_bf16(rnd) == gen.f32_to_bf16_bits(rnd.astype(np.float32))).mean() > 0.99  # double rounding rare
+    exact = rnd.astype(np.float32).astype(np.float64)
+    assert (oracle.round_bf16(exact) == gen.f32_to_bf16_bits(exact.astype(np.float32))).all()
+
+
+# --------------------------------------------------------------------------- paper-printed numbers
+def test_storage_ratios_paper_L86(oracle):
+    with open(os.path.join(HERE, "golden", "paper_L86_storage_ratios.txt")) as f:
+        rows = [ln.split() for ln in f if ln.strip() and not ln.startswith("#")]
+    assert len(rows) == 2
+    for m, n, r, pct in rows:
+        m, n, r, pct = int(m), int(n), int(r), float(pct)
+        ratio = 100.0 * oracle.lowrank_fp16_bytes(m, n, r) / oracle.residual_4bit_bytes(m, n)
+        assert abs(ratio - pct) < 1e-9
+
+
+# --------------------------------------------------------------------------- generator sanity
+def test_generator_statistics():
+    L = gen.config2_qproj(16)
+    assert L.X.shape == (16, 4096) and L.Rq.shape == (4096, 4096) and L.sw.shape == (4096, 32)
+    assert L.Rq.min() == -8 and L.Rq.max() == 7
+    assert abs(L.Rq.astype(np.float64).mean() + 0.5) < 0.01
+    assert abs((L.Rq.astype(np.float64) ** 2).mean() - 21.5) < 0.05
+    assert 0.005 * (1 - 2 ** -11) <= float(L.sw.min()) and float(L.sw.max()) <= 0.02 * (1 + 2 ** -11)  # FP16 RNE of U(0.005,0.02)
+    L1 = gen.config1_tiny()
+    assert (L1.M, L1.K, L1.N, L1.r, L1.G) == (8, 256, 512, 16, 64)
+    a = gen.config1_tiny()
+    assert (a.X == L1.X).all() and (a.Rq == L1.Rq).all()
