@@ -1,0 +1,131 @@
+/*
+ * twq.h -- C ABI of the B200 (sm_100a) TwinQuant dual-component 4-bit linear layer.
+ *
+ *     Y = deq( Q4(X*T) * R4^T ) + (X*L1)*L2
+ *
+ * PAPER.md = arxiv 2606.01556 (TwinQuant).  The operation is the inference form of
+ * Eq. 3 (section 2): a 4-bit activation x 4-bit weight residual GEMM
+ * (Eq. 2) with group scales along the reduction axis (L193, section 5.1) plus
+ * a two-stage rank-r product, merged by one epilogue and one store (L179-181,
+ * section 4.3).  The low-rank branch is the high-precision (FP16 factor) form that
+ * BASELINE.json's north_star fixes ("keeps the low-rank path in FP16").
+ *
+ * Conventions
+ *   - All data pointers are DEVICE pointers (cudaMalloc / torch CUDA tensors).  The
+ *     library never allocates, frees or copies user buffers and never synchronises.
+ *   - `stream` is a cudaStream_t passed as void* (NULL = legacy default stream).
+ *     Every call is asynchronous with respect to the host.
+ *   - All matrices are row-major.  M tokens, K in-features, N out-features,
+ *     G group size along K, ng = K/G groups, r rank.
+ *   - Errors are returned as twq_status; nothing throws or aborts.  Arguments are
+ *     validated BEFORE any CUDA call, so invalid arguments are reported without a GPU.
+ *   - Non-finite inputs give unspecified values, never a fault.
+ *   - There is no CPU fallback: without an sm_100 device the compute entry points
+ *     return TWQ_ERR_UNSUPPORTED / TWQ_ERR_CUDA.
+ */
+#ifndef TWQ_H_
+#define TWQ_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    TWQ_OK = 0,
+    TWQ_ERR_INVALID_ARG = 1,  /* null pointer, bad shape, bad alignment, buffer too small */
+    TWQ_ERR_UNSUPPORTED = 2,  /* device is not sm_100, or a shape outside the built kernels */
+    TWQ_ERR_WORKSPACE = 3,    /* ws_bytes < twq_workspace_bytes(...) */
+    TWQ_ERR_CUDA = 4          /* a CUDA runtime / driver call or the launch failed */
+} twq_status;
+
+typedef enum { TWQ_OUT_BF16 = 0, TWQ_OUT_FP16 = 1, TWQ_OUT_FP32 = 2 } twq_out_dtype;
+
+/* Shape rules shared by every entry point (checked, TWQ_ERR_INVALID_ARG otherwise):
+ *   M >= 1; G in {64,128}; K >= G, K % G == 0; N >= 16, N % 16 == 0;
+ *   0 <= r <= 256, r % 16 == 0 (r = 0: plain W4A4, no low-rank branch);
+ *   pointers 16-byte aligned; leading dimensions >= row length and a multiple of 8 elements.
+ */
+
+/* Human-readable name of a status code (static string, never NULL). */
+const char* twq_status_string(twq_status s);
+
+/* ---------------------------------------------------------------------------
+ * twq_packed_bytes -- size in bytes of the opaque kernel-native weight blob that
+ * twq_pack_weights writes for one layer (0 if the shape is invalid).
+ * Contents ("pre-processed offline"; L193 groups of G along K):
+ * 4-bit residual codes [N,K/2], FP32 group scales transposed [K/G,N], L1^T [r,K]
+ * FP16, L2^T [N,r] FP16; each section 256-byte aligned.
+ */
+size_t twq_packed_bytes(int N, int K, int r, int G);
+
+/* ---------------------------------------------------------------------------
+ * twq_pack_weights -- offline re-layout of one layer's weights (step a0).
+ *   Rq  [N,K]   int8   residual 4-bit codes, each in [-8,7] (two's complement INT4,
+ *                      symmetric quantizer of Eq. 1; values outside
+ *                      [-8,7] are truncated to their low 4 bits)
+ *   sw  [N,K/G] fp16   residual group scales (one per G contiguous k, per out channel)
+ *   L1  [K,r]   fp16   low-rank factor 1 (may be NULL iff r == 0)
+ *   L2  [r,N]   fp16   low-rank factor 2 (may be NULL iff r == 0)
+ *   packed      out    blob of twq_packed_bytes(N,K,r,G) bytes, 256-byte aligned
+ * The packed 4-bit interchange layout inside the blob is R4[N,K/2]: byte j of a row
+ * holds code k=2j in its low nibble and k=2j+1 in its high nibble.
+ * Returns TWQ_ERR_INVALID_ARG if packed_bytes is too small.
+ */
+twq_status twq_pack_weights(const int8_t* Rq, const void* sw, const void* L1, const void* L2,
+                            int N, int K, int r, int G,
+                            void* packed, size_t packed_bytes, void* stream);
+
+/* ---------------------------------------------------------------------------
+ * twq_quantize_act -- online per-token group quantizer (steps a1-a2).
+ * PAPER.md Eq. 1 (L43-47): Q_X = round(X/s_X), s_X = max|X|/q_max, q_max = 7;
+ * activation-side diagonal transform X*diag(lambda)^-1 (L54-58); groups of G (L193).
+ * Exact FP32 operation order (this order IS the specification; reading R8):
+ *     x~  = (float)X[m,k] * tinv[k]       (one RN multiply; skipped when tinv == NULL)
+ *     a   = max(max_{k in g} |x~|, 2^-30)
+ *     s   = a / 7.0f  (RN divide)   -> sx[m,g]
+ *     inv = 1.0f / s  (RN divide)
+ *     q   = clamp(rint_even(x~ * inv), -7, 7)
+ *   X    [M,ldx] bf16  activations (ldx >= K elements)
+ *   tinv [K]     fp32  diagonal of T (1/lambda), or NULL for T = identity
+ *   Xq   [M,K/2] u8    out: packed codes, low nibble = even k, two's complement
+ *   sx   [M,K/G] fp32  out: group scales
+ */
+twq_status twq_quantize_act(const void* X, int M, int K, int ldx, const float* tinv, int G,
+                            uint8_t* Xq, float* sx, void* stream);
+
+/* Bytes of scratch twq_dual_linear needs for this shape (0 is a legal answer). */
+size_t twq_workspace_bytes(int M, int N, int K, int r, int G);
+
+/* ---------------------------------------------------------------------------
+ * twq_dual_linear -- the fused dual-branch layer (steps a3-a7), ONE kernel launch.
+ *   residual : P[m,g,n] = sum_{k in g} qx[m,k]*qw[n,k]   exact int32   (Eq. 2; L177)
+ *              Yres     = sum_g sx[m,g]*sw[n,g]*P[m,g,n]  FP32          (L181 "folds the scale factors")
+ *   low-rank : H = X*L1 (FP32 accumulate, kept on chip), Ylr = H*L2    (Eq. 3; L177-179)
+ *   epilogue : Y = round_out(Yres + Ylr), one store                    (L181)
+ *   X      [M,ldx] bf16     raw activations (read by the low-rank branch; may be NULL iff r == 0)
+ *   Xq,sx                   outputs of twq_quantize_act for the same X
+ *   packed                  blob written by twq_pack_weights for (N,K,r,G)
+ *   Y      [M,ldy]          out, dtype ydt (ldy >= N elements)
+ *   ws, ws_bytes            scratch of at least twq_workspace_bytes(...) bytes, 256-byte aligned (may be
+ *                           NULL when that is 0).  It holds split-K partial sums and tile counters for
+ *                           decode-shaped calls.  The caller zero-fills it ONCE after allocation; every
+ *                           call leaves the counters zero again, so it can be reused without clearing.
+ *   dbg_P  [M,K/G,N] int32  NULL, or receives the integer group accumulators P taken from the
+ *                           same tensor-core path that feeds Y (parity evidence; slows the call)
+ */
+twq_status twq_dual_linear(const void* X, int ldx, const uint8_t* Xq, const float* sx,
+                           const void* packed, int M, int N, int K, int r, int G,
+                           void* Y, twq_out_dtype ydt, int ldy,
+                           void* ws, size_t ws_bytes, int32_t* dbg_P, void* stream);
+
+/* Number of kernel launches the last successful twq_dual_linear / twq_quantize_act /
+ * twq_pack_weights call on this thread issued (bench.py's gpu_launches accounting). */
+int twq_last_launch_count(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TWQ_H_ */

@@ -1,0 +1,11 @@
+"""paper_2606_01556_b200 -- B200 (sm_100a) TwinQuant dual-component 4-bit linear layer.
+
+Thin Python binding over the C-ABI library libtwq.so (include/twq.h).  The binding only
+marshals arguments (torch tensors -> device pointers, current stream); every step of the
+hot path runs in the CUDA kernels under csrc/.  There is NO CPU or PyTorch fallback: if
+the library is missing or the device is not sm_100 the calls raise.
+"""
+from .binding import (  # noqa: F401
+    TwqError, lib_path, load_library, packed_bytes, workspace_bytes, pack_weights, quantize_act,
+    dual_linear, last_launch_count, OUT_BF16, OUT_FP16, OUT_FP32, PackedLayer, algorithmic_bytes, flops,
+)

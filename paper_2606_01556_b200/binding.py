@@ -1,0 +1,165 @@
+"""ctypes binding of include/twq.h.  Names and argument order follow the C ABI."""
+from __future__ import annotations
+
+import ctypes
+import dataclasses
+import os
+
+import torch
+
+from . import _build
+
+OUT_BF16, OUT_FP16, OUT_FP32 = 0, 1, 2
+_STATUS = {0: "TWQ_OK", 1: "TWQ_ERR_INVALID_ARG", 2: "TWQ_ERR_UNSUPPORTED", 3: "TWQ_ERR_WORKSPACE", 4: "TWQ_ERR_CUDA"}
+_OUT_TORCH = {OUT_BF16: torch.bfloat16, OUT_FP16: torch.float16, OUT_FP32: torch.float32}
+
+EXPORTS = ("twq_status_string", "twq_packed_bytes", "twq_pack_weights", "twq_quantize_act",
+           "twq_workspace_bytes", "twq_dual_linear", "twq_last_launch_count")
+
+
+class TwqError(RuntimeError):
+    def __init__(self, code: int, where: str):
+        super().__init__(f"{where}: {_STATUS.get(code, code)}")
+        self.code = code
+
+
+_lib = None
+
+
+def lib_path() -> str:
+    return _build.LIB
+
+
+def load_library(build_if_missing: bool = True):
+    """Load libtwq.so (building it in-tree with nvcc if it is missing or stale)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = _build.LIB
+    if build_if_missing and _build.needs_build():
+        path = _build.build()
+    if not os.path.exists(path):
+        raise FileNotFoundError(f"{path} not built; run python -m paper_2606_01556_b200._build")
+    lib = ctypes.CDLL(path)
+    vp, i, sz = ctypes.c_void_p, ctypes.c_int, ctypes.c_size_t
+    lib.twq_status_string.restype = ctypes.c_char_p
+    lib.twq_status_string.argtypes = [i]
+    lib.twq_packed_bytes.restype = sz
+    lib.twq_packed_bytes.argtypes = [i, i, i, i]
+    lib.twq_pack_weights.restype = i
+    lib.twq_pack_weights.argtypes = [vp, vp, vp, vp, i, i, i, i, vp, sz, vp]
+    lib.twq_quantize_act.restype = i
+    lib.twq_quantize_act.argtypes = [vp, i, i, i, vp, i, vp, vp, vp]
+    lib.twq_workspace_bytes.restype = sz
+    lib.twq_workspace_bytes.argtypes = [i, i, i, i, i]
+    lib.twq_dual_linear.restype = i
+    lib.twq_dual_linear.argtypes = [vp, i, vp, vp, vp, i, i, i, i, i, vp, i, i, vp, sz, vp, vp]
+    lib.twq_last_launch_count.restype = i
+    lib.twq_last_launch_count.argtypes = []
+    _lib = lib
+    return lib
+
+
+def _ptr(t):
+    return None if t is None else ctypes.c_void_p(t.data_ptr())
+
+
+def _stream(stream=None):
+    s = torch.cuda.current_stream() if stream is None else stream
+    return ctypes.c_void_p(s.cuda_stream)
+
+
+def _check(code: int, where: str):
+    if code != 0:
+        raise TwqError(code, where)
+
+
+def packed_bytes(N: int, K: int, r: int, G: int) -> int:
+    return int(load_library().twq_packed_bytes(N, K, r, G))
+
+
+def workspace_bytes(M: int, N: int, K: int, r: int, G: int) -> int:
+    return int(load_library().twq_workspace_bytes(M, N, K, r, G))
+
+
+def last_launch_count() -> int:
+    return int(load_library().twq_last_launch_count())
+
+
+@dataclasses.dataclass
+class PackedLayer:
+    """Opaque packed weights of one layer + the shape they were packed for."""
+    blob: torch.Tensor
+    N: int
+    K: int
+    r: int
+    G: int
+
+
+def pack_weights(Rq: torch.Tensor, sw: torch.Tensor, L1, L2, G: int, stream=None) -> PackedLayer:
+    """twq_pack_weights.  Rq int8 [N,K] codes, sw fp16 [N,K/G], L1 fp16 [K,r], L2 fp16 [r,N] (device)."""
+    N, K = Rq.shape
+    r = 0 if L1 is None else int(L1.shape[1])
+    nbytes = packed_bytes(N, K, r, G)
+    if nbytes == 0:
+        raise TwqError(1, "twq_packed_bytes")
+    blob = torch.empty(nbytes, dtype=torch.uint8, device=Rq.device)
+    assert Rq.dtype == torch.int8 and Rq.is_contiguous() and sw.dtype == torch.float16 and sw.is_contiguous()
+    if r > 0:
+        assert L1.dtype == torch.float16 and L2.dtype == torch.float16 and L1.is_contiguous() and L2.is_contiguous()
+        assert tuple(L1.shape) == (K, r) and tuple(L2.shape) == (r, N)
+    code = load_library().twq_pack_weights(_ptr(Rq), _ptr(sw), _ptr(L1) if r else None, _ptr(L2) if r else None,
+                                           N, K, r, G, _ptr(blob), nbytes, _stream(stream))
+    _check(code, "twq_pack_weights")
+    return PackedLayer(blob, N, K, r, G)
+
+
+def quantize_act(X: torch.Tensor, G: int, tinv=None, out=None, stream=None):
+    """twq_quantize_act.  X bf16 [M,K] (row stride = X.stride(0)); returns (Xq u8 [M,K/2], sx f32 [M,K/G])."""
+    M, K = X.shape
+    assert X.dtype == torch.bfloat16 and X.stride(1) == 1
+    if out is None:
+        Xq = torch.empty((M, K // 2), dtype=torch.uint8, device=X.device)
+        sx = torch.empty((M, K // G), dtype=torch.float32, device=X.device)
+    else:
+        Xq, sx = out
+    code = load_library().twq_quantize_act(_ptr(X), M, K, X.stride(0), _ptr(tinv), G, _ptr(Xq), _ptr(sx),
+                                           _stream(stream))
+    _check(code, "twq_quantize_act")
+    return Xq, sx
+
+
+def dual_linear(X, Xq, sx, packed: PackedLayer, out_dtype: int = OUT_BF16, Y=None, ws=None, dbg_P=None,
+                stream=None):
+    """twq_dual_linear.  Returns Y [M,N] in out_dtype.  `ws` must be a zero-initialised uint8 tensor of at
+    least workspace_bytes(...) when that is non-zero (allocated here if omitted)."""
+    M = Xq.shape[0]
+    N, K, r, G = packed.N, packed.K, packed.r, packed.G
+    if Y is None:
+        Y = torch.empty((M, N), dtype=_OUT_TORCH[out_dtype], device=Xq.device)
+    need = workspace_bytes(M, N, K, r, G)
+    if need and ws is None:
+        ws = torch.zeros(need, dtype=torch.uint8, device=Xq.device)
+    ldx = X.stride(0) if X is not None else K
+    code = load_library().twq_dual_linear(_ptr(X) if r else None, ldx, _ptr(Xq), _ptr(sx), _ptr(packed.blob),
+                                          M, N, K, r, G, _ptr(Y), out_dtype, Y.stride(0), _ptr(ws),
+                                          0 if ws is None else ws.numel(), _ptr(dbg_P), _stream(stream))
+    _check(code, "twq_dual_linear")
+    return Y
+
+
+# ---- accounting used by bench.py (PAPER.md L86 byte arithmetic) ----
+def algorithmic_bytes(M: int, N: int, K: int, r: int, G: int, with_quantizer: bool = False, out_bytes: int = 2) -> int:
+    """Bytes the method must move for one twq_dual_linear call: packed residual, its scales (fp16 in the
+    interchange format), both factors, X, Xq, sx, Y.  with_quantizer adds the quantizer's own X read and
+    Xq/sx write."""
+    ng = K // G
+    w = N * K // 2 + 2 * N * ng + 2 * K * r + 2 * r * N
+    a = (2 * M * K if r > 0 else 0) + M * K // 2 + 4 * M * ng + out_bytes * M * N
+    q = 2 * M * K + M * K // 2 + 4 * M * ng if with_quantizer else 0
+    return w + a + q
+
+
+def flops(M: int, N: int, K: int, r: int):
+    """(int8 residual ops, 16-bit low-rank flops) of one call."""
+    return 2 * M * K * N, 2 * M * r * (K + N)

@@ -1,0 +1,458 @@
+// dual_linear.cu -- the fused dual-branch kernel (steps a3-a7), sm_100a only.
+//
+//   Y[m,n] = sum_g sx[m,g]*sw[n,g]*P[m,g,n]  +  sum_j H[m,j]*L2[j,n],
+//   P[m,g,n] = sum_{k in g} qx[m,k]*qw[n,k] (exact int32),   H = X*L1 (FP32 accumulate)
+//   PAPER.md Eq. 2 (L49-50), Eq. 3 (L62), L177-181 (section 4.3), L193 (groups of G).
+//
+// Tile: one CTA computes Y^T for 128 output channels (TMEM lanes = n, the MMA M dimension;
+// the weights are the A operand) x TN tokens (TMEM columns = m, the MMA N dimension; the
+// activations are the B operand).  Putting tokens on the N side lets decode-shaped calls
+// run N = 16 MMAs instead of padding M to 128.
+//
+// Phases inside the CTA (r > 0):
+//   1. stage 1   H^T[j,m] = sum_k L1T[j,k] X[m,k]    kind::f16 (A = f16, B = bf16), TMA-fed ring
+//      epilogue warps drain H^T from TMEM, round once to BF16 and write H[m,j] (K-major,
+//      128B-swizzled) into shared memory: the intermediate never leaves the SM.
+//   2. stage 2   Ylr^T[n,m] = sum_j L2T[n,j] H[m,j]  kind::f16, accumulator stays in TMEM
+//   3. residual  per group g: TMA brings packed INT4 rows of R4 and Xq; unpack warps expand
+//      each nibble c to the int8 value 16*c (one shift/and per word; sm_100 has no INT4 MMA)
+//      into 128B-swizzled K-major tiles; kind::i8 MMAs produce 256*P in a double-buffered
+//      TMEM accumulator; epilogue warps fold the two scales in FP32 into registers while the
+//      tensor core works on the next group.
+//   4. one epilogue: registers + Ylr from TMEM, one rounding, one store.
+#include <cuda_bf16.h>
+#include <cuda_fp16.h>
+
+#include "dual_linear.h"
+#include "sm100_ptx.cuh"
+
+namespace twq {
+
+namespace {
+
+constexpr int kThreads = 512;
+constexpr int kNumUnpackThreads = 128;  // warps 4..7
+constexpr int kNumEpiWarps = 8;         // warps 8..15
+constexpr int kTileN = 128;             // output channels per CTA (MMA M)
+constexpr int kNS1 = 3;                 // stage-1 ring depth
+constexpr int kNSU = 3;                 // unpacked-tile ring depth
+constexpr int kSxSlots = 8;             // per-group activation-scale slots (>= kNSU + 2)
+
+// TMEM columns (512 allocated): Ylr^T at 0; the two P buffers at 128 and 128+TN; the H^T
+// accumulators alias the P buffers (they are drained before the first residual MMA).
+constexpr int kColYlr = 0;
+constexpr int kColP = 128;
+constexpr int kColH = 128;
+
+template <int TN, int G>
+struct Cfg {
+    static constexpr int kXChunk = TN * 128;            // X tile, 64 bf16 per row
+    static constexpr int kL1Chunk = 128 * 128;          // L1T tile per 128-row block
+    static constexpr int kS1Stage = kXChunk + 2 * kL1Chunk;
+    static constexpr int kHBytes = TN * 512;            // H[m, 0..255] bf16 as 4 k-blocks of TN x 128 B
+    static constexpr int kL2TBytes = 4 * kL1Chunk;
+    static constexpr int kPA = kTileN * (G / 2);        // packed weight rows of one group
+    static constexpr int kPB = TN * (G / 2);
+    static constexpr int kPStage = kPA + kPB;
+    static constexpr int kUA = kTileN * G;              // unpacked int8 tiles of one group
+    static constexpr int kUB = TN * G;
+    static constexpr int kUStage = kUA + kUB;
+    static constexpr int kNSP = TN <= 32 ? 8 : 3;       // packed ring depth (deep at decode: bytes in flight)
+    static constexpr int kRing3 = kNSU * kUStage + kNSP * kPStage;
+    static constexpr int kRing1 = kNS1 * kS1Stage;
+    static constexpr int kRing = kRing1 > kRing3 ? (kRing1 > kL2TBytes ? kRing1 : kL2TBytes)
+                                                 : (kRing3 > kL2TBytes ? kRing3 : kL2TBytes);
+    static constexpr int kOffH = 0;
+    static constexpr int kOffRing = kHBytes;
+    static constexpr int kOffSx = kOffRing + kRing;
+    static constexpr int kOffBar = kOffSx + kSxSlots * TN * 4;
+    static constexpr int kNumBars = 2 * kNS1 + 2 * kNSP + 2 * kNSU + 4 + 4;
+    static constexpr int kSmemBytes = kOffBar + kNumBars * 8 + 16 + 1024;  // + TMEM slot + alignment slack
+    static_assert(kHBytes % 1024 == 0 && kXChunk % 1024 == 0 && kUA % 1024 == 0 && kUB % 512 == 0, "tile alignment");
+    static_assert(kSmemBytes <= 232448, "shared memory budget");
+};
+
+__device__ __forceinline__ uint32_t nib_lo16(uint32_t w) { return (w << 4) & 0xF0F0F0F0u; }  // 16*code, even k
+__device__ __forceinline__ uint32_t nib_hi16(uint32_t w) { return w & 0xF0F0F0F0u; }         // 16*code, odd k
+
+template <int TN, int G>
+__global__ void __launch_bounds__(kThreads, 1)
+dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CUtensorMap tmXq,
+                   const __grid_constant__ CUtensorMap tmX, const __grid_constant__ CUtensorMap tmL1T,
+                   const __grid_constant__ CUtensorMap tmL2T, const DualParams p) {
+    using C = Cfg<TN, G>;
+    extern __shared__ uint8_t smem_raw[];
+    uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+    uint8_t* sH = smem + C::kOffH;
+    uint8_t* sRing = smem + C::kOffRing;
+    float* sSx = reinterpret_cast<float*>(smem + C::kOffSx);
+    uint64_t* bars = reinterpret_cast<uint64_t*>(smem + C::kOffBar);
+    uint64_t* full1 = bars;                    // [kNS1]  TMA -> MMA (stage 1)
+    uint64_t* empty1 = full1 + kNS1;           // [kNS1]  MMA -> TMA
+    uint64_t* pfull = empty1 + kNS1;           // [kNSP]  TMA -> unpack
+    uint64_t* pempty = pfull + C::kNSP;        // [kNSP]  unpack -> TMA
+    uint64_t* ufull = pempty + C::kNSP;        // [kNSU]  unpack -> MMA
+    uint64_t* uempty = ufull + kNSU;           // [kNSU]  MMA -> unpack
+    uint64_t* tfull = uempty + kNSU;           // [2]     MMA -> epilogue (P buffer ready)
+    uint64_t* tempty = tfull + 2;              // [2]     epilogue -> MMA (P buffer drained)
+    uint64_t* h_full = tempty + 2;             // stage-1 accumulators complete
+    uint64_t* h_ready = h_full + 1;            // H written to shared memory
+    uint64_t* l2_full = h_ready + 1;           // L2T tile landed
+    uint64_t* ylr_done = l2_full + 1;          // stage-2 MMAs complete
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(ylr_done + 1);
+
+    const int warp = threadIdx.x >> 5;
+    const int lane = threadIdx.x & 31;
+    const int n0 = blockIdx.x * kTileN;
+    const int m0 = blockIdx.y * TN;
+    const int r = p.r;
+    const int nrb = (r + 127) >> 7;          // 128-row blocks of L1T / H^T
+    const int nkb = (r + 63) >> 6;           // 64-wide k-blocks of H / L2T
+    const int g_begin = p.g_per_split * blockIdx.z;
+    const int g_end = min(p.ng, g_begin + p.g_per_split);
+    // stage-1 K chunks (64 k each) of this split
+    const int kc_total = p.K >> 6;
+    const int kc_per = (kc_total + gridDim.z - 1) / gridDim.z;
+    const int kc_begin = kc_per * blockIdx.z;
+    const int kc_end = min(kc_total, kc_begin + kc_per);
+    const bool has_lr = r > 0 && kc_begin < kc_end;
+
+    if (threadIdx.x == 0) {
+        for (int i = 0; i < kNS1; ++i) { mbar_init(&full1[i], 1); mbar_init(&empty1[i], 1); }
+        for (int i = 0; i < C::kNSP; ++i) { mbar_init(&pfull[i], 1); mbar_init(&pempty[i], kNumUnpackThreads / 32); }
+        for (int i = 0; i < kNSU; ++i) { mbar_init(&ufull[i], kNumUnpackThreads / 32); mbar_init(&uempty[i], 1); }
+        for (int i = 0; i < 2; ++i) { mbar_init(&tfull[i], 1); mbar_init(&tempty[i], kNumEpiWarps); }
+        mbar_init(h_full, 1);
+        mbar_init(h_ready, kNumEpiWarps);
+        mbar_init(l2_full, 1);
+        mbar_init(ylr_done, 1);
+        fence_mbar_init();
+    }
+    if (warp == 0 && lane == 0) {
+        tma_prefetch_desc(&tmW);
+        tma_prefetch_desc(&tmXq);
+        if (r > 0) { tma_prefetch_desc(&tmX); tma_prefetch_desc(&tmL1T); tma_prefetch_desc(&tmL2T); }
+    }
+    if (warp == 2) tmem_alloc<512>(tmem_slot);
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem = *tmem_slot;
+
+    if (warp == 0) {
+        // ================================================================ TMA producer
+        if (lane == 0) {
+            if (has_lr) {
+                int it = 0;
+                for (int kc = kc_begin; kc < kc_end; ++kc, ++it) {
+                    const int s = it % kNS1, ph = (it / kNS1) & 1;
+                    mbar_wait(&empty1[s], ph ^ 1, 10);
+                    uint8_t* st = sRing + s * C::kS1Stage;
+                    mbar_arrive_expect_tx(&full1[s], C::kXChunk + nrb * C::kL1Chunk);
+                    tma_load_2d(st, &tmX, &full1[s], kc * 64, m0);
+                    for (int rb = 0; rb < nrb; ++rb)
+                        tma_load_2d(st + C::kXChunk + rb * C::kL1Chunk, &tmL1T, &full1[s], kc * 64, rb * 128);
+                }
+                // the L2T tile reuses ring memory: every stage-1 MMA must have completed
+                mbar_wait(h_full, 0, 11);
+                mbar_arrive_expect_tx(l2_full, nkb * C::kL1Chunk);
+                for (int kb = 0; kb < nkb; ++kb) tma_load_2d(sRing + kb * C::kL1Chunk, &tmL2T, l2_full, kb * 64, n0);
+                // the residual rings reuse it again: every stage-2 MMA must have completed
+                mbar_wait(ylr_done, 0, 12);
+            }
+            int it = 0;
+            for (int g = g_begin; g < g_end; ++g, ++it) {
+                const int s = it % C::kNSP, ph = (it / C::kNSP) & 1;
+                mbar_wait(&pempty[s], ph ^ 1, 13);
+                uint8_t* st = sRing + kNSU * C::kUStage + s * C::kPStage;
+                mbar_arrive_expect_tx(&pfull[s], C::kPStage);
+                tma_load_2d(st, &tmW, &pfull[s], g * (G / 2), n0);
+                tma_load_2d(st + C::kPA, &tmXq, &pfull[s], g * (G / 2), m0);
+            }
+        }
+    } else if (warp == 1) {
+        // ================================================================ MMA issuer (one thread)
+        if (lane == 0) {
+            if (has_lr) {
+                const uint32_t idesc1 = umma_idesc(1, 0, 1, 128, TN);  // D f32, A f16 (L1T), B bf16 (X)
+                int it = 0;
+                for (int kc = kc_begin; kc < kc_end; ++kc, ++it) {
+                    const int s = it % kNS1, ph = (it / kNS1) & 1;
+                    mbar_wait(&full1[s], ph, 20);
+                    tc_fence_after();
+                    const uint32_t xb = smem_u32(sRing + s * C::kS1Stage);
+                    const uint32_t lb = xb + C::kXChunk;
+#pragma unroll
+                    for (int ks = 0; ks < 4; ++ks)
+                        for (int rb = 0; rb < nrb; ++rb)
+                            umma_f16(tmem + kColH + rb * TN, umma_smem_desc<128>(lb + rb * C::kL1Chunk + ks * 32),
+                                     umma_smem_desc<128>(xb + ks * 32), idesc1, (it | ks) != 0);
+                    tc_commit(&empty1[s]);
+                }
+                tc_commit(h_full);
+                mbar_wait(h_ready, 0, 21);
+                mbar_wait(l2_full, 0, 22);
+                tc_fence_after();
+                const uint32_t idesc2 = umma_idesc(1, 0, 1, 128, TN);  // D f32, A f16 (L2T), B bf16 (H)
+                const uint32_t l2b = smem_u32(sRing), hb = smem_u32(sH);
+                const int nks = (r + 15) >> 4;
+                for (int ks = 0; ks < nks; ++ks) {
+                    const int kb = ks >> 2, kk = ks & 3;
+                    umma_f16(tmem + kColYlr, umma_smem_desc<128>(l2b + kb * C::kL1Chunk + kk * 32),
+                             umma_smem_desc<128>(hb + kb * (TN * 128) + kk * 32), idesc2, ks != 0);
+                }
+                tc_commit(ylr_done);
+            }
+            const uint32_t idesc3 = umma_idesc(2, 1, 1, 128, TN);  // D s32, A s8, B s8
+            int it = 0;
+            for (int g = g_begin; g < g_end; ++g, ++it) {
+                const int s = it % kNSU, ph = (it / kNSU) & 1;
+                const int b = it & 1, bph = (it >> 1) & 1;
+                mbar_wait(&tempty[b], bph ^ 1, 23);
+                mbar_wait(&ufull[s], ph, 24);
+                tc_fence_after();
+                const uint32_t ua = smem_u32(sRing + s * C::kUStage);
+                const uint32_t ub = ua + C::kUA;
+#pragma unroll
+                for (int ks = 0; ks < G / 32; ++ks)
+                    umma_i8(tmem + kColP + b * TN, umma_smem_desc<G>(ua + ks * 32), umma_smem_desc<G>(ub + ks * 32),
+                            idesc3, ks != 0);
+                tc_commit(&uempty[s]);
+                tc_commit(&tfull[b]);
+            }
+        }
+    } else if (warp >= 4 && warp < 8) {
+        // ================================================================ INT4 -> int8 unpack warps
+        const int u = threadIdx.x - 128;
+        constexpr int kCPR = (G / 2) / 16;  // 16-byte packed chunks per row
+        constexpr int kTasks = (kTileN + TN) * kCPR;
+        int it = 0;
+        for (int g = g_begin; g < g_end; ++g, ++it) {
+            const int sp = it % C::kNSP, pph = (it / C::kNSP) & 1;
+            const int su = it % kNSU, uph = (it / kNSU) & 1;
+            // activation scales of this group, pre-multiplied by 2^-8 (the MMA operands are 16*code)
+            for (int c = u; c < TN; c += kNumUnpackThreads) {
+                const int m = m0 + c;
+                sSx[(it & (kSxSlots - 1)) * TN + c] = m < p.M ? __ldg(p.sx + static_cast<size_t>(m) * p.ng + g) * 0x1p-8f : 0.0f;
+            }
+            mbar_wait(&pfull[sp], pph, 30);
+            mbar_wait(&uempty[su], uph ^ 1, 31);
+            const uint8_t* pa = sRing + kNSU * C::kUStage + sp * C::kPStage;
+            uint8_t* ua = sRing + su * C::kUStage;
+            for (int t = u; t < kTasks; t += kNumUnpackThreads) {
+                const int row = t / kCPR, j = t % kCPR;
+                const uint4 w = *reinterpret_cast<const uint4*>(pa + t * 16);  // A rows then B rows, contiguous
+                const uint4 o0 = make_uint4(nib_lo16(w.x), nib_hi16(w.x), nib_lo16(w.y), nib_hi16(w.y));
+                const uint4 o1 = make_uint4(nib_lo16(w.z), nib_hi16(w.z), nib_lo16(w.w), nib_hi16(w.w));
+                uint8_t* dst = row < kTileN ? ua : ua + C::kUA;
+                const uint32_t rr = row < kTileN ? row : row - kTileN;
+                *reinterpret_cast<uint4*>(dst + swizzled_chunk_offset<G>(rr, 2 * j)) = o0;
+                *reinterpret_cast<uint4*>(dst + swizzled_chunk_offset<G>(rr, 2 * j + 1)) = o1;
+            }
+            fence_proxy_async_smem();  // generic-proxy writes -> visible to the tensor core (async proxy)
+            __syncwarp();
+            if (lane == 0) { mbar_arrive(&ufull[su]); mbar_arrive(&pempty[sp]); }
+        }
+    } else if (warp >= 8) {
+        // ================================================================ epilogue warps
+        const int q = warp & 3;          // TMEM lane quarter this warp may access
+        const int h = (warp - 8) >> 2;   // which half of the token columns
+        constexpr int kCPW = TN >= 32 ? TN / 32 : 1;  // 16-column chunks per warp
+        const bool active = TN >= 32 || h == 0;
+        const int row = q * 32 + lane;
+        const int n = n0 + row;
+        const uint32_t tlane = tmem + (static_cast<uint32_t>(q * 32) << 16);
+        float acc[kCPW * 16];
+#pragma unroll
+        for (int i = 0; i < kCPW * 16; ++i) acc[i] = 0.0f;
+
+        if (has_lr) {
+            mbar_wait(h_full, 0, 40);
+            tc_fence_after();
+            if (active) {
+                for (int rb = 0; rb < nrb; ++rb) {
+#pragma unroll
+                    for (int i = 0; i < kCPW; ++i) {
+                        const int ch = h * kCPW + i;
+                        uint32_t v[16];
+                        tmem_ld16(tlane + kColH + rb * TN + ch * 16, v);
+                        tmem_ld_wait();
+                        const int j = rb * 128 + row;
+                        uint8_t* hk = sH + (j >> 6) * (TN * 128) + (j & 7) * 2;
+                        const uint32_t chunk = (j & 63) >> 3;
+#pragma unroll
+                        for (int c16 = 0; c16 < 16; ++c16) {
+                            const uint32_t c = ch * 16 + c16;
+                            *reinterpret_cast<__nv_bfloat16*>(hk + swizzled_chunk_offset<128>(c, chunk)) =
+                                __float2bfloat16_rn(__uint_as_float(v[c16]));
+                        }
+                    }
+                }
+            }
+            tc_fence_before();
+            fence_proxy_async_smem();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(h_ready);
+        }
+
+        int it = 0;
+        for (int g = g_begin; g < g_end; ++g, ++it) {
+            const int b = it & 1, bph = (it >> 1) & 1;
+            const float swn = n < p.N ? __ldg(p.swT + static_cast<size_t>(g) * p.N + n) : 0.0f;
+            const float cmagic = __fmul_rn(12582912.0f, swn);  // exact: sw has an 11-bit significand
+            mbar_wait(&tfull[b], bph, 41);
+            tc_fence_after();
+            if (active) {
+                const float* cs = sSx + (it & (kSxSlots - 1)) * TN;
+#pragma unroll
+                for (int i = 0; i < kCPW; ++i) {
+                    const int ch = h * kCPW + i;
+                    uint32_t v[16];
+                    tmem_ld16(tlane + kColP + b * TN + ch * 16, v);
+                    tmem_ld_wait();
+#pragma unroll
+                    for (int c4 = 0; c4 < 4; ++c4) {
+                        const float4 s4 = *reinterpret_cast<const float4*>(cs + ch * 16 + c4 * 4);
+                        const float sv[4] = {s4.x, s4.y, s4.z, s4.w};
+#pragma unroll
+                        for (int e = 0; e < 4; ++e) {
+                            const int c16 = c4 * 4 + e;
+                            // v = 256*P (|v| < 2^22): bits(1.5*2^23) + v is the float 1.5*2^23 + v exactly;
+                            // one FMA gives RN(v * sw) with no int->float conversion instruction.
+                            const float fp = __uint_as_float(v[c16] + 0x4B400000u);
+                            const float t = __fmaf_rn(fp, swn, -cmagic);
+                            acc[i * 16 + c16] = __fmaf_rn(t, sv[e], acc[i * 16 + c16]);
+                        }
+                    }
+                    if (p.dbgP != nullptr && n < p.N) {
+#pragma unroll
+                        for (int c16 = 0; c16 < 16; ++c16) {
+                            const int m = m0 + ch * 16 + c16;
+                            if (m < p.M)
+                                p.dbgP[(static_cast<size_t>(m) * p.ng + g) * p.N + n] = static_cast<int32_t>(v[c16]) >> 8;
+                        }
+                    }
+                }
+            }
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&tempty[b]);
+        }
+
+        if (has_lr) {
+            mbar_wait(ylr_done, 0, 42);
+            tc_fence_after();
+            if (active) {
+#pragma unroll
+                for (int i = 0; i < kCPW; ++i) {
+                    const int ch = h * kCPW + i;
+                    uint32_t v[16];
+                    tmem_ld16(tlane + kColYlr + ch * 16, v);
+                    tmem_ld_wait();
+#pragma unroll
+                    for (int c16 = 0; c16 < 16; ++c16) acc[i * 16 + c16] += __uint_as_float(v[c16]);
+                }
+            }
+            tc_fence_before();
+        }
+
+        if (active && n < p.N) {
+            if (gridDim.z == 1) {
+#pragma unroll
+                for (int i = 0; i < kCPW; ++i) {
+#pragma unroll
+                    for (int c16 = 0; c16 < 16; ++c16) {
+                        const int m = m0 + (h * kCPW + i) * 16 + c16;
+                        if (m < p.M) {
+                            const size_t o = static_cast<size_t>(m) * p.ldy + n;
+                            const float y = acc[i * 16 + c16];
+                            if (p.ydt == 0) static_cast<__nv_bfloat16*>(p.Y)[o] = __float2bfloat16_rn(y);
+                            else if (p.ydt == 1) static_cast<__half*>(p.Y)[o] = __float2half_rn(y);
+                            else static_cast<float*>(p.Y)[o] = y;
+                        }
+                    }
+                }
+            } else {
+                // split-K: park the FP32 partial of this split in the workspace [z][M][N]
+#pragma unroll
+                for (int i = 0; i < kCPW; ++i) {
+#pragma unroll
+                    for (int c16 = 0; c16 < 16; ++c16) {
+                        const int m = m0 + (h * kCPW + i) * 16 + c16;
+                        if (m < p.M)
+                            p.ws_part[(static_cast<size_t>(blockIdx.z) * p.M + m) * p.N + n] = acc[i * 16 + c16];
+                    }
+                }
+            }
+        }
+    }
+
+    // ---------------------------------------------------------------- teardown
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 2) {
+        tc_fence_after();
+        tmem_dealloc<512>(tmem);
+    }
+
+    if (gridDim.z > 1) {
+        // Deterministic split-K fix-up: the last CTA of this (n-tile, m-tile) to finish sums the
+        // partials in split order and writes Y; the tile counter is left at zero for the next call.
+        __shared__ int s_last;
+        __threadfence();
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            unsigned* ctr = p.ws_ctr + blockIdx.y * gridDim.x + blockIdx.x;
+            const unsigned prev = atomicAdd(ctr, 1u);
+            s_last = prev == gridDim.z - 1;
+            if (s_last) *ctr = 0;
+        }
+        __syncthreads();
+        if (s_last) {
+            __threadfence();
+            const int rows = min(TN, p.M - m0);
+            for (int idx = threadIdx.x; idx < rows * kTileN; idx += kThreads) {
+                const int mm = m0 + idx / kTileN, nn = n0 + idx % kTileN;
+                if (nn >= p.N) continue;
+                float y = 0.0f;
+                for (unsigned z = 0; z < gridDim.z; ++z)
+                    y += __ldcg(p.ws_part + (static_cast<size_t>(z) * p.M + mm) * p.N + nn);
+                const size_t o = static_cast<size_t>(mm) * p.ldy + nn;
+                if (p.ydt == 0) static_cast<__nv_bfloat16*>(p.Y)[o] = __float2bfloat16_rn(y);
+                else if (p.ydt == 1) static_cast<__half*>(p.Y)[o] = __float2half_rn(y);
+                else static_cast<float*>(p.Y)[o] = y;
+            }
+        }
+    }
+}
+
+template <int TN, int G>
+cudaError_t launch_one(const DualMaps& maps, const DualParams& p, dim3 grid, cudaStream_t stream) {
+    using C = Cfg<TN, G>;
+    auto kern = dual_linear_kernel<TN, G>;
+    static bool attr_set = false;
+    if (!attr_set) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::kSmemBytes);
+        if (e != cudaSuccess) return e;
+        attr_set = true;
+    }
+    kern<<<grid, kThreads, C::kSmemBytes, stream>>>(maps.W, maps.Xq, maps.X, maps.L1T, maps.L2T, p);
+    return cudaGetLastError();
+}
+
+}  // namespace
+
+int dual_pick_tn(int M) { return M <= 16 ? 16 : (M <= 32 ? 32 : (M <= 64 ? 64 : 128)); }
+
+cudaError_t launch_dual_linear(const DualMaps& maps, const DualParams& p, int TN, int G, int splits,
+                               cudaStream_t stream) {
+    dim3 grid((p.N + kTileN - 1) / kTileN, (p.M + TN - 1) / TN, splits);
+#define TWQ_CASE(tn, g) \
+    if (TN == tn && G == g) return launch_one<tn, g>(maps, p, grid, stream);
+    TWQ_CASE(16, 128) TWQ_CASE(32, 128) TWQ_CASE(64, 128) TWQ_CASE(128, 128)
+    TWQ_CASE(16, 64) TWQ_CASE(32, 64) TWQ_CASE(64, 64) TWQ_CASE(128, 64)
+#undef TWQ_CASE
+    return cudaErrorInvalidValue;
+}
+
+}  // namespace twq
