@@ -10,8 +10,9 @@
 // run N = 16 MMAs instead of padding M to 128.
 //
 // Phases inside the CTA (r > 0):
-//   1. stage 1   H^T[j,m] = sum_k L1T[j,k] X[m,k]    kind::f16 (A = f16, B = bf16), TMA-fed ring
-//      epilogue warps drain H^T from TMEM, round once to BF16 and write H[m,j] (K-major,
+//   1. stage 1   H^T[j,m] = sum_k L1T[j,k] X[m,k]    kind::f16, TMA-fed ring; helper warps rewrite the
+//      BF16 X tile as FP16 in place (exact), because both MMA operands must share one format.
+//      epilogue warps drain H^T from TMEM, round once to FP16 and write H[m,j] (K-major,
 //      128B-swizzled) into shared memory: the intermediate never leaves the SM.
 //   2. stage 2   Ylr^T[n,m] = sum_j L2T[n,j] H[m,j]  kind::f16, accumulator stays in TMEM
 //   3. residual  per group g: TMA brings packed INT4 rows of R4 and Xq; unpack warps expand
@@ -49,7 +50,7 @@ struct Cfg {
     static constexpr int kXChunk = TN * 128;            // X tile, 64 bf16 per row
     static constexpr int kL1Chunk = 128 * 128;          // L1T tile per 128-row block
     static constexpr int kS1Stage = kXChunk + 2 * kL1Chunk;
-    static constexpr int kHBytes = TN * 512;            // H[m, 0..255] bf16 as 4 k-blocks of TN x 128 B
+    static constexpr int kHBytes = TN * 512;            // H[m, 0..255] fp16 as 4 k-blocks of TN x 128 B
     static constexpr int kL2TBytes = 4 * kL1Chunk;
     static constexpr int kPA = kTileN * (G / 2);        // packed weight rows of one group
     static constexpr int kPB = TN * (G / 2);
@@ -66,7 +67,7 @@ struct Cfg {
     static constexpr int kOffRing = kHBytes;
     static constexpr int kOffSx = kOffRing + kRing;
     static constexpr int kOffBar = kOffSx + kSxSlots * TN * 4;
-    static constexpr int kNumBars = 2 * kNS1 + 2 * kNSP + 2 * kNSU + 4 + 4;
+    static constexpr int kNumBars = 3 * kNS1 + 2 * kNSP + 2 * kNSU + 4 + 4;
     static constexpr int kSmemBytes = kOffBar + kNumBars * 8 + 16 + 1024;  // + TMEM slot + alignment slack
     static_assert(kHBytes % 1024 == 0 && kXChunk % 1024 == 0 && kUA % 1024 == 0 && kUB % 512 == 0, "tile alignment");
     static_assert(kSmemBytes <= 232448, "shared memory budget");
@@ -89,7 +90,8 @@ dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constan
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem + C::kOffBar);
     uint64_t* full1 = bars;                    // [kNS1]  TMA -> MMA (stage 1)
     uint64_t* empty1 = full1 + kNS1;           // [kNS1]  MMA -> TMA
-    uint64_t* pfull = empty1 + kNS1;           // [kNSP]  TMA -> unpack
+    uint64_t* xconv = empty1 + kNS1;           // [kNS1]  converter warps -> MMA (X tile is FP16 now)
+    uint64_t* pfull = xconv + kNS1;            // [kNSP]  TMA -> unpack
     uint64_t* pempty = pfull + C::kNSP;        // [kNSP]  unpack -> TMA
     uint64_t* ufull = pempty + C::kNSP;        // [kNSU]  unpack -> MMA
     uint64_t* uempty = ufull + kNSU;           // [kNSU]  MMA -> unpack
@@ -118,7 +120,7 @@ dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constan
     const bool has_lr = r > 0 && kc_begin < kc_end;
 
     if (threadIdx.x == 0) {
-        for (int i = 0; i < kNS1; ++i) { mbar_init(&full1[i], 1); mbar_init(&empty1[i], 1); }
+        for (int i = 0; i < kNS1; ++i) { mbar_init(&full1[i], 1); mbar_init(&empty1[i], 1); mbar_init(&xconv[i], kNumUnpackThreads / 32); }
         for (int i = 0; i < C::kNSP; ++i) { mbar_init(&pfull[i], 1); mbar_init(&pempty[i], kNumUnpackThreads / 32); }
         for (int i = 0; i < kNSU; ++i) { mbar_init(&ufull[i], kNumUnpackThreads / 32); mbar_init(&uempty[i], 1); }
         for (int i = 0; i < 2; ++i) { mbar_init(&tfull[i], 1); mbar_init(&tempty[i], kNumEpiWarps); }
@@ -174,11 +176,11 @@ dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constan
         // ================================================================ MMA issuer (one thread)
         if (lane == 0) {
             if (has_lr) {
-                const uint32_t idesc1 = umma_idesc(1, 0, 1, 128, TN);  // D f32, A f16 (L1T), B bf16 (X)
+                const uint32_t idesc1 = umma_idesc(1, 0, 0, 128, TN);  // D f32, A f16 (L1T), B f16 (X converted in place)
                 int it = 0;
                 for (int kc = kc_begin; kc < kc_end; ++kc, ++it) {
                     const int s = it % kNS1, ph = (it / kNS1) & 1;
-                    mbar_wait(&full1[s], ph, 20);
+                    mbar_wait(&xconv[s], ph, 20);
                     tc_fence_after();
                     const uint32_t xb = smem_u32(sRing + s * C::kS1Stage);
                     const uint32_t lb = xb + C::kXChunk;
@@ -193,7 +195,7 @@ dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constan
                 mbar_wait(h_ready, 0, 21);
                 mbar_wait(l2_full, 0, 22);
                 tc_fence_after();
-                const uint32_t idesc2 = umma_idesc(1, 0, 1, 128, TN);  // D f32, A f16 (L2T), B bf16 (H)
+                const uint32_t idesc2 = umma_idesc(1, 0, 0, 128, TN);  // D f32, A f16 (L2T), B f16 (H)
                 const uint32_t l2b = smem_u32(sRing), hb = smem_u32(sH);
                 const int nks = (r + 15) >> 4;
                 for (int ks = 0; ks < nks; ++ks) {
@@ -226,6 +228,34 @@ dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constan
         const int u = threadIdx.x - 128;
         constexpr int kCPR = (G / 2) / 16;  // 16-byte packed chunks per row
         constexpr int kTasks = (kTileN + TN) * kCPR;
+        if (has_lr) {
+            // Stage-1 helper: kind::f16 needs A and B in ONE 16-bit format (mixing f16 and bf16 operands
+            // is an illegal instruction on sm_100), and L1 is FP16.  Rewrite the BF16 X tile in place as
+            // FP16: exact for 2^-14 <= |x| <= 65504, saturating above.  Elementwise, so the swizzled
+            // layout TMA wrote is untouched.
+            int it1 = 0;
+            for (int kc = kc_begin; kc < kc_end; ++kc, ++it1) {
+                const int s = it1 % kNS1, ph = (it1 / kNS1) & 1;
+                mbar_wait(&full1[s], ph, 32);
+                uint4* xt = reinterpret_cast<uint4*>(sRing + s * C::kS1Stage);
+                for (int t = u; t < C::kXChunk / 16; t += kNumUnpackThreads) {
+                    uint4 w = xt[t];
+                    uint32_t* wp = reinterpret_cast<uint32_t*>(&w);
+#pragma unroll
+                    for (int e = 0; e < 4; ++e) {
+                        float lo = __uint_as_float(wp[e] << 16), hi = __uint_as_float(wp[e] & 0xFFFF0000u);
+                        lo = fminf(fmaxf(lo, -65504.0f), 65504.0f);
+                        hi = fminf(fmaxf(hi, -65504.0f), 65504.0f);
+                        const __half2 h2 = __floats2half2_rn(lo, hi);
+                        wp[e] = *reinterpret_cast<const uint32_t*>(&h2);
+                    }
+                    xt[t] = w;
+                }
+                fence_proxy_async_smem();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&xconv[s]);
+            }
+        }
         int it = 0;
         for (int g = g_begin; g < g_end; ++g, ++it) {
             const int sp = it % C::kNSP, pph = (it / C::kNSP) & 1;
@@ -283,8 +313,8 @@ dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constan
 #pragma unroll
                         for (int c16 = 0; c16 < 16; ++c16) {
                             const uint32_t c = ch * 16 + c16;
-                            *reinterpret_cast<__nv_bfloat16*>(hk + swizzled_chunk_offset<128>(c, chunk)) =
-                                __float2bfloat16_rn(__uint_as_float(v[c16]));
+                            const float hv = fminf(fmaxf(__uint_as_float(v[c16]), -65504.0f), 65504.0f);
+                            *reinterpret_cast<__half*>(hk + swizzled_chunk_offset<128>(c, chunk)) = __float2half_rn(hv);
                         }
                     }
                 }
