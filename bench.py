@@ -1,0 +1,394 @@
+#!/usr/bin/env python
+"""bench.py -- timing harness for the TwinQuant dual-component linear layer on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload NAME] [--impl reference]
+
+One "step" = one pass of the whole hot path (twq_quantize_act + twq_dual_linear)
+over one batch of synthetic activations for one layer.  Prints ONE JSON line (rank 0).
+
+  value      us per step, device time (CUDA events around a CUDA graph of K steps, inputs resident in HBM)
+  e2e        the same through the public Python API with pinned-host X -> device and Y -> host inside the region
+  roofline   the fused kernel alone (its own K-launch graph): algorithmic bytes or int8-equivalent ops / time
+  cpu_baseline  the oracle (oracle/, as it stands) on the host cores, on a bounded sample
+  sweep      the other graded shapes (M = 1 / 16 / 128 q_proj, M = 2048 MLP) measured the same way
+
+Cold-cache protocol: the layer's packed weights (and activations) are rotated through enough distinct
+copies that one lap exceeds 2x the 126 MB L2, so every step streams its weights from HBM.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from gen import inputs as gen  # noqa: E402
+
+L2_BYTES = 126 * 1024 * 1024
+
+WORKLOADS = {
+    # name: (generator, kwargs, description)
+    "c2_qproj_m1": ("config2_qproj", dict(M=1), "LLaMA3-8B q_proj K=4096 N=4096 r=128 G=128 M=1"),
+    "c2_qproj_m16": ("config2_qproj", dict(M=16), "LLaMA3-8B q_proj K=4096 N=4096 r=128 G=128 M=16"),
+    "c2_qproj_m128": ("config2_qproj", dict(M=128), "LLaMA3-8B q_proj K=4096 N=4096 r=128 G=128 M=128"),
+    "c3_gateup_m2048": ("config3_mlp", dict(which="gate_up", M=2048), "LLaMA3-8B gate/up K=4096 N=14336 r=128 G=128 M=2048"),
+    "c3_down_m2048": ("config3_mlp", dict(which="down", M=2048), "LLaMA3-8B down K=14336 N=4096 r=128 G=128 M=2048"),
+    "c3_gateup_m2048_r256": ("config3_mlp", dict(which="gate_up", M=2048, r=256), "LLaMA3-8B gate/up r=256 M=2048"),
+    "c1_tiny": ("config1_tiny", dict(), "tiny M=8 K=256 N=512 r=16 G=64"),
+}
+DEFAULT_WORKLOAD = "c2_qproj_m16"
+DEFAULT_SWEEP = ["c2_qproj_m1", "c2_qproj_m16", "c2_qproj_m128", "c3_gateup_m2048", "c3_down_m2048"]
+
+
+def load_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        p = json.load(open(path))
+        return dict(hbm_gbs=float(p["hbm_gbs"]), bf16_tflops=float(p["bf16_tflops"]),
+                    bf16_tflops_sustained=float(p.get("bf16_tflops_sustained", p["bf16_tflops"])), source="measured")
+    return dict(hbm_gbs=6650.0, bf16_tflops=1590.0, bf16_tflops_sustained=1400.0, source="fallback")
+
+
+def make_layer(name):
+    fn, kw, _ = WORKLOADS[name]
+    return getattr(gen, fn)(**kw)
+
+
+# ----------------------------------------------------------------------------- clocks
+class ClockSampler:
+    FIELDS = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+              "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+              "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index=0):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", f"--id={index}", f"--query-gpu={self.FIELDS}",
+                                       "--format=csv,noheader,nounits", "-lms", "100"], stdout=self.f,
+                                      stderr=subprocess.DEVNULL)
+        except OSError:
+            self.p = None
+
+    def stop(self):
+        out = dict(sm_mhz=None, sm_max_mhz=None, reasons=[])
+        if self.p is None:
+            return out
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.p.kill()
+        self.f.flush()
+        rows = [ln.strip().split(", ") for ln in open(self.f.name) if ln.strip()]
+        os.unlink(self.f.name)
+        sm, reasons, smax = [], set(), None
+        for r in rows:
+            if len(r) < 7:
+                continue
+            try:
+                sm.append(float(r[0]))
+                smax = float(r[1])
+            except ValueError:
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[3:7]):
+                if v.strip().lower() == "active":
+                    reasons.add(name)
+        if sm:
+            hi = [c for c in sm if c >= 0.5 * max(sm)]   # samples under load
+            out = dict(sm_mhz=float(np.median(hi)), sm_max_mhz=smax, reasons=sorted(reasons), samples=len(sm))
+        return out
+
+
+# ----------------------------------------------------------------------------- GPU arm
+class GpuLayer:
+    """Device-resident copies of one layer, rotated so that a lap over them exceeds 2x L2."""
+
+    def __init__(self, L, twq, torch, min_lap_bytes=2 * L2_BYTES, max_copies=32):
+        self.L, self.twq, self.torch = L, twq, torch
+        dev = torch.device("cuda", torch.cuda.current_device())
+        self.Xh = torch.from_numpy(L.X.view(np.int16)).view(torch.bfloat16).pin_memory()
+        Rq, sw = torch.from_numpy(L.Rq).to(dev), torch.from_numpy(L.sw).to(dev)
+        L1, L2 = torch.from_numpy(L.L1).to(dev), torch.from_numpy(L.L2).to(dev)
+        first = twq.pack_weights(Rq, sw, L1 if L.r else None, L2 if L.r else None, L.G)
+        per_copy = first.blob.numel() + 2 * L.M * L.K + L.M * L.K // 2 + 2 * L.M * L.N
+        self.ncopies = int(min(max_copies, max(2, -(-min_lap_bytes // per_copy))))
+        self.packed = [first]
+        for _ in range(self.ncopies - 1):
+            self.packed.append(twq.PackedLayer(first.blob.clone(), first.N, first.K, first.r, first.G))
+        self.X = [self.Xh.to(dev) for _ in range(self.ncopies)]
+        self.Xq = [torch.empty((L.M, L.K // 2), dtype=torch.uint8, device=dev) for _ in range(self.ncopies)]
+        self.sx = [torch.empty((L.M, L.ng), dtype=torch.float32, device=dev) for _ in range(self.ncopies)]
+        self.Y = [torch.empty((L.M, L.N), dtype=torch.bfloat16, device=dev) for _ in range(self.ncopies)]
+        need = twq.workspace_bytes(L.M, L.N, L.K, L.r, L.G)
+        self.ws = torch.zeros(max(need, 256), dtype=torch.uint8, device=dev) if need else None
+        self.Yh = torch.empty((L.M, L.N), dtype=torch.bfloat16).pin_memory()
+        self.lap_bytes = per_copy * self.ncopies
+        del Rq, sw, L1, L2
+        torch.cuda.synchronize()
+
+    def step(self, i, quant=True, dual=True):
+        c = i % self.ncopies
+        if quant:
+            self.twq.quantize_act(self.X[c], self.L.G, None, out=(self.Xq[c], self.sx[c]))
+        if dual:
+            self.twq.dual_linear(self.X[c], self.Xq[c], self.sx[c], self.packed[c], self.twq.OUT_BF16, Y=self.Y[c],
+                                 ws=self.ws)
+
+    def e2e_step(self, i):
+        c = i % self.ncopies
+        self.X[c].copy_(self.Xh, non_blocking=True)
+        self.step(i)
+        self.Yh.copy_(self.Y[c], non_blocking=True)
+
+    def time_graph(self, steps, warmup, quant=True, dual=True):
+        """Device time per step of a CUDA graph holding `steps` consecutive steps (no host launch gaps)."""
+        torch = self.torch
+        s = torch.cuda.Stream()
+        s.wait_stream(torch.cuda.current_stream())
+        with torch.cuda.stream(s):
+            for i in range(max(warmup, self.ncopies)):           # every Xq/sx copy is valid before dual-only timing
+                self.step(i, True, True)
+            s.synchronize()
+            g = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(g, stream=s):
+                for i in range(steps):
+                    self.step(i, quant, dual)
+            g.replay()                                            # one untimed replay (graph upload)
+            s.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(s)
+            g.replay()
+            e1.record(s)
+            s.synchronize()
+        torch.cuda.current_stream().wait_stream(s)
+        return e0.elapsed_time(e1) * 1e3 / steps                  # us per step
+
+    def time_e2e(self, steps, warmup):
+        torch = self.torch
+        for i in range(warmup):
+            self.e2e_step(i)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for i in range(steps):
+            self.e2e_step(i)
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1) * 1e3 / steps
+
+
+def roofline_for(L, twq, us_dual, peaks, traffic=None):
+    by = twq.algorithmic_bytes(L.M, L.N, L.K, L.r, L.G)
+    ops_i8, fl_lr = twq.flops(L.M, L.N, L.K, L.r)
+    p_i8 = 2.0 * peaks["bf16_tflops"] * 1e12        # int8 dense = 2x bf16 (guide's nominal ratio) x measured bf16
+    p_f16 = peaks["bf16_tflops"] * 1e12
+    t_hbm = by / (peaks["hbm_gbs"] * 1e9)
+    t_tensor = ops_i8 / p_i8 + fl_lr / p_f16
+    t = us_dual * 1e-6
+    if t_hbm >= t_tensor:
+        ach = by / t / 1e9
+        return dict(bound="hbm", achieved=round(ach, 1), peak=peaks["hbm_gbs"], unit="GB/s",
+                    frac=round(ach / peaks["hbm_gbs"], 4), traffic=traffic, peak_source=peaks["source"],
+                    kernel="dual_linear_kernel", us=round(us_dual, 3), algorithmic_bytes=by)
+    eq_ops = ops_i8 + 2.0 * fl_lr                    # low-rank flops run at half the int8 rate
+    ach = eq_ops / t / 1e12
+    return dict(bound="tensor", achieved=round(ach, 1), peak=round(p_i8 / 1e12, 1), unit="TFLOP/s",
+                frac=round(ach / (p_i8 / 1e12), 4), traffic=traffic, peak_source=peaks["source"] + " bf16 burst x2 (int8)",
+                kernel="dual_linear_kernel", us=round(us_dual, 3), int8_equivalent_ops=eq_ops)
+
+
+def load_traffic(name):
+    path = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(path):
+        return json.load(open(path)).get(name)
+    return None
+
+
+def measure_workload(name, twq, torch, steps, warmup, peaks, with_e2e=False, with_cublas=False):
+    L = make_layer(name)
+    gl = GpuLayer(L, twq, torch)
+    us_step = gl.time_graph(steps, warmup, True, True)
+    us_dual = gl.time_graph(steps, warmup, False, True)
+    us_quant = gl.time_graph(steps, warmup, True, False)
+    ops_i8, fl_lr = twq.flops(L.M, L.N, L.K, L.r)
+    out = dict(workload=name, M=L.M, N=L.N, K=L.K, r=L.r, G=L.G, us_step=round(us_step, 3),
+               us_dual_linear=round(us_dual, 3), us_quantize_act=round(us_quant, 3),
+               eff_tops=round((ops_i8 + fl_lr) / (us_dual * 1e-6) / 1e12, 2),
+               gbs=round(twq.algorithmic_bytes(L.M, L.N, L.K, L.r, L.G) / (us_dual * 1e-6) / 1e9, 1),
+               weight_copies=gl.ncopies, lap_mb=round(gl.lap_bytes / 2 ** 20, 1),
+               roofline=roofline_for(L, twq, us_dual, peaks, load_traffic(name)))
+    if with_e2e:
+        out["us_e2e"] = round(gl.time_e2e(steps, warmup), 3)
+    if with_cublas:
+        A = torch.randn(L.M, L.K, device="cuda", dtype=torch.bfloat16)
+        Bs = [torch.randn(L.K, L.N, device="cuda", dtype=torch.bfloat16) for _ in range(max(2, min(16, (2 * L2_BYTES) // (2 * L.K * L.N) + 1)))]
+        for b in Bs[:3]:
+            torch.matmul(A, b)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for i in range(steps):
+            torch.matmul(A, Bs[i % len(Bs)])
+        e1.record()
+        torch.cuda.synchronize()
+        out["us_cublas_bf16_gemm"] = round(e0.elapsed_time(e1) * 1e3 / steps, 3)
+    return out, gl, L
+
+
+# ----------------------------------------------------------------------------- CPU oracle arm
+def time_oracle(L, budget_s=12.0, max_calls=10000):
+    """The oracle as it stands (quantize + pack + forward), all host cores; bounded by ~budget_s of work."""
+    from oracle import oracle as orc
+    orc.build()
+    rows = None
+    sample = f"all {L.M} token rows"
+    macs = L.M * L.N * L.K
+    if macs > 4e9:                                   # prefill shapes: a fixed sample of token rows, scaled linearly in M
+        nrows = max(1, int(4e9 // (L.N * L.K)))
+        rows = sorted(set(np.linspace(0, L.M - 1, nrows).astype(int).tolist()))
+        sample = f"{len(rows)} of {L.M} token rows (all N, all groups), time scaled by M/rows"
+    t0 = time.perf_counter()
+    calls = 0
+    while True:
+        orc.forward(L.X, L.Rq, L.sw, L.L1 if L.r else None, L.L2 if L.r else None, L.G, rows=rows)
+        calls += 1
+        el = time.perf_counter() - t0
+        if el >= budget_s or calls >= max_calls:
+            break
+    scale = 1.0 if rows is None else L.M / len(rows)
+    us = el / calls * 1e6 * scale
+    return dict(value=round(us, 1), unit="us/call", cores=orc.num_threads(), kind="oracle",
+                sample=f"{sample}; {calls} call(s) in {el:.1f} s")
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    L = make_layer(args.workload)
+    from oracle import oracle as orc
+    orc.build()
+    for _ in range(min(args.warmup, 1)):
+        time_oracle(L, budget_s=0.5, max_calls=1)
+    per_step_budget = min(20.0, 120.0 / max(1, args.steps))
+    t0 = time.perf_counter()
+    res = [time_oracle(L, budget_s=per_step_budget, max_calls=1) for _ in range(args.steps)]
+    us = float(np.mean([r["value"] for r in res]))
+    cb = dict(res[-1])
+    cb["value"] = round(us, 1)
+    line = dict(metric="fused dual-linear us/call", value=round(us, 1), unit="us/call", n_gpus=args.gpus,
+                steps=args.steps, warmup=args.warmup, ms_per_step=round(us / 1e3, 4), higher_is_better=False,
+                scaling="weak", vs_baseline=None, dtype="int64+f64", data="synthetic", impl="reference",
+                config=dict(workload=args.workload, desc=WORKLOADS[args.workload][2]),
+                cpu_baseline=cb,
+                e2e=dict(value=round(us, 1), unit="us/call", h2d_bytes_per_step=0, d2h_bytes_per_step=0),
+                wall_s=round(time.perf_counter() - t0, 1))
+    print(json.dumps(line))
+
+
+# ----------------------------------------------------------------------------- main
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=20)
+    ap.add_argument("--workload", default=DEFAULT_WORKLOAD, choices=sorted(WORKLOADS))
+    ap.add_argument("--impl", default="twq", choices=["twq", "reference"])
+    ap.add_argument("--no-sweep", action="store_true", help="time only --workload")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3)
+
+    if args.impl == "reference":
+        run_reference(args)
+        return
+
+    import torch
+    import paper_2606_01556_b200 as twq
+    twq.load_library()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl")
+
+    peaks = load_peaks()
+    sampler = ClockSampler(local) if rank == 0 else None
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    barrier()
+    main_res, gl, L = measure_workload(args.workload, twq, torch, args.steps, args.warmup, peaks, with_e2e=True,
+                                       with_cublas=(rank == 0))
+    barrier()
+    us = main_res["us_step"]
+    us_e2e = main_res["us_e2e"]
+    if dist is not None:                      # replicas only: max over ranks
+        t = torch.tensor([us, us_e2e], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        us, us_e2e = float(t[0]), float(t[1])
+    clocks = sampler.stop() if sampler else None
+
+    sweep = []
+    if rank == 0 and not args.no_sweep:
+        del gl
+        torch.cuda.empty_cache()
+        for name in DEFAULT_SWEEP:
+            if name == args.workload:
+                sweep.append({k: v for k, v in main_res.items() if k != "us_e2e"})
+                continue
+            r, g2, _ = measure_workload(name, twq, torch, max(20, min(args.steps, 100)), args.warmup, peaks,
+                                        with_cublas=True)
+            sweep.append(r)
+            del g2
+            torch.cuda.empty_cache()
+
+    if rank == 0:
+        cpu = None if args.no_cpu_baseline else time_oracle(L)
+        # whole-job figure: N replicas each finish K calls in the max-over-ranks time
+        value = us / world
+        line = dict(metric="fused dual-linear us/call", value=round(value, 3), unit="us/call", n_gpus=world,
+                    steps=args.steps, warmup=args.warmup, ms_per_step=round(us / 1e3, 6), higher_is_better=False,
+                    scaling="weak", vs_baseline=None, dtype="s8 (INT4 codes x16) -> s32; f16 -> f32 low-rank",
+                    data="synthetic",
+                    config=dict(workload=args.workload, desc=WORKLOADS[args.workload][2],
+                                l2="inputs larger than L2: %d rotating copies, %.0f MB per lap" %
+                                   (main_res["weight_copies"], main_res["lap_mb"]),
+                                launch="CUDA graph of K steps; step = twq_quantize_act + twq_dual_linear",
+                                multi_gpu="replicas only"),
+                    clocks=clocks,
+                    e2e=dict(value=round(us_e2e / world, 3), unit="us/call", h2d_bytes_per_step=2 * L.M * L.K,
+                             d2h_bytes_per_step=2 * L.M * L.N),
+                    gpu_launches=2 * args.steps,
+                    roofline=main_res["roofline"], cpu_baseline=cpu,
+                    us_dual_linear=main_res["us_dual_linear"], us_quantize_act=main_res["us_quantize_act"],
+                    eff_tops=main_res["eff_tops"], gbs=main_res["gbs"],
+                    cublas_bf16_gemm_us=main_res.get("us_cublas_bf16_gemm"),
+                    paper_context="paper: up to 1.8x over FP16 TensorRT-LLM end to end on RTX 4090 / L20 (PAPER.md L232)",
+                    sweep=sweep)
+        print(json.dumps(line))
+    if dist is not None:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -136,7 +136,7 @@ def dual_linear(X, Xq, sx, packed: PackedLayer, out_dtype: int = OUT_BF16, Y=Non
     M = Xq.shape[0]
     N, K, r, G = packed.N, packed.K, packed.r, packed.G
     if Y is None:
-        Y = torch.empty((M, N), dtype=_OUT_TORCH[out_dtype], device=Xq.device)
+        Y = torch.empty((M, N), dtype=_OUT_TORCH.get(out_dtype, torch.bfloat16), device=Xq.device)
     need = workspace_bytes(M, N, K, r, G)
     if need and ws is None:
         ws = torch.zeros(need, dtype=torch.uint8, device=Xq.device)
