@@ -295,6 +295,23 @@ def run_reference(args):
     print(json.dumps(line))
 
 
+# ----------------------------------------------------------------------------- multi-GPU (replicas only)
+def max_over_ranks(values, dist, device):
+    """Replicas only: every rank times its own replica; the job's time is the MAX
+    over ranks.  `dist` is torch.distributed (initialised) or None for a single process."""
+    import torch
+    if dist is None:
+        return [float(v) for v in values]
+    t = torch.tensor([float(v) for v in values], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(v) for v in t]
+
+
+def whole_job_us_per_call(us_max, world):
+    """N replicas each finish one call in `us_max` (max over ranks): the job completes N calls in that time."""
+    return us_max / world
+
+
 # ----------------------------------------------------------------------------- main
 def main():
     ap = argparse.ArgumentParser()
@@ -341,10 +358,7 @@ def main():
     barrier()
     us = main_res["us_step"]
     us_e2e = main_res["us_e2e"]
-    if dist is not None:                      # replicas only: max over ranks
-        t = torch.tensor([us, us_e2e], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        us, us_e2e = float(t[0]), float(t[1])
+    us, us_e2e = max_over_ranks([us, us_e2e], dist, "cuda")   # replicas only
     clocks = sampler.stop() if sampler else None
 
     sweep = []
@@ -364,7 +378,7 @@ def main():
     if rank == 0:
         cpu = None if args.no_cpu_baseline else time_oracle(L)
         # whole-job figure: N replicas each finish K calls in the max-over-ranks time
-        value = us / world
+        value = whole_job_us_per_call(us, world)
         line = dict(metric="fused dual-linear us/call", value=round(value, 3), unit="us/call", n_gpus=world,
                     steps=args.steps, warmup=args.warmup, ms_per_step=round(us / 1e3, 6), higher_is_better=False,
                     scaling="weak", vs_baseline=None, dtype="s8 (INT4 codes x16) -> s32; f16 -> f32 low-rank",
@@ -375,7 +389,7 @@ def main():
                                 launch="CUDA graph of K steps; step = twq_quantize_act + twq_dual_linear",
                                 multi_gpu="replicas only"),
                     clocks=clocks,
-                    e2e=dict(value=round(us_e2e / world, 3), unit="us/call", h2d_bytes_per_step=2 * L.M * L.K,
+                    e2e=dict(value=round(whole_job_us_per_call(us_e2e, world), 3), unit="us/call", h2d_bytes_per_step=2 * L.M * L.K,
                              d2h_bytes_per_step=2 * L.M * L.N),
                     gpu_launches=2 * args.steps,
                     roofline=main_res["roofline"], cpu_baseline=cpu,
