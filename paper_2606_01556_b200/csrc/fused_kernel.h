@@ -1,0 +1,52 @@
+// fused_kernel.h -- host-side interface between the C ABI (twq_api.cu) and the fused
+// dual-branch kernel (fused_kernel.cu).  Plain structs; all launch planning is host arithmetic.
+#pragma once
+#include <cuda.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace twq {
+
+// Work decomposition and shared-memory plan of one twq_dual_linear call (host-computed).
+struct FusedPlan {
+    int TN;                  // tokens per tile (MMA N): 16 / 32 / 64 / 128
+    int cs;                  // CTAs per cluster; the cluster shares the stage-1 product H through DSMEM
+    int splits;              // K splits (decode-shaped calls)
+    int g_per_split;         // residual groups per split
+    int n_tiles, m_tiles;    // 128-channel tiles, TN-token tiles
+    int n_blocks;            // n_tiles / cs
+    int units;               // splits * m_tiles * n_blocks  (one unit = cs n-tiles of one m-tile, one K split)
+    int nclusters;           // persistent clusters; cluster c owns units [c*units/nclusters, (c+1)*units/nclusters)
+    int nsp, nsu, ns1;       // ring depths: packed (TMA), expanded (MMA operands), stage-1
+    int alias;               // 1: the stage-1 ring and the FP32 H partial overlay the residual rings
+    int off_H, off_L2T, off_U, off_P, off_S1, off_Hpart, off_sx, off_bar;
+    int smem_bytes;
+    int tmem_cols;           // 256 or 512
+};
+
+struct FusedParams {
+    int M, N, K, r, ng;
+    int ldy, ydt;            // ydt: 0 bf16, 1 fp16, 2 fp32
+    const float* sx;         // [M][ng] activation group scales
+    const float* swT;        // [ng][N] weight group scales (FP32, transposed)
+    void* Y;                 // [M][ldy]
+    int32_t* dbgP;           // NULL or [M][ng][N]
+    float* ws_part;          // split-K partials [splits][M][N] (splits > 1 only)
+    unsigned* ws_ctr;        // split-K tile counters [m_tiles][n_tiles], zero between calls
+    FusedPlan plan;
+};
+
+struct FusedMaps {
+    CUtensorMap W, Xq, X, L1T, L2T;
+};
+
+// Fills `plan` for a shape; returns false if the shape cannot be planned (never for valid ABI shapes).
+bool fused_make_plan(int M, int N, int K, int r, int G, int num_sms, FusedPlan* plan);
+cudaError_t launch_fused(const FusedMaps& maps, const FusedParams& p, int G, cudaStream_t stream);
+
+cudaError_t launch_quantize_act(const void* X, int M, int K, int ldx, const float* tinv, int G, uint8_t* Xq,
+                                float* sx, cudaStream_t stream);
+cudaError_t launch_pack_weights(const int8_t* Rq, const void* sw, const void* L1, const void* L2, int N, int K, int r,
+                                int G, void* packed, cudaStream_t stream, int* launches);
+
+}  // namespace twq

@@ -6,7 +6,7 @@
 #include <string.h>
 
 #include "../../include/twq.h"
-#include "dual_linear.h"
+#include "fused_kernel.h"
 #include "packed_layout.h"
 
 namespace {
@@ -24,26 +24,23 @@ bool shape_ok(int M, int N, int K, int r, int G) {
     return true;
 }
 
-// Split the reduction over grid.z when the output tiles alone cannot fill 148 SMs
-// (decode-shaped M); each split owns a contiguous range of groups.
-int pick_splits(int M, int N, int K, int G) {
-    const int TN = twq::dual_pick_tn(M);
-    const long long tiles = static_cast<long long>((N + 127) / 128) * ((M + TN - 1) / TN);
-    const int ng = K / G;
-    if (tiles >= 111) return 1;  // >= 0.75 wave
-    long long s = 148 / tiles;
-    if (s > 16) s = 16;
-    if (s > ng) s = ng;
-    if (s < 1) s = 1;
-    // make every split non-empty
-    const int per = (ng + static_cast<int>(s) - 1) / static_cast<int>(s);
-    return (ng + per - 1) / per;
+// SM count of the current device (148 on B200; also the planning default when no device is present,
+// so twq_workspace_bytes gives the same answer on a CPU-only box).
+int num_sms() {
+    static thread_local int cached = 0;
+    if (cached == 0) {
+        int dev = 0, n = 0;
+        if (cudaGetDevice(&dev) == cudaSuccess &&
+            cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && n > 0)
+            cached = n;
+        else
+            return 148;
+    }
+    return cached;
 }
 
-size_t ctr_bytes(int M, int N) {
-    const int TN = twq::dual_pick_tn(M);
-    const size_t tiles = static_cast<size_t>((N + 127) / 128) * ((M + TN - 1) / TN);
-    return twq::align256(tiles * sizeof(unsigned));
+size_t ctr_bytes(const twq::FusedPlan& pl) {
+    return twq::align256(static_cast<size_t>(pl.n_tiles) * pl.m_tiles * sizeof(unsigned));
 }
 
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
@@ -142,9 +139,10 @@ twq_status twq_quantize_act(const void* X, int M, int K, int ldx, const float* t
 
 size_t twq_workspace_bytes(int M, int N, int K, int r, int G) {
     if (!shape_ok(M, N, K, r, G)) return 0;
-    const int s = pick_splits(M, N, K, G);
-    if (s <= 1) return 0;
-    return ctr_bytes(M, N) + static_cast<size_t>(s) * M * N * sizeof(float);
+    twq::FusedPlan pl;
+    if (!twq::fused_make_plan(M, N, K, r, G, num_sms(), &pl)) return 0;
+    if (pl.splits <= 1) return 0;
+    return ctr_bytes(pl) + static_cast<size_t>(pl.splits) * M * N * sizeof(float);
 }
 
 twq_status twq_dual_linear(const void* X, int ldx, const uint8_t* Xq, const float* sx, const void* packed, int M,
@@ -165,18 +163,21 @@ twq_status twq_dual_linear(const void* X, int ldx, const uint8_t* Xq, const floa
     if (need > 0 && (reinterpret_cast<uintptr_t>(ws) & 255u)) return TWQ_ERR_INVALID_ARG;
     if (!device_is_sm100()) return TWQ_ERR_UNSUPPORTED;
 
-    const int TN = twq::dual_pick_tn(M);
-    const int splits = pick_splits(M, N, K, G);
+    twq::FusedParams p;
+    memset(&p, 0, sizeof(p));
+    if (!twq::fused_make_plan(M, N, K, r, G, num_sms(), &p.plan)) return TWQ_ERR_UNSUPPORTED;
+    const int TN = p.plan.TN;
+    const int splits = p.plan.splits;
     const twq::PackedLayout lay = twq::packed_layout(N, K, r, G);
     const uint8_t* base = static_cast<const uint8_t*>(packed);
 
-    twq::DualMaps maps;
+    twq::FusedMaps maps;
     memset(&maps, 0, sizeof(maps));
     bool ok = true;
-    ok &= make_map(&maps.W, CU_TENSOR_MAP_DATA_TYPE_UINT8, 1, base + lay.off_r4, K / 2, N, K / 2, G / 2, 128,
-                   CU_TENSOR_MAP_SWIZZLE_NONE);
-    ok &= make_map(&maps.Xq, CU_TENSOR_MAP_DATA_TYPE_UINT8, 1, Xq, K / 2, M, K / 2, G / 2, TN,
-                   CU_TENSOR_MAP_SWIZZLE_NONE);
+    // packed INT4 tiles: rows of G/2 bytes, swizzled so that one-row-per-thread reads are conflict-free
+    const CUtensorMapSwizzle psw = G == 128 ? CU_TENSOR_MAP_SWIZZLE_64B : CU_TENSOR_MAP_SWIZZLE_32B;
+    ok &= make_map(&maps.W, CU_TENSOR_MAP_DATA_TYPE_UINT8, 1, base + lay.off_r4, K / 2, N, K / 2, G / 2, 128, psw);
+    ok &= make_map(&maps.Xq, CU_TENSOR_MAP_DATA_TYPE_UINT8, 1, Xq, K / 2, M, K / 2, G / 2, TN, psw);
     if (r > 0) {
         ok &= make_map(&maps.X, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, X, K, M, static_cast<uint64_t>(ldx) * 2, 64, TN,
                        CU_TENSOR_MAP_SWIZZLE_128B);
@@ -187,18 +188,15 @@ twq_status twq_dual_linear(const void* X, int ldx, const uint8_t* Xq, const floa
     }
     if (!ok) return TWQ_ERR_CUDA;
 
-    twq::DualParams p;
     p.M = M; p.N = N; p.K = K; p.r = r; p.ng = K / G;
     p.ldy = ldy; p.ydt = static_cast<int>(ydt);
-    p.g_per_split = (p.ng + splits - 1) / splits;
     p.sx = sx;
     p.swT = reinterpret_cast<const float*>(base + lay.off_swT);
     p.Y = Y;
     p.dbgP = dbg_P;
     p.ws_ctr = splits > 1 ? static_cast<unsigned*>(ws) : nullptr;
-    p.ws_part = splits > 1 ? reinterpret_cast<float*>(static_cast<uint8_t*>(ws) + ctr_bytes(M, N)) : nullptr;
-    if (twq::launch_dual_linear(maps, p, TN, G, splits, static_cast<cudaStream_t>(stream)) != cudaSuccess)
-        return TWQ_ERR_CUDA;
+    p.ws_part = splits > 1 ? reinterpret_cast<float*>(static_cast<uint8_t*>(ws) + ctr_bytes(p.plan)) : nullptr;
+    if (twq::launch_fused(maps, p, G, static_cast<cudaStream_t>(stream)) != cudaSuccess) return TWQ_ERR_CUDA;
     g_last_launches = 1;
     return TWQ_OK;
 }
