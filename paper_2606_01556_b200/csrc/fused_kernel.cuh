@@ -1,0 +1,832 @@
+// fused_kernel.cuh -- the fused dual-branch kernel template (steps a3-a7), sm_100a only.
+// Instantiated per (TN, G, debug) in fused_inst_*.cu; planned and dispatched by fused_kernel.cu.
+//
+//   Y[m,n] = sum_g sx[m,g]*sw[n,g]*P[m,g,n]  +  sum_j H[m,j]*L2[j,n],
+//   P[m,g,n] = sum_{k in g} qx[m,k]*qw[n,k] (exact int32),   H = X*L1 (FP32 accumulate)
+//   PAPER.md Eq. 2 (L49-50), Eq. 3 (L62), L177-181 (section 4.3), L193 (groups of G).
+//
+// Orientation: a CTA computes Y^T for 128 output channels (TMEM lanes = n, the MMA M
+// dimension; weights are the A operand) x TN tokens (TMEM columns = m, the MMA N dimension;
+// activations are the B operand).  Decode-shaped calls run N = 16 MMAs.
+//
+// Persistent clusters.  A cluster of `cs` CTAs owns `cs` adjacent n-tiles and walks a list of
+// units (K split, m-tile, n-block) with the m-tile changing slowest, so the stage-1 product
+// H = X*L1 of an m-tile is computed once per cluster, cooperatively: every CTA multiplies
+// 1/cs of the K range, the FP32 partials are reduce-scattered and the FP16 result all-gathered
+// through distributed shared memory.  H never leaves the chip.
+//
+// Warp roles (512 threads):
+//   warp 0      TMA producer: stage-1 tiles (X, L1T), L2T tile, packed INT4 tiles (R4, Xq)
+//   warp 1      MMA issuer (one thread): kind::f16 stage 1 / stage 2, kind::i8 residual
+//   warp 2      TMEM allocator
+//   warps 4-7   operand preparation: BF16->FP16 rewrite of the X tile (kind::f16 needs one
+//               16-bit format for both operands); INT4 -> int8 expansion: each nibble c becomes
+//               the byte 16*c (one shift/and per word, sign for free; sm_100 has no INT4 MMA).
+//               Weight rows go registers -> TMEM (the MMA reads A from TMEM, so expanded
+//               weights never touch shared memory); activation rows go to a swizzled smem tile.
+//   warps 8-15  epilogue: per group, tcgen05.ld the int32 accumulator, fold both scales in
+//               FP32 (two packed f32x2 FMAs per pair), accumulate in registers; add Ylr; store.
+//
+// Accumulator trick: each P buffer is pre-filled with the bit pattern of 1.5*2^23, and the
+// group's MMAs accumulate 256*P onto it (|256*P| < 2^22), so tcgen05.ld returns the float
+// 1.5*2^23 + 256*P directly: no int->float conversion instruction in the hot loop.
+//
+// Three P buffers rotate (MMA -> commit -> epilogue -> refill costs several hundred cycles of
+// latency per hand-off; two buffers cannot cover it).  The low-rank product Ylr = H*L2 of a tile
+// is accumulated (FP32) into the next P buffer at the START of the tile and becomes the initial
+// value of the epilogue's register accumulators, so it needs no TMEM columns of its own.
+// Group scales are staged ahead of use: the preparation warps fetch sx for 8 groups at a time,
+// one block ahead; the epilogue warps fetch sw two groups ahead.
+#pragma once
+#include <cuda_bf16.h>
+#include <cuda_fp16.h>
+
+#include "fused_kernel.h"
+#include "sm100_ptx.cuh"
+
+namespace twq {
+
+namespace {
+
+constexpr int kThreads = 512;
+constexpr int kPrepWarps = 4;           // warps 4..7
+constexpr int kPrepThreads = kPrepWarps * 32;
+constexpr int kEpiWarps = 8;            // warps 8..15
+constexpr int kTileN = 128;             // output channels per CTA (MMA M)
+constexpr int kSxSlots = 16;            // per-group activation-scale slots (two blocks of 8 groups)
+constexpr int kNB = 3;                  // P accumulator buffers in rotation
+constexpr int kMaxNS1 = 4, kMaxNSP = 8, kMaxNSU = 4;
+constexpr int kL1Chunk = 128 * 128;     // 128 rows x 64 fp16 (one 128B-swizzled tile)
+constexpr uint32_t kMagic = 0x4B400000u;  // bits of 1.5 * 2^23
+constexpr int kMaxDynSmem = 232448 - 64;
+
+// barrier slots (uint64 each)
+enum : int {
+    B_FULL1 = 0,
+    B_EMPTY1 = B_FULL1 + kMaxNS1,
+    B_XCONV = B_EMPTY1 + kMaxNS1,
+    B_PFULL = B_XCONV + kMaxNS1,
+    B_PEMPTY = B_PFULL + kMaxNSP,
+    B_UFULL = B_PEMPTY + kMaxNSP,
+    B_UEMPTY = B_UFULL + kMaxNSU,
+    B_TFULL = B_UEMPTY + kMaxNSU,
+    B_TEMPTY = B_TFULL + kNB,
+    B_HFULL = B_TEMPTY + kNB,   // stage-1 MMAs of this CTA complete
+    B_HDRAINED,                 // epilogue read H^T out of TMEM and re-initialised the P buffers
+    B_HREADY,                   // full FP16 H is in this CTA's shared memory
+    B_X1,                       // cluster: every CTA's FP32 partial is in its shared memory
+    B_X2,                       // cluster: every CTA finished reading partials and writing H
+    B_L2FULL,
+    B_L2EMPTY,
+    B_RESID,                    // all residual MMAs of a tile complete
+    B_COUNT
+};
+
+template <int TN, int G>
+struct Cfg {
+    static constexpr int kXChunk = TN * 128;          // X tile: TN rows x 64 bf16
+    static constexpr int kWB = kTileN * (G / 2);      // packed weight rows of one group
+    static constexpr int kXB = TN * (G / 2);          // packed activation rows of one group
+    static constexpr int kUB = TN * G;                // expanded activation tile of one group
+    static constexpr int kColP = 0;                   // P buffer b at b*TN; H^T block rb at rb*TN
+    static constexpr int kColA = (kNB * TN + 31) / 32 * 32;   // expanded weight rows (A operand), 32 cols / stage
+    static constexpr int kTmemCols = kColA + kMaxNSU * 32 <= 256 ? 256 : 512;
+    static constexpr int kCW = TN >= 32 ? TN / 2 : 16;   // token columns per epilogue warp
+    static constexpr int kCPW = kCW / 16;                // 16-column chunks per epilogue warp
+    static_assert(kColA + kMaxNSU * 32 <= 512, "TMEM budget");
+};
+
+__device__ __forceinline__ uint32_t nib_lo16(uint32_t w) { return (w << 4) & 0xF0F0F0F0u; }  // 16*code, even k
+__device__ __forceinline__ uint32_t nib_hi16(uint32_t w) { return w & 0xF0F0F0F0u; }         // 16*code, odd k
+
+// Position of 16-byte chunk `c` of row `row` in a packed tile whose rows are G/2 bytes
+// (TMA SWIZZLE_64B for G = 128, SWIZZLE_32B for G = 64).
+template <int G>
+__device__ __forceinline__ uint32_t packed_chunk_offset(uint32_t row, uint32_t c) {
+    if constexpr (G == 128) return row * 64u + ((c ^ ((row >> 1) & 3u)) << 4);
+    else return row * 32u + ((c ^ ((row >> 2) & 1u)) << 4);
+}
+
+// uses of P buffer b among the first q uses of the rotation
+__device__ __forceinline__ int buf_uses(int q, int b) { return (q + kNB - 1 - b) / kNB; }
+
+#ifdef TWQ_TRACE
+// Debug timeline: CTA 0 records (tag, clock64) per role.  Built only into the trace library.
+__device__ unsigned long long g_twq_trace[4 * 4096];
+#define TWQ_TR(role, n, tag)                                                                      \
+    do {                                                                                          \
+        if (blockIdx.x == 0 && (n) < 4096) g_twq_trace[(role) * 4096 + (n)++] =                   \
+            (static_cast<unsigned long long>(tag) << 48) | (static_cast<unsigned long long>(clock64()) & 0xFFFFFFFFFFFFull); \
+    } while (0)
+#else
+#define TWQ_TR(role, n, tag) do { } while (0)
+#endif
+
+struct Unit {
+    int n0, m0, g_begin, g_end, ctx, ks;
+};
+
+__device__ __forceinline__ Unit decode_unit(const FusedParams& p, int u, int rank) {
+    const FusedPlan& pl = p.plan;
+    Unit t;
+    const int nb = u % pl.n_blocks;
+    t.ctx = u / pl.n_blocks;
+    const int mt = t.ctx % pl.m_tiles;
+    t.ks = t.ctx / pl.m_tiles;
+    t.n0 = (nb * pl.cs + rank) * kTileN;
+    t.m0 = mt * pl.TN;
+    t.g_begin = t.ks * pl.g_per_split;
+    t.g_end = min(p.ng, t.g_begin + pl.g_per_split);
+    return t;
+}
+
+// 64-wide K chunks of stage 1 this CTA multiplies for a unit's context: 1/cs of the split's K range.
+template <int G>
+__device__ __forceinline__ void s1_range(const FusedParams& p, const Unit& t, int rank, int& kc0, int& kc1) {
+    const int b = t.g_begin * (G / 64), e = t.g_end * (G / 64);
+    const int per = (e - b + p.plan.cs - 1) / p.plan.cs;
+    kc0 = min(e, b + rank * per);
+    kc1 = min(e, kc0 + per);
+}
+
+template <int TN, int G, bool kDbg>
+__global__ void __launch_bounds__(kThreads, 1)
+fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CUtensorMap tmXq,
+                         const __grid_constant__ CUtensorMap tmX, const __grid_constant__ CUtensorMap tmL1T,
+                         const __grid_constant__ CUtensorMap tmL2T, const __grid_constant__ FusedParams p) {
+    using C = Cfg<TN, G>;
+    const FusedPlan& pl = p.plan;
+    extern __shared__ uint8_t smem_raw[];
+    // identical offset in every CTA of the cluster (DSMEM addresses are formed from local ones)
+    uint8_t* smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
+    uint8_t* sH = smem + pl.off_H;          // H[m, j] fp16, K-major, 64-wide k-blocks of TN x 128 B
+    uint8_t* sL2T = smem + pl.off_L2T;      // L2T tile: k-blocks of 128 x 128 B
+    uint8_t* sU = smem + pl.off_U;          // expanded activation tiles [nsu][TN x G]
+    uint8_t* sP = smem + pl.off_P;          // packed tiles [nsp][W 128 x G/2 | Xq TN x G/2]
+    uint8_t* sS1 = smem + pl.off_S1;        // stage-1 ring [ns1][X TN x 128 | L1T nrb x 16 KB]
+    float* sHpart = reinterpret_cast<float*>(smem + pl.off_Hpart);   // FP32 partial H[m][r]
+    float* sSx = reinterpret_cast<float*>(smem + pl.off_sx);
+    uint64_t* bars = reinterpret_cast<uint64_t*>(smem + pl.off_bar);
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + B_COUNT);
+    __shared__ int s_last;
+
+    const int warp = threadIdx.x >> 5;
+    const int lane = threadIdx.x & 31;
+    const int r = p.r;
+    const int nrb = (r + 127) >> 7;          // 128-row blocks of L1T / H^T
+    const int nkb = (r + 63) >> 6;           // 64-wide k-blocks of H / L2T
+    const int cs = pl.cs;
+    const int rank = cs > 1 ? static_cast<int>(cluster_ctarank()) : 0;
+    const int cid = cs > 1 ? static_cast<int>(cluster_id_x()) : static_cast<int>(blockIdx.x);
+    const int u_begin = static_cast<int>(static_cast<long long>(cid) * pl.units / pl.nclusters);
+    const int u_end = static_cast<int>(static_cast<long long>(cid + 1) * pl.units / pl.nclusters);
+    const int s1_stage_bytes = C::kXChunk + nrb * kL1Chunk;
+    const int p_stage_bytes = C::kWB + C::kXB;
+
+    if (threadIdx.x == 0) {
+        for (int i = 0; i < kMaxNS1; ++i) {
+            mbar_init(&bars[B_FULL1 + i], 1);
+            mbar_init(&bars[B_EMPTY1 + i], 1);
+            mbar_init(&bars[B_XCONV + i], kPrepWarps);
+        }
+        for (int i = 0; i < kMaxNSP; ++i) { mbar_init(&bars[B_PFULL + i], 1); mbar_init(&bars[B_PEMPTY + i], kPrepWarps); }
+        for (int i = 0; i < kMaxNSU; ++i) { mbar_init(&bars[B_UFULL + i], kPrepWarps); mbar_init(&bars[B_UEMPTY + i], 1); }
+        for (int i = 0; i < kNB; ++i) { mbar_init(&bars[B_TFULL + i], 1); mbar_init(&bars[B_TEMPTY + i], kEpiWarps); }
+        mbar_init(&bars[B_HFULL], 1);
+        mbar_init(&bars[B_HDRAINED], kEpiWarps);
+        mbar_init(&bars[B_HREADY], kEpiWarps);
+        mbar_init(&bars[B_X1], kEpiWarps * cs);
+        mbar_init(&bars[B_X2], kEpiWarps * cs);
+        mbar_init(&bars[B_L2FULL], 1);
+        mbar_init(&bars[B_L2EMPTY], 1);
+        mbar_init(&bars[B_RESID], 1);
+        fence_mbar_init();
+    }
+    if (warp == 0 && lane == 0) {
+        tma_prefetch_desc(&tmW);
+        tma_prefetch_desc(&tmXq);
+        if (r > 0) { tma_prefetch_desc(&tmX); tma_prefetch_desc(&tmL1T); tma_prefetch_desc(&tmL2T); }
+    }
+    if (warp == 2) tmem_alloc<C::kTmemCols>(tmem_slot);
+    tc_fence_before();
+    __syncthreads();
+    if (cs > 1) cluster_sync_all();   // peers' barriers are initialised before any remote arrive
+    tc_fence_after();
+    const uint32_t tmem = *tmem_slot;
+    pdl_launch_dependents();          // the next kernel may start its own prologue / weight prefetch
+
+    if (warp == 0) {
+        // ================================================================ TMA producer
+        if (lane == 0) {
+            int it1 = 0, itp = 0, tile_n = 0, ctx_n = 0, cur_ctx = -1;
+            bool waited = false;
+            for (int u = u_begin; u < u_end; ++u) {
+                const Unit t = decode_unit(p, u, rank);
+                if (r > 0 && t.ctx != cur_ctx) {
+                    cur_ctx = t.ctx;
+                    // the stage-1 ring overlays the residual rings: every residual MMA must be done
+                    if (pl.alias && tile_n > 0) mbar_wait(&bars[B_RESID], (tile_n - 1) & 1, 10);
+                    int kc0, kc1;
+                    s1_range<G>(p, t, rank, kc0, kc1);
+                    if (!waited && kc0 < kc1) { pdl_wait(); waited = true; }   // X comes from the previous kernel
+                    for (int kc = kc0; kc < kc1; ++kc, ++it1) {
+                        const int s = it1 % pl.ns1, ph = (it1 / pl.ns1) & 1;
+                        mbar_wait(&bars[B_EMPTY1 + s], ph ^ 1, 11);
+                        uint8_t* st = sS1 + s * s1_stage_bytes;
+                        mbar_arrive_expect_tx(&bars[B_FULL1 + s], s1_stage_bytes);
+                        tma_load_2d(st, &tmX, &bars[B_FULL1 + s], kc * 64, t.m0);
+                        for (int rb = 0; rb < nrb; ++rb)
+                            tma_load_2d(st + C::kXChunk + rb * kL1Chunk, &tmL1T, &bars[B_FULL1 + s], kc * 64, rb * 128);
+                    }
+                    // overlay: stage-1 MMAs done and the H exchange finished before residual tiles land
+                    if (pl.alias) mbar_wait(&bars[B_HREADY], ctx_n & 1, 12);
+                    ++ctx_n;
+                }
+                if (r > 0) {
+                    mbar_wait(&bars[B_L2EMPTY], (tile_n & 1) ^ 1, 13);
+                    mbar_arrive_expect_tx(&bars[B_L2FULL], nkb * kL1Chunk);
+                    for (int kb = 0; kb < nkb; ++kb)
+                        tma_load_2d(sL2T + kb * kL1Chunk, &tmL2T, &bars[B_L2FULL], kb * 64, t.n0);
+                }
+                for (int g = t.g_begin; g < t.g_end; ++g, ++itp) {
+                    const int s = itp % pl.nsp, ph = (itp / pl.nsp) & 1;
+                    mbar_wait(&bars[B_PEMPTY + s], ph ^ 1, 14);
+                    uint8_t* st = sP + s * p_stage_bytes;
+                    mbar_arrive_expect_tx(&bars[B_PFULL + s], p_stage_bytes);
+                    tma_load_2d(st, &tmW, &bars[B_PFULL + s], g * (G / 2), t.n0);
+                    if (!waited) { pdl_wait(); waited = true; }               // Xq comes from the quantizer
+                    tma_load_2d(st + C::kWB, &tmXq, &bars[B_PFULL + s], g * (G / 2), t.m0);
+                }
+                ++tile_n;
+            }
+        }
+    } else if (warp == 1) {
+        // ================================================================ MMA issuer (one thread)
+        if (lane == 0) {
+            const uint32_t idesc_lr = umma_idesc(1, 0, 0, 128, TN);  // D f32, A f16, B f16
+            const uint32_t idesc_i8 = umma_idesc(2, 1, 1, 128, TN);  // D s32, A s8, B s8
+            int it1 = 0, itp = 0, tile_n = 0, ctx_n = 0, cur_ctx = -1;
+            int q = 0;                    // P buffer uses so far (rotation over kNB buffers)
+            bool h_waited = true;
+#ifdef TWQ_TRACE
+            int trn = 0;
+#endif
+            for (int u = u_begin; u < u_end; ++u) {
+                const Unit t = decode_unit(p, u, rank);
+                if (r > 0 && t.ctx != cur_ctx) {
+                    cur_ctx = t.ctx;
+                    int kc0, kc1;
+                    s1_range<G>(p, t, rank, kc0, kc1);
+                    if (kc0 < kc1) {
+                        // H^T accumulates in the columns of P buffers 0..nrb-1: all their uses must be drained
+                        for (int b = 0; b < nrb; ++b) mbar_wait(&bars[B_TEMPTY + b], buf_uses(q, b) & 1, 20);
+                        tc_fence_after();
+                        for (int kc = kc0; kc < kc1; ++kc, ++it1) {
+                            const int s = it1 % pl.ns1, ph = (it1 / pl.ns1) & 1;
+                            mbar_wait(&bars[B_XCONV + s], ph, 21);
+                            tc_fence_after();
+                            const uint32_t xb = smem_u32(sS1 + s * s1_stage_bytes);
+                            const uint32_t lb = xb + C::kXChunk;
+#pragma unroll
+                            for (int ks = 0; ks < 4; ++ks)
+                                for (int rb = 0; rb < nrb; ++rb)
+                                    umma_f16(tmem + C::kColP + rb * TN, umma_smem_desc<128>(lb + rb * kL1Chunk + ks * 32),
+                                             umma_smem_desc<128>(xb + ks * 32), idesc_lr, (kc != kc0 || ks != 0) ? 1u : 0u);
+                            tc_commit(&bars[B_EMPTY1 + s]);
+                        }
+                        tc_commit(&bars[B_HFULL]);
+                    } else {
+                        mbar_arrive(&bars[B_HFULL]);   // empty K share: the epilogue contributes zeros
+                    }
+                    mbar_wait(&bars[B_HDRAINED], ctx_n & 1, 22);
+                    tc_fence_after();
+                    h_waited = false;
+                }
+                if (r > 0) {
+                    // stage 2 first: Ylr^T = L2T * H^T (FP32) into the next P buffer; the epilogue takes it
+                    // as the initial value of its accumulators
+                    if (!h_waited) { mbar_wait(&bars[B_HREADY], ctx_n & 1, 25); h_waited = true; ++ctx_n; }
+                    mbar_wait(&bars[B_L2FULL], tile_n & 1, 26);
+                    const int b = q % kNB, ub = q / kNB;
+                    mbar_wait(&bars[B_TEMPTY + b], ub & 1, 27);
+                    ++q;
+                    tc_fence_after();
+                    const uint32_t l2b = smem_u32(sL2T), hb = smem_u32(sH);
+                    const int nks = (r + 15) >> 4;
+                    for (int ks = 0; ks < nks; ++ks) {
+                        const int kb = ks >> 2, kk = ks & 3;
+                        umma_f16(tmem + C::kColP + b * TN, umma_smem_desc<128>(l2b + kb * kL1Chunk + kk * 32),
+                                 umma_smem_desc<128>(hb + kb * (TN * 128) + kk * 32), idesc_lr, ks != 0 ? 1u : 0u);
+                    }
+                    tc_commit(&bars[B_L2EMPTY]);
+                    tc_commit(&bars[B_TFULL + b]);
+                }
+                const int ngr = t.g_end - t.g_begin;
+                for (int gi = 0; gi < ngr; ++gi, ++itp) {
+                    const int su = itp % pl.nsu, ph = (itp / pl.nsu) & 1;
+                    const int b = q % kNB, ub = q / kNB;
+                    ++q;
+                    TWQ_TR(1, trn, 1);
+                    mbar_wait(&bars[B_TEMPTY + b], ub & 1, 23);
+                    TWQ_TR(1, trn, 2);
+                    mbar_wait(&bars[B_UFULL + su], ph, 24);
+                    TWQ_TR(1, trn, 3);
+                    tc_fence_after();
+                    const uint32_t ubase = smem_u32(sU + su * C::kUB);
+                    const uint32_t ta = tmem + C::kColA + su * 32;
+#pragma unroll
+                    for (int ks = 0; ks < G / 32; ++ks)   // accumulate onto the pre-filled 1.5*2^23 pattern
+                        umma_i8_ts(tmem + C::kColP + b * TN, ta + ks * 8, umma_smem_desc<G>(ubase + ks * 32), idesc_i8, 1u);
+                    tc_commit(&bars[B_UEMPTY + su]);
+                    tc_commit(&bars[B_TFULL + b]);
+                }
+                tc_commit(&bars[B_RESID]);
+                ++tile_n;
+            }
+        }
+    }
+    else if (warp >= 4 && warp < 8) {
+        // ================================================================ operand preparation warps
+        const int u_tid = threadIdx.x - 128;
+        const int q = warp & 3;                       // TMEM lane quarter this warp may write
+        const uint32_t arow = q * 32 + lane;          // weight row (output channel) of this thread
+        const uint32_t tlane = tmem + (static_cast<uint32_t>(q * 32) << 16);
+        constexpr int kCPR = (G / 2) / 16;            // 16-byte packed chunks per row
+        constexpr int kBTasks = TN * kCPR;
+        pdl_wait();                                   // reads sx (quantizer output)
+        int it1 = 0, itp = 0, cur_ctx = -1;
+        float sxv[8];                                 // scales of the next block of 8 groups for token row u_tid
+        {
+#pragma unroll
+            for (int j = 0; j < 8; ++j) sxv[j] = 0.0f;
+            if (u_begin < u_end) {
+                const Unit t0 = decode_unit(p, u_begin, rank);
+                const int m = t0.m0 + u_tid;
+                if (u_tid < TN && m < p.M) {
+                    const float* src = p.sx + static_cast<size_t>(m) * p.ng + t0.g_begin;
+                    const int left = t0.g_end - t0.g_begin;
+#pragma unroll
+                    for (int j = 0; j < 8; ++j) sxv[j] = j < left ? __ldg(src + j) : 0.0f;
+                }
+            }
+        }
+        for (int u = u_begin; u < u_end; ++u) {
+            const Unit t = decode_unit(p, u, rank);
+            if (r > 0 && t.ctx != cur_ctx) {
+                cur_ctx = t.ctx;
+                // kind::f16 needs A and B in ONE 16-bit format and L1 is FP16: rewrite the BF16 X tile in
+                // place as FP16 (exact for 2^-14 <= |x| <= 65504, saturating above).  Elementwise, so the
+                // swizzled layout TMA wrote is untouched.
+                int kc0, kc1;
+                s1_range<G>(p, t, rank, kc0, kc1);
+                for (int kc = kc0; kc < kc1; ++kc, ++it1) {
+                    const int s = it1 % pl.ns1, ph = (it1 / pl.ns1) & 1;
+                    mbar_wait(&bars[B_FULL1 + s], ph, 30);
+                    uint4* xt = reinterpret_cast<uint4*>(sS1 + s * s1_stage_bytes);
+                    for (int i = u_tid; i < C::kXChunk / 16; i += kPrepThreads) {
+                        uint4 w = xt[i];
+                        uint32_t* wp = reinterpret_cast<uint32_t*>(&w);
+#pragma unroll
+                        for (int e = 0; e < 4; ++e) {
+                            float lo = __uint_as_float(wp[e] << 16), hi = __uint_as_float(wp[e] & 0xFFFF0000u);
+                            lo = fminf(fmaxf(lo, -65504.0f), 65504.0f);
+                            hi = fminf(fmaxf(hi, -65504.0f), 65504.0f);
+                            const __half2 h2 = __floats2half2_rn(lo, hi);
+                            wp[e] = *reinterpret_cast<const uint32_t*>(&h2);
+                        }
+                        xt[i] = w;
+                    }
+                    fence_proxy_async_smem();
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(&bars[B_XCONV + s]);
+                }
+            }
+            const int ngr = t.g_end - t.g_begin;
+            for (int gi = 0; gi < ngr; ++gi, ++itp) {
+                const int sp = itp % pl.nsp, pph = (itp / pl.nsp) & 1;
+                const int su = itp % pl.nsu, uph = (itp / pl.nsu) & 1;
+                if ((gi & 7) == 0) {
+                    // activation scales of groups gi..gi+7 (fetched one block ahead), pre-multiplied by 2^-8
+                    // (the MMA operands are 16*code); then start the fetch of the next block
+                    if (u_tid < TN) {
+#pragma unroll
+                        for (int j = 0; j < 8; ++j) sSx[((itp + j) & (kSxSlots - 1)) * TN + u_tid] = sxv[j] * 0x1p-8f;
+                    }
+                    int nu = u, ngi = gi + 8;
+                    if (ngi >= ngr) { nu = u + 1; ngi = 0; }
+                    if (nu < u_end) {
+                        const Unit tn = decode_unit(p, nu, rank);
+                        const int m = tn.m0 + u_tid;
+                        const bool ok = u_tid < TN && m < p.M;
+                        const float* src = p.sx + static_cast<size_t>(ok ? m : 0) * p.ng + tn.g_begin + ngi;
+                        const int left = tn.g_end - tn.g_begin - ngi;
+#pragma unroll
+                        for (int j = 0; j < 8; ++j) sxv[j] = (ok && j < left) ? __ldg(src + j) : 0.0f;
+                    }
+                }
+                mbar_wait(&bars[B_PFULL + sp], pph, 31);
+                const uint8_t* pw = sP + sp * p_stage_bytes;
+                const uint8_t* px = pw + C::kWB;
+                // weight row -> registers
+                uint4 wv[kCPR];
+#pragma unroll
+                for (int c = 0; c < kCPR; ++c) wv[c] = *reinterpret_cast<const uint4*>(pw + packed_chunk_offset<G>(arow, c));
+                mbar_wait(&bars[B_UEMPTY + su], uph ^ 1, 32);
+                tc_fence_after();
+                // expanded weight row -> TMEM (A operand): 16 int8 words per packed chunk pair
+#pragma unroll
+                for (int c = 0; c < kCPR; c += 2) {
+                    uint32_t o[16];
+                    const uint32_t wi[8] = {wv[c].x, wv[c].y, wv[c].z, wv[c].w, wv[c + 1].x, wv[c + 1].y, wv[c + 1].z, wv[c + 1].w};
+#pragma unroll
+                    for (int i = 0; i < 8; ++i) { o[2 * i] = nib_lo16(wi[i]); o[2 * i + 1] = nib_hi16(wi[i]); }
+                    tmem_st16(tlane + C::kColA + su * 32 + c * 8, o);
+                }
+                // activation rows -> swizzled K-major smem tile (B operand)
+                uint8_t* ub = sU + su * C::kUB;
+                for (int i = u_tid; i < kBTasks; i += kPrepThreads) {
+                    const uint32_t row = i / kCPR, j = i % kCPR;
+                    const uint4 w = *reinterpret_cast<const uint4*>(px + packed_chunk_offset<G>(row, j));
+                    const uint4 o0 = make_uint4(nib_lo16(w.x), nib_hi16(w.x), nib_lo16(w.y), nib_hi16(w.y));
+                    const uint4 o1 = make_uint4(nib_lo16(w.z), nib_hi16(w.z), nib_lo16(w.w), nib_hi16(w.w));
+                    *reinterpret_cast<uint4*>(ub + swizzled_chunk_offset<G>(row, 2 * j)) = o0;
+                    *reinterpret_cast<uint4*>(ub + swizzled_chunk_offset<G>(row, 2 * j + 1)) = o1;
+                }
+                tmem_st_wait();
+                tc_fence_before();
+                fence_proxy_async_smem();  // generic-proxy writes -> visible to the tensor core (async proxy)
+                __syncwarp();
+                if (lane == 0) { mbar_arrive(&bars[B_UFULL + su]); mbar_arrive(&bars[B_PEMPTY + sp]); }
+            }
+        }
+    }
+    else if (warp >= 8) {
+        // ================================================================ epilogue warps
+        const int qd = warp & 3;             // TMEM lane quarter this warp may access
+        const int h = (warp - 8) >> 2;       // which half of the token columns
+        const bool active = TN >= 32 || h == 0;
+        const int col0 = h * C::kCW;
+        const int row = qd * 32 + lane;
+        const int et = threadIdx.x - 256;    // 0..255
+        const uint32_t tlane = tmem + (static_cast<uint32_t>(qd * 32) << 16);
+        constexpr int kNA = C::kCPW * 8;     // accumulator pairs per thread
+        uint64_t acc[kNA];
+#ifdef TWQ_TRACE
+        int trn = 0;
+        const bool trw = warp == 8 && lane == 0;
+#endif
+
+        // pre-fill this warp's slices of the P buffers with the 1.5*2^23 pattern
+        if (active) {
+#pragma unroll
+            for (int b = 0; b < kNB; ++b)
+#pragma unroll
+                for (int i = 0; i < C::kCPW; ++i) tmem_fill16(tlane + C::kColP + b * TN + col0 + i * 16, kMagic);
+            tmem_st_wait();
+        }
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) {
+#pragma unroll
+            for (int b = 0; b < kNB; ++b) mbar_arrive(&bars[B_TEMPTY + b]);
+        }
+        pdl_wait();                          // Y / workspace writes must follow the previous kernel
+
+        int itp = 0, ctx_n = 0, cur_ctx = -1;
+        int q = 0;                           // P buffer uses so far (same rotation as the MMA issuer)
+        for (int u = u_begin; u < u_end; ++u) {
+            const Unit t = decode_unit(p, u, rank);
+            const int n = t.n0 + row;
+            const bool n_ok = n < p.N;
+            const float* swp = p.swT + (n_ok ? n : 0);
+            // weight scales two groups ahead of use
+            float sw0 = n_ok ? __ldg(swp + static_cast<size_t>(t.g_begin) * p.N) : 0.0f;
+            float sw1 = (n_ok && t.g_begin + 1 < t.g_end) ? __ldg(swp + static_cast<size_t>(t.g_begin + 1) * p.N) : 0.0f;
+            if (r > 0 && t.ctx != cur_ctx) {
+                cur_ctx = t.ctx;
+                int kc0, kc1;
+                s1_range<G>(p, t, rank, kc0, kc1);
+                const bool has_s1 = kc0 < kc1;
+                mbar_wait(&bars[B_HFULL], ctx_n & 1, 40);
+                tc_fence_after();
+                if (active) {
+                    for (int rb = 0; rb < nrb; ++rb) {
+                        const int j = rb * 128 + row;
+#pragma unroll
+                        for (int i = 0; i < C::kCPW; ++i) {
+                            uint32_t v[16];
+                            if (has_s1) {
+                                tmem_ld16(tlane + C::kColP + rb * TN + col0 + i * 16, v);
+                                tmem_ld_wait();
+                            } else {
+#pragma unroll
+                                for (int c = 0; c < 16; ++c) v[c] = 0u;
+                            }
+                            if (j < r) {
+                                if (cs == 1) {
+                                    uint8_t* hk = sH + (j >> 6) * (TN * 128) + (j & 7) * 2;
+                                    const uint32_t chunk = (j & 63) >> 3;
+#pragma unroll
+                                    for (int c = 0; c < 16; ++c) {
+                                        const uint32_t m = col0 + i * 16 + c;
+                                        const float hv = fminf(fmaxf(__uint_as_float(v[c]), -65504.0f), 65504.0f);
+                                        *reinterpret_cast<__half*>(hk + swizzled_chunk_offset<128>(m, chunk)) = __float2half_rn(hv);
+                                    }
+                                } else {
+#pragma unroll
+                                    for (int c = 0; c < 16; ++c) sHpart[(col0 + i * 16 + c) * r + j] = __uint_as_float(v[c]);
+                                }
+                            }
+                        }
+                    }
+                    // the H^T columns are P buffers 0..nrb-1: restore their pre-fill
+                    for (int b = 0; b < nrb; ++b)
+#pragma unroll
+                        for (int i = 0; i < C::kCPW; ++i) tmem_fill16(tlane + C::kColP + b * TN + col0 + i * 16, kMagic);
+                    tmem_st_wait();
+                }
+                tc_fence_before();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&bars[B_HDRAINED]);
+                if (cs > 1) {
+                    // ---- reduce-scatter the FP32 partials, all-gather the FP16 result (DSMEM)
+                    if (lane < cs) mbar_arrive_remote(mapa_u32(smem_u32(&bars[B_X1]), lane));
+                    mbar_wait_cluster(&bars[B_X1], ctx_n & 1, 41);
+                    const int jcs = r >> 3;                     // 8-wide column chunks of H
+                    const int total = TN * jcs;
+                    for (int i = rank + cs * et; i < total; i += cs * 256) {
+                        const int m = i / jcs, jc = i - m * jcs;
+                        const uint32_t src = smem_u32(sHpart + m * r + jc * 8);
+                        float s[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+                        for (int pr = 0; pr < cs; ++pr) {       // fixed order: every CTA sees identical H
+                            const uint32_t a = mapa_u32(src, pr);
+                            const float4 x0 = ld_dsmem_f4(a), x1 = ld_dsmem_f4(a + 16);
+                            s[0] += x0.x; s[1] += x0.y; s[2] += x0.z; s[3] += x0.w;
+                            s[4] += x1.x; s[5] += x1.y; s[6] += x1.z; s[7] += x1.w;
+                        }
+                        uint32_t hw[4];
+#pragma unroll
+                        for (int e = 0; e < 4; ++e) {
+                            const float lo = fminf(fmaxf(s[2 * e], -65504.0f), 65504.0f);
+                            const float hi = fminf(fmaxf(s[2 * e + 1], -65504.0f), 65504.0f);
+                            const __half2 h2 = __floats2half2_rn(lo, hi);
+                            hw[e] = *reinterpret_cast<const uint32_t*>(&h2);
+                        }
+                        const uint32_t dst = smem_u32(sH + (jc >> 3) * (TN * 128) + swizzled_chunk_offset<128>(m, jc & 7));
+                        for (int pr = 0; pr < cs; ++pr) st_dsmem_u4(mapa_u32(dst, pr), make_uint4(hw[0], hw[1], hw[2], hw[3]));
+                    }
+                    fence_proxy_async_all();
+                    __syncwarp();
+                    if (lane < cs) mbar_arrive_remote(mapa_u32(smem_u32(&bars[B_X2]), lane));
+                    mbar_wait_cluster(&bars[B_X2], ctx_n & 1, 42);
+                }
+                fence_proxy_async_smem();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&bars[B_HREADY]);
+                ++ctx_n;
+            }
+
+            if (r > 0) {
+                // Ylr of this tile (FP32) is the initial value of the accumulators
+                const int b = q % kNB, ub = q / kNB;
+                ++q;
+                mbar_wait(&bars[B_TFULL + b], ub & 1, 44);
+                tc_fence_after();
+                if (active) {
+#pragma unroll
+                    for (int i = 0; i < C::kCPW; ++i) {
+                        uint32_t v[16];
+                        tmem_ld16(tlane + C::kColP + b * TN + col0 + i * 16, v);
+                        tmem_ld_wait();
+                        tmem_fill16(tlane + C::kColP + b * TN + col0 + i * 16, kMagic);
+#pragma unroll
+                        for (int c2 = 0; c2 < 8; ++c2)
+                            acc[i * 8 + c2] = (static_cast<uint64_t>(v[2 * c2 + 1]) << 32) | v[2 * c2];
+                    }
+                    tmem_st_wait();
+                }
+                tc_fence_before();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&bars[B_TEMPTY + b]);
+            } else {
+#pragma unroll
+                for (int i = 0; i < kNA; ++i) acc[i] = 0ull;
+            }
+
+            for (int g = t.g_begin; g < t.g_end; ++g, ++itp) {
+                const int b = q % kNB, ub = q / kNB;
+                ++q;
+                const float swn = sw0;
+                sw0 = sw1;
+                sw1 = (n_ok && g + 2 < t.g_end) ? __ldg(swp + static_cast<size_t>(g + 2) * p.N) : 0.0f;
+                const float cm = __fmul_rn(12582912.0f, swn);   // exact: sw has an 11-bit significand
+                const uint64_t sw2 = pack_f2(swn, swn), ncm2 = pack_f2(-cm, -cm);
+#ifdef TWQ_TRACE
+                if (trw) TWQ_TR(3, trn, 1);
+#endif
+                mbar_wait(&bars[B_TFULL + b], ub & 1, 43);
+#ifdef TWQ_TRACE
+                if (trw) TWQ_TR(3, trn, 2);
+#endif
+                tc_fence_after();
+                if (active) {
+                    const float* cs_ = sSx + (itp & (kSxSlots - 1)) * TN + col0;
+                    constexpr int kBatch = C::kCPW >= 2 ? 2 : 1;
+#pragma unroll
+                    for (int i0 = 0; i0 < C::kCPW; i0 += kBatch) {
+                        uint32_t v[kBatch][16];
+#pragma unroll
+                        for (int bi = 0; bi < kBatch; ++bi) tmem_ld16(tlane + C::kColP + b * TN + col0 + (i0 + bi) * 16, v[bi]);
+                        tmem_ld_wait();
+#pragma unroll
+                        for (int bi = 0; bi < kBatch; ++bi) tmem_fill16(tlane + C::kColP + b * TN + col0 + (i0 + bi) * 16, kMagic);
+                        if (i0 + kBatch >= C::kCPW) {    // last batch: hand the buffer back before the arithmetic
+                            tmem_st_wait();
+                            tc_fence_before();
+                            __syncwarp();
+                            if (lane == 0) mbar_arrive(&bars[B_TEMPTY + b]);
+#ifdef TWQ_TRACE
+                            if (trw) TWQ_TR(3, trn, 3);
+#endif
+                        }
+#pragma unroll
+                        for (int bi = 0; bi < kBatch; ++bi) {
+#pragma unroll
+                            for (int c4 = 0; c4 < 4; ++c4) {
+                                const float4 s4 = *reinterpret_cast<const float4*>(cs_ + (i0 + bi) * 16 + c4 * 4);
+                                // v = bits(1.5*2^23 + 256*P): one FMA gives RN(256*P * sw), the next accumulates * sx*2^-8
+                                const uint64_t f01 = (static_cast<uint64_t>(v[bi][c4 * 4 + 1]) << 32) | v[bi][c4 * 4];
+                                const uint64_t f23 = (static_cast<uint64_t>(v[bi][c4 * 4 + 3]) << 32) | v[bi][c4 * 4 + 2];
+                                const uint64_t t01 = fma2(f01, sw2, ncm2), t23 = fma2(f23, sw2, ncm2);
+                                const int a = (i0 + bi) * 8 + c4 * 2;
+                                acc[a] = fma2(t01, pack_f2(s4.x, s4.y), acc[a]);
+                                acc[a + 1] = fma2(t23, pack_f2(s4.z, s4.w), acc[a + 1]);
+                            }
+                            if (kDbg) {
+                                if (p.dbgP != nullptr && n_ok) {
+#pragma unroll
+                                    for (int c = 0; c < 16; ++c) {
+                                        const int m = t.m0 + col0 + (i0 + bi) * 16 + c;
+                                        if (m < p.M)
+                                            p.dbgP[(static_cast<size_t>(m) * p.ng + g) * p.N + n] =
+                                                static_cast<int32_t>(v[bi][c] - kMagic) >> 8;
+                                    }
+                                }
+                            }
+                        }
+                    }
+                } else {
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(&bars[B_TEMPTY + b]);
+                }
+#ifdef TWQ_TRACE
+                if (trw) TWQ_TR(3, trn, 4);
+#endif
+            }
+
+            if (active && n_ok) {
+#pragma unroll
+                for (int i = 0; i < kNA; ++i) {
+                    float y2[2];
+                    unpack_f2(acc[i], y2[0], y2[1]);
+#pragma unroll
+                    for (int e = 0; e < 2; ++e) {
+                        const int m = t.m0 + col0 + i * 2 + e;
+                        if (m < p.M) {
+                            const float y = y2[e];
+                            if (pl.splits == 1) {
+                                const size_t o = static_cast<size_t>(m) * p.ldy + n;
+                                if (p.ydt == 0) static_cast<__nv_bfloat16*>(p.Y)[o] = __float2bfloat16_rn(y);
+                                else if (p.ydt == 1) static_cast<__half*>(p.Y)[o] = __float2half_rn(y);
+                                else static_cast<float*>(p.Y)[o] = y;
+                            } else {   // split-K: park the FP32 partial of this split in the workspace [ks][M][N]
+                                p.ws_part[(static_cast<size_t>(t.ks) * p.M + m) * p.N + n] = y;
+                            }
+                        }
+                    }
+                }
+            }
+        }
+    }
+
+    // ---------------------------------------------------------------- teardown
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 2) {
+        tc_fence_after();
+        tmem_dealloc<C::kTmemCols>(tmem);
+    }
+
+    if (pl.splits > 1) {
+        // Deterministic split-K fix-up (one unit per cluster when splits > 1): the last CTA of this
+        // (n-tile, m-tile) to finish sums the partials in split order and writes Y; the tile counter is
+        // left at zero for the next call.
+        const Unit t = decode_unit(p, u_begin, rank);
+        __threadfence();
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            unsigned* ctr = p.ws_ctr + (t.m0 / TN) * pl.n_tiles + t.n0 / kTileN;
+            const unsigned prev = atomicAdd(ctr, 1u);
+            s_last = prev == static_cast<unsigned>(pl.splits - 1);
+            if (s_last) *ctr = 0;
+        }
+        __syncthreads();
+        if (s_last) {
+            __threadfence();
+            const int rows = min(TN, p.M - t.m0);
+            for (int idx = threadIdx.x; idx < rows * kTileN; idx += kThreads) {
+                const int mm = t.m0 + idx / kTileN, nn = t.n0 + idx % kTileN;
+                if (nn >= p.N) continue;
+                float y = 0.0f;
+                for (int z = 0; z < pl.splits; ++z)
+                    y += __ldcg(p.ws_part + (static_cast<size_t>(z) * p.M + mm) * p.N + nn);
+                const size_t o = static_cast<size_t>(mm) * p.ldy + nn;
+                if (p.ydt == 0) static_cast<__nv_bfloat16*>(p.Y)[o] = __float2bfloat16_rn(y);
+                else if (p.ydt == 1) static_cast<__half*>(p.Y)[o] = __float2half_rn(y);
+                else static_cast<float*>(p.Y)[o] = y;
+            }
+        }
+    }
+    if (cs > 1) cluster_sync_all();   // no CTA exits while a peer may still touch its shared memory
+}
+
+
+}  // namespace
+
+template <int TN, int G, bool kDbg>
+cudaError_t launch_fused_inst(const FusedMaps& maps, const FusedParams& p, cudaStream_t stream) {
+    auto kern = fused_dual_linear_kernel<TN, G, kDbg>;
+    static int attr_smem = 0;
+    if (attr_smem < p.plan.smem_bytes) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxDynSmem);
+        if (e != cudaSuccess) return e;
+        attr_smem = kMaxDynSmem;
+    }
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(static_cast<unsigned>(p.plan.nclusters * p.plan.cs));
+    cfg.blockDim = dim3(kThreads);
+    cfg.dynamicSmemBytes = static_cast<size_t>(p.plan.smem_bytes);
+    cfg.stream = stream;
+    cudaLaunchAttribute attrs[2];
+    int na = 0;
+    if (p.plan.cs > 1) {
+        attrs[na].id = cudaLaunchAttributeClusterDimension;
+        attrs[na].val.clusterDim.x = static_cast<unsigned>(p.plan.cs);
+        attrs[na].val.clusterDim.y = 1;
+        attrs[na].val.clusterDim.z = 1;
+        ++na;
+    }
+    attrs[na].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attrs[na].val.programmaticStreamSerializationAllowed = 1;
+    ++na;
+    cfg.attrs = attrs;
+    cfg.numAttrs = static_cast<unsigned>(na);
+    return cudaLaunchKernelEx(&cfg, kern, maps.W, maps.Xq, maps.X, maps.L1T, maps.L2T, p);
+}
+
+// How many clusters of `cs` CTAs (one CTA per SM) the device can hold at once; 0 on failure.
+template <int TN, int G, bool kDbg>
+int max_active_clusters_inst(int cs, int num_sms) {
+    auto kern = fused_dual_linear_kernel<TN, G, kDbg>;
+    if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxDynSmem) != cudaSuccess) {
+        cudaGetLastError();
+        return 0;
+    }
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(static_cast<unsigned>(num_sms / cs * cs));
+    cfg.blockDim = dim3(kThreads);
+    cfg.dynamicSmemBytes = kMaxDynSmem;
+    cudaLaunchAttribute attr;
+    attr.id = cudaLaunchAttributeClusterDimension;
+    attr.val.clusterDim.x = static_cast<unsigned>(cs);
+    attr.val.clusterDim.y = 1;
+    attr.val.clusterDim.z = 1;
+    cfg.attrs = &attr;
+    cfg.numAttrs = 1;
+    int n = 0;
+    if (cudaOccupancyMaxActiveClusters(&n, kern, &cfg) != cudaSuccess) {
+        cudaGetLastError();
+        return 0;
+    }
+    return n;
+}
+
+
+// Explicit instantiations live in fused_inst_tn*.cu (one file per token-tile size, compiled in parallel).
+#define TWQ_EXTERN_INST(tn)                                                                                         \
+    extern template cudaError_t launch_fused_inst<tn, 128, false>(const FusedMaps&, const FusedParams&, cudaStream_t); \
+    extern template cudaError_t launch_fused_inst<tn, 128, true>(const FusedMaps&, const FusedParams&, cudaStream_t);  \
+    extern template cudaError_t launch_fused_inst<tn, 64, false>(const FusedMaps&, const FusedParams&, cudaStream_t);  \
+    extern template cudaError_t launch_fused_inst<tn, 64, true>(const FusedMaps&, const FusedParams&, cudaStream_t);
+TWQ_EXTERN_INST(16)
+TWQ_EXTERN_INST(32)
+TWQ_EXTERN_INST(64)
+TWQ_EXTERN_INST(128)
+extern template int max_active_clusters_inst<128, 128, false>(int, int);
+#define TWQ_DEFINE_INST(tn)                                                                                  \
+    template cudaError_t launch_fused_inst<tn, 128, false>(const FusedMaps&, const FusedParams&, cudaStream_t); \
+    template cudaError_t launch_fused_inst<tn, 128, true>(const FusedMaps&, const FusedParams&, cudaStream_t);  \
+    template cudaError_t launch_fused_inst<tn, 64, false>(const FusedMaps&, const FusedParams&, cudaStream_t);  \
+    template cudaError_t launch_fused_inst<tn, 64, true>(const FusedMaps&, const FusedParams&, cudaStream_t);
+
+}  // namespace twq
