@@ -72,7 +72,7 @@ static bool make_plan_tn(int TN, int M, int N, int K, int r, int G, int num_sms,
     const int ub = TN * G, pb = kTileN * (G / 2) + TN * (G / 2);
     const int s1b = TN * 128 + nrb * kL1Chunk;
     const int hpart = pl.cs > 1 ? round_up(TN * r * 4, 1024) : 0;
-    const int fixed = kSxSlots * TN * 4 + B_COUNT * 8 + 64;
+    const int fixed = kSxSlots * TN * 4 + B_COUNT * 8 + 256;
     const int budget = kMaxDynSmem - 1024 - fixed;             // dynamic limit minus alignment slack
     pl.nsu = kMaxNSU;
     pl.nsp = TN <= 32 ? kMaxNSP : 4;
@@ -106,7 +106,7 @@ static bool make_plan_tn(int TN, int M, int N, int K, int r, int G, int num_sms,
     }
     o = round_up(o, 16);
     pl.off_sx = o; o += kSxSlots * TN * 4;
-    pl.off_bar = o; o += B_COUNT * 8 + 64;
+    pl.off_bar = o; o += B_COUNT * 8 + 256;
     pl.smem_bytes = o + 1024;
     pl.tmem_cols = Cfg<16, 128>::kTmemCols;   // informational
     *out = pl;

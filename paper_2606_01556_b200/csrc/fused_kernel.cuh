@@ -15,17 +15,19 @@
 // 1/cs of the K range, the FP32 partials are reduce-scattered and the FP16 result all-gathered
 // through distributed shared memory.  H never leaves the chip.
 //
-// Warp roles (512 threads):
+// Warp roles (640 threads; registers re-balanced per role with setmaxnreg):
 //   warp 0      TMA producer: stage-1 tiles (X, L1T), L2T tile, packed INT4 tiles (R4, Xq)
 //   warp 1      MMA issuer (one thread): kind::f16 stage 1 / stage 2, kind::i8 residual
 //   warp 2      TMEM allocator
-//   warps 4-7   operand preparation: BF16->FP16 rewrite of the X tile (kind::f16 needs one
-//               16-bit format for both operands); INT4 -> int8 expansion: each nibble c becomes
+//   warps 4-11  operand preparation.  All: BF16->FP16 rewrite of the X tile (kind::f16 needs one
+//               16-bit format for both operands).  INT4 -> int8 expansion: each nibble c becomes
 //               the byte 16*c (one shift/and per word, sign for free; sm_100 has no INT4 MMA).
-//               Weight rows go registers -> TMEM (the MMA reads A from TMEM, so expanded
-//               weights never touch shared memory); activation rows go to a swizzled smem tile.
-//   warps 8-15  epilogue: per group, tcgen05.ld the int32 accumulator, fold both scales in
+//               Warps 4-7: weight rows, registers -> TMEM (the MMA reads A from TMEM, so expanded
+//               weights never touch shared memory).  Warps 8-11: activation rows -> swizzled smem
+//               tile (B operand), and the activation group scales.
+//   warps 12-19 epilogue: per group, tcgen05.ld the int32 accumulator, fold both scales in
 //               FP32 (two packed f32x2 FMAs per pair), accumulate in registers; add Ylr; store.
+// The single-thread roles keep stage indices and phases in counters (no division in any loop).
 //
 // Accumulator trick: each P buffer is pre-filled with the bit pattern of 1.5*2^23, and the
 // group's MMAs accumulate 256*P onto it (|256*P| < 2^22), so tcgen05.ld returns the float
@@ -48,10 +50,14 @@ namespace twq {
 
 namespace {
 
-constexpr int kThreads = 512;
-constexpr int kPrepWarps = 4;           // warps 4..7
+constexpr int kThreads = 640;
+constexpr int kPrepWarps = 8;           // warps 4..7 expand weight rows, warps 8..11 expand activation rows
 constexpr int kPrepThreads = kPrepWarps * 32;
-constexpr int kEpiWarps = 8;            // warps 8..15
+constexpr int kEpiWarp0 = 12;           // first epilogue warp (a multiple of 4: TMEM lane quarter = warp % 4)
+constexpr int kEpiWarps = 8;            // warps 12..19
+// register budgets after setmaxnreg: the pool is what the CTA was launched with (640 x 96 = 61440);
+// 128*40 + 256*64 + 256*152 = 60416
+constexpr int kRegsCtl = 40, kRegsPrep = 64, kRegsEpi = 152;
 constexpr int kTileN = 128;             // output channels per CTA (MMA M)
 constexpr int kSxSlots = 16;            // per-group activation-scale slots (two blocks of 8 groups)
 constexpr int kNB = 3;                  // P accumulator buffers in rotation
@@ -207,19 +213,30 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
         tma_prefetch_desc(&tmXq);
         if (r > 0) { tma_prefetch_desc(&tmX); tma_prefetch_desc(&tmL1T); tma_prefetch_desc(&tmL2T); }
     }
+    if (threadIdx.x < 32) tmem_slot[8 + threadIdx.x] = kMagic;   // read back by the epilogue warps (see kfill)
     if (warp == 2) tmem_alloc<C::kTmemCols>(tmem_slot);
     tc_fence_before();
     __syncthreads();
     if (cs > 1) cluster_sync_all();   // peers' barriers are initialised before any remote arrive
     tc_fence_after();
     const uint32_t tmem = *tmem_slot;
+    const uint32_t bar0 = smem_u32(bars);   // shared-window address of barrier slot 0 (slot i at bar0 + 8*i)
+#define TWQ_BAR(i) (bar0 + 8u * static_cast<uint32_t>(i))
     pdl_launch_dependents();          // the next kernel may start its own prologue / weight prefetch
 
+    if (warp < 4) {
+        reg_dec<kRegsCtl>();
     if (warp == 0) {
         // ================================================================ TMA producer
         if (lane == 0) {
-            int it1 = 0, itp = 0, tile_n = 0, ctx_n = 0, cur_ctx = -1;
+            int tile_n = 0, ctx_n = 0, cur_ctx = -1;
+            int s1 = 0, ph1 = 0;          // stage-1 ring position / phase
+            int sp = 0, php = 0;          // packed ring position / phase
             bool waited = false;
+            const uint32_t sP_a = smem_u32(sP);
+#ifdef TWQ_TRACE
+            int trn = 0;
+#endif
             for (int u = u_begin; u < u_end; ++u) {
                 const Unit t = decode_unit(p, u, rank);
                 if (r > 0 && t.ctx != cur_ctx) {
@@ -229,14 +246,14 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
                     int kc0, kc1;
                     s1_range<G>(p, t, rank, kc0, kc1);
                     if (!waited && kc0 < kc1) { pdl_wait(); waited = true; }   // X comes from the previous kernel
-                    for (int kc = kc0; kc < kc1; ++kc, ++it1) {
-                        const int s = it1 % pl.ns1, ph = (it1 / pl.ns1) & 1;
-                        mbar_wait(&bars[B_EMPTY1 + s], ph ^ 1, 11);
-                        uint8_t* st = sS1 + s * s1_stage_bytes;
-                        mbar_arrive_expect_tx(&bars[B_FULL1 + s], s1_stage_bytes);
-                        tma_load_2d(st, &tmX, &bars[B_FULL1 + s], kc * 64, t.m0);
+                    for (int kc = kc0; kc < kc1; ++kc) {
+                        mbar_wait(&bars[B_EMPTY1 + s1], ph1 ^ 1, 11);
+                        uint8_t* st = sS1 + s1 * s1_stage_bytes;
+                        mbar_arrive_expect_tx(&bars[B_FULL1 + s1], s1_stage_bytes);
+                        tma_load_2d(st, &tmX, &bars[B_FULL1 + s1], kc * 64, t.m0);
                         for (int rb = 0; rb < nrb; ++rb)
-                            tma_load_2d(st + C::kXChunk + rb * kL1Chunk, &tmL1T, &bars[B_FULL1 + s], kc * 64, rb * 128);
+                            tma_load_2d(st + C::kXChunk + rb * kL1Chunk, &tmL1T, &bars[B_FULL1 + s1], kc * 64, rb * 128);
+                        if (++s1 == pl.ns1) { s1 = 0; ph1 ^= 1; }
                     }
                     // overlay: stage-1 MMAs done and the H exchange finished before residual tiles land
                     if (pl.alias) mbar_wait(&bars[B_HREADY], ctx_n & 1, 12);
@@ -248,14 +265,17 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
                     for (int kb = 0; kb < nkb; ++kb)
                         tma_load_2d(sL2T + kb * kL1Chunk, &tmL2T, &bars[B_L2FULL], kb * 64, t.n0);
                 }
-                for (int g = t.g_begin; g < t.g_end; ++g, ++itp) {
-                    const int s = itp % pl.nsp, ph = (itp / pl.nsp) & 1;
-                    mbar_wait(&bars[B_PEMPTY + s], ph ^ 1, 14);
-                    uint8_t* st = sP + s * p_stage_bytes;
-                    mbar_arrive_expect_tx(&bars[B_PFULL + s], p_stage_bytes);
-                    tma_load_2d(st, &tmW, &bars[B_PFULL + s], g * (G / 2), t.n0);
+                int c0 = t.g_begin * (G / 2);
+                for (int g = t.g_begin; g < t.g_end; ++g, c0 += G / 2) {
+                    TWQ_TR(0, trn, 1);
+                    mbar_wait_a(TWQ_BAR(B_PEMPTY + sp), php ^ 1);
+                    TWQ_TR(0, trn, 2);
+                    const uint32_t st = sP_a + sp * p_stage_bytes;
+                    mbar_arrive_expect_tx_a(TWQ_BAR(B_PFULL + sp), p_stage_bytes);
+                    tma_load_2d_a(st, &tmW, TWQ_BAR(B_PFULL + sp), c0, t.n0);
                     if (!waited) { pdl_wait(); waited = true; }               // Xq comes from the quantizer
-                    tma_load_2d(st + C::kWB, &tmXq, &bars[B_PFULL + s], g * (G / 2), t.m0);
+                    tma_load_2d_a(st + C::kWB, &tmXq, TWQ_BAR(B_PFULL + sp), c0, t.m0);
+                    if (++sp == pl.nsp) { sp = 0; php ^= 1; }
                 }
                 ++tile_n;
             }
@@ -265,9 +285,12 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
         if (lane == 0) {
             const uint32_t idesc_lr = umma_idesc(1, 0, 0, 128, TN);  // D f32, A f16, B f16
             const uint32_t idesc_i8 = umma_idesc(2, 1, 1, 128, TN);  // D s32, A s8, B s8
-            int it1 = 0, itp = 0, tile_n = 0, ctx_n = 0, cur_ctx = -1;
-            int q = 0;                    // P buffer uses so far (rotation over kNB buffers)
+            int tile_n = 0, ctx_n = 0, cur_ctx = -1;
+            int s1 = 0, ph1 = 0;          // stage-1 ring position / phase
+            int su = 0, phu = 0;          // expanded-operand ring position / phase
+            int b = 0, pb = 0;            // next P buffer of the rotation / parity of its use count
             bool h_waited = true;
+            const uint64_t udesc0 = umma_smem_desc<G>(smem_u32(sU));   // + stage * kUB/16 + k-step * 2
 #ifdef TWQ_TRACE
             int trn = 0;
 #endif
@@ -279,20 +302,20 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
                     s1_range<G>(p, t, rank, kc0, kc1);
                     if (kc0 < kc1) {
                         // H^T accumulates in the columns of P buffers 0..nrb-1: all their uses must be drained
-                        for (int b = 0; b < nrb; ++b) mbar_wait(&bars[B_TEMPTY + b], buf_uses(q, b) & 1, 20);
+                        for (int bb = 0; bb < nrb; ++bb) mbar_wait(&bars[B_TEMPTY + bb], bb < b ? (pb ^ 1) : pb, 20);
                         tc_fence_after();
-                        for (int kc = kc0; kc < kc1; ++kc, ++it1) {
-                            const int s = it1 % pl.ns1, ph = (it1 / pl.ns1) & 1;
-                            mbar_wait(&bars[B_XCONV + s], ph, 21);
+                        for (int kc = kc0; kc < kc1; ++kc) {
+                            mbar_wait(&bars[B_XCONV + s1], ph1, 21);
                             tc_fence_after();
-                            const uint32_t xb = smem_u32(sS1 + s * s1_stage_bytes);
+                            const uint32_t xb = smem_u32(sS1 + s1 * s1_stage_bytes);
                             const uint32_t lb = xb + C::kXChunk;
 #pragma unroll
                             for (int ks = 0; ks < 4; ++ks)
                                 for (int rb = 0; rb < nrb; ++rb)
                                     umma_f16(tmem + C::kColP + rb * TN, umma_smem_desc<128>(lb + rb * kL1Chunk + ks * 32),
                                              umma_smem_desc<128>(xb + ks * 32), idesc_lr, (kc != kc0 || ks != 0) ? 1u : 0u);
-                            tc_commit(&bars[B_EMPTY1 + s]);
+                            tc_commit(&bars[B_EMPTY1 + s1]);
+                            if (++s1 == pl.ns1) { s1 = 0; ph1 ^= 1; }
                         }
                         tc_commit(&bars[B_HFULL]);
                     } else {
@@ -307,9 +330,7 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
                     // as the initial value of its accumulators
                     if (!h_waited) { mbar_wait(&bars[B_HREADY], ctx_n & 1, 25); h_waited = true; ++ctx_n; }
                     mbar_wait(&bars[B_L2FULL], tile_n & 1, 26);
-                    const int b = q % kNB, ub = q / kNB;
-                    mbar_wait(&bars[B_TEMPTY + b], ub & 1, 27);
-                    ++q;
+                    mbar_wait(&bars[B_TEMPTY + b], pb, 27);
                     tc_fence_after();
                     const uint32_t l2b = smem_u32(sL2T), hb = smem_u32(sH);
                     const int nks = (r + 15) >> 4;
@@ -320,46 +341,75 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
                     }
                     tc_commit(&bars[B_L2EMPTY]);
                     tc_commit(&bars[B_TFULL + b]);
+                    if (++b == kNB) { b = 0; pb ^= 1; }
                 }
                 const int ngr = t.g_end - t.g_begin;
-                for (int gi = 0; gi < ngr; ++gi, ++itp) {
-                    const int su = itp % pl.nsu, ph = (itp / pl.nsu) & 1;
-                    const int b = q % kNB, ub = q / kNB;
-                    ++q;
+                for (int gi = 0; gi < ngr; ++gi) {
                     TWQ_TR(1, trn, 1);
-                    mbar_wait(&bars[B_TEMPTY + b], ub & 1, 23);
+                    mbar_wait_a(TWQ_BAR(B_TEMPTY + b), pb);
                     TWQ_TR(1, trn, 2);
-                    mbar_wait(&bars[B_UFULL + su], ph, 24);
+                    mbar_wait_a(TWQ_BAR(B_UFULL + su), phu);
                     TWQ_TR(1, trn, 3);
                     tc_fence_after();
-                    const uint32_t ubase = smem_u32(sU + su * C::kUB);
+                    const uint64_t ud = udesc0 + static_cast<uint64_t>(su * (C::kUB >> 4));
                     const uint32_t ta = tmem + C::kColA + su * 32;
+                    const uint32_t td = tmem + C::kColP + b * TN;
 #pragma unroll
                     for (int ks = 0; ks < G / 32; ++ks)   // accumulate onto the pre-filled 1.5*2^23 pattern
-                        umma_i8_ts(tmem + C::kColP + b * TN, ta + ks * 8, umma_smem_desc<G>(ubase + ks * 32), idesc_i8, 1u);
-                    tc_commit(&bars[B_UEMPTY + su]);
-                    tc_commit(&bars[B_TFULL + b]);
+                        umma_i8_ts(td, ta + ks * 8, ud + static_cast<uint64_t>(ks * 2), idesc_i8, 1u);
+                    tc_commit_a(TWQ_BAR(B_UEMPTY + su));
+                    tc_commit_a(TWQ_BAR(B_TFULL + b));
+                    TWQ_TR(1, trn, 4);
+                    if (++su == pl.nsu) { su = 0; phu ^= 1; }
+                    if (++b == kNB) { b = 0; pb ^= 1; }
                 }
                 tc_commit(&bars[B_RESID]);
                 ++tile_n;
             }
         }
     }
-    else if (warp >= 4 && warp < 8) {
+    }  // control warps
+    else if (warp < kEpiWarp0) {
         // ================================================================ operand preparation warps
-        const int u_tid = threadIdx.x - 128;
-        const int q = warp & 3;                       // TMEM lane quarter this warp may write
-        const uint32_t arow = q * 32 + lane;          // weight row (output channel) of this thread
-        const uint32_t tlane = tmem + (static_cast<uint32_t>(q * 32) << 16);
+        reg_dec<kRegsPrep>();
+        const bool w_role = warp < 8;                 // warps 4-7: weight rows -> TMEM; warps 8-11: activation rows -> smem
+        const int c_tid = threadIdx.x - 128;          // 0..255, stage-1 conversion index
+        const int u_tid = (threadIdx.x - 128) & 127;  // index inside the role
+        const int qd = warp & 3;                      // TMEM lane quarter a weight warp may write
+        const uint32_t arow = qd * 32 + lane;         // weight row (output channel) of this thread
+        const uint32_t tlane = tmem + (static_cast<uint32_t>(qd * 32) << 16);
         constexpr int kCPR = (G / 2) / 16;            // 16-byte packed chunks per row
-        constexpr int kBTasks = TN * kCPR;
+        // activation rows: kTPR threads share a row, each expands kXC of its kCPR chunks
+        constexpr int kTPR = (128 / TN) < kCPR ? (128 / TN) : kCPR;
+        constexpr int kXC = kCPR / kTPR;
+        const uint32_t xrow = u_tid % TN;
+        const uint32_t xpart = u_tid / TN;
+        const bool x_on = xpart < kTPR;
+        uint32_t in_off[kCPR];                        // packed chunk offsets (weight role: all; activation role: first kXC)
+        uint32_t out_off[2 * kXC];
+        if (w_role) {
+#pragma unroll
+            for (int c = 0; c < kCPR; ++c) in_off[c] = packed_chunk_offset<G>(arow, c);
+        } else {
+#pragma unroll
+            for (int j = 0; j < kXC; ++j) {
+                const uint32_t ch = xpart + j * kTPR;
+                in_off[j] = C::kWB + packed_chunk_offset<G>(xrow, ch);
+                out_off[2 * j] = swizzled_chunk_offset<G>(xrow, 2 * ch);
+                out_off[2 * j + 1] = swizzled_chunk_offset<G>(xrow, 2 * ch + 1);
+            }
+        }
         pdl_wait();                                   // reads sx (quantizer output)
-        int it1 = 0, itp = 0, cur_ctx = -1;
+        int cur_ctx = -1, itp = 0;
+        int s1 = 0, ph1 = 0, sp = 0, php = 0, su = 0, phu = 0;
+#ifdef TWQ_TRACE
+        int trn = (warp == 8 && lane == 0) ? 0 : 4096;
+#endif
         float sxv[8];                                 // scales of the next block of 8 groups for token row u_tid
         {
 #pragma unroll
             for (int j = 0; j < 8; ++j) sxv[j] = 0.0f;
-            if (u_begin < u_end) {
+            if (!w_role && u_begin < u_end) {
                 const Unit t0 = decode_unit(p, u_begin, rank);
                 const int m = t0.m0 + u_tid;
                 if (u_tid < TN && m < p.M) {
@@ -379,11 +429,10 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
                 // swizzled layout TMA wrote is untouched.
                 int kc0, kc1;
                 s1_range<G>(p, t, rank, kc0, kc1);
-                for (int kc = kc0; kc < kc1; ++kc, ++it1) {
-                    const int s = it1 % pl.ns1, ph = (it1 / pl.ns1) & 1;
-                    mbar_wait(&bars[B_FULL1 + s], ph, 30);
-                    uint4* xt = reinterpret_cast<uint4*>(sS1 + s * s1_stage_bytes);
-                    for (int i = u_tid; i < C::kXChunk / 16; i += kPrepThreads) {
+                for (int kc = kc0; kc < kc1; ++kc) {
+                    mbar_wait(&bars[B_FULL1 + s1], ph1, 30);
+                    uint4* xt = reinterpret_cast<uint4*>(sS1 + s1 * s1_stage_bytes);
+                    for (int i = c_tid; i < C::kXChunk / 16; i += kPrepThreads) {
                         uint4 w = xt[i];
                         uint32_t* wp = reinterpret_cast<uint32_t*>(&w);
 #pragma unroll
@@ -398,14 +447,13 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
                     }
                     fence_proxy_async_smem();
                     __syncwarp();
-                    if (lane == 0) mbar_arrive(&bars[B_XCONV + s]);
+                    if (lane == 0) mbar_arrive(&bars[B_XCONV + s1]);
+                    if (++s1 == pl.ns1) { s1 = 0; ph1 ^= 1; }
                 }
             }
             const int ngr = t.g_end - t.g_begin;
             for (int gi = 0; gi < ngr; ++gi, ++itp) {
-                const int sp = itp % pl.nsp, pph = (itp / pl.nsp) & 1;
-                const int su = itp % pl.nsu, uph = (itp / pl.nsu) & 1;
-                if ((gi & 7) == 0) {
+                if (!w_role && (gi & 7) == 0) {
                     // activation scales of groups gi..gi+7 (fetched one block ahead), pre-multiplied by 2^-8
                     // (the MMA operands are 16*code); then start the fetch of the next block
                     if (u_tid < TN) {
@@ -424,56 +472,82 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
                         for (int j = 0; j < 8; ++j) sxv[j] = (ok && j < left) ? __ldg(src + j) : 0.0f;
                     }
                 }
-                mbar_wait(&bars[B_PFULL + sp], pph, 31);
+                TWQ_TR(2, trn, 1);
+                mbar_wait_a(TWQ_BAR(B_PFULL + sp), php);
+                TWQ_TR(2, trn, 2);
                 const uint8_t* pw = sP + sp * p_stage_bytes;
-                const uint8_t* px = pw + C::kWB;
-                // weight row -> registers
-                uint4 wv[kCPR];
+                if (w_role) {
+                    // weight row -> registers -> 16*code bytes -> TMEM (A operand): 16 int8 words per packed chunk pair
+                    uint4 wv[kCPR];
 #pragma unroll
-                for (int c = 0; c < kCPR; ++c) wv[c] = *reinterpret_cast<const uint4*>(pw + packed_chunk_offset<G>(arow, c));
-                mbar_wait(&bars[B_UEMPTY + su], uph ^ 1, 32);
-                tc_fence_after();
-                // expanded weight row -> TMEM (A operand): 16 int8 words per packed chunk pair
+                    for (int c = 0; c < kCPR; ++c) wv[c] = *reinterpret_cast<const uint4*>(pw + in_off[c]);
+                    mbar_wait_a(TWQ_BAR(B_UEMPTY + su), phu ^ 1);
+                    tc_fence_after();
 #pragma unroll
-                for (int c = 0; c < kCPR; c += 2) {
-                    uint32_t o[16];
-                    const uint32_t wi[8] = {wv[c].x, wv[c].y, wv[c].z, wv[c].w, wv[c + 1].x, wv[c + 1].y, wv[c + 1].z, wv[c + 1].w};
+                    for (int c = 0; c < kCPR; c += 2) {
+                        uint32_t o[16];
+                        const uint32_t wi[8] = {wv[c].x, wv[c].y, wv[c].z, wv[c].w, wv[c + 1].x, wv[c + 1].y, wv[c + 1].z, wv[c + 1].w};
 #pragma unroll
-                    for (int i = 0; i < 8; ++i) { o[2 * i] = nib_lo16(wi[i]); o[2 * i + 1] = nib_hi16(wi[i]); }
-                    tmem_st16(tlane + C::kColA + su * 32 + c * 8, o);
+                        for (int i = 0; i < 8; ++i) { o[2 * i] = nib_lo16(wi[i]); o[2 * i + 1] = nib_hi16(wi[i]); }
+                        tmem_st16(tlane + C::kColA + su * 32 + c * 8, o);
+                    }
+                    tmem_st_wait();
+                    tc_fence_before();
+                } else {
+                    // activation rows -> swizzled K-major smem tile (B operand)
+                    uint4 xv[kXC];
+                    if (x_on) {
+#pragma unroll
+                        for (int j = 0; j < kXC; ++j) xv[j] = *reinterpret_cast<const uint4*>(pw + in_off[j]);
+                    }
+                    mbar_wait_a(TWQ_BAR(B_UEMPTY + su), phu ^ 1);
+                    TWQ_TR(2, trn, 3);
+                    if (x_on) {
+                        uint8_t* ub = sU + su * C::kUB;
+#pragma unroll
+                        for (int j = 0; j < kXC; ++j) {
+                            const uint4 w = xv[j];
+                            *reinterpret_cast<uint4*>(ub + out_off[2 * j]) =
+                                make_uint4(nib_lo16(w.x), nib_hi16(w.x), nib_lo16(w.y), nib_hi16(w.y));
+                            *reinterpret_cast<uint4*>(ub + out_off[2 * j + 1]) =
+                                make_uint4(nib_lo16(w.z), nib_hi16(w.z), nib_lo16(w.w), nib_hi16(w.w));
+                        }
+                    }
+                    fence_proxy_async_smem();  // generic-proxy writes -> visible to the tensor core (async proxy)
                 }
-                // activation rows -> swizzled K-major smem tile (B operand)
-                uint8_t* ub = sU + su * C::kUB;
-                for (int i = u_tid; i < kBTasks; i += kPrepThreads) {
-                    const uint32_t row = i / kCPR, j = i % kCPR;
-                    const uint4 w = *reinterpret_cast<const uint4*>(px + packed_chunk_offset<G>(row, j));
-                    const uint4 o0 = make_uint4(nib_lo16(w.x), nib_hi16(w.x), nib_lo16(w.y), nib_hi16(w.y));
-                    const uint4 o1 = make_uint4(nib_lo16(w.z), nib_hi16(w.z), nib_lo16(w.w), nib_hi16(w.w));
-                    *reinterpret_cast<uint4*>(ub + swizzled_chunk_offset<G>(row, 2 * j)) = o0;
-                    *reinterpret_cast<uint4*>(ub + swizzled_chunk_offset<G>(row, 2 * j + 1)) = o1;
-                }
-                tmem_st_wait();
-                tc_fence_before();
-                fence_proxy_async_smem();  // generic-proxy writes -> visible to the tensor core (async proxy)
                 __syncwarp();
-                if (lane == 0) { mbar_arrive(&bars[B_UFULL + su]); mbar_arrive(&bars[B_PEMPTY + sp]); }
+                if (lane == 0) { mbar_arrive_a(TWQ_BAR(B_UFULL + su)); mbar_arrive_a(TWQ_BAR(B_PEMPTY + sp)); }
+                TWQ_TR(2, trn, 4);
+                if (++sp == pl.nsp) { sp = 0; php ^= 1; }
+                if (++su == pl.nsu) { su = 0; phu ^= 1; }
             }
         }
     }
-    else if (warp >= 8) {
+    else {
         // ================================================================ epilogue warps
+        reg_inc<kRegsEpi>();
         const int qd = warp & 3;             // TMEM lane quarter this warp may access
-        const int h = (warp - 8) >> 2;       // which half of the token columns
+        const int h = (warp - kEpiWarp0) >> 2;   // which half of the token columns
         const bool active = TN >= 32 || h == 0;
         const int col0 = h * C::kCW;
         const int row = qd * 32 + lane;
-        const int et = threadIdx.x - 256;    // 0..255
+        const int et = threadIdx.x - kEpiWarp0 * 32;    // 0..255
         const uint32_t tlane = tmem + (static_cast<uint32_t>(qd * 32) << 16);
         constexpr int kNA = C::kCPW * 8;     // accumulator pairs per thread
         uint64_t acc[kNA];
+        // the 1.5*2^23 pattern in 16 registers that stay allocated (a tcgen05.st source is a register vector;
+        // opaque to the compiler so that it is not re-materialised per store)
+        uint32_t kfill[16];
+        {
+            // one word per lane, so that the values are not warp-uniform to the compiler (uniform registers
+            // would be copied into a fresh vector before every store)
+            const volatile uint32_t* mg = reinterpret_cast<const volatile uint32_t*>(tmem_slot + 8) + lane;
+#pragma unroll
+            for (int i = 0; i < 16; ++i) kfill[i] = *mg;
+        }
 #ifdef TWQ_TRACE
         int trn = 0;
-        const bool trw = warp == 8 && lane == 0;
+        const bool trw = warp == kEpiWarp0 && lane == 0;
 #endif
 
         // pre-fill this warp's slices of the P buffers with the 1.5*2^23 pattern
@@ -481,7 +555,7 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
 #pragma unroll
             for (int b = 0; b < kNB; ++b)
 #pragma unroll
-                for (int i = 0; i < C::kCPW; ++i) tmem_fill16(tlane + C::kColP + b * TN + col0 + i * 16, kMagic);
+                for (int i = 0; i < C::kCPW; ++i) tmem_st16(tlane + C::kColP + b * TN + col0 + i * 16, kfill);
             tmem_st_wait();
         }
         tc_fence_before();
@@ -493,7 +567,7 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
         pdl_wait();                          // Y / workspace writes must follow the previous kernel
 
         int itp = 0, ctx_n = 0, cur_ctx = -1;
-        int q = 0;                           // P buffer uses so far (same rotation as the MMA issuer)
+        int b = 0, pb = 0;                   // next P buffer / parity of its use count (same rotation as the MMA issuer)
         for (int u = u_begin; u < u_end; ++u) {
             const Unit t = decode_unit(p, u, rank);
             const int n = t.n0 + row;
@@ -540,9 +614,9 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
                         }
                     }
                     // the H^T columns are P buffers 0..nrb-1: restore their pre-fill
-                    for (int b = 0; b < nrb; ++b)
+                    for (int bb = 0; bb < nrb; ++bb)
 #pragma unroll
-                        for (int i = 0; i < C::kCPW; ++i) tmem_fill16(tlane + C::kColP + b * TN + col0 + i * 16, kMagic);
+                        for (int i = 0; i < C::kCPW; ++i) tmem_st16(tlane + C::kColP + bb * TN + col0 + i * 16, kfill);
                     tmem_st_wait();
                 }
                 tc_fence_before();
@@ -588,9 +662,7 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
 
             if (r > 0) {
                 // Ylr of this tile (FP32) is the initial value of the accumulators
-                const int b = q % kNB, ub = q / kNB;
-                ++q;
-                mbar_wait(&bars[B_TFULL + b], ub & 1, 44);
+                mbar_wait(&bars[B_TFULL + b], pb, 44);
                 tc_fence_after();
                 if (active) {
 #pragma unroll
@@ -598,7 +670,7 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
                         uint32_t v[16];
                         tmem_ld16(tlane + C::kColP + b * TN + col0 + i * 16, v);
                         tmem_ld_wait();
-                        tmem_fill16(tlane + C::kColP + b * TN + col0 + i * 16, kMagic);
+                        tmem_st16(tlane + C::kColP + b * TN + col0 + i * 16, kfill);
 #pragma unroll
                         for (int c2 = 0; c2 < 8; ++c2)
                             acc[i * 8 + c2] = (static_cast<uint64_t>(v[2 * c2 + 1]) << 32) | v[2 * c2];
@@ -608,14 +680,13 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
                 tc_fence_before();
                 __syncwarp();
                 if (lane == 0) mbar_arrive(&bars[B_TEMPTY + b]);
+                if (++b == kNB) { b = 0; pb ^= 1; }
             } else {
 #pragma unroll
                 for (int i = 0; i < kNA; ++i) acc[i] = 0ull;
             }
 
             for (int g = t.g_begin; g < t.g_end; ++g, ++itp) {
-                const int b = q % kNB, ub = q / kNB;
-                ++q;
                 const float swn = sw0;
                 sw0 = sw1;
                 sw1 = (n_ok && g + 2 < t.g_end) ? __ldg(swp + static_cast<size_t>(g + 2) * p.N) : 0.0f;
@@ -624,27 +695,28 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
 #ifdef TWQ_TRACE
                 if (trw) TWQ_TR(3, trn, 1);
 #endif
-                mbar_wait(&bars[B_TFULL + b], ub & 1, 43);
+                mbar_wait_a(TWQ_BAR(B_TFULL + b), pb);
 #ifdef TWQ_TRACE
                 if (trw) TWQ_TR(3, trn, 2);
 #endif
                 tc_fence_after();
                 if (active) {
                     const float* cs_ = sSx + (itp & (kSxSlots - 1)) * TN + col0;
-                    constexpr int kBatch = C::kCPW >= 2 ? 2 : 1;
+                    const uint32_t tcol = tlane + C::kColP + b * TN + col0;
+                    constexpr int kBatch = C::kCPW == 2 ? 2 : 1;   // registers: 64 accumulators + 16 fill at TN = 128
 #pragma unroll
                     for (int i0 = 0; i0 < C::kCPW; i0 += kBatch) {
                         uint32_t v[kBatch][16];
 #pragma unroll
-                        for (int bi = 0; bi < kBatch; ++bi) tmem_ld16(tlane + C::kColP + b * TN + col0 + (i0 + bi) * 16, v[bi]);
+                        for (int bi = 0; bi < kBatch; ++bi) tmem_ld16(tcol + (i0 + bi) * 16, v[bi]);
                         tmem_ld_wait();
 #pragma unroll
-                        for (int bi = 0; bi < kBatch; ++bi) tmem_fill16(tlane + C::kColP + b * TN + col0 + (i0 + bi) * 16, kMagic);
+                        for (int bi = 0; bi < kBatch; ++bi) tmem_st16(tcol + (i0 + bi) * 16, kfill);
                         if (i0 + kBatch >= C::kCPW) {    // last batch: hand the buffer back before the arithmetic
                             tmem_st_wait();
                             tc_fence_before();
                             __syncwarp();
-                            if (lane == 0) mbar_arrive(&bars[B_TEMPTY + b]);
+                            if (lane == 0) mbar_arrive_a(TWQ_BAR(B_TEMPTY + b));
 #ifdef TWQ_TRACE
                             if (trw) TWQ_TR(3, trn, 3);
 #endif
@@ -677,11 +749,12 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
                     }
                 } else {
                     __syncwarp();
-                    if (lane == 0) mbar_arrive(&bars[B_TEMPTY + b]);
+                    if (lane == 0) mbar_arrive_a(TWQ_BAR(B_TEMPTY + b));
                 }
 #ifdef TWQ_TRACE
                 if (trw) TWQ_TR(3, trn, 4);
 #endif
+                if (++b == kNB) { b = 0; pb ^= 1; }
             }
 
             if (active && n_ok) {

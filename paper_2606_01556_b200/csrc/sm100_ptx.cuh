@@ -48,17 +48,42 @@ __device__ __forceinline__ bool mbar_try_wait(uint64_t* bar, uint32_t parity) {
         : "memory");
     return ok != 0;
 }
-// Bounded wait: a protocol bug becomes a trap (reported as a launch failure) instead of
-// a hung GPU.  The bound is ~4 s of wall clock, far above any legitimate wait.
+// Bounded wait: a protocol bug becomes a trap (reported as a launch failure) instead of a hung
+// GPU.  try_wait itself suspends the thread for a hardware-defined time slice, so the bound of
+// 2^26 polls is far above any legitimate wait.  Kept to a handful of instructions: single-thread
+// roles (TMA producer, MMA issuer) execute one of these per pipeline hand-off.
 __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity, int tag = 0) {
-    if (mbar_try_wait(bar, parity)) return;
-    long long t0 = clock64();
+    (void)tag;
+    uint32_t spins = 0;
     while (!mbar_try_wait(bar, parity)) {
-        if (clock64() - t0 > 8000000000LL) {
-            printf("twq: mbarrier timeout tag=%d block=(%d,%d,%d) thread=%d parity=%u\n", tag, blockIdx.x,
-                   blockIdx.y, blockIdx.z, threadIdx.x, parity);
-            __trap();
-        }
+        if (++spins > (1u << 26)) __trap();
+    }
+}
+
+
+// ---- the same operations on shared-window addresses (uint32), for hot loops: the address is formed
+// once per role instead of being re-derived from a generic pointer at every call site
+__device__ __forceinline__ void mbar_arrive_a(uint32_t bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx_a(uint32_t bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ bool mbar_try_wait_a(uint32_t bar, uint32_t parity) {
+    uint32_t ok;
+    asm volatile(
+        "{\n\t.reg .pred P;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 P, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, P;\n\t}\n"
+        : "=r"(ok)
+        : "r"(bar), "r"(parity)
+        : "memory");
+    return ok != 0;
+}
+__device__ __forceinline__ void mbar_wait_a(uint32_t bar, uint32_t parity) {
+    uint32_t spins = 0;
+    while (!mbar_try_wait_a(bar, parity)) {
+        if (++spins > (1u << 26)) __trap();
     }
 }
 
@@ -127,6 +152,15 @@ __device__ __forceinline__ void tmem_ld16(uint32_t taddr, uint32_t (&v)[16]) {
         : "r"(taddr)
         : "memory");
 }
+__device__ __forceinline__ void tc_commit_a(uint32_t bar) {
+    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void tma_load_2d_a(uint32_t smem_dst, const CUtensorMap* m, uint32_t bar, int c0, int c1) {
+    asm volatile(
+        "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];"
+        ::"r"(smem_dst), "l"(reinterpret_cast<uint64_t>(m)), "r"(bar), "r"(c0), "r"(c1)
+        : "memory");
+}
 __device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 
 // 32 lanes x 16 columns store (registers -> TMEM), thread i writes lane (base_lane+i).
@@ -144,6 +178,11 @@ __device__ __forceinline__ void tmem_fill16(uint32_t taddr, uint32_t c) {
         ::"r"(taddr), "r"(c)
         : "memory");
 }
+// setmaxnreg: warpgroup-wide register reallocation (all 4 warps of an aligned group execute it)
+template <int kRegs>
+__device__ __forceinline__ void reg_dec() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kRegs)); }
+template <int kRegs>
+__device__ __forceinline__ void reg_inc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(kRegs)); }
 __device__ __forceinline__ void tmem_st_wait() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
 
 // ------------------------------------------------------------------ clusters / DSMEM / PDL
@@ -187,14 +226,10 @@ __device__ __forceinline__ bool mbar_try_wait_cluster(uint64_t* bar, uint32_t pa
     return ok != 0;
 }
 __device__ __forceinline__ void mbar_wait_cluster(uint64_t* bar, uint32_t parity, int tag = 0) {
-    if (mbar_try_wait_cluster(bar, parity)) return;
-    long long t0 = clock64();
+    (void)tag;
+    uint32_t spins = 0;
     while (!mbar_try_wait_cluster(bar, parity)) {
-        if (clock64() - t0 > 8000000000LL) {
-            printf("twq: cluster mbarrier timeout tag=%d block=(%d,%d,%d) thread=%d parity=%u\n", tag, blockIdx.x,
-                   blockIdx.y, blockIdx.z, threadIdx.x, parity);
-            __trap();
-        }
+        if (++spins > (1u << 26)) __trap();
     }
 }
 __device__ __forceinline__ float4 ld_dsmem_f4(uint32_t cluster_addr) {
