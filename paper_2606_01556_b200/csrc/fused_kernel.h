@@ -40,6 +40,28 @@ struct FusedMaps {
     CUtensorMap W, Xq, X, L1T, L2T;
 };
 
+
+// Decode-shaped calls (M <= 16): parameters and plan of decode_kernel.cu (host-computed).
+struct DecodeParams {
+    int M, N, K, r, ng;
+    int ldx, ldy, ydt;       // ydt: 0 bf16, 1 fp16, 2 fp32
+    int n_tiles;             // N / 16
+    int cs, grid;            // CTAs per cluster, CTAs in the grid (a multiple of cs)
+    int T, P;                // 16-channel tiles per CTA, K-parts per tile
+    int off_res, off_hpart, off_h, off_ylr, off_sx, smem_bytes;
+    const uint8_t* R4;       // [N][K/2]
+    const float* swT;        // [ng][N]
+    const void* L1T;         // [r][K] f16
+    const void* L2T;         // [N][r] f16
+    const void* X;           // [M][ldx] bf16
+    const uint8_t* Xq;       // [M][K/2]
+    const float* sx;         // [M][ng]
+    void* Y;
+    int32_t* dbgP;
+};
+bool decode_make_plan(int M, int N, int K, int r, int G, int num_sms, DecodeParams* out);
+cudaError_t launch_decode(const DecodeParams& p, int G, cudaStream_t stream);
+
 // Fills `plan` for a shape; returns false if the shape cannot be planned (never for valid ABI shapes).
 bool fused_make_plan(int M, int N, int K, int r, int G, int num_sms, FusedPlan* plan);
 cudaError_t launch_fused(const FusedMaps& maps, const FusedParams& p, int G, cudaStream_t stream);

@@ -20,6 +20,9 @@ template <int kG, bool kHasT>
 __global__ void __launch_bounds__(256) quantize_act_kernel(const uint16_t* __restrict__ X, int M, int K, int ldx,
                                                            const float* __restrict__ tinv,
                                                            uint8_t* __restrict__ Xq, float* __restrict__ sx) {
+    // programmatic dependent launch: the next kernel (twq_dual_linear) may start its prologue and weight
+    // prefetch now; it waits (griddepcontrol.wait) for this grid to finish before it reads Xq / sx
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     constexpr int kLanesPerGroup = kG / 8;
     const int chunks_per_row = K >> 3;  // 8-element chunks
     const long long total = static_cast<long long>(M) * chunks_per_row;

@@ -139,6 +139,8 @@ twq_status twq_quantize_act(const void* X, int M, int K, int ldx, const float* t
 
 size_t twq_workspace_bytes(int M, int N, int K, int r, int G) {
     if (!shape_ok(M, N, K, r, G)) return 0;
+    twq::DecodeParams dp;
+    if (twq::decode_make_plan(M, N, K, r, G, num_sms(), &dp)) return 0;   // decode-shaped calls need no scratch
     twq::FusedPlan pl;
     if (!twq::fused_make_plan(M, N, K, r, G, num_sms(), &pl)) return 0;
     if (pl.splits <= 1) return 0;
@@ -163,13 +165,28 @@ twq_status twq_dual_linear(const void* X, int ldx, const uint8_t* Xq, const floa
     if (need > 0 && (reinterpret_cast<uintptr_t>(ws) & 255u)) return TWQ_ERR_INVALID_ARG;
     if (!device_is_sm100()) return TWQ_ERR_UNSUPPORTED;
 
+    const twq::PackedLayout lay = twq::packed_layout(N, K, r, G);
+    const uint8_t* base = static_cast<const uint8_t*>(packed);
+
+    // decode-shaped calls (M <= 16): the register-resident kernel of decode_kernel.cu
+    twq::DecodeParams dp;
+    if (twq::decode_make_plan(M, N, K, r, G, num_sms(), &dp)) {
+        dp.ldx = ldx; dp.ldy = ldy; dp.ydt = static_cast<int>(ydt);
+        dp.R4 = base + lay.off_r4;
+        dp.swT = reinterpret_cast<const float*>(base + lay.off_swT);
+        dp.L1T = base + lay.off_l1t;
+        dp.L2T = base + lay.off_l2t;
+        dp.X = X; dp.Xq = Xq; dp.sx = sx; dp.Y = Y; dp.dbgP = dbg_P;
+        if (twq::launch_decode(dp, G, static_cast<cudaStream_t>(stream)) != cudaSuccess) return TWQ_ERR_CUDA;
+        g_last_launches = 1;
+        return TWQ_OK;
+    }
+
     twq::FusedParams p;
     memset(&p, 0, sizeof(p));
     if (!twq::fused_make_plan(M, N, K, r, G, num_sms(), &p.plan)) return TWQ_ERR_UNSUPPORTED;
     const int TN = p.plan.TN;
     const int splits = p.plan.splits;
-    const twq::PackedLayout lay = twq::packed_layout(N, K, r, G);
-    const uint8_t* base = static_cast<const uint8_t*>(packed);
 
     twq::FusedMaps maps;
     memset(&maps, 0, sizeof(maps));

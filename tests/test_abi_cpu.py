@@ -50,8 +50,10 @@ def test_packed_bytes_accounts_for_every_section(lib):
 def test_workspace_rule(lib):
     import paper_2606_01556_b200 as twq
     assert twq.workspace_bytes(2048, 14336, 4096, 128, 128) == 0      # prefill: tiles fill the GPU, no split
-    w = twq.workspace_bytes(1, 4096, 4096, 128, 128)                   # decode: split-K partials + counters
-    assert w > 0 and (w - 256) % (1 * 4096 * 4) == 0
+    assert twq.workspace_bytes(1, 4096, 4096, 128, 128) == 0           # decode kernel (M <= 16): no scratch
+    assert twq.workspace_bytes(16, 4096, 4096, 128, 128) == 0
+    w = twq.workspace_bytes(32, 4096, 4096, 128, 128)                  # few tiles: split-K partials + counters
+    assert w > 0 and (w - 256) % (32 * 4096 * 4) == 0
     assert twq.workspace_bytes(0, 4096, 4096, 128, 128) == 0           # invalid shape
 
 
@@ -74,7 +76,7 @@ def test_argument_validation_happens_before_cuda(lib):
     assert lib.twq_dual_linear(None, 256, p, p, p, 8, 512, 256, 16, 64, p, 0, 512, None, 0, None, None) == 1
     assert lib.twq_dual_linear(p, 256, p, p, p, 8, 512, 256, 16, 64, p, 7, 512, None, 0, None, None) == 1
     assert lib.twq_dual_linear(p, 256, p, p, p, 8, 512, 256, 16, 64, p, 0, 256, None, 0, None, None) == 1
-    assert lib.twq_dual_linear(p, 256, p, p, p, 8, 512, 256, 16, 64, p, 0, 512, None, 0, None, None) == 3
+    assert lib.twq_dual_linear(p, 256, p, p, p, 24, 512, 256, 16, 64, p, 0, 512, None, 0, None, None) == 3
     # valid arguments but no sm_100 device here -> UNSUPPORTED or CUDA error, never a crash, never OK
     import torch
     if not torch.cuda.is_available():

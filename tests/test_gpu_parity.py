@@ -172,9 +172,28 @@ def test_exactly_representable_output_is_bit_exact(twq, oracle):
     assert (ref["Y"] == gen.bf16_bits_to_f32(oracle.round_bf16(ref["Y"])).astype(np.float64)).all()  # truly exact
 
 
-def test_strides_fp16_output_and_workspace_reuse(twq, oracle):
+def test_decode_kernel_strides_fp16_output_no_workspace(twq, oracle):
+    """M <= 16 runs the register-resident decode kernel: no scratch, padded Y rows untouched, repeatable."""
     import torch
     L = gen.make_layer(9, 512, 256, 32, 128, seed=41)
+    X, packed, _ = _upload(twq, L)
+    Xq, sx = twq.quantize_act(X, L.G)
+    assert twq.workspace_bytes(L.M, L.N, L.K, L.r, L.G) == 0
+    Ybig = torch.full((L.M, L.N + 64), 7.0, dtype=torch.float16, device="cuda")
+    Yv = Ybig[:, :L.N]
+    twq.dual_linear(X, Xq, sx, packed, twq.OUT_FP16, Y=Yv)
+    a = Yv.clone()
+    twq.dual_linear(X, Xq, sx, packed, twq.OUT_FP16, Y=Yv)
+    assert torch.equal(a, Yv)
+    assert (Ybig[:, L.N:] == 7.0).all()
+    ref = oracle.forward(L.X, L.Rq, L.sw, L.L1, L.L2, L.G)["Y"]
+    y = Yv.float().cpu().numpy().astype(np.float64)
+    assert np.abs(y - ref).max() / np.abs(ref).max() <= TOL + 2.0 ** -11
+
+
+def test_strides_fp16_output_and_workspace_reuse(twq, oracle):
+    import torch
+    L = gen.make_layer(24, 512, 256, 32, 128, seed=41)
     X, packed, _ = _upload(twq, L)
     Xq, sx = twq.quantize_act(X, L.G)
     need = twq.workspace_bytes(L.M, L.N, L.K, L.r, L.G)
@@ -196,7 +215,7 @@ def test_strides_fp16_output_and_workspace_reuse(twq, oracle):
 
 def test_errors_are_reported_not_thrown_by_cuda(twq):
     import torch
-    L = gen.make_layer(4, 256, 128, 0, 128, seed=5)
+    L = gen.make_layer(20, 256, 128, 0, 128, seed=5)
     X, packed, _ = _upload(twq, L)
     Xq, sx = twq.quantize_act(X, L.G)
     with pytest.raises(twq.TwqError):
