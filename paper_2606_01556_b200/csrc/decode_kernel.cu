@@ -28,6 +28,8 @@
 // for the weights and for the activations alike, so every global load is a 128-bit load.
 #include <cuda_bf16.h>
 #include <cuda_fp16.h>
+#include <stdio.h>
+#include <stdlib.h>
 
 #include "fused_kernel.h"
 #include "sm100_ptx.cuh"
@@ -118,6 +120,7 @@ __global__ void __launch_bounds__(kDecThreads, 1) decode_dual_linear_kernel(cons
     __half* sH = reinterpret_cast<__half*>(dsm + p.off_h);        // [16 tokens][r + 8]
     float* sYlr = reinterpret_cast<float*>(dsm + p.off_ylr);      // [16 tokens][T*16]
     float* sSx = reinterpret_cast<float*>(dsm + p.off_sx);        // [8*MT tokens][ng]
+    __half* sXs = reinterpret_cast<__half*>(dsm + p.off_xs);      // [8*MT tokens][K slice + 8] FP16 copy of X
 
     constexpr int kW = G / 32;
     constexpr int kTok = 8 * MT;
@@ -125,8 +128,9 @@ __global__ void __launch_bounds__(kDecThreads, 1) decode_dual_linear_kernel(cons
     const int gid = lane >> 2, tid4 = lane & 3;
     const int r = p.r, ng = p.ng, cs = p.cs;
     const int rank = cs > 1 ? static_cast<int>(cluster_ctarank()) : 0;
-    const int tile0 = static_cast<int>(blockIdx.x) * p.T;                       // first 16-channel tile of this CTA
-    const int ntile = max(0, min(p.T, p.n_tiles - tile0));
+    // 16-channel tiles of this CTA: an even split of the n_tiles over the grid (at most T each)
+    const int tile0 = static_cast<int>(static_cast<long long>(blockIdx.x) * p.n_tiles / gridDim.x);
+    const int ntile = static_cast<int>(static_cast<long long>(blockIdx.x + 1) * p.n_tiles / gridDim.x) - tile0;
     const int items = ntile * p.P;
     const int rowbytes = p.K >> 1;
     const int hstride = r + 8;
@@ -178,32 +182,50 @@ __global__ void __launch_bounds__(kDecThreads, 1) decode_dual_linear_kernel(cons
         const int units = p.K >> 5;                                  // 32-wide K units
         const int u0 = static_cast<int>(static_cast<long long>(units) * rank / cs);
         const int u1 = static_cast<int>(static_cast<long long>(units) * (rank + 1) / cs);
-        const uint16_t* X = static_cast<const uint16_t*>(p.X);
-        for (int jt = warp; jt < (r >> 3); jt += kDecWarps) {
+        const int nu = u1 - u0;
+        constexpr int kDL = 8;                                       // L1T loads in flight per thread
+        // first j-tile's L1T loads go out before the X slice is staged
+        int jt = warp;
+        const uint8_t* lrow = reinterpret_cast<const uint8_t*>(p.L1T) + (static_cast<size_t>(jt * 8 + gid) * p.K + tid4 * 8) * 2;
+        uint4 lv[kDL];
+        const bool j_ok = jt < (r >> 3);
+#pragma unroll
+        for (int s = 0; s < kDL; ++s)
+            if (j_ok && s < nu) lv[s] = ldg_nc(lrow + static_cast<size_t>(u0 + s) * 64);
+        // X slice (tokens x 32*nu k, BF16 -> FP16) into shared memory, rows padded by 16 bytes
+        const int xs_stride = nu * 32 + 8;                           // halves
+        {
+            const uint16_t* X = static_cast<const uint16_t*>(p.X);
+            const int chunks = nu * 4;                               // 16-byte chunks per token row
+            for (int i = threadIdx.x; i < kTok * chunks; i += kDecThreads) {
+                const int m = i / chunks, c = i - m * chunks;
+                uint4 v = make_uint4(0, 0, 0, 0);
+                if (m < p.M) v = __ldg(reinterpret_cast<const uint4*>(X + static_cast<size_t>(m) * p.ldx + u0 * 32 + c * 8));
+                v.x = bf2_to_h2(v.x); v.y = bf2_to_h2(v.y); v.z = bf2_to_h2(v.z); v.w = bf2_to_h2(v.w);
+                *reinterpret_cast<uint4*>(sXs + m * xs_stride + c * 8) = v;
+            }
+        }
+        __syncthreads();
+        for (; jt < (r >> 3); jt += kDecWarps) {
             float d[4] = {0.f, 0.f, 0.f, 0.f};
-            const uint8_t* lrow = reinterpret_cast<const uint8_t*>(p.L1T) + (static_cast<size_t>(jt * 8 + gid) * p.K + tid4 * 8) * 2;
-            const uint8_t* xa = reinterpret_cast<const uint8_t*>(X) + (static_cast<size_t>(gid) * p.ldx + tid4 * 8) * 2;
-            const uint8_t* xb = xa + static_cast<size_t>(8) * p.ldx * 2;
-            const bool a_ok = gid < p.M, b_ok = gid + 8 < p.M;
-            uint4 lv[kD], av[kD], bv[kD];
-            auto ld1 = [&](int s, int uu) {
-                const size_t off = static_cast<size_t>(uu) * 64;
-                lv[s] = ldg_nc(lrow + off);
-                av[s] = a_ok ? __ldg(reinterpret_cast<const uint4*>(xa + off)) : make_uint4(0, 0, 0, 0);
-                bv[s] = b_ok ? __ldg(reinterpret_cast<const uint4*>(xb + off)) : make_uint4(0, 0, 0, 0);
-            };
+            if (jt != warp) {
+                lrow = reinterpret_cast<const uint8_t*>(p.L1T) + (static_cast<size_t>(jt * 8 + gid) * p.K + tid4 * 8) * 2;
 #pragma unroll
-            for (int s = 0; s < kD; ++s)
-                if (u0 + s < u1) ld1(s, u0 + s);
-            for (int ub = u0; ub < u1; ub += kD) {
+                for (int s = 0; s < kDL; ++s)
+                    if (s < nu) lv[s] = ldg_nc(lrow + static_cast<size_t>(u0 + s) * 64);
+            }
+            const __half* xa = sXs + gid * xs_stride + tid4 * 8;
+            const __half* xb = xa + 8 * xs_stride;
+            for (int ub = 0; ub < nu; ub += kDL) {
 #pragma unroll
-                for (int s = 0; s < kD; ++s) {
-                    if (ub + s < u1) {
-                        const uint32_t a[4] = {bf2_to_h2(av[s].x), bf2_to_h2(av[s].y), bf2_to_h2(av[s].z), bf2_to_h2(av[s].w)};
-                        const uint32_t b[4] = {bf2_to_h2(bv[s].x), bf2_to_h2(bv[s].y), bf2_to_h2(bv[s].z), bf2_to_h2(bv[s].w)};
-                        hmma_16816(d, a[0], b[0], a[1], b[1], lv[s].x, lv[s].y);
-                        hmma_16816(d, a[2], b[2], a[3], b[3], lv[s].z, lv[s].w);
-                        if (ub + s + kD < u1) ld1(s, ub + s + kD);
+                for (int s = 0; s < kDL; ++s) {
+                    if (ub + s < nu) {
+                        const uint4 a = *reinterpret_cast<const uint4*>(xa + (ub + s) * 32);
+                        uint4 b = make_uint4(0, 0, 0, 0);
+                        if (MT == 2) b = *reinterpret_cast<const uint4*>(xb + (ub + s) * 32);
+                        hmma_16816(d, a.x, b.x, a.y, b.y, lv[s].x, lv[s].y);
+                        hmma_16816(d, a.z, b.z, a.w, b.w, lv[s].z, lv[s].w);
+                        if (ub + s + kDL < nu) lv[s] = ldg_nc(lrow + static_cast<size_t>(u0 + ub + s + kDL) * 64);
                     }
                 }
             }
@@ -449,11 +471,15 @@ bool decode_make_plan(int M, int N, int K, int r, int G, int num_sms, DecodePara
     p.cs = 1;
     int cap = num_sms;
     if (r > 0) {
+        // every cluster streams all of L1 (K*r*2 bytes) from L2, so the largest cluster that still covers
+        // 80 % of the SMs wins; otherwise the size covering the most SMs
         int best = 0;
-        for (int c = 16; c >= 1; c >>= 1) {
+        bool done = false;
+        for (int c = 16; c >= 1 && !done; c >>= 1) {
             if (r % c != 0 || (K >> 5) < c) continue;
             const int n = decode_cluster_capacity(c, num_sms);
-            if (n * c > best + best / 16) { best = n * c; p.cs = c; cap = n; }
+            if (n * c > best) { best = n * c; p.cs = c; cap = n; }
+            if (n * c * 5 >= num_sms * 4) done = true;
         }
     }
     int nclusters = cap;
@@ -473,6 +499,8 @@ bool decode_make_plan(int M, int N, int K, int r, int G, int num_sms, DecodePara
     p.off_h = o; o += 16 * (r + 8) * 2;
     p.off_ylr = o; o += 16 * p.T * 16 * 4;
     p.off_sx = o; o += kTok * p.ng * 4;
+    o = (o + 15) & ~15;
+    p.off_xs = o; o += r > 0 ? kTok * (((K >> 5) + p.cs - 1) / p.cs * 32 + 8) * 2 : 0;
     p.smem_bytes = (o + 15) & ~15;
     if (p.smem_bytes > 200 * 1024) return false;
     *out = p;
@@ -481,6 +509,10 @@ bool decode_make_plan(int M, int N, int K, int r, int G, int num_sms, DecodePara
 
 cudaError_t launch_decode(const DecodeParams& p, int G, cudaStream_t stream) {
     const bool dbg = p.dbgP != nullptr;
+    static const bool trace = getenv("TWQ_DEBUG_PLAN") != nullptr;
+    if (trace)
+        fprintf(stderr, "twq decode plan: M=%d N=%d K=%d r=%d cs=%d grid=%d T=%d P=%d smem=%d\n", p.M, p.N, p.K, p.r,
+                p.cs, p.grid, p.T, p.P, p.smem_bytes);
     const int mt = p.M <= 8 ? 1 : 2;
 #define TWQ_DCASE(g, m)                                                                   \
     if (G == g && mt == m) return dbg ? decode_launch_inst<g, m, true>(p, stream) : decode_launch_inst<g, m, false>(p, stream);

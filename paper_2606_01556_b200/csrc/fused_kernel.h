@@ -48,7 +48,7 @@ struct DecodeParams {
     int n_tiles;             // N / 16
     int cs, grid;            // CTAs per cluster, CTAs in the grid (a multiple of cs)
     int T, P;                // 16-channel tiles per CTA, K-parts per tile
-    int off_res, off_hpart, off_h, off_ylr, off_sx, smem_bytes;
+    int off_res, off_hpart, off_h, off_ylr, off_sx, off_xs, smem_bytes;
     const uint8_t* R4;       // [N][K/2]
     const float* swT;        // [ng][N]
     const void* L1T;         // [r][K] f16
