@@ -80,7 +80,7 @@ __device__ __forceinline__ uint32_t bf2_to_h2(uint32_t w) {
 
 __device__ __forceinline__ float ld_dsmem_f(uint32_t cluster_addr) {
     float v;
-    asm volatile("ld.shared::cluster.f32 %0, [%1];" : "=f"(v) : "r"(cluster_addr) : "memory");
+    asm volatile("ld.shared::cluster.f32 %0, [%1];" : "=f"(v) : "r"(cluster_addr));
     return v;
 }
 __device__ __forceinline__ void st_dsmem_u16(uint32_t cluster_addr, uint16_t v) {
@@ -112,6 +112,20 @@ __device__ __forceinline__ void load_words(uint32_t (&dst)[kW], const uint8_t* p
     }
 }
 
+#ifdef TWQ_TRACE
+__device__ unsigned long long g_twq_dtrace[4 * 32];
+#define TWQ_DT(k)                                                                                     \
+    do {                                                                                              \
+        if ((threadIdx.x & 31) == 0 && (threadIdx.x >> 5) < 2 && (blockIdx.x == 0 || blockIdx.x == 61)) { \
+            unsigned long long t_;                                                                    \
+            asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t_));                                    \
+            g_twq_dtrace[((blockIdx.x != 0) * 2 + (threadIdx.x >> 5)) * 32 + (k)] = t_;               \
+        }                                                                                             \
+    } while (0)
+#else
+#define TWQ_DT(k) do { } while (0)
+#endif
+
 template <int G, int MT, bool kDbg>
 __global__ void __launch_bounds__(kDecThreads, 1) decode_dual_linear_kernel(const __grid_constant__ DecodeParams p) {
     extern __shared__ __align__(16) uint8_t dsm[];
@@ -136,6 +150,7 @@ __global__ void __launch_bounds__(kDecThreads, 1) decode_dual_linear_kernel(cons
     const int hstride = r + 8;
 
     pdl_launch_dependents();
+    TWQ_DT(0);
 
     // ---------------------------------------------------------------- residual: first loads in flight
     constexpr int kD = 4;
@@ -170,12 +185,9 @@ __global__ void __launch_bounds__(kDecThreads, 1) decode_dual_linear_kernel(cons
             }
         }
     };
-    if (item < items) {
-        setup_item();
-#pragma unroll
-        for (int s = 0; s < kD; ++s)
-            if (s < cnt) load_w(sl[s], s);
-    }
+    // The low-rank chain (L1T slice -> partial H -> cluster exchange -> stage 2) is the critical path of a
+    // decode call, so its loads go out first; the residual weight stream is started right after and lands
+    // while the cluster exchanges H.
 
     // ---------------------------------------------------------------- low-rank stage 1: H partial of this CTA's K slice
     if (r > 0) {
@@ -184,7 +196,19 @@ __global__ void __launch_bounds__(kDecThreads, 1) decode_dual_linear_kernel(cons
         const int u1 = static_cast<int>(static_cast<long long>(units) * (rank + 1) / cs);
         const int nu = u1 - u0;
         constexpr int kDL = 8;                                       // L1T loads in flight per thread
-        // first j-tile's L1T loads go out before the X slice is staged
+        // loads in the order the dependent chain needs them: X slice, first j-tile's L1T ring, residual weights
+        const int xs_stride = nu * 32 + 8;                           // halves; rows padded by 16 bytes
+        const uint16_t* X = static_cast<const uint16_t*>(p.X);
+        const int chunks = nu * 4;                                   // 16-byte chunks per token row
+        constexpr int kXV = 2;                                       // staged X chunks per thread per pass
+        uint4 xv[kXV];
+#pragma unroll
+        for (int q = 0; q < kXV; ++q) {
+            const int i = threadIdx.x + q * kDecThreads;
+            const int m = i / chunks, c = i - m * chunks;
+            xv[q] = make_uint4(0, 0, 0, 0);
+            if (i < kTok * chunks && m < p.M) xv[q] = __ldg(reinterpret_cast<const uint4*>(X + static_cast<size_t>(m) * p.ldx + u0 * 32 + c * 8));
+        }
         int jt = warp;
         const uint8_t* lrow = reinterpret_cast<const uint8_t*>(p.L1T) + (static_cast<size_t>(jt * 8 + gid) * p.K + tid4 * 8) * 2;
         uint4 lv[kDL];
@@ -192,22 +216,34 @@ __global__ void __launch_bounds__(kDecThreads, 1) decode_dual_linear_kernel(cons
 #pragma unroll
         for (int s = 0; s < kDL; ++s)
             if (j_ok && s < nu) lv[s] = ldg_nc(lrow + static_cast<size_t>(u0 + s) * 64);
-        // X slice (tokens x 32*nu k, BF16 -> FP16) into shared memory, rows padded by 16 bytes
-        const int xs_stride = nu * 32 + 8;                           // halves
-        {
-            const uint16_t* X = static_cast<const uint16_t*>(p.X);
-            const int chunks = nu * 4;                               // 16-byte chunks per token row
-            for (int i = threadIdx.x; i < kTok * chunks; i += kDecThreads) {
+        // X slice (tokens x 32*nu k, BF16 -> FP16) into shared memory
+#pragma unroll
+        for (int q = 0; q < kXV; ++q) {
+            const int i = threadIdx.x + q * kDecThreads;
+            if (i < kTok * chunks) {
                 const int m = i / chunks, c = i - m * chunks;
-                uint4 v = make_uint4(0, 0, 0, 0);
-                if (m < p.M) v = __ldg(reinterpret_cast<const uint4*>(X + static_cast<size_t>(m) * p.ldx + u0 * 32 + c * 8));
+                uint4 v = xv[q];
                 v.x = bf2_to_h2(v.x); v.y = bf2_to_h2(v.y); v.z = bf2_to_h2(v.z); v.w = bf2_to_h2(v.w);
                 *reinterpret_cast<uint4*>(sXs + m * xs_stride + c * 8) = v;
             }
         }
+        for (int i = threadIdx.x + kXV * kDecThreads; i < kTok * chunks; i += kDecThreads) {   // long K slices
+            const int m = i / chunks, c = i - m * chunks;
+            uint4 v = make_uint4(0, 0, 0, 0);
+            if (m < p.M) v = __ldg(reinterpret_cast<const uint4*>(X + static_cast<size_t>(m) * p.ldx + u0 * 32 + c * 8));
+            v.x = bf2_to_h2(v.x); v.y = bf2_to_h2(v.y); v.z = bf2_to_h2(v.z); v.w = bf2_to_h2(v.w);
+            *reinterpret_cast<uint4*>(sXs + m * xs_stride + c * 8) = v;
+        }
         __syncthreads();
+        TWQ_DT(1);
         for (; jt < (r >> 3); jt += kDecWarps) {
-            float d[4] = {0.f, 0.f, 0.f, 0.f};
+            // a warp-level MMA has a latency of several hundred cycles on this part: eight independent
+            // accumulators keep the dependent chain at nu/4 instead of 2*nu
+            float d8[8][4];
+#pragma unroll
+            for (int q = 0; q < 8; ++q)
+#pragma unroll
+                for (int e = 0; e < 4; ++e) d8[q][e] = 0.0f;
             if (jt != warp) {
                 lrow = reinterpret_cast<const uint8_t*>(p.L1T) + (static_cast<size_t>(jt * 8 + gid) * p.K + tid4 * 8) * 2;
 #pragma unroll
@@ -223,23 +259,50 @@ __global__ void __launch_bounds__(kDecThreads, 1) decode_dual_linear_kernel(cons
                         const uint4 a = *reinterpret_cast<const uint4*>(xa + (ub + s) * 32);
                         uint4 b = make_uint4(0, 0, 0, 0);
                         if (MT == 2) b = *reinterpret_cast<const uint4*>(xb + (ub + s) * 32);
-                        hmma_16816(d, a.x, b.x, a.y, b.y, lv[s].x, lv[s].y);
-                        hmma_16816(d, a.z, b.z, a.w, b.w, lv[s].z, lv[s].w);
+                        hmma_16816(d8[(2 * s) & 7], a.x, b.x, a.y, b.y, lv[s].x, lv[s].y);
+                        hmma_16816(d8[(2 * s + 1) & 7], a.z, b.z, a.w, b.w, lv[s].z, lv[s].w);
                         if (ub + s + kDL < nu) lv[s] = ldg_nc(lrow + static_cast<size_t>(u0 + ub + s + kDL) * 64);
                     }
                 }
             }
+            float d[4];
+#pragma unroll
+            for (int e = 0; e < 4; ++e)
+                d[e] = ((d8[0][e] + d8[1][e]) + (d8[2][e] + d8[3][e])) + ((d8[4][e] + d8[5][e]) + (d8[6][e] + d8[7][e]));
             const int j = jt * 8 + tid4 * 2;
             sHpart[gid * r + j] = d[0];
             sHpart[gid * r + j + 1] = d[1];
             sHpart[(gid + 8) * r + j] = d[2];
             sHpart[(gid + 8) * r + j + 1] = d[3];
         }
+        TWQ_DT(2);
         if (cs > 1) cluster_arrive();   // release: this CTA's partial is in its shared memory
+        TWQ_DT(3);
+    }
+    // residual weight stream: issued after the arrive (its release fence would otherwise wait for these loads)
+    if (item < items) {
+        setup_item();
+#pragma unroll
+        for (int s = 0; s < kD; ++s)
+            if (s < cnt) load_w(sl[s], s);
+    }
+
+    // stage-2 operand of this warp's first 8-channel step (L2T rows), prefetched behind the weights
+    constexpr int kL2 = 8;                             // 32-wide j steps held in registers (r <= 256)
+    uint4 l2v[kL2];
+    const bool l2_ok = r > 0 && warp < ntile * 2;
+    if (l2_ok) {
+        const uint8_t* lrow = reinterpret_cast<const uint8_t*>(p.L2T) +
+                              (static_cast<size_t>(tile0 * 16 + warp * 8 + gid) * r + tid4 * 8) * 2;
+#pragma unroll
+        for (int js = 0; js < kL2; ++js)
+            l2v[js] = (js * 32 + tid4 * 8 < r) ? ldg_nc(lrow + js * 64) : make_uint4(0, 0, 0, 0);
     }
 
     // ---------------------------------------------------------------- quantizer outputs from here on
+    TWQ_DT(4);
     pdl_wait();
+    TWQ_DT(5);
     for (int i = threadIdx.x; i < kTok * ng; i += kDecThreads) {
         const int m = i / ng, g = i - m * ng;
         sSx[i] = m < p.M ? __ldg(p.sx + static_cast<size_t>(m) * ng + g) * 0x1p-8f : 0.0f;   // MMA operands are 16*code
@@ -249,7 +312,9 @@ __global__ void __launch_bounds__(kDecThreads, 1) decode_dual_linear_kernel(cons
         for (int s = 0; s < kD; ++s)
             if (s < cnt) load_x(sl[s], s);
     }
-    __syncthreads();
+
+    __syncthreads();                                   // sSx visible to every warp
+    TWQ_DT(9);
 
     // ---------------------------------------------------------------- residual items of this warp
     while (item < items) {
@@ -260,43 +325,53 @@ __global__ void __launch_bounds__(kDecThreads, 1) decode_dual_linear_kernel(cons
             for (int e = 0; e < 4; ++e) acc[t][e] = 0.0f;
         const int n_a = (tile0 + tile) * 16 + gid;   // output channel of rows gid (n_a) and gid+8 (n_a + 8)
         for (int ib = 0; ib < cnt; ib += kD) {
+            // the kD groups in flight form independent MMA chains (one int32 tile each); issuing them
+            // interleaved hides the warp-level MMA latency
+            int d[kD][MT][4];
+#pragma unroll
+            for (int s = 0; s < kD; ++s)
+#pragma unroll
+                for (int t = 0; t < MT; ++t)
+#pragma unroll
+                    for (int e = 0; e < 4; ++e) d[s][t][e] = 0;
+#pragma unroll
+            for (int w = 0; w < kW; ++w) {              // one K-step of 32 codes per packed word
+#pragma unroll
+                for (int s = 0; s < kD; ++s) {
+                    if (ib + s < cnt) {
+                        const Slot<G, MT>& c = sl[s];
+                        const uint32_t a0 = d_lo16(c.wa[w]), a2 = d_hi16(c.wa[w]);
+                        const uint32_t a1 = d_lo16(c.wb[w]), a3 = d_hi16(c.wb[w]);
+#pragma unroll
+                        for (int t = 0; t < MT; ++t)
+                            imma_16832(d[s][t], a0, a1, a2, a3, d_lo16(c.xq[t][w]), d_hi16(c.xq[t][w]));
+                    }
+                }
+            }
 #pragma unroll
             for (int s = 0; s < kD; ++s) {
                 const int i = ib + s;
                 if (i < cnt) {
                     const int g = kpart + i * p.P;
                     Slot<G, MT>& c = sl[s];
-                    int d[MT][4];
-#pragma unroll
-                    for (int t = 0; t < MT; ++t)
-#pragma unroll
-                        for (int e = 0; e < 4; ++e) d[t][e] = 0;
-#pragma unroll
-                    for (int w = 0; w < kW; ++w) {      // one K-step of 32 codes per packed word
-                        const uint32_t a0 = d_lo16(c.wa[w]), a2 = d_hi16(c.wa[w]);
-                        const uint32_t a1 = d_lo16(c.wb[w]), a3 = d_hi16(c.wb[w]);
-#pragma unroll
-                        for (int t = 0; t < MT; ++t)
-                            imma_16832(d[t], a0, a1, a2, a3, d_lo16(c.xq[t][w]), d_hi16(c.xq[t][w]));
-                    }
                     // d = 256 * P (exact); fold both scales in FP32 (sx already carries 2^-8)
 #pragma unroll
                     for (int t = 0; t < MT; ++t) {
                         const float s0 = sSx[(8 * t + tid4 * 2) * ng + g], s1 = sSx[(8 * t + tid4 * 2 + 1) * ng + g];
-                        acc[t][0] = fmaf(__fmul_rn(static_cast<float>(d[t][0]), c.swa), s0, acc[t][0]);
-                        acc[t][1] = fmaf(__fmul_rn(static_cast<float>(d[t][1]), c.swa), s1, acc[t][1]);
-                        acc[t][2] = fmaf(__fmul_rn(static_cast<float>(d[t][2]), c.swb), s0, acc[t][2]);
-                        acc[t][3] = fmaf(__fmul_rn(static_cast<float>(d[t][3]), c.swb), s1, acc[t][3]);
+                        acc[t][0] = fmaf(__fmul_rn(static_cast<float>(d[s][t][0]), c.swa), s0, acc[t][0]);
+                        acc[t][1] = fmaf(__fmul_rn(static_cast<float>(d[s][t][1]), c.swa), s1, acc[t][1]);
+                        acc[t][2] = fmaf(__fmul_rn(static_cast<float>(d[s][t][2]), c.swb), s0, acc[t][2]);
+                        acc[t][3] = fmaf(__fmul_rn(static_cast<float>(d[s][t][3]), c.swb), s1, acc[t][3]);
                         if (kDbg) {
                             if (p.dbgP != nullptr) {
                                 const int m0 = 8 * t + tid4 * 2;
                                 if (m0 < p.M) {
-                                    p.dbgP[(static_cast<size_t>(m0) * ng + g) * p.N + n_a] = d[t][0] >> 8;
-                                    p.dbgP[(static_cast<size_t>(m0) * ng + g) * p.N + n_a + 8] = d[t][2] >> 8;
+                                    p.dbgP[(static_cast<size_t>(m0) * ng + g) * p.N + n_a] = d[s][t][0] >> 8;
+                                    p.dbgP[(static_cast<size_t>(m0) * ng + g) * p.N + n_a + 8] = d[s][t][2] >> 8;
                                 }
                                 if (m0 + 1 < p.M) {
-                                    p.dbgP[(static_cast<size_t>(m0 + 1) * ng + g) * p.N + n_a] = d[t][1] >> 8;
-                                    p.dbgP[(static_cast<size_t>(m0 + 1) * ng + g) * p.N + n_a + 8] = d[t][3] >> 8;
+                                    p.dbgP[(static_cast<size_t>(m0 + 1) * ng + g) * p.N + n_a] = d[s][t][1] >> 8;
+                                    p.dbgP[(static_cast<size_t>(m0 + 1) * ng + g) * p.N + n_a + 8] = d[s][t][3] >> 8;
                                 }
                             }
                         }
@@ -323,24 +398,31 @@ __global__ void __launch_bounds__(kDecThreads, 1) decode_dual_linear_kernel(cons
         }
     }
 
-    // ---------------------------------------------------------------- low-rank: H exchange, stage 2
-    const int nloc = p.T * 16;                         // channels of this CTA (row stride of sYlr)
+    // ---------------------------------------------------------------- low-rank: H exchange
     if (r > 0) {
         if (cs > 1) {
             cluster_wait();                            // every CTA's FP32 partial is visible
+            TWQ_DT(6);
             const int jc = r / cs;                     // columns of H this CTA reduces
-            for (int i = threadIdx.x; i < 16 * jc; i += kDecThreads) {
+            for (int i = threadIdx.x; i < p.M * jc; i += kDecThreads) {   // rows m >= M of H are zero everywhere
                 const int m = i / jc, j = rank * jc + (i - m * jc);
                 const uint32_t src = smem_u32(sHpart + m * r + j);
                 float s = 0.0f;
-                for (int pr = 0; pr < cs; ++pr) s += ld_dsmem_f(mapa_u32(src, pr));   // fixed order: identical H everywhere
+                for (int pr = 0; pr < cs; pr += 4) {   // four remote loads in flight; fixed order: identical H everywhere
+                    float v[4];
+#pragma unroll
+                    for (int q = 0; q < 4; ++q) v[q] = pr + q < cs ? ld_dsmem_f(mapa_u32(src, pr + q)) : 0.0f;
+#pragma unroll
+                    for (int q = 0; q < 4; ++q) s += v[q];
+                }
                 s = fminf(fmaxf(s, -65504.0f), 65504.0f);
                 const __half hv = __float2half_rn(s);
                 const uint32_t dsta = smem_u32(sH + m * hstride + j);
                 for (int pr = 0; pr < cs; ++pr) st_dsmem_u16(mapa_u32(dsta, pr), *reinterpret_cast<const uint16_t*>(&hv));
             }
-            cluster_arrive();
-            cluster_wait();                            // the full FP16 H is in this CTA's shared memory
+            TWQ_DT(7);
+            cluster_arrive();                          // waited for after the residual items
+            TWQ_DT(8);
         } else {
             __syncthreads();
             for (int i = threadIdx.x; i < 16 * r; i += kDecThreads) {
@@ -350,22 +432,36 @@ __global__ void __launch_bounds__(kDecThreads, 1) decode_dual_linear_kernel(cons
             }
             __syncthreads();
         }
-        // stage 2: Ylr[m, n] = sum_j H[m,j] * L2T[n,j] for this CTA's channels, 8 channels per warp step
+    }
+    // ---------------------------------------------------------------- low-rank stage 2
+    const int nloc = p.T * 16;                         // channels of this CTA (row stride of sYlr)
+    if (r > 0) {
+        TWQ_DT(10);
+        if (cs > 1) cluster_wait();                    // the full FP16 H is in this CTA's shared memory
+        TWQ_DT(11);
+        // Ylr[m, n] = sum_j H[m,j] * L2T[n,j] for this CTA's channels, 8 channels per warp step
         for (int nt = warp; nt < ntile * 2; nt += kDecWarps) {
             float d[4] = {0.f, 0.f, 0.f, 0.f};
-            const int n = tile0 * 16 + nt * 8 + gid;
-            const uint8_t* lrow = reinterpret_cast<const uint8_t*>(p.L2T) + (static_cast<size_t>(n) * r + tid4 * 8) * 2;
+            if (nt != warp) {
+                const uint8_t* lrow = reinterpret_cast<const uint8_t*>(p.L2T) +
+                                      (static_cast<size_t>(tile0 * 16 + nt * 8 + gid) * r + tid4 * 8) * 2;
+#pragma unroll
+                for (int js = 0; js < kL2; ++js)
+                    l2v[js] = (js * 32 + tid4 * 8 < r) ? ldg_nc(lrow + js * 64) : make_uint4(0, 0, 0, 0);
+            }
             const __half* ha = sH + gid * hstride + tid4 * 8;
             const __half* hb = ha + 8 * hstride;
-            for (int jb = 0; jb < r; jb += 32) {
-                uint4 lv = make_uint4(0, 0, 0, 0), a = lv, b = lv;
-                if (jb + tid4 * 8 < r) {               // r is a multiple of 16: the last step may be half empty
-                    lv = ldg_nc(lrow + jb * 2);
-                    a = *reinterpret_cast<const uint4*>(ha + jb);
-                    b = *reinterpret_cast<const uint4*>(hb + jb);
+#pragma unroll
+            for (int js = 0; js < kL2; ++js) {
+                if (js * 32 < r) {                     // warp-uniform
+                    uint4 a = make_uint4(0, 0, 0, 0), b = a;
+                    if (js * 32 + tid4 * 8 < r) {      // r is a multiple of 16: the last step may be half empty
+                        a = *reinterpret_cast<const uint4*>(ha + js * 32);
+                        b = *reinterpret_cast<const uint4*>(hb + js * 32);
+                    }
+                    hmma_16816(d, a.x, b.x, a.y, b.y, l2v[js].x, l2v[js].y);
+                    hmma_16816(d, a.z, b.z, a.w, b.w, l2v[js].z, l2v[js].w);
                 }
-                hmma_16816(d, a.x, b.x, a.y, b.y, lv.x, lv.y);
-                hmma_16816(d, a.z, b.z, a.w, b.w, lv.z, lv.w);
             }
             const int nl = nt * 8 + tid4 * 2;
             sYlr[gid * nloc + nl] = d[0];
@@ -376,6 +472,7 @@ __global__ void __launch_bounds__(kDecThreads, 1) decode_dual_linear_kernel(cons
     }
     __syncthreads();
 
+    TWQ_DT(12);
     // ---------------------------------------------------------------- single epilogue: sum the K-parts, add Ylr, one store
     for (int i = threadIdx.x; i < ntile * 16 * p.M; i += kDecThreads) {
         const int m = i / (ntile * 16), nl = i - m * (ntile * 16);
@@ -388,6 +485,7 @@ __global__ void __launch_bounds__(kDecThreads, 1) decode_dual_linear_kernel(cons
         else if (p.ydt == 1) static_cast<__half*>(p.Y)[o] = __float2half_rn(y);
         else static_cast<float*>(p.Y)[o] = y;
     }
+    TWQ_DT(13);
     // no trailing cluster barrier: the last remote access of any CTA precedes its second arrive, which
     // every CTA has waited for
 }
@@ -472,15 +570,19 @@ bool decode_make_plan(int M, int N, int K, int r, int G, int num_sms, DecodePara
     int cap = num_sms;
     if (r > 0) {
         // every cluster streams all of L1 (K*r*2 bytes) from L2, so the largest cluster that still covers
-        // 80 % of the SMs wins; otherwise the size covering the most SMs
+        // 70 % of the SMs wins; otherwise the size covering the most SMs
         int best = 0;
         bool done = false;
         for (int c = 16; c >= 1 && !done; c >>= 1) {
             if (r % c != 0 || (K >> 5) < c) continue;
             const int n = decode_cluster_capacity(c, num_sms);
             if (n * c > best) { best = n * c; p.cs = c; cap = n; }
-            if (n * c * 5 >= num_sms * 4) done = true;
+            if (n * c * 10 >= num_sms * 7) done = true;
         }
+    }
+    if (const char* e = getenv("TWQ_DEBUG_DECODE_CS")) {   // debugging aid: force the cluster size
+        const int c = atoi(e);
+        if (r > 0 && c >= 1 && c <= 16 && (c & (c - 1)) == 0 && r % c == 0) { p.cs = c; cap = decode_cluster_capacity(c, num_sms); }
     }
     int nclusters = cap;
     const int need = (p.n_tiles + p.cs - 1) / p.cs;           // clusters needed at one tile per CTA
