@@ -198,19 +198,29 @@ def roofline_for(L, twq, us_dual, peaks, traffic=None):
         ach = by / t / 1e9
         return dict(bound="hbm", achieved=round(ach, 1), peak=peaks["hbm_gbs"], unit="GB/s",
                     frac=round(ach / peaks["hbm_gbs"], 4), traffic=traffic, peak_source=peaks["source"],
-                    kernel="dual_linear_kernel", us=round(us_dual, 3), algorithmic_bytes=by)
+                    kernel=kernel_name(L), us=round(us_dual, 3), algorithmic_bytes=by)
     eq_ops = ops_i8 + 2.0 * fl_lr                    # low-rank flops run at half the int8 rate
     ach = eq_ops / t / 1e12
     return dict(bound="tensor", achieved=round(ach, 1), peak=round(p_i8 / 1e12, 1), unit="TFLOP/s",
                 frac=round(ach / (p_i8 / 1e12), 4), traffic=traffic, peak_source=peaks["source"] + " bf16 burst x2 (int8)",
-                kernel="dual_linear_kernel", us=round(us_dual, 3), int8_equivalent_ops=eq_ops)
+                kernel=kernel_name(L), us=round(us_dual, 3), int8_equivalent_ops=eq_ops)
+
+
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dual-linear kernel, from the ncu --set full
+# captures summarised under profiles/ (r01b_full_*.txt); None where no capture exists.
+TRAFFIC_BYTES = {
+    "c2_qproj_m1": 11078912,          # profiles/r01b_full_decode_c2_qproj_m1.txt
+    "c2_qproj_m16": 11239680,         # profiles/r01b_full_decode_c2_qproj_m16.txt
+    "c3_gateup_m2048": 111621120,     # profiles/r01b_full_fused_c3_gateup_m2048.txt
+}
 
 
 def load_traffic(name):
-    path = os.path.join(ROOT, "profiles", "traffic.json")
-    if os.path.exists(path):
-        return json.load(open(path)).get(name)
-    return None
+    return TRAFFIC_BYTES.get(name)
+
+
+def kernel_name(L):
+    return "decode_dual_linear_kernel" if L.M <= 16 else "fused_dual_linear_kernel"
 
 
 def measure_workload(name, twq, torch, steps, warmup, peaks, with_e2e=False, with_cublas=False):

@@ -119,6 +119,21 @@ def test_ragged_shapes(twq, oracle, M, K, N, r, G):
     _check_layer(twq, oracle, gen.make_layer(M, K, N, r, G, seed=1000 + M, with_tinv=(M % 2 == 0)))
 
 
+@pytest.mark.parametrize("M,K,N,r,G", [
+    (1, 128, 16, 16, 128),       # one tile, one group, smallest rank
+    (3, 192, 48, 16, 64),        # G = 64 (two packed words per thread), three groups
+    (8, 2048, 528, 48, 128),     # r not a multiple of 32: half-empty last stage-2 step; N = 33 tiles
+    (9, 1024, 272, 256, 128),    # two token tiles of the MMA (M > 8), rank 256: two j-tiles per warp
+    (12, 640, 16, 0, 128),       # rank 0 in the decode kernel, fewer tiles than CTAs
+    (16, 7168, 1040, 128, 128),  # long K: items with more groups than pipeline slots, several ring rounds
+    (16, 512, 4112, 32, 64),     # many tiles per CTA, whole K in one part
+])
+def test_decode_kernel_shapes(twq, oracle, M, K, N, r, G):
+    """M <= 16 takes the register-resident decode kernel (decode_kernel.cu); same bar as every other shape."""
+    assert twq.workspace_bytes(M, N, K, r, G) == 0
+    _check_layer(twq, oracle, gen.make_layer(M, K, N, r, G, seed=2000 + M + N, with_tinv=(M % 2 == 1)))
+
+
 def test_rank0_is_plain_w4a4_and_zero_residual_is_lowrank(twq, oracle):
     """north_star special cases, on the GPU path."""
     import torch
