@@ -83,10 +83,20 @@ __device__ __forceinline__ float ld_dsmem_f(uint32_t cluster_addr) {
     asm volatile("ld.shared::cluster.f32 %0, [%1];" : "=f"(v) : "r"(cluster_addr));
     return v;
 }
+__device__ __forceinline__ float4 ld_dsmem_f4_nc(uint32_t cluster_addr) {
+    float4 v;
+    asm volatile("ld.shared::cluster.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(cluster_addr));
+    return v;
+}
 __device__ __forceinline__ void st_dsmem_u16(uint32_t cluster_addr, uint16_t v) {
     asm volatile("st.shared::cluster.u16 [%0], %1;" ::"r"(cluster_addr), "h"(v) : "memory");
 }
 __device__ __forceinline__ void cluster_arrive() { asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory"); }
+// Arrive without a per-thread release fence: used after __syncthreads() + one fence.acq_rel.cluster by
+// thread 0 (the CTA's writes are ordered before that fence by the block barrier), or where the arrive only
+// says "done reading".  The per-thread release form costs every warp a full memory fence (~0.5-0.9 us here).
+__device__ __forceinline__ void cluster_arrive_relaxed() { asm volatile("barrier.cluster.arrive.relaxed.aligned;" ::: "memory"); }
+__device__ __forceinline__ void fence_cluster() { asm volatile("fence.acq_rel.cluster;" ::: "memory"); }
 __device__ __forceinline__ void cluster_wait() { asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory"); }
 
 }  // namespace
@@ -145,12 +155,19 @@ __global__ void __launch_bounds__(kDecThreads, 1) decode_dual_linear_kernel(cons
     // 16-channel tiles of this CTA: an even split of the n_tiles over the grid (at most T each)
     const int tile0 = static_cast<int>(static_cast<long long>(blockIdx.x) * p.n_tiles / gridDim.x);
     const int ntile = static_cast<int>(static_cast<long long>(blockIdx.x + 1) * p.n_tiles / gridDim.x) - tile0;
-    const int items = ntile * p.P;
+    // K-parts per tile, chosen per CTA so that its ntile * P items fill the 16 warps in ONE round where
+    // possible (a second item per warp would expose another DRAM round trip): P = 16 / ntile, any integer
+    int P = ntile > 0 ? kDecWarps / ntile : 1;
+    P = max(1, min(P, p.P));
+    const int items = ntile * P;
     const int rowbytes = p.K >> 1;
     const int hstride = r + 8;
 
     pdl_launch_dependents();
     TWQ_DT(0);
+#ifdef TWQ_TRACE
+    if (p.ydt >= 100) return;     // launch-overhead probe (trace build only)
+#endif
 
     // ---------------------------------------------------------------- residual: first loads in flight
     constexpr int kD = 4;
@@ -159,13 +176,13 @@ __global__ void __launch_bounds__(kDecThreads, 1) decode_dual_linear_kernel(cons
     int tile = 0, kpart = 0, cnt = 0;      // its tile, K-part and number of groups
     const uint8_t* wrow = nullptr;         // row gid of the tile in R4
     auto setup_item = [&]() {
-        tile = item / p.P;
-        kpart = item - tile * p.P;
-        cnt = kpart < ng ? (ng - kpart + p.P - 1) / p.P : 0;
+        tile = item / P;
+        kpart = item - tile * P;
+        cnt = kpart < ng ? (ng - kpart + P - 1) / P : 0;
         wrow = p.R4 + static_cast<size_t>((tile0 + tile) * 16 + gid) * rowbytes + tid4 * (kW * 4);
     };
     auto load_w = [&](Slot<G, MT>& s, int i) {   // weights + weight scales of the i-th group of the item
-        const int g = kpart + i * p.P;
+        const int g = kpart + i * P;
         load_words<kW>(s.wa, wrow + static_cast<size_t>(g) * (G / 2), true);
         load_words<kW>(s.wb, wrow + static_cast<size_t>(g) * (G / 2) + static_cast<size_t>(8) * rowbytes, true);
         const float* sp = p.swT + static_cast<size_t>(g) * p.N + (tile0 + tile) * 16 + gid;
@@ -173,7 +190,7 @@ __global__ void __launch_bounds__(kDecThreads, 1) decode_dual_linear_kernel(cons
         s.swb = __ldg(sp + 8);
     };
     auto load_x = [&](Slot<G, MT>& s, int i) {   // packed activations of tokens gid (, gid+8)
-        const int g = kpart + i * p.P;
+        const int g = kpart + i * P;
 #pragma unroll
         for (int t = 0; t < MT; ++t) {
             const int m = gid + 8 * t;
@@ -276,7 +293,11 @@ __global__ void __launch_bounds__(kDecThreads, 1) decode_dual_linear_kernel(cons
             sHpart[(gid + 8) * r + j + 1] = d[3];
         }
         TWQ_DT(2);
-        if (cs > 1) cluster_arrive();   // release: this CTA's partial is in its shared memory
+        if (cs > 1) {                   // release: this CTA's partial is in its shared memory
+            __syncthreads();
+            if (threadIdx.x == 0) fence_cluster();
+            cluster_arrive_relaxed();
+        }
         TWQ_DT(3);
     }
     // residual weight stream: issued after the arrive (its release fence would otherwise wait for these loads)
@@ -352,7 +373,7 @@ __global__ void __launch_bounds__(kDecThreads, 1) decode_dual_linear_kernel(cons
             for (int s = 0; s < kD; ++s) {
                 const int i = ib + s;
                 if (i < cnt) {
-                    const int g = kpart + i * p.P;
+                    const int g = kpart + i * P;
                     Slot<G, MT>& c = sl[s];
                     // d = 256 * P (exact); fold both scales in FP32 (sx already carries 2^-8)
 #pragma unroll
@@ -403,26 +424,32 @@ __global__ void __launch_bounds__(kDecThreads, 1) decode_dual_linear_kernel(cons
         if (cs > 1) {
             cluster_wait();                            // every CTA's FP32 partial is visible
             TWQ_DT(6);
-            const int jc = r / cs;                     // columns of H this CTA reduces
-            for (int i = threadIdx.x; i < p.M * jc; i += kDecThreads) {   // rows m >= M of H are zero everywhere
-                const int m = i / jc, j = rank * jc + (i - m * jc);
+            // all-reduce by reading: every CTA sums the cs partials of the M live rows itself (fixed order, so
+            // H is identical everywhere) -- one cluster barrier instead of a reduce-scatter plus an all-gather
+            const int r4 = r >> 2;
+            for (int i = threadIdx.x; i < p.M * r4; i += kDecThreads) {
+                const int m = i / r4, j = (i - m * r4) * 4;
                 const uint32_t src = smem_u32(sHpart + m * r + j);
-                float s = 0.0f;
-                for (int pr = 0; pr < cs; pr += 4) {   // four remote loads in flight; fixed order: identical H everywhere
-                    float v[4];
+                float4 s4 = make_float4(0.f, 0.f, 0.f, 0.f);
+                for (int pr = 0; pr < cs; pr += 4) {   // four remote loads in flight
+                    float4 v[4];
 #pragma unroll
-                    for (int q = 0; q < 4; ++q) v[q] = pr + q < cs ? ld_dsmem_f(mapa_u32(src, pr + q)) : 0.0f;
+                    for (int q = 0; q < 4; ++q)
+                        v[q] = pr + q < cs ? ld_dsmem_f4_nc(mapa_u32(src, pr + q)) : make_float4(0.f, 0.f, 0.f, 0.f);
 #pragma unroll
-                    for (int q = 0; q < 4; ++q) s += v[q];
+                    for (int q = 0; q < 4; ++q) { s4.x += v[q].x; s4.y += v[q].y; s4.z += v[q].z; s4.w += v[q].w; }
                 }
-                s = fminf(fmaxf(s, -65504.0f), 65504.0f);
-                const __half hv = __float2half_rn(s);
-                const uint32_t dsta = smem_u32(sH + m * hstride + j);
-                for (int pr = 0; pr < cs; ++pr) st_dsmem_u16(mapa_u32(dsta, pr), *reinterpret_cast<const uint16_t*>(&hv));
+                const __half2 h01 = __floats2half2_rn(fminf(fmaxf(s4.x, -65504.0f), 65504.0f), fminf(fmaxf(s4.y, -65504.0f), 65504.0f));
+                const __half2 h23 = __floats2half2_rn(fminf(fmaxf(s4.z, -65504.0f), 65504.0f), fminf(fmaxf(s4.w, -65504.0f), 65504.0f));
+                uint2 o;
+                o.x = *reinterpret_cast<const uint32_t*>(&h01);
+                o.y = *reinterpret_cast<const uint32_t*>(&h23);
+                *reinterpret_cast<uint2*>(sH + m * hstride + j) = o;
             }
             TWQ_DT(7);
-            cluster_arrive();                          // waited for after the residual items
+            cluster_arrive_relaxed();                  // this CTA no longer reads its peers (waited for before exit)
             TWQ_DT(8);
+            __syncthreads();
         } else {
             __syncthreads();
             for (int i = threadIdx.x; i < 16 * r; i += kDecThreads) {
@@ -437,8 +464,6 @@ __global__ void __launch_bounds__(kDecThreads, 1) decode_dual_linear_kernel(cons
     const int nloc = p.T * 16;                         // channels of this CTA (row stride of sYlr)
     if (r > 0) {
         TWQ_DT(10);
-        if (cs > 1) cluster_wait();                    // the full FP16 H is in this CTA's shared memory
-        TWQ_DT(11);
         // Ylr[m, n] = sum_j H[m,j] * L2T[n,j] for this CTA's channels, 8 channels per warp step
         for (int nt = warp; nt < ntile * 2; nt += kDecWarps) {
             float d[4] = {0.f, 0.f, 0.f, 0.f};
@@ -478,7 +503,7 @@ __global__ void __launch_bounds__(kDecThreads, 1) decode_dual_linear_kernel(cons
         const int m = i / (ntile * 16), nl = i - m * (ntile * 16);
         const int tl = nl >> 4, row = nl & 15;
         float y = 0.0f;
-        for (int pp = 0; pp < p.P; ++pp) y += sRes[(static_cast<size_t>(tl * p.P + pp) * 16 + row) * kTok + m];
+        for (int pp = 0; pp < P; ++pp) y += sRes[(static_cast<size_t>(tl * P + pp) * 16 + row) * kTok + m];
         if (r > 0) y += sYlr[m * nloc + nl];
         const size_t o = static_cast<size_t>(m) * p.ldy + tile0 * 16 + nl;
         if (p.ydt == 0) static_cast<__nv_bfloat16*>(p.Y)[o] = __float2bfloat16_rn(y);
@@ -486,8 +511,7 @@ __global__ void __launch_bounds__(kDecThreads, 1) decode_dual_linear_kernel(cons
         else static_cast<float*>(p.Y)[o] = y;
     }
     TWQ_DT(13);
-    // no trailing cluster barrier: the last remote access of any CTA precedes its second arrive, which
-    // every CTA has waited for
+    if (r > 0 && cs > 1) cluster_wait();               // no CTA exits while a peer may still read its partial
 }
 
 // ------------------------------------------------------------------------------------------------ host
@@ -590,13 +614,11 @@ bool decode_make_plan(int M, int N, int K, int r, int G, int num_sms, DecodePara
     if (nclusters < 1) nclusters = 1;
     p.grid = nclusters * p.cs;
     p.T = (p.n_tiles + p.grid - 1) / p.grid;
-    int P = 1;
-    while (P * p.T < kDecWarps && P * 2 <= p.ng && P < 16) P *= 2;
-    p.P = P;
-    if (p.T * p.P > kDecWarps * kMaxItemsPerWarp) return false;
+    p.P = p.ng < kDecWarps ? p.ng : kDecWarps;            // upper bound; each CTA takes 16 / (its tiles), see the kernel
+    if (p.T > kDecWarps * kMaxItemsPerWarp) return false;
     const int kTok = M <= 8 ? 8 : 16;
     int o = 0;
-    p.off_res = o; o += p.T * p.P * 16 * kTok * 4;
+    p.off_res = o; o += (p.T > kDecWarps ? p.T : kDecWarps) * 16 * kTok * 4;   // items <= max(16, T)
     p.off_hpart = o; o += 16 * r * 4;
     p.off_h = o; o += 16 * (r + 8) * 2;
     p.off_ylr = o; o += 16 * p.T * 16 * 4;
