@@ -424,8 +424,10 @@ __global__ void __launch_bounds__(kDecThreads, 1) decode_dual_linear_kernel(cons
         if (cs > 1) {
             cluster_wait();                            // every CTA's FP32 partial is visible
             TWQ_DT(6);
+            if (p.M <= 2) {
             // all-reduce by reading: every CTA sums the cs partials of the M live rows itself (fixed order, so
-            // H is identical everywhere) -- one cluster barrier instead of a reduce-scatter plus an all-gather
+            // H is identical everywhere) -- one cluster barrier instead of a reduce-scatter plus an all-gather.
+            // Distributed-shared-memory reads are slow (about 8 KB per microsecond per CTA here), so only for M <= 2.
             const int r4 = r >> 2;
             for (int i = threadIdx.x; i < p.M * r4; i += kDecThreads) {
                 const int m = i / r4, j = (i - m * r4) * 4;
@@ -445,6 +447,31 @@ __global__ void __launch_bounds__(kDecThreads, 1) decode_dual_linear_kernel(cons
                 o.x = *reinterpret_cast<const uint32_t*>(&h01);
                 o.y = *reinterpret_cast<const uint32_t*>(&h23);
                 *reinterpret_cast<uint2*>(sH + m * hstride + j) = o;
+            }
+            } else {
+                // reduce-scatter (this CTA sums r/cs columns of the M live rows over the cs partials, fixed
+                // order) + all-gather (the FP16 result goes to every CTA's sH)
+                const int jc = r / cs;
+                for (int i = threadIdx.x; i < p.M * jc; i += kDecThreads) {
+                    const int m = i / jc, j = rank * jc + (i - m * jc);
+                    const uint32_t src = smem_u32(sHpart + m * r + j);
+                    float s = 0.0f;
+                    for (int pr = 0; pr < cs; pr += 4) {
+                        float v[4];
+#pragma unroll
+                        for (int q = 0; q < 4; ++q) v[q] = pr + q < cs ? ld_dsmem_f(mapa_u32(src, pr + q)) : 0.0f;
+#pragma unroll
+                        for (int q = 0; q < 4; ++q) s += v[q];
+                    }
+                    s = fminf(fmaxf(s, -65504.0f), 65504.0f);
+                    const __half hv = __float2half_rn(s);
+                    const uint32_t dsta = smem_u32(sH + m * hstride + j);
+                    for (int pr = 0; pr < cs; ++pr) st_dsmem_u16(mapa_u32(dsta, pr), *reinterpret_cast<const uint16_t*>(&hv));
+                }
+                __syncthreads();
+                if (threadIdx.x == 0) fence_cluster();     // release this CTA's remote stores
+                cluster_arrive_relaxed();
+                cluster_wait();                            // every CTA's slice of H has arrived
             }
             TWQ_DT(7);
             cluster_arrive_relaxed();                  // this CTA no longer reads its peers (waited for before exit)
