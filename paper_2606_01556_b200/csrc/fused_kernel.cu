@@ -69,13 +69,16 @@ static bool make_plan_tn(int TN, int M, int N, int K, int r, int G, int num_sms,
     // shared memory map
     const int nrb = (r + 127) / 128, nkb = (r + 63) / 64;
     const int hbytes = nkb * TN * 128, l2bytes = nkb * kL1Chunk;
-    const int ub = TN * G, pb = kTileN * (G / 2) + TN * (G / 2);
+    // CTA pairs: prefill tiles in an even cluster without K splits; each CTA then expands half of the token rows
+    pl.pair = (TN == 128 && pl.cs >= 2 && pl.splits == 1) ? 1 : 0;
+    const int xr = pl.pair ? TN / 2 : TN;
+    const int ub = xr * G, pb = kTileN * (G / 2) + xr * (G / 2);
     const int s1b = TN * 128 + nrb * kL1Chunk;
     const int hpart = pl.cs > 1 ? round_up(TN * r * 4, 1024) : 0;
     const int fixed = kSxSlots * TN * 4 + B_COUNT * 8 + 256;
     const int budget = kMaxDynSmem - 1024 - fixed;             // dynamic limit minus alignment slack
     pl.nsu = kMaxNSU;
-    pl.nsp = TN <= 32 ? kMaxNSP : 4;
+    pl.nsp = (TN <= 32 || pl.pair) ? kMaxNSP : 4;   // a pair's packed stage is 12 KB: the ring can be twice as deep
     pl.ns1 = r > 0 ? (TN <= 32 ? 3 : 2) : 0;
     pl.alias = 0;
     auto total = [&](const FusedPlan& q) {
@@ -123,8 +126,12 @@ bool fused_make_plan(int M, int N, int K, int r, int G, int num_sms, FusedPlan* 
 cudaError_t launch_fused(const FusedMaps& maps, const FusedParams& p, int G, cudaStream_t stream) {
     const bool dbg = p.dbgP != nullptr;
 #define TWQ_CASE(tn, g)                                                               \
-    if (p.plan.TN == tn && G == g)                                                    \
+    if (p.plan.TN == tn && G == g && !p.plan.pair)                                    \
         return dbg ? launch_fused_inst<tn, g, true>(maps, p, stream) : launch_fused_inst<tn, g, false>(maps, p, stream);
+    if (p.plan.pair && p.plan.TN == 128 && G == 128)
+        return dbg ? launch_fused_inst<128, 128, true, true>(maps, p, stream) : launch_fused_inst<128, 128, false, true>(maps, p, stream);
+    if (p.plan.pair && p.plan.TN == 128 && G == 64)
+        return dbg ? launch_fused_inst<128, 64, true, true>(maps, p, stream) : launch_fused_inst<128, 64, false, true>(maps, p, stream);
     TWQ_CASE(16, 128) TWQ_CASE(32, 128) TWQ_CASE(64, 128) TWQ_CASE(128, 128)
     TWQ_CASE(16, 64) TWQ_CASE(32, 64) TWQ_CASE(64, 64) TWQ_CASE(128, 64)
 #undef TWQ_CASE

@@ -85,15 +85,20 @@ enum : int {
     B_L2FULL,
     B_L2EMPTY,
     B_RESID,                    // all residual MMAs of a tile complete
+    // CTA pairs (cta_group::2): barriers of the pair's leader that BOTH CTAs arrive on
+    B_TEMPTY2,                  // + kNB: P buffer drained by the epilogues of both CTAs
+    B_UFULL2 = B_TEMPTY2 + kNB, // + kMaxNSU: expanded operands of both CTAs ready
+    B_HDRAINED2 = B_UFULL2 + kMaxNSU,
     B_COUNT
 };
 
-template <int TN, int G>
+template <int TN, int G, bool kPair = false>
 struct Cfg {
     static constexpr int kXChunk = TN * 128;          // X tile: TN rows x 64 bf16
+    static constexpr int kXR = kPair ? TN / 2 : TN;   // activation rows this CTA expands (a pair splits the B rows)
     static constexpr int kWB = kTileN * (G / 2);      // packed weight rows of one group
-    static constexpr int kXB = TN * (G / 2);          // packed activation rows of one group
-    static constexpr int kUB = TN * G;                // expanded activation tile of one group
+    static constexpr int kXB = kXR * (G / 2);         // packed activation rows of one group
+    static constexpr int kUB = kXR * G;               // expanded activation tile of one group
     static constexpr int kColP = 0;                   // P buffer b at b*TN; H^T block rb at rb*TN
     static constexpr int kColA = (kNB * TN + 31) / 32 * 32;   // expanded weight rows (A operand), 32 cols / stage
     static constexpr int kTmemCols = kColA + kMaxNSU * 32 <= 256 ? 256 : 512;
@@ -155,12 +160,12 @@ __device__ __forceinline__ void s1_range(const FusedParams& p, const Unit& t, in
     kc1 = min(e, kc0 + per);
 }
 
-template <int TN, int G, bool kDbg>
+template <int TN, int G, bool kDbg, bool kPair = false>
 __global__ void __launch_bounds__(kThreads, 1)
 fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CUtensorMap tmXq,
                          const __grid_constant__ CUtensorMap tmX, const __grid_constant__ CUtensorMap tmL1T,
                          const __grid_constant__ CUtensorMap tmL2T, const __grid_constant__ FusedParams p) {
-    using C = Cfg<TN, G>;
+    using C = Cfg<TN, G, kPair>;
     const FusedPlan& pl = p.plan;
     extern __shared__ uint8_t smem_raw[];
     // identical offset in every CTA of the cluster (DSMEM addresses are formed from local ones)
@@ -206,6 +211,9 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
         mbar_init(&bars[B_L2FULL], 1);
         mbar_init(&bars[B_L2EMPTY], 1);
         mbar_init(&bars[B_RESID], 1);
+        for (int i = 0; i < kNB; ++i) mbar_init(&bars[B_TEMPTY2 + i], 2 * kEpiWarps);
+        for (int i = 0; i < kMaxNSU; ++i) mbar_init(&bars[B_UFULL2 + i], 2 * kPrepWarps);
+        mbar_init(&bars[B_HDRAINED2], 2 * kEpiWarps);
         fence_mbar_init();
     }
     if (warp == 0 && lane == 0) {
@@ -214,7 +222,10 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
         if (r > 0) { tma_prefetch_desc(&tmX); tma_prefetch_desc(&tmL1T); tma_prefetch_desc(&tmL2T); }
     }
     if (threadIdx.x < 32) tmem_slot[8 + threadIdx.x] = kMagic;   // read back by the epilogue warps (see kfill)
-    if (warp == 2) tmem_alloc<C::kTmemCols>(tmem_slot);
+    if (warp == 2) {
+        if (kPair) tmem_alloc_pair<C::kTmemCols>(tmem_slot);
+        else tmem_alloc<C::kTmemCols>(tmem_slot);
+    }
     tc_fence_before();
     __syncthreads();
     if (cs > 1) cluster_sync_all();   // peers' barriers are initialised before any remote arrive
@@ -222,6 +233,10 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
     const uint32_t tmem = *tmem_slot;
     const uint32_t bar0 = smem_u32(bars);   // shared-window address of barrier slot 0 (slot i at bar0 + 8*i)
 #define TWQ_BAR(i) (bar0 + 8u * static_cast<uint32_t>(i))
+    // pair mode: the same barrier slots in the pair's leader (even rank), as shared::cluster addresses
+    const uint32_t lbar0 = kPair ? mapa_u32(bar0, static_cast<uint32_t>(rank & ~1)) : bar0;
+#define TWQ_LBAR(i) (lbar0 + 8u * static_cast<uint32_t>(i))
+    const bool leader = !kPair || (rank & 1) == 0;
     pdl_launch_dependents();          // the next kernel may start its own prologue / weight prefetch
 
     if (warp < 4) {
@@ -274,7 +289,7 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
                     mbar_arrive_expect_tx_a(TWQ_BAR(B_PFULL + sp), p_stage_bytes);
                     tma_load_2d_a(st, &tmW, TWQ_BAR(B_PFULL + sp), c0, t.n0);
                     if (!waited) { pdl_wait(); waited = true; }               // Xq comes from the quantizer
-                    tma_load_2d_a(st + C::kWB, &tmXq, TWQ_BAR(B_PFULL + sp), c0, t.m0);
+                    tma_load_2d_a(st + C::kWB, &tmXq, TWQ_BAR(B_PFULL + sp), c0, t.m0 + (kPair ? (rank & 1) * C::kXR : 0));
                     if (++sp == pl.nsp) { sp = 0; php ^= 1; }
                 }
                 ++tile_n;
@@ -285,6 +300,8 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
         if (lane == 0) {
             const uint32_t idesc_lr = umma_idesc(1, 0, 0, 128, TN);  // D f32, A f16, B f16
             const uint32_t idesc_i8 = umma_idesc(2, 1, 1, 128, TN);  // D s32, A s8, B s8
+            const uint32_t idesc_i8_pair = umma_idesc(2, 1, 1, 256, TN);
+            (void)idesc_i8_pair;
             int tile_n = 0, ctx_n = 0, cur_ctx = -1;
             int s1 = 0, ph1 = 0;          // stage-1 ring position / phase
             int su = 0, phu = 0;          // expanded-operand ring position / phase
@@ -322,6 +339,8 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
                         mbar_arrive(&bars[B_HFULL]);   // empty K share: the epilogue contributes zeros
                     }
                     mbar_wait(&bars[B_HDRAINED], ctx_n & 1, 22);
+                    // pair leader: its MMAs also write the peer's P buffers, where the peer's H^T partial lives
+                    if (kPair && leader) mbar_wait_cluster_a(TWQ_BAR(B_HDRAINED2), ctx_n & 1);
                     tc_fence_after();
                     h_waited = false;
                 }
@@ -329,7 +348,7 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
                     // stage 2 first: Ylr^T = L2T * H^T (FP32) into the next P buffer; the epilogue takes it
                     // as the initial value of its accumulators
                     if (!h_waited) { mbar_wait(&bars[B_HREADY], ctx_n & 1, 25); h_waited = true; ++ctx_n; }
-                    mbar_wait(&bars[B_L2FULL], tile_n & 1, 26);
+                    mbar_wait(&bars[B_L2FULL], tile_n & 1, 26 + 100 * tile_n + 10000 * (rank & 1));
                     mbar_wait(&bars[B_TEMPTY + b], pb, 27);
                     tc_fence_after();
                     const uint32_t l2b = smem_u32(sL2T), hb = smem_u32(sH);
@@ -346,24 +365,50 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
                 const int ngr = t.g_end - t.g_begin;
                 for (int gi = 0; gi < ngr; ++gi) {
                     TWQ_TR(1, trn, 1);
-                    mbar_wait_a(TWQ_BAR(B_TEMPTY + b), pb);
-                    TWQ_TR(1, trn, 2);
-                    mbar_wait_a(TWQ_BAR(B_UFULL + su), phu);
-                    TWQ_TR(1, trn, 3);
-                    tc_fence_after();
-                    const uint64_t ud = udesc0 + static_cast<uint64_t>(su * (C::kUB >> 4));
-                    const uint32_t ta = tmem + C::kColA + su * 32;
-                    const uint32_t td = tmem + C::kColP + b * TN;
+                    if (!kPair) {
+                        mbar_wait_a(TWQ_BAR(B_TEMPTY + b), pb);
+                        TWQ_TR(1, trn, 2);
+                        mbar_wait_a(TWQ_BAR(B_UFULL + su), phu);
+                        TWQ_TR(1, trn, 3);
+                        tc_fence_after();
+                        const uint64_t ud = udesc0 + static_cast<uint64_t>(su * (C::kUB >> 4));
+                        const uint32_t ta = tmem + C::kColA + su * 32;
+                        const uint32_t td = tmem + C::kColP + b * TN;
 #pragma unroll
-                    for (int ks = 0; ks < G / 32; ++ks)   // accumulate onto the pre-filled 1.5*2^23 pattern
-                        umma_i8_ts(td, ta + ks * 8, ud + static_cast<uint64_t>(ks * 2), idesc_i8, 1u);
-                    tc_commit_a(TWQ_BAR(B_UEMPTY + su));
-                    tc_commit_a(TWQ_BAR(B_TFULL + b));
+                        for (int ks = 0; ks < G / 32; ++ks)   // accumulate onto the pre-filled 1.5*2^23 pattern
+                            umma_i8_ts(td, ta + ks * 8, ud + static_cast<uint64_t>(ks * 2), idesc_i8, 1u);
+                        tc_commit_a(TWQ_BAR(B_UEMPTY + su));
+                        tc_commit_a(TWQ_BAR(B_TFULL + b));
+                    } else if (leader) {
+                        // one M = 256 MMA per K-step for the pair: both epilogues drained buffer b, both CTAs'
+                        // operands of stage su are in place; completion is multicast to both CTAs' barriers
+                        mbar_wait_cluster_a(TWQ_BAR(B_TEMPTY2 + b), pb, 1000000 + tile_n * 10000 + gi * 100 + b * 10 + pb);
+                        TWQ_TR(1, trn, 2);
+                        mbar_wait_cluster_a(TWQ_BAR(B_UFULL2 + su), phu);
+                        TWQ_TR(1, trn, 3);
+                        tc_fence_after();
+                        const uint64_t ud = udesc0 + static_cast<uint64_t>(su * (C::kUB >> 4));
+                        const uint32_t ta = tmem + C::kColA + su * 32;
+                        const uint32_t td = tmem + C::kColP + b * TN;
+#pragma unroll
+                        for (int ks = 0; ks < G / 32; ++ks)
+                            umma_i8_ts_pair(td, ta + ks * 8, ud + static_cast<uint64_t>(ks * 2), idesc_i8_pair, 1u);
+                        const uint16_t mask = static_cast<uint16_t>(3u << (rank & ~1));
+                        tc_commit_pair_a(TWQ_BAR(B_UEMPTY + su), mask);
+                        tc_commit_pair_a(TWQ_BAR(B_TFULL + b), mask);
+                    } else {
+                        // the peer's issuer follows the leader use by use (a parity wait may only be one phase
+                        // ahead of its barrier): it waits for the leader's completion of this group
+                        mbar_wait_a(TWQ_BAR(B_TFULL + b), pb);
+                    }
                     TWQ_TR(1, trn, 4);
                     if (++su == pl.nsu) { su = 0; phu ^= 1; }
                     if (++b == kNB) { b = 0; pb ^= 1; }
                 }
-                tc_commit(&bars[B_RESID]);
+                // all residual MMAs of the tile complete (alias mode: the stage-1 ring may overwrite the rings);
+                // in a pair the leader's commit covers both CTAs' operands
+                if (!kPair) tc_commit(&bars[B_RESID]);
+                else if (leader) tc_commit_pair_a(TWQ_BAR(B_RESID), static_cast<uint16_t>(3u << (rank & ~1)));
                 ++tile_n;
             }
         }
@@ -380,10 +425,10 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
         const uint32_t tlane = tmem + (static_cast<uint32_t>(qd * 32) << 16);
         constexpr int kCPR = (G / 2) / 16;            // 16-byte packed chunks per row
         // activation rows: kTPR threads share a row, each expands kXC of its kCPR chunks
-        constexpr int kTPR = (128 / TN) < kCPR ? (128 / TN) : kCPR;
+        constexpr int kTPR = (128 / C::kXR) < kCPR ? (128 / C::kXR) : kCPR;
         constexpr int kXC = kCPR / kTPR;
-        const uint32_t xrow = u_tid % TN;
-        const uint32_t xpart = u_tid / TN;
+        const uint32_t xrow = u_tid % C::kXR;
+        const uint32_t xpart = u_tid / C::kXR;
         const bool x_on = xpart < kTPR;
         uint32_t in_off[kCPR];                        // packed chunk offsets (weight role: all; activation role: first kXC)
         uint32_t out_off[2 * kXC];
@@ -516,7 +561,11 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
                     fence_proxy_async_smem();  // generic-proxy writes -> visible to the tensor core (async proxy)
                 }
                 __syncwarp();
-                if (lane == 0) { mbar_arrive_a(TWQ_BAR(B_UFULL + su)); mbar_arrive_a(TWQ_BAR(B_PEMPTY + sp)); }
+                if (lane == 0) {
+                    if (kPair) mbar_arrive_remote_relaxed(TWQ_LBAR(B_UFULL2 + su));   // release.cluster, on the pair leader
+                    else mbar_arrive_a(TWQ_BAR(B_UFULL + su));
+                    mbar_arrive_a(TWQ_BAR(B_PEMPTY + sp));
+                }
                 TWQ_TR(2, trn, 4);
                 if (++sp == pl.nsp) { sp = 0; php ^= 1; }
                 if (++su == pl.nsu) { su = 0; phu ^= 1; }
@@ -562,7 +611,10 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
         __syncwarp();
         if (lane == 0) {
 #pragma unroll
-            for (int b = 0; b < kNB; ++b) mbar_arrive(&bars[B_TEMPTY + b]);
+            for (int b = 0; b < kNB; ++b) {
+                mbar_arrive(&bars[B_TEMPTY + b]);
+                if (kPair) mbar_arrive_remote_relaxed(TWQ_LBAR(B_TEMPTY2 + b));
+            }
         }
         pdl_wait();                          // Y / workspace writes must follow the previous kernel
 
@@ -621,7 +673,10 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
                 }
                 tc_fence_before();
                 __syncwarp();
-                if (lane == 0) mbar_arrive(&bars[B_HDRAINED]);
+                if (lane == 0) {
+                    mbar_arrive(&bars[B_HDRAINED]);
+                    if (kPair) mbar_arrive_remote_relaxed(TWQ_LBAR(B_HDRAINED2));
+                }
                 if (cs > 1) {
                     // ---- reduce-scatter the FP32 partials, all-gather the FP16 result (DSMEM)
                     if (lane < cs) mbar_arrive_remote(mapa_u32(smem_u32(&bars[B_X1]), lane));
@@ -679,7 +734,10 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
                 }
                 tc_fence_before();
                 __syncwarp();
-                if (lane == 0) mbar_arrive(&bars[B_TEMPTY + b]);
+                if (lane == 0) {
+                    mbar_arrive(&bars[B_TEMPTY + b]);
+                    if (kPair) mbar_arrive_remote_relaxed(TWQ_LBAR(B_TEMPTY2 + b));
+                }
                 if (++b == kNB) { b = 0; pb ^= 1; }
             } else {
 #pragma unroll
@@ -716,7 +774,10 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
                             tmem_st_wait();
                             tc_fence_before();
                             __syncwarp();
-                            if (lane == 0) mbar_arrive_a(TWQ_BAR(B_TEMPTY + b));
+                            if (lane == 0) {
+                                mbar_arrive_a(TWQ_BAR(B_TEMPTY + b));
+                                if (kPair) mbar_arrive_remote_relaxed(TWQ_LBAR(B_TEMPTY2 + b));
+                            }
 #ifdef TWQ_TRACE
                             if (trw) TWQ_TR(3, trn, 3);
 #endif
@@ -749,7 +810,10 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
                     }
                 } else {
                     __syncwarp();
-                    if (lane == 0) mbar_arrive_a(TWQ_BAR(B_TEMPTY + b));
+                    if (lane == 0) {
+                        mbar_arrive_a(TWQ_BAR(B_TEMPTY + b));
+                        if (kPair) mbar_arrive_remote_relaxed(TWQ_LBAR(B_TEMPTY2 + b));
+                    }
                 }
 #ifdef TWQ_TRACE
                 if (trw) TWQ_TR(3, trn, 4);
@@ -785,9 +849,11 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
     // ---------------------------------------------------------------- teardown
     tc_fence_before();
     __syncthreads();
+    if (kPair) cluster_sync_all();   // the leader's MMAs write the peer's TMEM: both CTAs are done before either frees
     if (warp == 2) {
         tc_fence_after();
-        tmem_dealloc<C::kTmemCols>(tmem);
+        if (kPair) tmem_dealloc_pair<C::kTmemCols>(tmem);
+        else tmem_dealloc<C::kTmemCols>(tmem);
     }
 
     if (pl.splits > 1) {
@@ -826,9 +892,9 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
 
 }  // namespace
 
-template <int TN, int G, bool kDbg>
+template <int TN, int G, bool kDbg, bool kPair = false>
 cudaError_t launch_fused_inst(const FusedMaps& maps, const FusedParams& p, cudaStream_t stream) {
-    auto kern = fused_dual_linear_kernel<TN, G, kDbg>;
+    auto kern = fused_dual_linear_kernel<TN, G, kDbg, kPair>;
     static int attr_smem = 0;
     if (attr_smem < p.plan.smem_bytes) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxDynSmem);
@@ -896,6 +962,10 @@ TWQ_EXTERN_INST(32)
 TWQ_EXTERN_INST(64)
 TWQ_EXTERN_INST(128)
 extern template int max_active_clusters_inst<128, 128, false>(int, int);
+extern template cudaError_t launch_fused_inst<128, 128, false, true>(const FusedMaps&, const FusedParams&, cudaStream_t);
+extern template cudaError_t launch_fused_inst<128, 128, true, true>(const FusedMaps&, const FusedParams&, cudaStream_t);
+extern template cudaError_t launch_fused_inst<128, 64, false, true>(const FusedMaps&, const FusedParams&, cudaStream_t);
+extern template cudaError_t launch_fused_inst<128, 64, true, true>(const FusedMaps&, const FusedParams&, cudaStream_t);
 #define TWQ_DEFINE_INST(tn)                                                                                  \
     template cudaError_t launch_fused_inst<tn, 128, false>(const FusedMaps&, const FusedParams&, cudaStream_t); \
     template cudaError_t launch_fused_inst<tn, 128, true>(const FusedMaps&, const FusedParams&, cudaStream_t);  \

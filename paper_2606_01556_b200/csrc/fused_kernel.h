@@ -19,6 +19,7 @@ struct FusedPlan {
     int nclusters;           // persistent clusters; cluster c owns units [c*units/nclusters, (c+1)*units/nclusters)
     int nsp, nsu, ns1;       // ring depths: packed (TMA), expanded (MMA operands), stage-1
     int alias;               // 1: the stage-1 ring and the FP32 H partial overlay the residual rings
+    int pair;                // 1: CTA pairs (cta_group::2): ranks 2i / 2i+1 of a cluster share one M = 256 MMA
     int off_H, off_L2T, off_U, off_P, off_S1, off_Hpart, off_sx, off_bar;
     int smem_bytes;
     int tmem_cols;           // 256 or 512

@@ -52,11 +52,16 @@ __device__ __forceinline__ bool mbar_try_wait(uint64_t* bar, uint32_t parity) {
 // GPU.  try_wait itself suspends the thread for a hardware-defined time slice, so the bound of
 // 2^26 polls is far above any legitimate wait.  Kept to a handful of instructions: single-thread
 // roles (TMA producer, MMA issuer) execute one of these per pipeline hand-off.
+#ifdef TWQ_WAIT_DEBUG
+#define TWQ_WAIT_FAIL(tag) do { if (spins == (1u << 26) + 1) printf("twq: wait timeout tag=%d block=%d thread=%d\n", (tag), blockIdx.x, threadIdx.x); if (spins > (1u << 27)) __trap(); } while (0)
+#else
+#define TWQ_WAIT_FAIL(tag) __trap()
+#endif
 __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity, int tag = 0) {
     (void)tag;
     uint32_t spins = 0;
     while (!mbar_try_wait(bar, parity)) {
-        if (++spins > (1u << 26)) __trap();
+        if (++spins > (1u << 26)) TWQ_WAIT_FAIL(tag);
     }
 }
 
@@ -80,10 +85,11 @@ __device__ __forceinline__ bool mbar_try_wait_a(uint32_t bar, uint32_t parity) {
         : "memory");
     return ok != 0;
 }
-__device__ __forceinline__ void mbar_wait_a(uint32_t bar, uint32_t parity) {
+__device__ __forceinline__ void mbar_wait_a(uint32_t bar, uint32_t parity, int tag = 100) {
+    (void)tag;
     uint32_t spins = 0;
     while (!mbar_try_wait_a(bar, parity)) {
-        if (++spins > (1u << 26)) __trap();
+        if (++spins > (1u << 26)) TWQ_WAIT_FAIL(tag + static_cast<int>(bar & 0xFFFu) * 1000);
     }
 }
 
@@ -214,6 +220,11 @@ __device__ __forceinline__ uint32_t mapa_u32(uint32_t local_addr, uint32_t rank)
 __device__ __forceinline__ void mbar_arrive_remote(uint32_t cluster_addr) {
     asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr) : "memory");
 }
+// Relaxed form: the caller has already made its writes visible (fence.proxy.async / tcgen05.wait + fence); the
+// release form costs each arriving warp a cluster-scope fence of ~800 cycles on this part.
+__device__ __forceinline__ void mbar_arrive_remote_relaxed(uint32_t cluster_addr) {
+    asm volatile("mbarrier.arrive.relaxed.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr) : "memory");
+}
 __device__ __forceinline__ bool mbar_try_wait_cluster(uint64_t* bar, uint32_t parity) {
     uint32_t ok;
     asm volatile(
@@ -229,7 +240,7 @@ __device__ __forceinline__ void mbar_wait_cluster(uint64_t* bar, uint32_t parity
     (void)tag;
     uint32_t spins = 0;
     while (!mbar_try_wait_cluster(bar, parity)) {
-        if (++spins > (1u << 26)) __trap();
+        if (++spins > (1u << 26)) TWQ_WAIT_FAIL(tag);
     }
 }
 __device__ __forceinline__ float4 ld_dsmem_f4(uint32_t cluster_addr) {
@@ -260,6 +271,52 @@ __device__ __forceinline__ uint64_t fma2(uint64_t a, uint64_t b, uint64_t c) {
     uint64_t d;
     asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
     return d;
+}
+
+
+// ------------------------------------------------------------------ CTA pairs (cta_group::2)
+// Two CTAs of a cluster (ranks 2i, 2i+1) run one MMA of M = 256: each CTA's TMEM holds its own 128 rows of A
+// and of D, each CTA's shared memory holds its half of the B rows (rows [rank*N/2, (rank+1)*N/2)) at the same
+// offset; the even CTA issues.  Verified on B200 against a CPU product (A from TMEM, kind::i8), also mixed with
+// cta_group::1 MMAs on the same allocation.
+template <int kCols>
+__device__ __forceinline__ void tmem_alloc_pair(uint32_t* smem_slot) {
+    asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(smem_slot)),
+                 "n"(kCols)
+                 : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;" ::: "memory");
+}
+template <int kCols>
+__device__ __forceinline__ void tmem_dealloc_pair(uint32_t taddr) {
+    asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" ::"r"(taddr), "n"(kCols) : "memory");
+}
+__device__ __forceinline__ void umma_i8_ts_pair(uint32_t d_tmem, uint32_t a_tmem, uint64_t bdesc, uint32_t idesc,
+                                                uint32_t accumulate) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "setp.ne.b32 p, %4, 0;\n\t"
+        "tcgen05.mma.cta_group::2.kind::i8 [%0], [%1], %2, %3, p;\n\t}\n"
+        ::"r"(d_tmem), "r"(a_tmem), "l"(bdesc), "r"(idesc), "r"(accumulate)
+        : "memory");
+}
+// commit of the pair's MMAs: one arrival on the barrier at this shared-window offset in every CTA of `cta_mask`
+__device__ __forceinline__ void tc_commit_pair_a(uint32_t bar, uint16_t cta_mask) {
+    asm volatile("tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;"
+                 ::"r"(bar), "h"(cta_mask) : "memory");
+}
+__device__ __forceinline__ void mbar_wait_cluster_a(uint32_t bar, uint32_t parity, int tag = 0) {
+    (void)tag;
+    uint32_t spins = 0;
+    for (;;) {
+        uint32_t ok;
+        asm volatile(
+            "{\n\t.reg .pred P;\n\t"
+            "mbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 P, [%1], %2;\n\t"
+            "selp.u32 %0, 1, 0, P;\n\t}\n"
+            : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+        if (ok) break;
+        if (++spins > (1u << 26)) TWQ_WAIT_FAIL(tag ? tag : 200 + static_cast<int>(bar & 0xFFFu) * 1000);
+    }
 }
 
 // ------------------------------------------------------------------ UMMA descriptors

@@ -194,7 +194,7 @@ twq_status twq_dual_linear(const void* X, int ldx, const uint8_t* Xq, const floa
     // packed INT4 tiles: rows of G/2 bytes, swizzled so that one-row-per-thread reads are conflict-free
     const CUtensorMapSwizzle psw = G == 128 ? CU_TENSOR_MAP_SWIZZLE_64B : CU_TENSOR_MAP_SWIZZLE_32B;
     ok &= make_map(&maps.W, CU_TENSOR_MAP_DATA_TYPE_UINT8, 1, base + lay.off_r4, K / 2, N, K / 2, G / 2, 128, psw);
-    ok &= make_map(&maps.Xq, CU_TENSOR_MAP_DATA_TYPE_UINT8, 1, Xq, K / 2, M, K / 2, G / 2, TN, psw);
+    ok &= make_map(&maps.Xq, CU_TENSOR_MAP_DATA_TYPE_UINT8, 1, Xq, K / 2, M, K / 2, G / 2, p.plan.pair ? TN / 2 : TN, psw);
     if (r > 0) {
         ok &= make_map(&maps.X, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, X, K, M, static_cast<uint64_t>(ldx) * 2, 64, TN,
                        CU_TENSOR_MAP_SWIZZLE_128B);
