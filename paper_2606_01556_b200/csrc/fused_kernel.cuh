@@ -53,11 +53,15 @@ namespace {
 constexpr int kThreads = 640;
 constexpr int kPrepWarps = 8;           // warps 4..7 expand weight rows, warps 8..11 expand activation rows
 constexpr int kPrepThreads = kPrepWarps * 32;
-constexpr int kEpiWarp0 = 12;           // first epilogue warp (a multiple of 4: TMEM lane quarter = warp % 4)
+constexpr int kEpiWarp0 = 8;            // first epilogue warp (a multiple of 4: TMEM lane quarter = warp % 4)
+// The single-thread roles get the HIGHEST warp ids: the warp scheduler of a sub-partition favours higher warp
+// ids, and with the issuer in warp 1 every step of its loop waited ~300 cycles for an issue slot behind the
+// spinning / streaming warps of its sub-partition (in-kernel timeline, r01b).
+constexpr int kCtlWarp0 = 16;           // 16 TMA producer, 17 MMA issuer, 18 TMEM allocator, 19 idle
 constexpr int kEpiWarps = 8;            // warps 12..19
 // register budgets after setmaxnreg: the pool is what the CTA was launched with (640 x 96 = 61440);
-// 128*40 + 256*64 + 256*152 = 60416
-constexpr int kRegsCtl = 40, kRegsPrep = 64, kRegsEpi = 152;
+// 128*40 + 256*56 + 256*160 = 60416
+constexpr int kRegsCtl = 40, kRegsPrep = 56, kRegsEpi = 160;
 constexpr int kTileN = 128;             // output channels per CTA (MMA M)
 constexpr int kSxSlots = 16;            // per-group activation-scale slots (two blocks of 8 groups)
 constexpr int kNB = 3;                  // P accumulator buffers in rotation
@@ -216,13 +220,13 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
         mbar_init(&bars[B_HDRAINED2], 2 * kEpiWarps);
         fence_mbar_init();
     }
-    if (warp == 0 && lane == 0) {
+    if (warp == kCtlWarp0 && lane == 0) {
         tma_prefetch_desc(&tmW);
         tma_prefetch_desc(&tmXq);
         if (r > 0) { tma_prefetch_desc(&tmX); tma_prefetch_desc(&tmL1T); tma_prefetch_desc(&tmL2T); }
     }
     if (threadIdx.x < 32) tmem_slot[8 + threadIdx.x] = kMagic;   // read back by the epilogue warps (see kfill)
-    if (warp == 2) {
+    if (warp == kCtlWarp0 + 2) {
         if (kPair) tmem_alloc_pair<C::kTmemCols>(tmem_slot);
         else tmem_alloc<C::kTmemCols>(tmem_slot);
     }
@@ -239,9 +243,9 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
     const bool leader = !kPair || (rank & 1) == 0;
     pdl_launch_dependents();          // the next kernel may start its own prologue / weight prefetch
 
-    if (warp < 4) {
+    if (warp >= kCtlWarp0) {
         reg_dec<kRegsCtl>();
-    if (warp == 0) {
+    if (warp == kCtlWarp0) {
         // ================================================================ TMA producer
         if (lane == 0) {
             int tile_n = 0, ctx_n = 0, cur_ctx = -1;
@@ -295,9 +299,13 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
                 ++tile_n;
             }
         }
-    } else if (warp == 1) {
-        // ================================================================ MMA issuer (one thread)
-        if (lane == 0) {
+    } else if (warp == kCtlWarp0 + 1) {
+        // ================================================================ MMA issuer
+        // The whole warp runs the loop converged and one elected lane issues: inside an `if (lane == 0)` region
+        // the compiler wraps EVERY tcgen05 instruction in its own elect / branch loop (~50 cycles each), which
+        // together with two dependent barrier polls (~150 cycles each even when already complete) made the
+        // issuer itself the slowest stage of the pipeline (in-kernel timeline + micro-benchmark, r01b).
+        {
             const uint32_t idesc_lr = umma_idesc(1, 0, 0, 128, TN);  // D f32, A f16, B f16
             const uint32_t idesc_i8 = umma_idesc(2, 1, 1, 128, TN);  // D s32, A s8, B s8
             const uint32_t idesc_i8_pair = umma_idesc(2, 1, 1, 256, TN);
@@ -326,17 +334,22 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
                             tc_fence_after();
                             const uint32_t xb = smem_u32(sS1 + s1 * s1_stage_bytes);
                             const uint32_t lb = xb + C::kXChunk;
+                            if (elect_one()) {
 #pragma unroll
-                            for (int ks = 0; ks < 4; ++ks)
-                                for (int rb = 0; rb < nrb; ++rb)
-                                    umma_f16(tmem + C::kColP + rb * TN, umma_smem_desc<128>(lb + rb * kL1Chunk + ks * 32),
-                                             umma_smem_desc<128>(xb + ks * 32), idesc_lr, (kc != kc0 || ks != 0) ? 1u : 0u);
-                            tc_commit(&bars[B_EMPTY1 + s1]);
+                                for (int ks = 0; ks < 4; ++ks)
+                                    for (int rb = 0; rb < nrb; ++rb)
+                                        umma_f16(tmem + C::kColP + rb * TN, umma_smem_desc<128>(lb + rb * kL1Chunk + ks * 32),
+                                                 umma_smem_desc<128>(xb + ks * 32), idesc_lr, (kc != kc0 || ks != 0) ? 1u : 0u);
+                                tc_commit(&bars[B_EMPTY1 + s1]);
+                            }
+                            __syncwarp();
                             if (++s1 == pl.ns1) { s1 = 0; ph1 ^= 1; }
                         }
-                        tc_commit(&bars[B_HFULL]);
+                        if (elect_one()) tc_commit(&bars[B_HFULL]);
+                        __syncwarp();
                     } else {
-                        mbar_arrive(&bars[B_HFULL]);   // empty K share: the epilogue contributes zeros
+                        if (elect_one()) mbar_arrive(&bars[B_HFULL]);   // empty K share: the epilogue contributes zeros
+                        __syncwarp();
                     }
                     mbar_wait(&bars[B_HDRAINED], ctx_n & 1, 22);
                     // pair leader: its MMAs also write the peer's P buffers, where the peer's H^T partial lives
@@ -353,49 +366,66 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
                     tc_fence_after();
                     const uint32_t l2b = smem_u32(sL2T), hb = smem_u32(sH);
                     const int nks = (r + 15) >> 4;
-                    for (int ks = 0; ks < nks; ++ks) {
-                        const int kb = ks >> 2, kk = ks & 3;
-                        umma_f16(tmem + C::kColP + b * TN, umma_smem_desc<128>(l2b + kb * kL1Chunk + kk * 32),
-                                 umma_smem_desc<128>(hb + kb * (TN * 128) + kk * 32), idesc_lr, ks != 0 ? 1u : 0u);
+                    if (elect_one()) {
+                        for (int ks = 0; ks < nks; ++ks) {
+                            const int kb = ks >> 2, kk = ks & 3;
+                            umma_f16(tmem + C::kColP + b * TN, umma_smem_desc<128>(l2b + kb * kL1Chunk + kk * 32),
+                                     umma_smem_desc<128>(hb + kb * (TN * 128) + kk * 32), idesc_lr, ks != 0 ? 1u : 0u);
+                        }
+                        tc_commit(&bars[B_L2EMPTY]);
+                        tc_commit(&bars[B_TFULL + b]);
                     }
-                    tc_commit(&bars[B_L2EMPTY]);
-                    tc_commit(&bars[B_TFULL + b]);
+                    __syncwarp();
                     if (++b == kNB) { b = 0; pb ^= 1; }
                 }
                 const int ngr = t.g_end - t.g_begin;
                 for (int gi = 0; gi < ngr; ++gi) {
                     TWQ_TR(1, trn, 1);
                     if (!kPair) {
-                        mbar_wait_a(TWQ_BAR(B_TEMPTY + b), pb);
-                        TWQ_TR(1, trn, 2);
-                        mbar_wait_a(TWQ_BAR(B_UFULL + su), phu);
+                        {   // both polls in flight together
+                            const bool ok1 = mbar_try_wait_a(TWQ_BAR(B_TEMPTY + b), pb);
+                            const bool ok2 = mbar_try_wait_a(TWQ_BAR(B_UFULL + su), phu);
+                            if (!ok1) mbar_wait_a(TWQ_BAR(B_TEMPTY + b), pb);
+                            TWQ_TR(1, trn, 2);
+                            if (!ok2) mbar_wait_a(TWQ_BAR(B_UFULL + su), phu);
+                        }
                         TWQ_TR(1, trn, 3);
                         tc_fence_after();
                         const uint64_t ud = udesc0 + static_cast<uint64_t>(su * (C::kUB >> 4));
                         const uint32_t ta = tmem + C::kColA + su * 32;
                         const uint32_t td = tmem + C::kColP + b * TN;
+                        if (elect_one()) {
 #pragma unroll
-                        for (int ks = 0; ks < G / 32; ++ks)   // accumulate onto the pre-filled 1.5*2^23 pattern
-                            umma_i8_ts(td, ta + ks * 8, ud + static_cast<uint64_t>(ks * 2), idesc_i8, 1u);
-                        tc_commit_a(TWQ_BAR(B_UEMPTY + su));
-                        tc_commit_a(TWQ_BAR(B_TFULL + b));
+                            for (int ks = 0; ks < G / 32; ++ks)   // accumulate onto the pre-filled 1.5*2^23 pattern
+                                umma_i8_ts(td, ta + ks * 8, ud + static_cast<uint64_t>(ks * 2), idesc_i8, 1u);
+                            tc_commit_a(TWQ_BAR(B_UEMPTY + su));
+                            tc_commit_a(TWQ_BAR(B_TFULL + b));
+                        }
+                        __syncwarp();
                     } else if (leader) {
                         // one M = 256 MMA per K-step for the pair: both epilogues drained buffer b, both CTAs'
                         // operands of stage su are in place; completion is multicast to both CTAs' barriers
-                        mbar_wait_cluster_a(TWQ_BAR(B_TEMPTY2 + b), pb, 1000000 + tile_n * 10000 + gi * 100 + b * 10 + pb);
-                        TWQ_TR(1, trn, 2);
-                        mbar_wait_cluster_a(TWQ_BAR(B_UFULL2 + su), phu);
+                        {   // both polls in flight together
+                            const bool ok1 = mbar_try_wait_cluster_a(TWQ_BAR(B_TEMPTY2 + b), pb);
+                            const bool ok2 = mbar_try_wait_cluster_a(TWQ_BAR(B_UFULL2 + su), phu);
+                            if (!ok1) mbar_wait_cluster_a(TWQ_BAR(B_TEMPTY2 + b), pb);
+                            TWQ_TR(1, trn, 2);
+                            if (!ok2) mbar_wait_cluster_a(TWQ_BAR(B_UFULL2 + su), phu);
+                        }
                         TWQ_TR(1, trn, 3);
                         tc_fence_after();
                         const uint64_t ud = udesc0 + static_cast<uint64_t>(su * (C::kUB >> 4));
                         const uint32_t ta = tmem + C::kColA + su * 32;
                         const uint32_t td = tmem + C::kColP + b * TN;
+                        if (elect_one()) {
 #pragma unroll
-                        for (int ks = 0; ks < G / 32; ++ks)
-                            umma_i8_ts_pair(td, ta + ks * 8, ud + static_cast<uint64_t>(ks * 2), idesc_i8_pair, 1u);
-                        const uint16_t mask = static_cast<uint16_t>(3u << (rank & ~1));
-                        tc_commit_pair_a(TWQ_BAR(B_UEMPTY + su), mask);
-                        tc_commit_pair_a(TWQ_BAR(B_TFULL + b), mask);
+                            for (int ks = 0; ks < G / 32; ++ks)
+                                umma_i8_ts_pair(td, ta + ks * 8, ud + static_cast<uint64_t>(ks * 2), idesc_i8_pair, 1u);
+                            const uint16_t mask = static_cast<uint16_t>(3u << (rank & ~1));
+                            tc_commit_pair_a(TWQ_BAR(B_UEMPTY + su), mask);
+                            tc_commit_pair_a(TWQ_BAR(B_TFULL + b), mask);
+                        }
+                        __syncwarp();
                     } else {
                         // the peer's issuer follows the leader use by use (a parity wait may only be one phase
                         // ahead of its barrier): it waits for the leader's completion of this group
@@ -407,8 +437,11 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
                 }
                 // all residual MMAs of the tile complete (alias mode: the stage-1 ring may overwrite the rings);
                 // in a pair the leader's commit covers both CTAs' operands
-                if (!kPair) tc_commit(&bars[B_RESID]);
-                else if (leader) tc_commit_pair_a(TWQ_BAR(B_RESID), static_cast<uint16_t>(3u << (rank & ~1)));
+                if (elect_one()) {
+                    if (!kPair) tc_commit(&bars[B_RESID]);
+                    else if (leader) tc_commit_pair_a(TWQ_BAR(B_RESID), static_cast<uint16_t>(3u << (rank & ~1)));
+                }
+                __syncwarp();
                 ++tile_n;
             }
         }
@@ -417,9 +450,9 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
     else if (warp < kEpiWarp0) {
         // ================================================================ operand preparation warps
         reg_dec<kRegsPrep>();
-        const bool w_role = warp < 8;                 // warps 4-7: weight rows -> TMEM; warps 8-11: activation rows -> smem
-        const int c_tid = threadIdx.x - 128;          // 0..255, stage-1 conversion index
-        const int u_tid = (threadIdx.x - 128) & 127;  // index inside the role
+        const bool w_role = warp < 4;                 // warps 0-3: weight rows -> TMEM; warps 4-7: activation rows -> smem
+        const int c_tid = threadIdx.x;                // 0..255, stage-1 conversion index
+        const int u_tid = threadIdx.x & 127;          // index inside the role
         const int qd = warp & 3;                      // TMEM lane quarter a weight warp may write
         const uint32_t arow = qd * 32 + lane;         // weight row (output channel) of this thread
         const uint32_t tlane = tmem + (static_cast<uint32_t>(qd * 32) << 16);
@@ -448,7 +481,7 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
         int cur_ctx = -1, itp = 0;
         int s1 = 0, ph1 = 0, sp = 0, php = 0, su = 0, phu = 0;
 #ifdef TWQ_TRACE
-        int trn = (warp == 8 && lane == 0) ? 0 : 4096;
+        int trn = (warp == 4 && lane == 0) ? 0 : 4096;
 #endif
         float sxv[8];                                 // scales of the next block of 8 groups for token row u_tid
         {
@@ -761,7 +794,7 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
                 if (active) {
                     const float* cs_ = sSx + (itp & (kSxSlots - 1)) * TN + col0;
                     const uint32_t tcol = tlane + C::kColP + b * TN + col0;
-                    constexpr int kBatch = C::kCPW == 2 ? 2 : 1;   // registers: 64 accumulators + 16 fill at TN = 128
+                    constexpr int kBatch = C::kCPW >= 2 ? 2 : 1;   // two 16-column loads per tcgen05.wait::ld
 #pragma unroll
                     for (int i0 = 0; i0 < C::kCPW; i0 += kBatch) {
                         uint32_t v[kBatch][16];
@@ -850,7 +883,7 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
     tc_fence_before();
     __syncthreads();
     if (kPair) cluster_sync_all();   // the leader's MMAs write the peer's TMEM: both CTAs are done before either frees
-    if (warp == 2) {
+    if (warp == kCtlWarp0 + 2) {
         tc_fence_after();
         if (kPair) tmem_dealloc_pair<C::kTmemCols>(tmem);
         else tmem_dealloc<C::kTmemCols>(tmem);

@@ -304,16 +304,20 @@ __device__ __forceinline__ void tc_commit_pair_a(uint32_t bar, uint16_t cta_mask
     asm volatile("tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;"
                  ::"r"(bar), "h"(cta_mask) : "memory");
 }
+__device__ __forceinline__ bool mbar_try_wait_cluster_a(uint32_t bar, uint32_t parity) {
+    uint32_t ok;
+    asm volatile(
+        "{\n\t.reg .pred P;\n\t"
+        "mbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 P, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, P;\n\t}\n"
+        : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+    return ok != 0;
+}
 __device__ __forceinline__ void mbar_wait_cluster_a(uint32_t bar, uint32_t parity, int tag = 0) {
     (void)tag;
     uint32_t spins = 0;
     for (;;) {
-        uint32_t ok;
-        asm volatile(
-            "{\n\t.reg .pred P;\n\t"
-            "mbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 P, [%1], %2;\n\t"
-            "selp.u32 %0, 1, 0, P;\n\t}\n"
-            : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+        const bool ok = mbar_try_wait_cluster_a(bar, parity);
         if (ok) break;
         if (++spins > (1u << 26)) TWQ_WAIT_FAIL(tag ? tag : 200 + static_cast<int>(bar & 0xFFFu) * 1000);
     }
