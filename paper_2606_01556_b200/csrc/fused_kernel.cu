@@ -1,5 +1,7 @@
 // fused_kernel.cu -- launch planning and dispatch for the fused dual-branch kernel
 // (kernel template: fused_kernel.cuh; instantiations: fused_inst_*.cu).  Host arithmetic only.
+#include <stdlib.h>
+
 #include "fused_kernel.cuh"
 
 namespace twq {
@@ -70,7 +72,7 @@ static bool make_plan_tn(int TN, int M, int N, int K, int r, int G, int num_sms,
     const int nrb = (r + 127) / 128, nkb = (r + 63) / 64;
     const int hbytes = nkb * TN * 128, l2bytes = nkb * kL1Chunk;
     // CTA pairs: prefill tiles in an even cluster without K splits; each CTA then expands half of the token rows
-    pl.pair = (TN == 128 && pl.cs >= 2 && pl.splits == 1) ? 1 : 0;
+    pl.pair = (TN == 128 && pl.cs >= 2 && pl.splits == 1 && getenv("TWQ_DEBUG_NO_PAIR") == nullptr) ? 1 : 0;
     const int xr = pl.pair ? TN / 2 : TN;
     const int ub = xr * G, pb = kTileN * (G / 2) + xr * (G / 2);
     const int s1b = TN * 128 + nrb * kL1Chunk;

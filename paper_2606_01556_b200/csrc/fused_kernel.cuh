@@ -16,17 +16,26 @@
 // through distributed shared memory.  H never leaves the chip.
 //
 // Warp roles (640 threads; registers re-balanced per role with setmaxnreg):
-//   warp 0      TMA producer: stage-1 tiles (X, L1T), L2T tile, packed INT4 tiles (R4, Xq)
-//   warp 1      MMA issuer (one thread): kind::f16 stage 1 / stage 2, kind::i8 residual
-//   warp 2      TMEM allocator
-//   warps 4-11  operand preparation.  All: BF16->FP16 rewrite of the X tile (kind::f16 needs one
+//   warps 0-7   operand preparation.  All: BF16->FP16 rewrite of the X tile (kind::f16 needs one
 //               16-bit format for both operands).  INT4 -> int8 expansion: each nibble c becomes
 //               the byte 16*c (one shift/and per word, sign for free; sm_100 has no INT4 MMA).
-//               Warps 4-7: weight rows, registers -> TMEM (the MMA reads A from TMEM, so expanded
-//               weights never touch shared memory).  Warps 8-11: activation rows -> swizzled smem
+//               Warps 0-3: weight rows, registers -> TMEM (the MMA reads A from TMEM, so expanded
+//               weights never touch shared memory).  Warps 4-7: activation rows -> swizzled smem
 //               tile (B operand), and the activation group scales.
-//   warps 12-19 epilogue: per group, tcgen05.ld the int32 accumulator, fold both scales in
+//   warps 8-15  epilogue: per group, tcgen05.ld the int32 accumulator, fold both scales in
 //               FP32 (two packed f32x2 FMAs per pair), accumulate in registers; add Ylr; store.
+//   warp 16     TMA producer: stage-1 tiles (X, L1T), L2T tile, packed INT4 tiles (R4, Xq)
+//   warp 17     MMA issuer (the warp runs converged, one elected lane issues): kind::f16 stage 1 /
+//               stage 2, kind::i8 residual
+//   warp 18     TMEM allocator
+//
+// CTA pairs (kPair, 128-token tiles in an even cluster): ranks 2i / 2i+1 share ONE tcgen05.mma of M = 256
+// (cta_group::2).  Each CTA keeps its own 128 weight rows in its TMEM and expands only HALF of the token
+// rows (B rows [rank*64, rank*64+64)), which halves the activation-side shared-memory traffic and
+// expansion work; the even CTA issues after both CTAs' preparation warps and epilogues have arrived on
+// ITS barriers (relaxed remote arrives: the data is already fenced locally; a release at cluster scope
+// costs ~800 cycles per warp here) and multicasts the completion to both CTAs' barriers.  The odd CTA's
+// issuer still runs its own stage-1 / stage-2 MMAs (cta_group::1) and follows the leader use by use.
 // The single-thread roles keep stage indices and phases in counters (no division in any loop).
 //
 // Accumulator trick: each P buffer is pre-filled with the bit pattern of 1.5*2^23, and the
