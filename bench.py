@@ -207,11 +207,11 @@ def roofline_for(L, twq, us_dual, peaks, traffic=None):
 
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dual-linear kernel, from the ncu --set full
-# captures summarised under profiles/ (r01b_full_*.txt); None where no capture exists.
+# captures summarised under profiles/ (r01c_full_*.txt); None where no capture exists.
 TRAFFIC_BYTES = {
-    "c2_qproj_m1": 11078912,          # profiles/r01b_full_decode_c2_qproj_m1.txt
-    "c2_qproj_m16": 11239680,         # profiles/r01b_full_decode_c2_qproj_m16.txt
-    "c3_gateup_m2048": 111621120,     # profiles/r01b_full_fused_c3_gateup_m2048.txt
+    "c2_qproj_m1": 11086848,          # profiles/r01c_full_decode_c2_qproj_m1.txt
+    "c2_qproj_m16": 11246080,         # profiles/r01c_full_decode_c2_qproj_m16.txt
+    "c3_gateup_m2048": 112169216,     # profiles/r01c_full_fused_c3_gateup_m2048.txt
 }
 
 
