@@ -915,16 +915,24 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
         if (s_last) {
             __threadfence();
             const int rows = min(TN, p.M - t.m0);
-            for (int idx = threadIdx.x; idx < rows * kTileN; idx += kThreads) {
-                const int mm = t.m0 + idx / kTileN, nn = t.n0 + idx % kTileN;
+            // four channels per thread and step (N is a multiple of 16, the workspace 256-byte aligned): the
+            // loads of all splits are independent, the sum is in split order
+            for (int idx = threadIdx.x; idx < rows * (kTileN / 4); idx += kThreads) {
+                const int mm = t.m0 + idx / (kTileN / 4), nn = t.n0 + (idx % (kTileN / 4)) * 4;
                 if (nn >= p.N) continue;
-                float y = 0.0f;
-                for (int z = 0; z < pl.splits; ++z)
-                    y += __ldcg(p.ws_part + (static_cast<size_t>(z) * p.M + mm) * p.N + nn);
+                float4 y = make_float4(0.f, 0.f, 0.f, 0.f);
+                for (int z = 0; z < pl.splits; ++z) {
+                    const float4 v = __ldcg(reinterpret_cast<const float4*>(p.ws_part + (static_cast<size_t>(z) * p.M + mm) * p.N + nn));
+                    y.x += v.x; y.y += v.y; y.z += v.z; y.w += v.w;
+                }
+                const float yv[4] = {y.x, y.y, y.z, y.w};
                 const size_t o = static_cast<size_t>(mm) * p.ldy + nn;
-                if (p.ydt == 0) static_cast<__nv_bfloat16*>(p.Y)[o] = __float2bfloat16_rn(y);
-                else if (p.ydt == 1) static_cast<__half*>(p.Y)[o] = __float2half_rn(y);
-                else static_cast<float*>(p.Y)[o] = y;
+#pragma unroll
+                for (int e = 0; e < 4; ++e) {
+                    if (p.ydt == 0) static_cast<__nv_bfloat16*>(p.Y)[o + e] = __float2bfloat16_rn(yv[e]);
+                    else if (p.ydt == 1) static_cast<__half*>(p.Y)[o + e] = __float2half_rn(yv[e]);
+                    else static_cast<float*>(p.Y)[o + e] = yv[e];
+                }
             }
         }
     }
