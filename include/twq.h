@@ -111,7 +111,8 @@ size_t twq_workspace_bytes(int M, int N, int K, int r, int G);
  *   Y      [M,ldy]          out, dtype ydt (ldy >= N elements)
  *   ws, ws_bytes            scratch of at least twq_workspace_bytes(...) bytes, 256-byte aligned (may be
  *                           NULL when that is 0).  It holds split-K partial sums and tile counters for
- *                           decode-shaped calls.  The caller zero-fills it ONCE after allocation; every
+ *                           calls with few output tiles (16 < M, roughly M*N < 1.5 M outputs); calls with
+ *                           M <= 16 and prefill-shaped calls need none.  The caller zero-fills it ONCE after allocation; every
  *                           call leaves the counters zero again, so it can be reused without clearing.
  *   dbg_P  [M,K/G,N] int32  NULL, or receives the integer group accumulators P taken from the
  *                           same tensor-core path that feeds Y (parity evidence; slows the call)
