@@ -139,7 +139,7 @@ __device__ unsigned long long g_twq_dtrace[4 * 32];
 template <int G, int MT, bool kDbg>
 __global__ void __launch_bounds__(kDecThreads, 1) decode_dual_linear_kernel(const __grid_constant__ DecodeParams p) {
     extern __shared__ __align__(16) uint8_t dsm[];
-    float* sRes = reinterpret_cast<float*>(dsm + p.off_res);      // [items][16 rows][8*MT tokens]
+    float* sRes = reinterpret_cast<float*>(dsm + p.off_res);      // [items][8*MT tokens][16 rows]: the epilogue reads rows contiguously
     float* sHpart = reinterpret_cast<float*>(dsm + p.off_hpart);  // [16 tokens][r]
     __half* sH = reinterpret_cast<__half*>(dsm + p.off_h);        // [16 tokens][r + 8]
     float* sYlr = reinterpret_cast<float*>(dsm + p.off_ylr);      // [16 tokens][T*16]
@@ -405,10 +405,10 @@ __global__ void __launch_bounds__(kDecThreads, 1) decode_dual_linear_kernel(cons
 #pragma unroll
         for (int t = 0; t < MT; ++t) {
             const int m0 = 8 * t + tid4 * 2;
-            dst[gid * kTok + m0] = acc[t][0];
-            dst[gid * kTok + m0 + 1] = acc[t][1];
-            dst[(gid + 8) * kTok + m0] = acc[t][2];
-            dst[(gid + 8) * kTok + m0 + 1] = acc[t][3];
+            dst[m0 * 16 + gid] = acc[t][0];
+            dst[(m0 + 1) * 16 + gid] = acc[t][1];
+            dst[m0 * 16 + gid + 8] = acc[t][2];
+            dst[(m0 + 1) * 16 + gid + 8] = acc[t][3];
         }
         item += kDecWarps;
         if (item < items) {
@@ -530,7 +530,7 @@ __global__ void __launch_bounds__(kDecThreads, 1) decode_dual_linear_kernel(cons
         const int m = i / (ntile * 16), nl = i - m * (ntile * 16);
         const int tl = nl >> 4, row = nl & 15;
         float y = 0.0f;
-        for (int pp = 0; pp < P; ++pp) y += sRes[(static_cast<size_t>(tl * P + pp) * 16 + row) * kTok + m];
+        for (int pp = 0; pp < P; ++pp) y += sRes[(static_cast<size_t>(tl * P + pp) * kTok + m) * 16 + row];
         if (r > 0) y += sYlr[m * nloc + nl];
         const size_t o = static_cast<size_t>(m) * p.ldy + tile0 * 16 + nl;
         if (p.ydt == 0) static_cast<__nv_bfloat16*>(p.Y)[o] = __float2bfloat16_rn(y);
