@@ -69,6 +69,8 @@ __device__ __forceinline__ uint4 ldg_nc(const void* p) {
     return v;
 }
 
+__device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
+
 // two BF16 (packed) -> two FP16 (packed), exact for 2^-14 <= |x| <= 65504, saturating above
 __device__ __forceinline__ uint32_t bf2_to_h2(uint32_t w) {
     float lo = __uint_as_float(w << 16), hi = __uint_as_float(w & 0xFFFF0000u);
@@ -306,6 +308,13 @@ __global__ void __launch_bounds__(kDecThreads, 1) decode_dual_linear_kernel(cons
 #pragma unroll
         for (int s = 0; s < kD; ++s)
             if (s < cnt) load_w(sl[s], s);
+        // groups beyond the register ring: pull their lines into L2 now, so that the ring's refills are L2 hits
+        // instead of a second DRAM round trip (CTAs with an odd tile count have 6-7 groups per item)
+        for (int i = kD; i < cnt && i < 3 * kD; ++i) {
+            const uint8_t* a = wrow + static_cast<size_t>(kpart + i * P) * (G / 2);
+            prefetch_l2(a);
+            prefetch_l2(a + static_cast<size_t>(8) * rowbytes);
+        }
     }
 
     // stage-2 operand of this warp's first 8-channel step (L2T rows), prefetched behind the weights
