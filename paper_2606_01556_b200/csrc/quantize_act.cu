@@ -20,8 +20,12 @@ template <int kG, bool kHasT>
 __global__ void __launch_bounds__(256) quantize_act_kernel(const uint16_t* __restrict__ X, int M, int K, int ldx,
                                                            const float* __restrict__ tinv,
                                                            uint8_t* __restrict__ Xq, float* __restrict__ sx) {
-    // programmatic dependent launch: the next kernel (twq_dual_linear) may start its prologue and weight
-    // prefetch now; it waits (griddepcontrol.wait) for this grid to finish before it reads Xq / sx
+    // Programmatic dependent launch on both sides.  This kernel is itself launched as a programmatic
+    // dependent, so its blocks are scheduled while the previous kernel of the stream drains; it waits for that
+    // kernel (which may have produced X, and may still read the Xq / sx buffers) before touching memory, and
+    // only then lets the next kernel (twq_dual_linear) start its prologue and weight prefetch -- that kernel
+    // reads X before its own griddepcontrol.wait, so the order wait -> launch_dependents matters.
+    asm volatile("griddepcontrol.wait;" ::: "memory");
     asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     constexpr int kLanesPerGroup = kG / 8;
     const int chunks_per_row = K >> 3;  // 8-element chunks
@@ -83,14 +87,25 @@ cudaError_t launch_quantize_act(const void* X, int M, int K, int ldx, const floa
     if (blocks > 148LL * 64) blocks = 148LL * 64;  // grid-stride beyond 64 CTAs per SM
     if (blocks < 1) blocks = 1;
     const uint16_t* Xp = static_cast<const uint16_t*>(X);
-    dim3 grid(static_cast<unsigned>(blocks));
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(static_cast<unsigned>(blocks));
+    cfg.blockDim = dim3(threads);
+    cfg.dynamicSmemBytes = 0;
+    cfg.stream = stream;
+    cudaLaunchAttribute attr;
+    attr.id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr.val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = &attr;
+    cfg.numAttrs = 1;
+    cudaError_t e;
     if (G == 128) {
-        if (tinv) quantize_act_kernel<128, true><<<grid, threads, 0, stream>>>(Xp, M, K, ldx, tinv, Xq, sx);
-        else quantize_act_kernel<128, false><<<grid, threads, 0, stream>>>(Xp, M, K, ldx, tinv, Xq, sx);
+        if (tinv) e = cudaLaunchKernelEx(&cfg, quantize_act_kernel<128, true>, Xp, M, K, ldx, tinv, Xq, sx);
+        else e = cudaLaunchKernelEx(&cfg, quantize_act_kernel<128, false>, Xp, M, K, ldx, tinv, Xq, sx);
     } else {
-        if (tinv) quantize_act_kernel<64, true><<<grid, threads, 0, stream>>>(Xp, M, K, ldx, tinv, Xq, sx);
-        else quantize_act_kernel<64, false><<<grid, threads, 0, stream>>>(Xp, M, K, ldx, tinv, Xq, sx);
+        if (tinv) e = cudaLaunchKernelEx(&cfg, quantize_act_kernel<64, true>, Xp, M, K, ldx, tinv, Xq, sx);
+        else e = cudaLaunchKernelEx(&cfg, quantize_act_kernel<64, false>, Xp, M, K, ldx, tinv, Xq, sx);
     }
+    if (e != cudaSuccess) return e;
     return cudaGetLastError();
 }
 
