@@ -52,7 +52,8 @@ static bool make_plan_tn(int TN, int M, int N, int K, int r, int G, int num_sms,
     // K splits when the output tiles alone cannot fill the machine (decode-shaped M)
     const long long tiles = static_cast<long long>(pl.n_tiles) * pl.m_tiles;
     int s = 1;
-    if (tiles < (3 * num_sms) / 4) {
+    // TWQ_DEBUG_NO_SPLIT: testing aid -- small shapes then take the unsplit path (and CTA pairs) of large ones
+    if (tiles < (3 * num_sms) / 4 && getenv("TWQ_DEBUG_NO_SPLIT") == nullptr) {
         s = static_cast<int>(static_cast<long long>(max_clusters) * pl.cs / tiles);
         if (s > 16) s = 16;
         if (s > ng) s = ng;

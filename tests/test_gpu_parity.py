@@ -134,6 +134,21 @@ def test_decode_kernel_shapes(twq, oracle, M, K, N, r, G):
     _check_layer(twq, oracle, gen.make_layer(M, K, N, r, G, seed=2000 + M + N, with_tinv=(M % 2 == 1)))
 
 
+@pytest.mark.parametrize("M,K,N,r,G", [
+    (256, 512, 512, 64, 64),      # CTA pairs with 64-wide groups
+    (300, 1024, 1024, 128, 128),  # ragged last token tile: the odd CTA's half of the B rows is all padding
+    (129, 256, 256, 16, 128),     # one live row in the second tile; smallest rank
+    (640, 2048, 2304, 128, 128),  # several tiles per cluster and a change of token tile inside a cluster's list
+])
+def test_fused_kernel_cta_pairs(twq, oracle, monkeypatch, M, K, N, r, G):
+    """128-token tiles in an even cluster run as CTA pairs (cta_group::2, fused_kernel.cuh); same bar.
+    Shapes this small would split K instead; the planner's testing switch sends them down the unsplit path."""
+    monkeypatch.setenv("TWQ_DEBUG_NO_SPLIT", "1")
+    assert twq.workspace_bytes(M, N, K, r, G) == 0
+    rows = None if M * N * K <= 2 ** 29 else sorted(set(np.linspace(0, M - 1, 96).astype(int).tolist()))
+    _check_layer(twq, oracle, gen.make_layer(M, K, N, r, G, seed=3000 + M, with_tinv=(M % 2 == 0)), rows=rows)
+
+
 def test_rank0_is_plain_w4a4_and_zero_residual_is_lowrank(twq, oracle):
     """north_star special cases, on the GPU path."""
     import torch
