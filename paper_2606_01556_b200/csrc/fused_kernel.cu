@@ -40,12 +40,36 @@ static bool make_plan_tn(int TN, int M, int N, int K, int r, int G, int num_sms,
     // that keeps the most SMs busy; ties go to the larger cluster (less redundant stage-1 work)
     pl.cs = 1;
     if (r > 0) {
-        int best = 0;
-        for (int c = 8; c >= 1; c >>= 1) {
-            if (pl.n_tiles % c != 0) continue;
-            const int sms = cluster_capacity(c, num_sms) * c;
-            if (sms > best + best / 16) { best = sms; pl.cs = c; }
+        const long long tiles0 = static_cast<long long>(pl.n_tiles) * pl.m_tiles;
+        if (tiles0 < (3 * num_sms) / 4) {
+            // few tiles (K will be split): the size that keeps the most SMs busy; ties go to the larger cluster
+            int best = 0;
+            for (int c = 8; c >= 1; c >>= 1) {
+                if (pl.n_tiles % c != 0) continue;
+                const int sms = cluster_capacity(c, num_sms) * c;
+                if (sms > best + best / 16) { best = sms; pl.cs = c; }
+            }
+        } else {
+            // unsplit path: a cost model in cycles per CTA.  A cluster recomputes H = X*L1 once per token tile it
+            // touches, each CTA a serial chain of K/(64*cs) chunks (~700 cycles each); the residual costs ~1450 cycles
+            // per K-group per tile (both fitted to gate/up and down at M = 2048 over cs = 2 / 4 / 8, r01c).  Small
+            // clusters cover more SMs, large ones share stage 1 further.
+            long long best_cost = -1;
+            for (int c = 8; c >= 1; c >>= 1) {
+                if (pl.n_tiles % c != 0) continue;
+                const int nb = pl.n_tiles / c;
+                const long long units = static_cast<long long>(pl.m_tiles) * nb;
+                const long long ncl = units < cluster_capacity(c, num_sms) ? units : cluster_capacity(c, num_sms);
+                const long long upc = (units + ncl - 1) / ncl;                       // units per cluster (the longest)
+                const long long ctxs = (upc + nb - 1) / nb + ((upc > 1 && nb > 1) ? 1 : 0);
+                const long long cost = ctxs * ((K / 64 + c - 1) / c) * 700 + upc * ng * 1450;
+                if (best_cost < 0 || cost < best_cost) { best_cost = cost; pl.cs = c; }
+            }
         }
+    }
+    if (const char* e = getenv("TWQ_DEBUG_FUSED_CS")) {   // debugging aid: force the cluster size
+        const int c = atoi(e);
+        if (r > 0 && (c == 1 || c == 2 || c == 4 || c == 8) && pl.n_tiles % c == 0) pl.cs = c;
     }
     pl.n_blocks = pl.n_tiles / pl.cs;
     const int max_clusters = cluster_capacity(pl.cs, num_sms);
