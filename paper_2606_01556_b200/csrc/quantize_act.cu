@@ -6,10 +6,9 @@
 // (reading R8) and must reproduce the oracle's codes and scales bit for bit, so
 // this file is compiled WITHOUT fast-math and uses the *_rn intrinsics (no FMA contraction).
 //
-// HBM-bound: 2 B/element in, 0.5 B/element + 4 B/group out.  Each thread owns 16
-// consecutive k (two 16-byte loads of one 32-byte sector, one 8-byte store); G/16 adjacent lanes
-// form a group and reduce their amax with xor-shuffles, so a warp covers 512 contiguous elements of
-// one row (1 KB in, 256 B out).  Sixteen elements per thread halve the per-group work (two IEEE
+// HBM-bound: 2 B/element in, 0.5 B/element + 4 B/group out.  Each thread owns kE = 16 or 32
+// consecutive k (16-byte loads, one 8- or 16-byte store); G/kE adjacent lanes form a group and
+// reduce their amax with xor-shuffles.  More elements per thread mean less per-group work (two IEEE
 // divides, index arithmetic) per byte: with eight the kernel was instruction-bound, not HBM-bound.
 #include <cuda_bf16.h>
 #include <cuda_runtime.h>
@@ -19,7 +18,7 @@ namespace twq {
 
 // kIdx: index type of the chunk counter -- unsigned (32-bit divide, ~20 instructions) whenever M*K/8 < 2^31,
 // which is every realistic shape; the 64-bit divide it replaces made this kernel instruction-bound (ncu r01c).
-template <int kG, bool kHasT, typename kIdx = unsigned>
+template <int kG, bool kHasT, typename kIdx = unsigned, int kE = 16>
 __global__ void __launch_bounds__(256) quantize_act_kernel(const uint16_t* __restrict__ X, int M, int K, int ldx,
                                                            const float* __restrict__ tinv,
                                                            uint8_t* __restrict__ Xq, float* __restrict__ sx) {
@@ -30,10 +29,12 @@ __global__ void __launch_bounds__(256) quantize_act_kernel(const uint16_t* __res
     // reads X before its own griddepcontrol.wait, so the order wait -> launch_dependents matters.
     asm volatile("griddepcontrol.wait;" ::: "memory");
     asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
-    constexpr int kLanesPerGroup = kG / 16;
-    const int chunks_per_row = K >> 4;  // 16-element chunks
+    // kE = elements per thread: 32 for large problems (fewer divides and index arithmetic per byte), 16 below
+    // (more threads: the small calls are latency-bound)
+    constexpr int kLanesPerGroup = kG / kE;
+    const int chunks_per_row = K / kE;
     const kIdx total = static_cast<kIdx>(M) * static_cast<kIdx>(chunks_per_row);
-    // K % G == 0 and G % 16 == 0 guarantee that a group never straddles rows and that the
+    // K % G == 0 and G % 32 == 0 guarantee that a group never straddles rows and that the
     // kLanesPerGroup lanes of a group are either all active or all inactive.
     const kIdx total_pad = (total + 31) & ~static_cast<kIdx>(31);
     for (kIdx idx = static_cast<kIdx>(blockIdx.x) * blockDim.x + threadIdx.x; idx < total_pad;
@@ -41,20 +42,25 @@ __global__ void __launch_bounds__(256) quantize_act_kernel(const uint16_t* __res
         const bool active = idx < total;
         const int m = active ? static_cast<int>(idx / static_cast<kIdx>(chunks_per_row)) : 0;
         const int c = active ? static_cast<int>(idx - static_cast<kIdx>(m) * static_cast<kIdx>(chunks_per_row)) : 0;
-        float x[16];
+        float x[kE];
         if (active) {
-            const uint4* src = reinterpret_cast<const uint4*>(X + static_cast<size_t>(m) * ldx + c * 16);
-            const uint4 r0 = __ldg(src), r1 = __ldg(src + 1);
-            const uint32_t w[8] = {r0.x, r0.y, r0.z, r0.w, r1.x, r1.y, r1.z, r1.w};
+            const uint4* src = reinterpret_cast<const uint4*>(X + static_cast<size_t>(m) * ldx + c * kE);
+            uint4 rr[kE / 8];
 #pragma unroll
-            for (int i = 0; i < 8; ++i) {
-                x[2 * i] = __uint_as_float(w[i] << 16);              // BF16 -> FP32, exact
-                x[2 * i + 1] = __uint_as_float(w[i] & 0xFFFF0000u);
+            for (int q = 0; q < kE / 8; ++q) rr[q] = __ldg(src + q);
+#pragma unroll
+            for (int q = 0; q < kE / 8; ++q) {
+                const uint32_t w[4] = {rr[q].x, rr[q].y, rr[q].z, rr[q].w};
+#pragma unroll
+                for (int i = 0; i < 4; ++i) {
+                    x[8 * q + 2 * i] = __uint_as_float(w[i] << 16);              // BF16 -> FP32, exact
+                    x[8 * q + 2 * i + 1] = __uint_as_float(w[i] & 0xFFFF0000u);
+                }
             }
             if (kHasT) {
-                const float4* tp = reinterpret_cast<const float4*>(tinv + c * 16);
+                const float4* tp = reinterpret_cast<const float4*>(tinv + c * kE);
 #pragma unroll
-                for (int q = 0; q < 4; ++q) {
+                for (int q = 0; q < kE / 4; ++q) {
                     const float4 t = __ldg(tp + q);
                     x[4 * q] = __fmul_rn(x[4 * q], t.x);
                     x[4 * q + 1] = __fmul_rn(x[4 * q + 1], t.y);
@@ -64,25 +70,29 @@ __global__ void __launch_bounds__(256) quantize_act_kernel(const uint16_t* __res
             }
         } else {
 #pragma unroll
-            for (int i = 0; i < 16; ++i) x[i] = 0.0f;
+            for (int i = 0; i < kE; ++i) x[i] = 0.0f;
         }
         float amax = 0.0f;
 #pragma unroll
-        for (int i = 0; i < 16; ++i) amax = fmaxf(amax, fabsf(x[i]));
+        for (int i = 0; i < kE; ++i) amax = fmaxf(amax, fabsf(x[i]));
 #pragma unroll
         for (int d = kLanesPerGroup / 2; d >= 1; d >>= 1) amax = fmaxf(amax, __shfl_xor_sync(0xffffffffu, amax, d));
         const float amax_c = fmaxf(amax, 0x1p-30f);
         const float s = __fdiv_rn(amax_c, 7.0f);
         const float inv = __fdiv_rn(1.0f, s);
-        uint32_t packed[2] = {0u, 0u};
+        uint32_t packed[kE / 8];
 #pragma unroll
-        for (int i = 0; i < 16; ++i) {
+        for (int q = 0; q < kE / 8; ++q) packed[q] = 0u;
+#pragma unroll
+        for (int i = 0; i < kE; ++i) {
             int q = __float2int_rn(__fmul_rn(x[i], inv));  // round-half-to-even
             q = max(-7, min(7, q));
             packed[i >> 3] |= (static_cast<uint32_t>(q) & 0xFu) << (4 * (i & 7));  // low nibble = even k
         }
         if (active) {
-            *reinterpret_cast<uint2*>(Xq + static_cast<size_t>(m) * (K >> 1) + c * 8) = make_uint2(packed[0], packed[1]);
+            uint8_t* dst = Xq + static_cast<size_t>(m) * (K >> 1) + c * (kE / 2);
+            if constexpr (kE == 32) *reinterpret_cast<uint4*>(dst) = make_uint4(packed[0], packed[1], packed[2], packed[3]);
+            else *reinterpret_cast<uint2*>(dst) = make_uint2(packed[0], packed[1]);
             if ((c % kLanesPerGroup) == 0) sx[static_cast<size_t>(m) * (K / kG) + c / kLanesPerGroup] = s;
         }
     }
@@ -90,7 +100,8 @@ __global__ void __launch_bounds__(256) quantize_act_kernel(const uint16_t* __res
 
 cudaError_t launch_quantize_act(const void* X, int M, int K, int ldx, const float* tinv, int G, uint8_t* Xq,
                                 float* sx, cudaStream_t stream) {
-    const long long total = static_cast<long long>(M) * (K >> 4);
+    const bool big = static_cast<long long>(M) * K >= (1LL << 22);   // 32 elements per thread from 4 Mi elements
+    const long long total = static_cast<long long>(M) * (big ? K >> 5 : K >> 4);
     const int threads = 256;
     long long blocks = (total + threads - 1) / threads;
     if (blocks > 148LL * 64) blocks = 148LL * 64;  // grid-stride beyond 64 CTAs per SM
@@ -108,9 +119,10 @@ cudaError_t launch_quantize_act(const void* X, int M, int K, int ldx, const floa
     cfg.numAttrs = 1;
     cudaError_t e;
     const bool wide = total + 8192LL * 256 >= (1LL << 31);   // 64-bit chunk counter only for > 1.7e10 elements
-#define TWQ_QLAUNCH(g, t)                                                                                        \
-    (wide ? cudaLaunchKernelEx(&cfg, quantize_act_kernel<g, t, unsigned long long>, Xp, M, K, ldx, tinv, Xq, sx)  \
-          : cudaLaunchKernelEx(&cfg, quantize_act_kernel<g, t, unsigned>, Xp, M, K, ldx, tinv, Xq, sx))
+#define TWQ_QLAUNCH(g, t)                                                                                              \
+    (wide  ? cudaLaunchKernelEx(&cfg, quantize_act_kernel<g, t, unsigned long long, 32>, Xp, M, K, ldx, tinv, Xq, sx)   \
+     : big ? cudaLaunchKernelEx(&cfg, quantize_act_kernel<g, t, unsigned, 32>, Xp, M, K, ldx, tinv, Xq, sx)             \
+           : cudaLaunchKernelEx(&cfg, quantize_act_kernel<g, t, unsigned, 16>, Xp, M, K, ldx, tinv, Xq, sx))
     if (G == 128) e = tinv ? TWQ_QLAUNCH(128, true) : TWQ_QLAUNCH(128, false);
     else e = tinv ? TWQ_QLAUNCH(64, true) : TWQ_QLAUNCH(64, false);
 #undef TWQ_QLAUNCH
