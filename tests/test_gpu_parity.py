@@ -296,3 +296,10 @@ def test_config4_qwen(twq, oracle, which, M, nrows):
 @pytest.mark.parametrize("which,M", [("q", 1), ("k", 8), ("down", 16), ("gate_up", 2)])
 def test_config5_llama70b(twq, oracle, which, M):
     _check_layer(twq, oracle, gen.config5_llama70b(which, M), check_P=(which != "gate_up"))
+
+
+def test_config5_llama70b_largest_prefill_sampled(twq, oracle):
+    """configs[4] at its largest layer and a prefill batch: gate/up K = 8192, N = 28672, r = 256, M = 2048 (the
+    rank-256 buffers force the 64-token tile); 24 token rows x all N are compared, without the P dump (60 GB)."""
+    L = gen.config5_llama70b("gate_up", 2048)
+    _check_layer(twq, oracle, L, rows=_sample_rows(2048, 24), check_P=False)
