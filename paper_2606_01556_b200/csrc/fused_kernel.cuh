@@ -560,7 +560,10 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
                     }
                 }
                 TWQ_TR(2, trn, 1);
-                mbar_wait_a(TWQ_BAR(B_PFULL + sp), php);
+                // both barrier polls in flight together (a poll costs ~150 cycles even when the phase is complete)
+                const bool pf_ok = mbar_try_wait_a(TWQ_BAR(B_PFULL + sp), php);
+                const bool ue_ok = mbar_try_wait_a(TWQ_BAR(B_UEMPTY + su), phu ^ 1);
+                if (!pf_ok) mbar_wait_a(TWQ_BAR(B_PFULL + sp), php);
                 TWQ_TR(2, trn, 2);
                 const uint8_t* pw = sP + sp * p_stage_bytes;
                 if (w_role) {
@@ -568,7 +571,7 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
                     uint4 wv[kCPR];
 #pragma unroll
                     for (int c = 0; c < kCPR; ++c) wv[c] = *reinterpret_cast<const uint4*>(pw + in_off[c]);
-                    mbar_wait_a(TWQ_BAR(B_UEMPTY + su), phu ^ 1);
+                    if (!ue_ok) mbar_wait_a(TWQ_BAR(B_UEMPTY + su), phu ^ 1);
                     tc_fence_after();
 #pragma unroll
                     for (int c = 0; c < kCPR; c += 2) {
@@ -587,7 +590,7 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
 #pragma unroll
                         for (int j = 0; j < kXC; ++j) xv[j] = *reinterpret_cast<const uint4*>(pw + in_off[j]);
                     }
-                    mbar_wait_a(TWQ_BAR(B_UEMPTY + su), phu ^ 1);
+                    if (!ue_ok) mbar_wait_a(TWQ_BAR(B_UEMPTY + su), phu ^ 1);
                     TWQ_TR(2, trn, 3);
                     if (x_on) {
                         uint8_t* ub = sU + su * C::kUB;
