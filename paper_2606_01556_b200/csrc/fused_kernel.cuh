@@ -784,6 +784,9 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
                     if (kPair) mbar_arrive_remote_relaxed(TWQ_LBAR(B_TEMPTY2 + b));
                 }
                 if (++b == kNB) { b = 0; pb ^= 1; }
+#ifdef TWQ_TRACE
+                if (trw) TWQ_TR(3, trn, 7);
+#endif
             } else {
 #pragma unroll
                 for (int i = 0; i < kNA; ++i) acc[i] = 0ull;
@@ -866,7 +869,36 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
                 if (++b == kNB) { b = 0; pb ^= 1; }
             }
 
-            if (active && n_ok) {
+#ifdef TWQ_TRACE
+            if (trw) TWQ_TR(3, trn, 5);
+#endif
+#ifndef TWQ_EXP_NOSTORE
+            if (active && pl.splits == 1 && (p.ldy & 1) == 0) {
+                // Lane = output channel, register = token: neighbouring lanes trade one value per token pair, so the
+                // even lane holds channels (n, n+1) of token 2i and the odd lane channels (n-1, n) of token 2i+1 --
+                // half as many store instructions, each lane a 4-byte (FP32 output: 8-byte) word.  N is even.
+                const bool odd = lane & 1;
+                const int nn = n - (odd ? 1 : 0);
+#pragma unroll
+                for (int i = 0; i < kNA; ++i) {
+                    float y0, y1;
+                    unpack_f2(acc[i], y0, y1);
+                    const float got = __shfl_xor_sync(0xffffffffu, odd ? y0 : y1, 1);
+                    const float lo = odd ? got : y0, hi = odd ? y1 : got;   // channels nn, nn + 1
+                    const int m = t.m0 + col0 + i * 2 + (odd ? 1 : 0);
+                    if (n_ok && m < p.M) {
+                        const size_t o = static_cast<size_t>(m) * p.ldy + nn;
+                        if (p.ydt == 0) {
+                            const __nv_bfloat162 v = __floats2bfloat162_rn(lo, hi);
+                            *reinterpret_cast<__nv_bfloat162*>(static_cast<__nv_bfloat16*>(p.Y) + o) = v;
+                        } else if (p.ydt == 1) {
+                            *reinterpret_cast<__half2*>(static_cast<__half*>(p.Y) + o) = __floats2half2_rn(lo, hi);
+                        } else {
+                            *reinterpret_cast<float2*>(static_cast<float*>(p.Y) + o) = make_float2(lo, hi);
+                        }
+                    }
+                }
+            } else if (active && n_ok) {   // split-K partial (FP32, workspace [ks][M][N]) or an odd row pitch
 #pragma unroll
                 for (int i = 0; i < kNA; ++i) {
                     float y2[2];
@@ -874,20 +906,19 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
 #pragma unroll
                     for (int e = 0; e < 2; ++e) {
                         const int m = t.m0 + col0 + i * 2 + e;
-                        if (m < p.M) {
-                            const float y = y2[e];
-                            if (pl.splits == 1) {
-                                const size_t o = static_cast<size_t>(m) * p.ldy + n;
-                                if (p.ydt == 0) static_cast<__nv_bfloat16*>(p.Y)[o] = __float2bfloat16_rn(y);
-                                else if (p.ydt == 1) static_cast<__half*>(p.Y)[o] = __float2half_rn(y);
-                                else static_cast<float*>(p.Y)[o] = y;
-                            } else {   // split-K: park the FP32 partial of this split in the workspace [ks][M][N]
-                                p.ws_part[(static_cast<size_t>(t.ks) * p.M + m) * p.N + n] = y;
-                            }
-                        }
+                        if (m >= p.M) continue;
+                        const size_t o = static_cast<size_t>(m) * p.ldy + n;
+                        if (pl.splits > 1) p.ws_part[(static_cast<size_t>(t.ks) * p.M + m) * p.N + n] = y2[e];
+                        else if (p.ydt == 0) static_cast<__nv_bfloat16*>(p.Y)[o] = __float2bfloat16_rn(y2[e]);
+                        else if (p.ydt == 1) static_cast<__half*>(p.Y)[o] = __float2half_rn(y2[e]);
+                        else static_cast<float*>(p.Y)[o] = y2[e];
                     }
                 }
             }
+#endif
+#ifdef TWQ_TRACE
+            if (trw) TWQ_TR(3, trn, 6);
+#endif
         }
     }
 
