@@ -873,7 +873,53 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
             if (trw) TWQ_TR(3, trn, 5);
 #endif
 #ifndef TWQ_EXP_NOSTORE
-            if (active && pl.splits == 1 && (p.ldy & 1) == 0) {
+            if (active && pl.splits == 1 && p.ydt <= 1 && (p.ldy & 7) == 0) {
+                // 16-bit outputs, 16-byte aligned rows.  Lane = output channel, register = token: an 8 x 8 transpose
+                // among groups of 8 lanes (three butterfly rounds, 8 shuffles per 8 tokens) leaves each lane with 8
+                // consecutive channels of ONE token: 8 16-byte stores per thread instead of 64 2-byte ones (a store
+                // instruction cost ~115 cycles per warp here whatever its width: 7500 cycles per tile before).
+                const bool b0 = lane & 1, b1 = lane & 2, b2 = lane & 4;
+                const int n8 = t.n0 + qd * 32 + (lane & 24);
+                const bool n8_ok = n8 < p.N;                      // N is a multiple of 16
+#pragma unroll
+                for (int blk = 0; blk < kNA / 4; ++blk) {
+                    uint32_t rA[4];
+#pragma unroll
+                    for (int k = 0; k < 4; ++k) {
+                        float y0, y1;
+                        unpack_f2(acc[blk * 4 + k], y0, y1);
+                        uint32_t w;                               // [token 2k | token 2k+1] of the own channel
+                        if (p.ydt == 0) { const __nv_bfloat162 v = __floats2bfloat162_rn(y0, y1); w = *reinterpret_cast<const uint32_t*>(&v); }
+                        else { const __half2 v = __floats2half2_rn(y0, y1); w = *reinterpret_cast<const uint32_t*>(&v); }
+                        const uint32_t got = __shfl_xor_sync(0xffffffffu, w, 1);
+                        // even lane: token 2k, channels (own, partner); odd lane: token 2k+1, channels (partner, own)
+                        rA[k] = b0 ? __byte_perm(got, w, 0x7632) : __byte_perm(w, got, 0x5410);
+                    }
+                    // round 2: lane bit 1 <-> token bit 1 (k & 1); two channel pairs per token
+                    uint32_t rB[2][2];
+#pragma unroll
+                    for (int s2 = 0; s2 < 2; ++s2) {
+                        const uint32_t keep = b1 ? rA[2 * s2 + 1] : rA[2 * s2], send = b1 ? rA[2 * s2] : rA[2 * s2 + 1];
+                        const uint32_t got = __shfl_xor_sync(0xffffffffu, send, 2);
+                        rB[s2][0] = b1 ? got : keep;
+                        rB[s2][1] = b1 ? keep : got;
+                    }
+                    // round 3: lane bit 2 <-> token bit 2; four channel pairs of one token
+                    uint32_t o4[4];
+                    {
+                        const uint32_t k0 = b2 ? rB[1][0] : rB[0][0], k1 = b2 ? rB[1][1] : rB[0][1];
+                        const uint32_t s0 = b2 ? rB[0][0] : rB[1][0], s1 = b2 ? rB[0][1] : rB[1][1];
+                        const uint32_t g0 = __shfl_xor_sync(0xffffffffu, s0, 4), g1 = __shfl_xor_sync(0xffffffffu, s1, 4);
+                        o4[0] = b2 ? g0 : k0; o4[1] = b2 ? g1 : k1;
+                        o4[2] = b2 ? k0 : g0; o4[3] = b2 ? k1 : g1;
+                    }
+                    const int m = t.m0 + col0 + blk * 8 + (lane & 7);
+                    if (n8_ok && m < p.M) {
+                        uint8_t* dst = static_cast<uint8_t*>(p.Y) + (static_cast<size_t>(m) * p.ldy + n8) * 2;
+                        *reinterpret_cast<uint4*>(dst) = make_uint4(o4[0], o4[1], o4[2], o4[3]);
+                    }
+                }
+            } else if (active && pl.splits == 1 && (p.ldy & 1) == 0) {
                 // Lane = output channel, register = token: neighbouring lanes trade one value per token pair, so the
                 // even lane holds channels (n, n+1) of token 2i and the odd lane channels (n-1, n) of token 2i+1 --
                 // half as many store instructions, each lane a 4-byte (FP32 output: 8-byte) word.  N is even.
