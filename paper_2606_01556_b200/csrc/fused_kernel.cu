@@ -104,6 +104,11 @@ static bool make_plan_tn(int TN, int M, int N, int K, int r, int G, int num_sms,
     const int hpart = pl.cs > 1 ? round_up(TN * r * 4, 1024) : 0;
     const int fixed = kSxSlots * TN * 4 + B_COUNT * 8 + 256;
     const int budget = kMaxDynSmem - 1024 - fixed;             // dynamic limit minus alignment slack
+    // output staging for the asynchronous (TMA) store of a finished 128-token tile of 16-bit outputs: two 128-byte-
+    // swizzled halves of 64 channels; taken only where it fits beside a packed ring of at least 6 (pairs) / 4 stages.
+    // The caller clears the flag for FP32 outputs and row pitches that are not a multiple of 16 bytes.
+    const int ybytes = TN * kTileN * 2;
+    pl.ystage = (TN == 128 && pl.splits == 1 && getenv("TWQ_DEBUG_NO_YSTAGE") == nullptr) ? 1 : 0;
     pl.nsu = kMaxNSU;
     pl.nsp = (TN <= 32 || pl.pair) ? kMaxNSP : 4;   // a pair's packed stage is 12 KB: the ring can be twice as deep
     pl.ns1 = r > 0 ? (TN <= 32 ? 3 : 2) : 0;
@@ -111,8 +116,15 @@ static bool make_plan_tn(int TN, int M, int N, int K, int r, int G, int num_sms,
     auto total = [&](const FusedPlan& q) {
         const int resid = q.nsu * ub + round_up(q.nsp * pb, 1024);
         const int s1 = q.alias ? (q.ns1 * s1b > hpart ? q.ns1 * s1b : hpart) : q.ns1 * s1b + hpart;
-        return hbytes + l2bytes + (q.alias ? (resid > s1 ? resid : s1) : resid + s1);
+        return hbytes + l2bytes + (q.alias ? (resid > s1 ? resid : s1) : resid + s1) + (q.ystage ? ybytes + 1024 : 0);
     };
+    if (pl.ystage) {
+        FusedPlan q = pl;
+        q.alias = 1; q.ns1 = r > 0 ? 3 : 0;
+        if (total(q) > budget && pl.pair) q.nsp = 6;
+        if (total(q) > budget) pl.ystage = 0;
+        else if (total(pl) > budget) pl.nsp = q.nsp;
+    }
     if (total(pl) > budget) { pl.alias = 1; pl.ns1 = r > 0 ? 3 : 0; }
     while (total(pl) > budget && pl.nsp > 2) --pl.nsp;
     while (total(pl) > budget && pl.nsu > 2) --pl.nsu;
@@ -135,6 +147,7 @@ static bool make_plan_tn(int TN, int M, int N, int K, int r, int G, int num_sms,
         pl.off_Hpart = o; o += hpart;
     }
     o = round_up(o, 16);
+    if (pl.ystage) { o = round_up(o, 1024); pl.off_Y = o; o += ybytes; }
     pl.off_sx = o; o += kSxSlots * TN * 4;
     pl.off_bar = o; o += B_COUNT * 8 + 256;
     pl.smem_bytes = o + 1024;

@@ -52,6 +52,8 @@
 #include <cuda_bf16.h>
 #include <cuda_fp16.h>
 
+#include <type_traits>
+
 #include "fused_kernel.h"
 #include "sm100_ptx.cuh"
 
@@ -177,7 +179,8 @@ template <int TN, int G, bool kDbg, bool kPair = false>
 __global__ void __launch_bounds__(kThreads, 1)
 fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_constant__ CUtensorMap tmXq,
                          const __grid_constant__ CUtensorMap tmX, const __grid_constant__ CUtensorMap tmL1T,
-                         const __grid_constant__ CUtensorMap tmL2T, const __grid_constant__ FusedParams p) {
+                         const __grid_constant__ CUtensorMap tmL2T, const __grid_constant__ CUtensorMap tmY,
+                         const __grid_constant__ FusedParams p) {
     using C = Cfg<TN, G, kPair>;
     const FusedPlan& pl = p.plan;
     extern __shared__ uint8_t smem_raw[];
@@ -190,6 +193,7 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
     uint8_t* sS1 = smem + pl.off_S1;        // stage-1 ring [ns1][X TN x 128 | L1T nrb x 16 KB]
     float* sHpart = reinterpret_cast<float*>(smem + pl.off_Hpart);   // FP32 partial H[m][r]
     float* sSx = reinterpret_cast<float*>(smem + pl.off_sx);
+    uint8_t* sY = smem + pl.off_Y;          // output staging (only when pl.ystage): 2 x [TN][64 channels], 128B-swizzled
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem + pl.off_bar);
     uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + B_COUNT);
     __shared__ int s_last;
@@ -628,6 +632,7 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
         const int et = threadIdx.x - kEpiWarp0 * 32;    // 0..255
         const uint32_t tlane = tmem + (static_cast<uint32_t>(qd * 32) << 16);
         constexpr int kNA = C::kCPW * 8;     // accumulator pairs per thread
+        bool y_pending = false;              // first epilogue warp: bulk stores of the previous tile in flight
         uint64_t acc[kNA];
         // the 1.5*2^23 pattern in 16 registers that stay allocated (a tcgen05.st source is a register vector;
         // opaque to the compiler so that it is not re-materialised per store)
@@ -874,6 +879,15 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
 #endif
 #ifndef TWQ_EXP_NOSTORE
             if (active && pl.splits == 1 && p.ydt <= 1 && (p.ldy & 7) == 0) {
+                const bool staged = pl.ystage != 0;
+                if (staged) {
+                    // the bulk copies of the previous tile have read the staging tile (issued a whole tile ago)
+                    if (warp == kEpiWarp0 && y_pending) bulk_wait_read0();
+                    named_bar_sync(1, kEpiWarps * 32);
+                }
+#ifdef TWQ_TRACE
+                if (trw) TWQ_TR(3, trn, 8);
+#endif
                 // 16-bit outputs, 16-byte aligned rows.  Lane = output channel, register = token: an 8 x 8 transpose
                 // among groups of 8 lanes (three butterfly rounds, 8 shuffles per 8 tokens) leaves each lane with 8
                 // consecutive channels of ONE token: 8 16-byte stores per thread instead of 64 2-byte ones (a store
@@ -881,6 +895,9 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
                 const bool b0 = lane & 1, b1 = lane & 2, b2 = lane & 4;
                 const int n8 = t.n0 + qd * 32 + (lane & 24);
                 const bool n8_ok = n8 < p.N;                      // N is a multiple of 16
+                // one straight-line copy per (format, staged) case: with the two uniform branches inside the loop the
+                // eight blocks ran one after the other, each a chain of three shuffle latencies (2200 cycles per tile)
+                auto store16 = [&](auto kBf16, auto kStaged) {
 #pragma unroll
                 for (int blk = 0; blk < kNA / 4; ++blk) {
                     uint32_t rA[4];
@@ -889,7 +906,7 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
                         float y0, y1;
                         unpack_f2(acc[blk * 4 + k], y0, y1);
                         uint32_t w;                               // [token 2k | token 2k+1] of the own channel
-                        if (p.ydt == 0) { const __nv_bfloat162 v = __floats2bfloat162_rn(y0, y1); w = *reinterpret_cast<const uint32_t*>(&v); }
+                        if (decltype(kBf16)::value) { const __nv_bfloat162 v = __floats2bfloat162_rn(y0, y1); w = *reinterpret_cast<const uint32_t*>(&v); }
                         else { const __half2 v = __floats2half2_rn(y0, y1); w = *reinterpret_cast<const uint32_t*>(&v); }
                         const uint32_t got = __shfl_xor_sync(0xffffffffu, w, 1);
                         // even lane: token 2k, channels (own, partner); odd lane: token 2k+1, channels (partner, own)
@@ -913,10 +930,42 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
                         o4[0] = b2 ? g0 : k0; o4[1] = b2 ? g1 : k1;
                         o4[2] = b2 ? k0 : g0; o4[3] = b2 ? k1 : g1;
                     }
-                    const int m = t.m0 + col0 + blk * 8 + (lane & 7);
-                    if (n8_ok && m < p.M) {
+                    const int mrow = col0 + blk * 8 + (lane & 7);
+                    const int m = t.m0 + mrow;
+                    if (decltype(kStaged)::value) {
+                        // channel half (qd >> 1), row of 128 bytes, 16-byte chunk XOR (row & 7): the layout TMA expects
+                        const int c16 = ((qd & 1) * 32 + (lane & 24)) >> 3;
+                        *reinterpret_cast<uint4*>(sY + (qd >> 1) * (TN * 128) + mrow * 128 + ((c16 ^ (mrow & 7)) << 4)) =
+                            make_uint4(o4[0], o4[1], o4[2], o4[3]);
+                    } else if (n8_ok && m < p.M) {
                         uint8_t* dst = static_cast<uint8_t*>(p.Y) + (static_cast<size_t>(m) * p.ldy + n8) * 2;
                         *reinterpret_cast<uint4*>(dst) = make_uint4(o4[0], o4[1], o4[2], o4[3]);
+                    }
+                }
+                };
+                using TrueT = std::integral_constant<bool, true>;
+                using FalseT = std::integral_constant<bool, false>;
+                if (p.ydt == 0) { if (staged) store16(TrueT{}, TrueT{}); else store16(TrueT{}, FalseT{}); }
+                else { if (staged) store16(FalseT{}, TrueT{}); else store16(FalseT{}, FalseT{}); }
+#ifdef TWQ_TRACE
+                if (trw) TWQ_TR(3, trn, 9);
+#endif
+                if (staged) {
+                    // Asynchronous store: the memory system takes ~2900 cycles to absorb the 32 KB every SM writes at a
+                    // tile boundary (all SMs at once); two TMA stores drain that while the next tile is computed.
+                    // Rows beyond M and channels beyond N are clipped by the tensor map.
+                    fence_proxy_async_smem();
+                    named_bar_sync(1, kEpiWarps * 32);
+#ifdef TWQ_TRACE
+                    if (trw) TWQ_TR(3, trn, 10);
+#endif
+                    if (warp == kEpiWarp0) {
+                        if (lane == 0) {
+                            tma_store_2d(&tmY, smem_u32(sY), t.n0, t.m0);
+                            if (t.n0 + 64 < p.N) tma_store_2d(&tmY, smem_u32(sY + TN * 128), t.n0 + 64, t.m0);
+                            bulk_commit();
+                        }
+                        y_pending = true;
                     }
                 }
             } else if (active && pl.splits == 1 && (p.ldy & 1) == 0) {
@@ -966,6 +1015,7 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
             if (trw) TWQ_TR(3, trn, 6);
 #endif
         }
+        if (y_pending) bulk_wait_all0();     // the staged tiles are in global memory before the CTA goes away
     }
 
     // ---------------------------------------------------------------- teardown
@@ -1050,7 +1100,7 @@ cudaError_t launch_fused_inst(const FusedMaps& maps, const FusedParams& p, cudaS
     ++na;
     cfg.attrs = attrs;
     cfg.numAttrs = static_cast<unsigned>(na);
-    return cudaLaunchKernelEx(&cfg, kern, maps.W, maps.Xq, maps.X, maps.L1T, maps.L2T, p);
+    return cudaLaunchKernelEx(&cfg, kern, maps.W, maps.Xq, maps.X, maps.L1T, maps.L2T, maps.Y, p);
 }
 
 // How many clusters of `cs` CTAs (one CTA per SM) the device can hold at once; 0 on failure.

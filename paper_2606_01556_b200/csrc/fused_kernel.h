@@ -20,7 +20,8 @@ struct FusedPlan {
     int nsp, nsu, ns1;       // ring depths: packed (TMA), expanded (MMA operands), stage-1
     int alias;               // 1: the stage-1 ring and the FP32 H partial overlay the residual rings
     int pair;                // 1: CTA pairs (cta_group::2): ranks 2i / 2i+1 of a cluster share one M = 256 MMA
-    int off_H, off_L2T, off_U, off_P, off_S1, off_Hpart, off_sx, off_bar;
+    int ystage;              // 1: the epilogue parks the finished tile in shared memory and bulk-copies it out (async)
+    int off_H, off_L2T, off_U, off_P, off_S1, off_Hpart, off_sx, off_bar, off_Y;
     int smem_bytes;
     int tmem_cols;           // 256 or 512
 };
@@ -38,7 +39,7 @@ struct FusedParams {
 };
 
 struct FusedMaps {
-    CUtensorMap W, Xq, X, L1T, L2T;
+    CUtensorMap W, Xq, X, L1T, L2T, Y;
 };
 
 

@@ -203,6 +203,14 @@ twq_status twq_dual_linear(const void* X, int ldx, const uint8_t* Xq, const floa
         ok &= make_map(&maps.L2T, CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 2, base + lay.off_l2t, r, N,
                        static_cast<uint64_t>(r) * 2, 64, 128, CU_TENSOR_MAP_SWIZZLE_128B);
     }
+    if (p.plan.ystage) {
+        // asynchronous tile store: 16-bit outputs with a row pitch TMA accepts (a multiple of 16 bytes)
+        if (static_cast<int>(ydt) <= 1 && (ldy & 7) == 0)
+            ok &= make_map(&maps.Y, CU_TENSOR_MAP_DATA_TYPE_UINT16, 2, Y, N, M, static_cast<uint64_t>(ldy) * 2, 64, TN,
+                           CU_TENSOR_MAP_SWIZZLE_128B);
+        else
+            p.plan.ystage = 0;     // the kernel stores from registers (the staging bytes stay unused)
+    }
     if (!ok) return TWQ_ERR_CUDA;
 
     p.M = M; p.N = N; p.K = K; p.r = r; p.ng = K / G;
