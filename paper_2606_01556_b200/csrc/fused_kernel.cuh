@@ -196,7 +196,6 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
     uint8_t* sY = smem + pl.off_Y;          // output staging (only when pl.ystage): 2 x [TN][64 channels], 128B-swizzled
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem + pl.off_bar);
     uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + B_COUNT);
-    __shared__ int s_last;
 
     const int warp = threadIdx.x >> 5;
     const int lane = threadIdx.x & 31;
@@ -770,15 +769,18 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
                 mbar_wait(&bars[B_TFULL + b], pb, 44);
                 tc_fence_after();
                 if (active) {
+                    // all loads in flight, one wait (the accumulator registers are free at this point)
+                    uint32_t v[C::kCPW][16];
+#pragma unroll
+                    for (int i = 0; i < C::kCPW; ++i) tmem_ld16(tlane + C::kColP + b * TN + col0 + i * 16, v[i]);
+                    tmem_ld_wait();
+#pragma unroll
+                    for (int i = 0; i < C::kCPW; ++i) tmem_st16(tlane + C::kColP + b * TN + col0 + i * 16, kfill);
 #pragma unroll
                     for (int i = 0; i < C::kCPW; ++i) {
-                        uint32_t v[16];
-                        tmem_ld16(tlane + C::kColP + b * TN + col0 + i * 16, v);
-                        tmem_ld_wait();
-                        tmem_st16(tlane + C::kColP + b * TN + col0 + i * 16, kfill);
 #pragma unroll
                         for (int c2 = 0; c2 < 8; ++c2)
-                            acc[i * 8 + c2] = (static_cast<uint64_t>(v[2 * c2 + 1]) << 32) | v[2 * c2];
+                            acc[i * 8 + c2] = (static_cast<uint64_t>(v[i][2 * c2 + 1]) << 32) | v[i][2 * c2];
                     }
                     tmem_st_wait();
                 }
@@ -968,12 +970,16 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
                         y_pending = true;
                     }
                 }
-            } else if (active && pl.splits == 1 && (p.ldy & 1) == 0) {
+            } else if (active && (pl.splits > 1 || (p.ldy & 1) == 0)) {
                 // Lane = output channel, register = token: neighbouring lanes trade one value per token pair, so the
                 // even lane holds channels (n, n+1) of token 2i and the odd lane channels (n-1, n) of token 2i+1 --
                 // half as many store instructions, each lane a 4-byte (FP32 output: 8-byte) word.  N is even.
+                // Split-K partials (FP32, workspace [ks][M][N]) take the FP32 form of it.
                 const bool odd = lane & 1;
                 const int nn = n - (odd ? 1 : 0);
+                const bool part = pl.splits > 1;
+                float* const y32 = part ? p.ws_part + static_cast<size_t>(t.ks) * p.M * p.N : static_cast<float*>(p.Y);
+                const int ld32 = part ? p.N : p.ldy;
 #pragma unroll
                 for (int i = 0; i < kNA; ++i) {
                     float y0, y1;
@@ -983,17 +989,17 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
                     const int m = t.m0 + col0 + i * 2 + (odd ? 1 : 0);
                     if (n_ok && m < p.M) {
                         const size_t o = static_cast<size_t>(m) * p.ldy + nn;
-                        if (p.ydt == 0) {
+                        if (part || p.ydt == 2) {
+                            *reinterpret_cast<float2*>(y32 + static_cast<size_t>(m) * ld32 + nn) = make_float2(lo, hi);
+                        } else if (p.ydt == 0) {
                             const __nv_bfloat162 v = __floats2bfloat162_rn(lo, hi);
                             *reinterpret_cast<__nv_bfloat162*>(static_cast<__nv_bfloat16*>(p.Y) + o) = v;
-                        } else if (p.ydt == 1) {
-                            *reinterpret_cast<__half2*>(static_cast<__half*>(p.Y) + o) = __floats2half2_rn(lo, hi);
                         } else {
-                            *reinterpret_cast<float2*>(static_cast<float*>(p.Y) + o) = make_float2(lo, hi);
+                            *reinterpret_cast<__half2*>(static_cast<__half*>(p.Y) + o) = __floats2half2_rn(lo, hi);
                         }
                     }
                 }
-            } else if (active && n_ok) {   // split-K partial (FP32, workspace [ks][M][N]) or an odd row pitch
+            } else if (active && n_ok) {   // odd row pitch: element stores
 #pragma unroll
                 for (int i = 0; i < kNA; ++i) {
                     float y2[2];
@@ -1003,8 +1009,7 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
                         const int m = t.m0 + col0 + i * 2 + e;
                         if (m >= p.M) continue;
                         const size_t o = static_cast<size_t>(m) * p.ldy + n;
-                        if (pl.splits > 1) p.ws_part[(static_cast<size_t>(t.ks) * p.M + m) * p.N + n] = y2[e];
-                        else if (p.ydt == 0) static_cast<__nv_bfloat16*>(p.Y)[o] = __float2bfloat16_rn(y2[e]);
+                        if (p.ydt == 0) static_cast<__nv_bfloat16*>(p.Y)[o] = __float2bfloat16_rn(y2[e]);
                         else if (p.ydt == 1) static_cast<__half*>(p.Y)[o] = __float2half_rn(y2[e]);
                         else static_cast<float*>(p.Y)[o] = y2[e];
                     }
@@ -1029,41 +1034,65 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
     }
 
     if (pl.splits > 1) {
-        // Deterministic split-K fix-up (one unit per cluster when splits > 1): the last CTA of this
-        // (n-tile, m-tile) to finish sums the partials in split order and writes Y; the tile counter is
-        // left at zero for the next call.
+        // Deterministic split-K fix-up (one unit per cluster when splits > 1, so every CTA of the grid is resident):
+        // the CTAs that hold the K splits of one (n-tile, m-tile) wait for one another on the tile counter, then each
+        // sums a share of the rows over all partials in split order and writes Y.  The counter runs 0 .. splits
+        // (partials parked) .. 2*splits (shares written) and the last CTA leaves it at zero for the next call.
         const Unit t = decode_unit(p, u_begin, rank);
+        unsigned* ctr = p.ws_ctr + (t.m0 / TN) * pl.n_tiles + t.n0 / kTileN;
         __threadfence();
         __syncthreads();
         if (threadIdx.x == 0) {
-            unsigned* ctr = p.ws_ctr + (t.m0 / TN) * pl.n_tiles + t.n0 / kTileN;
-            const unsigned prev = atomicAdd(ctr, 1u);
-            s_last = prev == static_cast<unsigned>(pl.splits - 1);
-            if (s_last) *ctr = 0;
+            atomicAdd(ctr, 1u);
+            unsigned seen;
+            do {
+                asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(seen) : "l"(ctr) : "memory");
+                if (seen < static_cast<unsigned>(pl.splits)) __nanosleep(64);
+            } while (seen < static_cast<unsigned>(pl.splits));
+            __threadfence();
         }
         __syncthreads();
-        if (s_last) {
-            __threadfence();
+        {
             const int rows = min(TN, p.M - t.m0);
+            const int r0 = rows * t.ks / pl.splits, r1 = rows * (t.ks + 1) / pl.splits;
             // four channels per thread and step (N is a multiple of 16, the workspace 256-byte aligned): the
             // loads of all splits are independent, the sum is in split order
-            for (int idx = threadIdx.x; idx < rows * (kTileN / 4); idx += kThreads) {
-                const int mm = t.m0 + idx / (kTileN / 4), nn = t.n0 + (idx % (kTileN / 4)) * 4;
+            for (int idx = threadIdx.x; idx < (r1 - r0) * (kTileN / 4); idx += kThreads) {
+                const int mm = t.m0 + r0 + idx / (kTileN / 4), nn = t.n0 + (idx % (kTileN / 4)) * 4;
                 if (nn >= p.N) continue;
                 float4 y = make_float4(0.f, 0.f, 0.f, 0.f);
                 for (int z = 0; z < pl.splits; ++z) {
                     const float4 v = __ldcg(reinterpret_cast<const float4*>(p.ws_part + (static_cast<size_t>(z) * p.M + mm) * p.N + nn));
                     y.x += v.x; y.y += v.y; y.z += v.z; y.w += v.w;
                 }
-                const float yv[4] = {y.x, y.y, y.z, y.w};
                 const size_t o = static_cast<size_t>(mm) * p.ldy + nn;
+                if (p.ydt == 2 && (p.ldy & 3) == 0) {
+                    *reinterpret_cast<float4*>(static_cast<float*>(p.Y) + o) = y;
+                } else if (p.ydt <= 1 && (p.ldy & 3) == 0) {
+                    uint2 w;
+                    if (p.ydt == 0) {
+                        const __nv_bfloat162 a = __floats2bfloat162_rn(y.x, y.y), c = __floats2bfloat162_rn(y.z, y.w);
+                        w = make_uint2(*reinterpret_cast<const uint32_t*>(&a), *reinterpret_cast<const uint32_t*>(&c));
+                    } else {
+                        const __half2 a = __floats2half2_rn(y.x, y.y), c = __floats2half2_rn(y.z, y.w);
+                        w = make_uint2(*reinterpret_cast<const uint32_t*>(&a), *reinterpret_cast<const uint32_t*>(&c));
+                    }
+                    *reinterpret_cast<uint2*>(static_cast<uint8_t*>(p.Y) + o * 2) = w;
+                } else {
+                    const float yv[4] = {y.x, y.y, y.z, y.w};
 #pragma unroll
-                for (int e = 0; e < 4; ++e) {
-                    if (p.ydt == 0) static_cast<__nv_bfloat16*>(p.Y)[o + e] = __float2bfloat16_rn(yv[e]);
-                    else if (p.ydt == 1) static_cast<__half*>(p.Y)[o + e] = __float2half_rn(yv[e]);
-                    else static_cast<float*>(p.Y)[o + e] = yv[e];
+                    for (int e = 0; e < 4; ++e) {
+                        if (p.ydt == 0) static_cast<__nv_bfloat16*>(p.Y)[o + e] = __float2bfloat16_rn(yv[e]);
+                        else if (p.ydt == 1) static_cast<__half*>(p.Y)[o + e] = __float2half_rn(yv[e]);
+                        else static_cast<float*>(p.Y)[o + e] = yv[e];
+                    }
                 }
             }
+        }
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            const unsigned prev = atomicAdd(ctr, 1u);
+            if (prev == static_cast<unsigned>(2 * pl.splits - 1)) atomicExch(ctr, 0u);
         }
     }
     if (cs > 1) cluster_sync_all();   // no CTA exits while a peer may still touch its shared memory
