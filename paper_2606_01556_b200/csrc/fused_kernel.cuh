@@ -980,25 +980,41 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
                 const bool part = pl.splits > 1;
                 float* const y32 = part ? p.ws_part + static_cast<size_t>(t.ks) * p.M * p.N : static_cast<float*>(p.Y);
                 const int ld32 = part ? p.N : p.ldy;
+                // one straight-line copy per format; the shuffles of eight token pairs are issued together, ahead of
+                // the (predicated) stores: with a branch per pair each store waited for its own shuffle (~130 cycles)
+                auto store_pairs = [&](auto kKind) {
+                    constexpr int kind = decltype(kKind)::value;   // 0 bf16, 1 fp16, 2 fp32
 #pragma unroll
-                for (int i = 0; i < kNA; ++i) {
-                    float y0, y1;
-                    unpack_f2(acc[i], y0, y1);
-                    const float got = __shfl_xor_sync(0xffffffffu, odd ? y0 : y1, 1);
-                    const float lo = odd ? got : y0, hi = odd ? y1 : got;   // channels nn, nn + 1
-                    const int m = t.m0 + col0 + i * 2 + (odd ? 1 : 0);
-                    if (n_ok && m < p.M) {
-                        const size_t o = static_cast<size_t>(m) * p.ldy + nn;
-                        if (part || p.ydt == 2) {
-                            *reinterpret_cast<float2*>(y32 + static_cast<size_t>(m) * ld32 + nn) = make_float2(lo, hi);
-                        } else if (p.ydt == 0) {
-                            const __nv_bfloat162 v = __floats2bfloat162_rn(lo, hi);
-                            *reinterpret_cast<__nv_bfloat162*>(static_cast<__nv_bfloat16*>(p.Y) + o) = v;
-                        } else {
-                            *reinterpret_cast<__half2*>(static_cast<__half*>(p.Y) + o) = __floats2half2_rn(lo, hi);
+                    for (int i0 = 0; i0 < kNA; i0 += 8) {
+                        float lo[8], hi[8];
+#pragma unroll
+                        for (int j = 0; j < 8; ++j) {
+                            float y0, y1;
+                            unpack_f2(acc[i0 + j], y0, y1);
+                            const float got = __shfl_xor_sync(0xffffffffu, odd ? y0 : y1, 1);
+                            lo[j] = odd ? got : y0;               // channels nn, nn + 1
+                            hi[j] = odd ? y1 : got;
+                        }
+#pragma unroll
+                        for (int j = 0; j < 8; ++j) {
+                            const int m = t.m0 + col0 + (i0 + j) * 2 + (odd ? 1 : 0);
+                            if (n_ok && m < p.M) {
+                                if (kind == 2) {
+                                    *reinterpret_cast<float2*>(y32 + static_cast<size_t>(m) * ld32 + nn) = make_float2(lo[j], hi[j]);
+                                } else if (kind == 0) {
+                                    *reinterpret_cast<__nv_bfloat162*>(static_cast<__nv_bfloat16*>(p.Y) + static_cast<size_t>(m) * p.ldy + nn) =
+                                        __floats2bfloat162_rn(lo[j], hi[j]);
+                                } else {
+                                    *reinterpret_cast<__half2*>(static_cast<__half*>(p.Y) + static_cast<size_t>(m) * p.ldy + nn) =
+                                        __floats2half2_rn(lo[j], hi[j]);
+                                }
+                            }
                         }
                     }
-                }
+                };
+                if (part || p.ydt == 2) store_pairs(std::integral_constant<int, 2>{});
+                else if (p.ydt == 0) store_pairs(std::integral_constant<int, 0>{});
+                else store_pairs(std::integral_constant<int, 1>{});
             } else if (active && n_ok) {   // odd row pitch: element stores
 #pragma unroll
                 for (int i = 0; i < kNA; ++i) {
