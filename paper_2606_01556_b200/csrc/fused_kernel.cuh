@@ -496,18 +496,29 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
         int trn = (warp == 4 && lane == 0) ? 0 : 4096;
 #endif
         float sxv[8];                                 // scales of the next block of 8 groups for token row u_tid
+        // scales of the unit the last fetch came from: row pointer (at the unit's first group) and validity.  A fetch
+        // inside the same unit only advances along the row; decode_unit (integer divisions, ~500 cycles) runs once per unit.
+        const float* fx_row = p.sx;
+        bool fx_ok = false;
+        auto fetch_sx = [&](const float* src, int left) {
+            if (fx_ok && left >= 8 && (reinterpret_cast<uintptr_t>(src) & 15u) == 0) {
+                const float4 a = __ldg(reinterpret_cast<const float4*>(src)), c = __ldg(reinterpret_cast<const float4*>(src) + 1);
+                sxv[0] = a.x; sxv[1] = a.y; sxv[2] = a.z; sxv[3] = a.w;
+                sxv[4] = c.x; sxv[5] = c.y; sxv[6] = c.z; sxv[7] = c.w;
+            } else {
+#pragma unroll
+                for (int j = 0; j < 8; ++j) sxv[j] = (fx_ok && j < left) ? __ldg(src + j) : 0.0f;
+            }
+        };
         {
 #pragma unroll
             for (int j = 0; j < 8; ++j) sxv[j] = 0.0f;
             if (!w_role && u_begin < u_end) {
                 const Unit t0 = decode_unit(p, u_begin, rank);
                 const int m = t0.m0 + u_tid;
-                if (u_tid < TN && m < p.M) {
-                    const float* src = p.sx + static_cast<size_t>(m) * p.ng + t0.g_begin;
-                    const int left = t0.g_end - t0.g_begin;
-#pragma unroll
-                    for (int j = 0; j < 8; ++j) sxv[j] = j < left ? __ldg(src + j) : 0.0f;
-                }
+                fx_ok = u_tid < TN && m < p.M;
+                fx_row = p.sx + static_cast<size_t>(fx_ok ? m : 0) * p.ng + t0.g_begin;
+                fetch_sx(fx_row, t0.g_end - t0.g_begin);
             }
         }
         for (int u = u_begin; u < u_end; ++u) {
@@ -550,16 +561,14 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
 #pragma unroll
                         for (int j = 0; j < 8; ++j) sSx[((itp + j) & (kSxSlots - 1)) * TN + u_tid] = sxv[j] * 0x1p-8f;
                     }
-                    int nu = u, ngi = gi + 8;
-                    if (ngi >= ngr) { nu = u + 1; ngi = 0; }
-                    if (nu < u_end) {
-                        const Unit tn = decode_unit(p, nu, rank);
+                    if (gi + 8 < ngr) {
+                        fetch_sx(fx_row + gi + 8, ngr - gi - 8);          // same unit: fx_row is this unit's row
+                    } else if (u + 1 < u_end) {
+                        const Unit tn = decode_unit(p, u + 1, rank);
                         const int m = tn.m0 + u_tid;
-                        const bool ok = u_tid < TN && m < p.M;
-                        const float* src = p.sx + static_cast<size_t>(ok ? m : 0) * p.ng + tn.g_begin + ngi;
-                        const int left = tn.g_end - tn.g_begin - ngi;
-#pragma unroll
-                        for (int j = 0; j < 8; ++j) sxv[j] = (ok && j < left) ? __ldg(src + j) : 0.0f;
+                        fx_ok = u_tid < TN && m < p.M;
+                        fx_row = p.sx + static_cast<size_t>(fx_ok ? m : 0) * p.ng + tn.g_begin;
+                        fetch_sx(fx_row, tn.g_end - tn.g_begin);
                     }
                 }
                 TWQ_TR(2, trn, 1);
