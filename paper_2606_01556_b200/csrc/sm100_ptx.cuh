@@ -93,7 +93,6 @@ __device__ __forceinline__ void mbar_wait_a(uint32_t bar, uint32_t parity, int t
     }
 }
 
-// ------------------------------------------------------------------ fences
 // ---- asynchronous tile store shared -> global (TMA, bulk-group completion) -----------------------------------
 __device__ __forceinline__ void tma_store_2d(const CUtensorMap* m, uint32_t src_smem, int c0, int c1) {
     asm volatile("cp.async.bulk.tensor.2d.global.shared::cta.bulk_group [%0, {%2, %3}], [%1];"
@@ -109,6 +108,7 @@ __device__ __forceinline__ void named_bar_sync(int id, int count) {
     asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(count) : "memory");
 }
 
+// ------------------------------------------------------------------ fences
 __device__ __forceinline__ void fence_proxy_async_smem() {
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
 }
@@ -183,6 +183,15 @@ __device__ __forceinline__ void tma_load_2d_a(uint32_t smem_dst, const CUtensorM
         : "memory");
 }
 __device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+// The same wait, tied to the registers an earlier tcgen05.ld wrote: the compiler sees them redefined here, so no use of
+// them can be scheduled above the wait (needed when other work sits between the load and its wait).
+__device__ __forceinline__ void tmem_ld_wait_on(uint32_t (&v)[16]) {
+    asm volatile("tcgen05.wait::ld.sync.aligned;"
+                 : "+r"(v[0]), "+r"(v[1]), "+r"(v[2]), "+r"(v[3]), "+r"(v[4]), "+r"(v[5]), "+r"(v[6]), "+r"(v[7]),
+                   "+r"(v[8]), "+r"(v[9]), "+r"(v[10]), "+r"(v[11]), "+r"(v[12]), "+r"(v[13]), "+r"(v[14]), "+r"(v[15])
+                 :
+                 : "memory");
+}
 
 // 32 lanes x 16 columns store (registers -> TMEM), thread i writes lane (base_lane+i).
 __device__ __forceinline__ void tmem_st16(uint32_t taddr, const uint32_t (&v)[16]) {
