@@ -211,7 +211,7 @@ def roofline_for(L, twq, us_dual, peaks, traffic=None):
 TRAFFIC_BYTES = {
     "c2_qproj_m1": 11086848,          # profiles/r01c_full_decode_c2_qproj_m1.txt
     "c2_qproj_m16": 11246080,         # profiles/r01c_full_decode_c2_qproj_m16.txt
-    "c3_gateup_m2048": 112169216,     # profiles/r01c_full_fused_c3_gateup_m2048.txt
+    "c3_gateup_m2048": 111107840,     # profiles/r01d_full_fused_c3_gateup_m2048.txt
 }
 
 
