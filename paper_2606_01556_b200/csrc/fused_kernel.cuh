@@ -954,10 +954,31 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
                     }
                 }
                 };
+                // Staged tiles need no transpose: the lane writes its own 2-byte elements into the swizzled tile (a warp
+                // covers 64 contiguous bytes of one token row: one wavefront), 64 stores and no shuffle chains.
+                auto stage16 = [&](auto kBf16) {
+                    // byte address of this lane's channel in a row with (row & 7) == j; rows are col0 + 2i + e
+                    const int chan = (qd & 1) * 32 + lane;                 // channel inside the 64-channel half
+                    uint8_t* const half = sY + (qd >> 1) * (TN * 128) + col0 * 128 + (chan & 7) * 2;
+                    uint8_t* rowp[8];
+#pragma unroll
+                    for (int j = 0; j < 8; ++j) rowp[j] = half + ((((chan >> 3) ^ j) & 7) << 4);
+#pragma unroll
+                    for (int i = 0; i < kNA; ++i) {
+                        float y0, y1;
+                        unpack_f2(acc[i], y0, y1);
+                        uint32_t w;
+                        if (decltype(kBf16)::value) { const __nv_bfloat162 v = __floats2bfloat162_rn(y0, y1); w = *reinterpret_cast<const uint32_t*>(&v); }
+                        else { const __half2 v = __floats2half2_rn(y0, y1); w = *reinterpret_cast<const uint32_t*>(&v); }
+                        *reinterpret_cast<uint16_t*>(rowp[(2 * i) & 7] + (2 * i) * 128) = static_cast<uint16_t>(w);
+                        *reinterpret_cast<uint16_t*>(rowp[(2 * i + 1) & 7] + (2 * i + 1) * 128) = static_cast<uint16_t>(w >> 16);
+                    }
+                };
                 using TrueT = std::integral_constant<bool, true>;
                 using FalseT = std::integral_constant<bool, false>;
-                if (p.ydt == 0) { if (staged) store16(TrueT{}, TrueT{}); else store16(TrueT{}, FalseT{}); }
-                else { if (staged) store16(FalseT{}, TrueT{}); else store16(FalseT{}, FalseT{}); }
+                if (staged) { if (p.ydt == 0) stage16(TrueT{}); else stage16(FalseT{}); }
+                else if (p.ydt == 0) store16(TrueT{}, FalseT{});
+                else store16(FalseT{}, FalseT{});
 #ifdef TWQ_TRACE
                 if (trw) TWQ_TR(3, trn, 9);
 #endif
