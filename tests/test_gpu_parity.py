@@ -149,6 +149,34 @@ def test_fused_kernel_cta_pairs(twq, oracle, monkeypatch, M, K, N, r, G):
     _check_layer(twq, oracle, gen.make_layer(M, K, N, r, G, seed=3000 + M, with_tinv=(M % 2 == 0)), rows=rows)
 
 
+@pytest.mark.parametrize("pad", [0, 8, 2, 1])
+@pytest.mark.parametrize("split,N", [(False, 1232), (False, 1200), (True, 1232)])
+def test_fused_kernel_store_paths(twq, oracle, monkeypatch, pad, split, N):
+    """Every store path of the fused kernel writes the same Y (fused_kernel.cuh, 'The store of a finished tile' in
+    DESIGN.md 6.2): row pitch N + pad selects staged TMA tiles / 16-byte transposed stores (pad % 8 == 0), lane pairs
+    (even pad) or element stores (odd pad); unsplit 128-token tiles (CTA pairs: 10 channel tiles) or the split-K
+    fix-up.  Ragged last token tile and a last channel tile of 80 / 48 channels (the second half-tile store is
+    clipped / skipped); columns beyond N must stay untouched."""
+    import torch
+    M, K, r, G = 300, 512, 64, 128
+    if not split:
+        monkeypatch.setenv("TWQ_DEBUG_NO_SPLIT", "1")
+    L = gen.make_layer(M, K, N, r, G, seed=4100)
+    X, packed, _ = _upload(twq, L)
+    Xq, sx = twq.quantize_act(X, G)
+    ref = oracle.forward(L.X, L.Rq, L.sw, L.L1, L.L2, G, want_P=False)["Y"]
+    Y32 = twq.dual_linear(X, Xq, sx, packed, twq.OUT_FP32)
+    assert np.abs(Y32.cpu().numpy().astype(np.float64) - ref).max() / np.abs(ref).max() <= TOL
+    for od, dt in ((twq.OUT_FP32, torch.float32), (twq.OUT_BF16, torch.bfloat16), (twq.OUT_FP16, torch.float16)):
+        buf = torch.full((M, N + pad), -77.0, dtype=dt, device="cuda")
+        Y = buf[:, :N]
+        twq.dual_linear(X, Xq, sx, packed, od, Y=Y)
+        torch.cuda.synchronize()
+        assert (_bits(Y.contiguous()) == _bits(Y32.to(dt))).all(), (od, pad)
+        if pad:
+            assert (buf[:, N:] == -77.0).all(), "wrote beyond N"
+
+
 def test_rank0_is_plain_w4a4_and_zero_residual_is_lowrank(twq, oracle):
     """north_star special cases, on the GPU path."""
     import torch
