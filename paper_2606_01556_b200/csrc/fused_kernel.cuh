@@ -48,6 +48,12 @@
 // value of the epilogue's register accumulators, so it needs no TMEM columns of its own.
 // Group scales are staged ahead of use: the preparation warps fetch sx for 8 groups at a time,
 // one block ahead; the epilogue warps fetch sw two groups ahead.
+//
+// Store of a finished tile (a thread owns one channel x TN/2 tokens): 128-token tiles of 16-bit outputs are
+// written into a 128B-swizzled shared-memory tile and leave through two asynchronous TMA stores while the
+// next tile is computed; other 16-bit cases transpose 8 x 8 among lanes to 16-byte stores; FP32 outputs and
+// split-K partials pair neighbouring lanes (8-byte stores).  Split-K calls (one unit per cluster, whole grid
+// resident): the CTAs holding the splits of a tile meet on the tile counter and each sums a share of the rows.
 #pragma once
 #include <cuda_bf16.h>
 #include <cuda_fp16.h>
