@@ -116,7 +116,9 @@ static bool make_plan_tn(int TN, int M, int N, int K, int r, int G, int num_sms,
     auto total = [&](const FusedPlan& q) {
         const int resid = q.nsu * ub + round_up(q.nsp * pb, 1024);
         const int s1 = q.alias ? (q.ns1 * s1b > hpart ? q.ns1 * s1b : hpart) : q.ns1 * s1b + hpart;
-        return hbytes + l2bytes + (q.alias ? (resid > s1 ? resid : s1) : resid + s1) + (q.ystage ? ybytes + 1024 : 0);
+        const int ys = q.ystage ? ybytes + 1024 : 0;
+        if (q.alias == 2) return hbytes + (l2bytes + resid > s1 ? l2bytes + resid : s1) + ys;
+        return hbytes + l2bytes + (q.alias ? (resid > s1 ? resid : s1) : resid + s1) + ys;
     };
     if (pl.ystage) {
         FusedPlan q = pl;
@@ -126,6 +128,17 @@ static bool make_plan_tn(int TN, int M, int N, int K, int r, int G, int num_sms,
         else if (total(pl) > budget) pl.nsp = q.nsp;
     }
     if (total(pl) > budget) { pl.alias = 1; pl.ns1 = r > 0 ? 3 : 0; }
+    if (total(pl) > budget && r > 0 && getenv("TWQ_DEBUG_NO_ALIAS2") == nullptr) {
+        // Rank-256 buffers beside a 128-token tile: the stage-1 ring and the FP32 partial of H overlay the L2T tile as
+        // well as the residual rings.  L2T is dead whenever stage 1 runs: its stage-2 MMAs were issued at the start
+        // of the previous tile, whose residual MMAs (B_RESID) the producer waits for before the first stage-1 load,
+        // and the next L2T load follows B_HREADY (the same two waits that protect the rings).
+        FusedPlan q = pl;
+        q.alias = 2;
+        q.ystage = 0;
+        while (total(q) > budget && q.nsp > 4) --q.nsp;
+        if (total(q) <= budget) pl = q;
+    }
     while (total(pl) > budget && pl.nsp > 2) --pl.nsp;
     while (total(pl) > budget && pl.nsu > 2) --pl.nsu;
     while (total(pl) > budget && pl.ns1 > 2) --pl.ns1;
@@ -136,7 +149,12 @@ static bool make_plan_tn(int TN, int M, int N, int K, int r, int G, int num_sms,
     pl.off_U = o;
     pl.off_P = o + pl.nsu * ub;
     const int resid = pl.nsu * ub + round_up(pl.nsp * pb, 1024);
-    if (pl.alias) {
+    if (pl.alias == 2) {
+        pl.off_S1 = pl.off_L2T;
+        pl.off_Hpart = pl.off_L2T;
+        const int s1 = pl.ns1 * s1b > hpart ? pl.ns1 * s1b : hpart;
+        o = pl.off_L2T + (l2bytes + resid > s1 ? l2bytes + resid : s1);
+    } else if (pl.alias) {
         pl.off_S1 = o;
         pl.off_Hpart = o;   // the FP32 partial is written after the stage-1 MMAs completed
         const int s1 = pl.ns1 * s1b > hpart ? pl.ns1 * s1b : hpart;

@@ -139,6 +139,9 @@ def test_decode_kernel_shapes(twq, oracle, M, K, N, r, G):
     (300, 1024, 1024, 128, 128),  # ragged last token tile: the odd CTA's half of the B rows is all padding
     (129, 256, 256, 16, 128),     # one live row in the second tile; smallest rank
     (640, 2048, 2304, 128, 128),  # several tiles per cluster and a change of token tile inside a cluster's list
+    (640, 1024, 2304, 256, 128),  # rank 256: the stage-1 ring / H partial overlay the L2T tile too (plan.alias == 2),
+                                  # with a new token tile's stage 1 following tiles that used L2T
+    (300, 512, 1280, 256, 64),    # the same overlay with G = 64 and a ragged token tile
 ])
 def test_fused_kernel_cta_pairs(twq, oracle, monkeypatch, M, K, N, r, G):
     """128-token tiles in an even cluster run as CTA pairs (cta_group::2, fused_kernel.cuh); same bar.
