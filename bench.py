@@ -10,7 +10,7 @@ over one batch of synthetic activations for one layer.  Prints ONE JSON line (ra
   e2e        the same through the public Python API with pinned-host X -> device and Y -> host inside the region
   roofline   the fused kernel alone (its own K-launch graph): algorithmic bytes or int8-equivalent ops / time
   cpu_baseline  the oracle (oracle/, as it stands) on the host cores, on a bounded sample
-  sweep      the other graded shapes (M = 1 / 16 / 128 q_proj, M = 2048 MLP) measured the same way
+  sweep      the other graded shapes (M = 1 / 16 / 128 q_proj, M = 2048 MLP at r = 128 and 256) measured the same way
 
 Cold-cache protocol: the layer's packed weights (and activations) are rotated through enough distinct
 copies that one lap exceeds 2x the 126 MB L2, so every step streams its weights from HBM.
@@ -46,7 +46,8 @@ WORKLOADS = {
     "c1_tiny": ("config1_tiny", dict(), "tiny M=8 K=256 N=512 r=16 G=64"),
 }
 DEFAULT_WORKLOAD = "c2_qproj_m16"
-DEFAULT_SWEEP = ["c2_qproj_m1", "c2_qproj_m16", "c2_qproj_m128", "c3_gateup_m2048", "c3_down_m2048"]
+DEFAULT_SWEEP = ["c2_qproj_m1", "c2_qproj_m16", "c2_qproj_m128", "c3_gateup_m2048", "c3_down_m2048",
+                 "c3_gateup_m2048_r256"]
 
 
 def load_peaks():
