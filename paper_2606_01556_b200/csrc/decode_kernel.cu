@@ -211,8 +211,11 @@ __global__ void __launch_bounds__(kDecThreads, 1) decode_dual_linear_kernel(cons
     // ---------------------------------------------------------------- low-rank stage 1: H partial of this CTA's K slice
     if (r > 0) {
         const int units = p.K >> 5;                                  // 32-wide K units
-        const int u0 = static_cast<int>(static_cast<long long>(units) * rank / cs);
-        const int u1 = static_cast<int>(static_cast<long long>(units) * (rank + 1) / cs);
+        // K slice of this CTA: 1/cs of K, or (stage 1 over all clusters) 1/grid of K
+        const int kslice = p.ncl_k > 1 ? static_cast<int>(blockIdx.x) : rank;
+        const int kslices = p.ncl_k > 1 ? static_cast<int>(gridDim.x) : cs;
+        const int u0 = static_cast<int>(static_cast<long long>(units) * kslice / kslices);
+        const int u1 = static_cast<int>(static_cast<long long>(units) * (kslice + 1) / kslices);
         const int nu = u1 - u0;
         constexpr int kDL = 8;                                       // L1T loads in flight per thread
         // loads in the order the dependent chain needs them: X slice, first j-tile's L1T ring, residual weights
@@ -433,7 +436,59 @@ __global__ void __launch_bounds__(kDecThreads, 1) decode_dual_linear_kernel(cons
         if (cs > 1) {
             cluster_wait();                            // every CTA's FP32 partial is visible
             TWQ_DT(6);
-            if (p.M <= 2) {
+            if (p.ncl_k > 1) {
+                // Stage 1 over all clusters.  (a) reduce-scatter inside the cluster as below, but the FP32 sums of
+                // this CTA's r/cs columns go to the workspace [cluster][16][r]; (b) grid-wide barrier on the
+                // workspace counter; (c) sum over the clusters in fixed order (H is identical everywhere), FP16,
+                // all-gather through distributed shared memory.
+                const int jc = r / cs;
+                const int cl = static_cast<int>(blockIdx.x) / cs;
+                for (int i = threadIdx.x; i < p.M * jc; i += kDecThreads) {
+                    const int m = i / jc, j = rank * jc + (i - m * jc);
+                    const uint32_t src = smem_u32(sHpart + m * r + j);
+                    float s = 0.0f;
+                    for (int pr = 0; pr < cs; pr += 4) {
+                        float v[4];
+#pragma unroll
+                        for (int q = 0; q < 4; ++q) v[q] = pr + q < cs ? ld_dsmem_f(mapa_u32(src, pr + q)) : 0.0f;
+#pragma unroll
+                        for (int q = 0; q < 4; ++q) s += v[q];
+                    }
+                    p.ws_h[(static_cast<size_t>(cl) * 16 + m) * r + j] = s;
+                }
+                __syncthreads();
+                if (threadIdx.x == 0) {
+                    __threadfence();
+                    atomicAdd(p.ws_ctr, 1u);
+                    unsigned seen, spins = 0;
+                    do {
+                        asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(seen) : "l"(p.ws_ctr) : "memory");
+                        if (seen < gridDim.x) {
+                            __nanosleep(32);
+                            if (++spins > (1u << 24)) __trap();   // a CTA of the grid never arrived: fail loudly, do not hang
+                        }
+                    } while (seen < gridDim.x);
+                    __threadfence();
+                }
+                __syncthreads();
+                for (int i = threadIdx.x; i < p.M * jc; i += kDecThreads) {
+                    const int m = i / jc, j = rank * jc + (i - m * jc);
+                    float s = 0.0f;
+                    for (int c = 0; c < p.ncl_k; ++c) s += __ldcg(p.ws_h + (static_cast<size_t>(c) * 16 + m) * r + j);
+                    s = fminf(fmaxf(s, -65504.0f), 65504.0f);
+                    const __half hv = __float2half_rn(s);
+                    const uint32_t dsta = smem_u32(sH + m * hstride + j);
+                    for (int pr = 0; pr < cs; ++pr) st_dsmem_u16(mapa_u32(dsta, pr), *reinterpret_cast<const uint16_t*>(&hv));
+                }
+                __syncthreads();
+                if (threadIdx.x == 0) {
+                    fence_cluster();                       // release this CTA's remote stores
+                    const unsigned prev = atomicAdd(p.ws_ctr, 1u);   // second round: the last CTA leaves the counter at zero
+                    if (prev == 2u * gridDim.x - 1u) atomicExch(p.ws_ctr, 0u);
+                }
+                cluster_arrive_relaxed();
+                cluster_wait();                            // every CTA's slice of H has arrived
+            } else if (p.M <= 2) {
             // all-reduce by reading: every CTA sums the cs partials of the M live rows itself (fixed order, so
             // H is identical everywhere) -- one cluster barrier instead of a reduce-scatter plus an all-gather.
             // Distributed-shared-memory reads are slow (about 8 KB per microsecond per CTA here), so only for M <= 2.
@@ -650,6 +705,18 @@ bool decode_make_plan(int M, int N, int K, int r, int G, int num_sms, DecodePara
     if (nclusters < 1) nclusters = 1;
     p.grid = nclusters * p.cs;
     p.T = (p.n_tiles + p.grid - 1) / p.grid;
+    // Stage 1 over all clusters: every cluster otherwise streams ALL of L1T from L2 (K*r*2 bytes each), which is most
+    // of the traffic of a decode call on the larger layers.  With the K range split over the whole grid L1T is read
+    // once; the cluster-level partials of H then meet in the caller's workspace behind one grid-wide barrier (every
+    // CTA is resident: the grid is at most the occupancy-queried cluster capacity).  Worth its barrier from ~16 MB
+    // of avoided re-reads.
+    p.ncl_k = 1;
+    if (r > 0 && p.cs > 1 && nclusters > 1 && (K >> 5) >= p.grid) {
+        const long long avoided = 2LL * K * r * (nclusters - 1);
+        bool on = avoided >= (16LL << 20);
+        if (const char* e = getenv("TWQ_DEBUG_DECODE_GRIDK")) on = atoi(e) != 0;   // testing aid: force on / off
+        if (on) p.ncl_k = nclusters;
+    }
     p.P = p.ng < kDecWarps ? p.ng : kDecWarps;            // upper bound; each CTA takes 16 / (its tiles), see the kernel
     if (p.T > kDecWarps * kMaxItemsPerWarp) return false;
     const int kTok = M <= 8 ? 8 : 16;

@@ -51,6 +51,9 @@ struct DecodeParams {
     int cs, grid;            // CTAs per cluster, CTAs in the grid (a multiple of cs)
     int T, P;                // 16-channel tiles per CTA, K-parts per tile
     int off_res, off_hpart, off_h, off_ylr, off_sx, off_xs, smem_bytes;
+    int ncl_k;               // > 1: stage 1 splits K over ALL ncl_k clusters (L1T read once per call); partials meet in ws_h
+    float* ws_h;             // [ncl_k][16][r] FP32 cluster-level partials of H (caller's workspace)
+    unsigned* ws_ctr;        // grid barrier counter (zero between calls)
     const uint8_t* R4;       // [N][K/2]
     const float* swT;        // [ng][N]
     const void* L1T;         // [r][K] f16
@@ -62,6 +65,9 @@ struct DecodeParams {
     int32_t* dbgP;
 };
 bool decode_make_plan(int M, int N, int K, int r, int G, int num_sms, DecodeParams* out);
+inline size_t decode_workspace_bytes(const DecodeParams& p) {
+    return p.ncl_k > 1 ? 256 + ((static_cast<size_t>(p.ncl_k) * 16 * p.r * sizeof(float) + 255) & ~static_cast<size_t>(255)) : 0;
+}
 cudaError_t launch_decode(const DecodeParams& p, int G, cudaStream_t stream);
 
 // Fills `plan` for a shape; returns false if the shape cannot be planned (never for valid ABI shapes).

@@ -140,7 +140,7 @@ twq_status twq_quantize_act(const void* X, int M, int K, int ldx, const float* t
 size_t twq_workspace_bytes(int M, int N, int K, int r, int G) {
     if (!shape_ok(M, N, K, r, G)) return 0;
     twq::DecodeParams dp;
-    if (twq::decode_make_plan(M, N, K, r, G, num_sms(), &dp)) return 0;   // decode-shaped calls need no scratch
+    if (twq::decode_make_plan(M, N, K, r, G, num_sms(), &dp)) return twq::decode_workspace_bytes(dp);   // 0 for most
     twq::FusedPlan pl;
     if (!twq::fused_make_plan(M, N, K, r, G, num_sms(), &pl)) return 0;
     if (pl.splits <= 1) return 0;
@@ -177,6 +177,8 @@ twq_status twq_dual_linear(const void* X, int ldx, const uint8_t* Xq, const floa
         dp.L1T = base + lay.off_l1t;
         dp.L2T = base + lay.off_l2t;
         dp.X = X; dp.Xq = Xq; dp.sx = sx; dp.Y = Y; dp.dbgP = dbg_P;
+        dp.ws_ctr = static_cast<unsigned*>(ws);
+        dp.ws_h = dp.ncl_k > 1 ? reinterpret_cast<float*>(static_cast<uint8_t*>(ws) + 256) : nullptr;
         if (twq::launch_decode(dp, G, static_cast<cudaStream_t>(stream)) != cudaSuccess) return TWQ_ERR_CUDA;
         g_last_launches = 1;
         return TWQ_OK;

@@ -233,6 +233,32 @@ def test_exactly_representable_output_is_bit_exact(twq, oracle):
     assert (ref["Y"] == gen.bf16_bits_to_f32(oracle.round_bf16(ref["Y"])).astype(np.float64)).all()  # truly exact
 
 
+@pytest.mark.parametrize("M,K,N,r,G", [(1, 8192, 4096, 128, 128), (16, 8192, 2048, 256, 128), (5, 4096, 4096, 64, 64)])
+def test_decode_kernel_stage1_over_all_clusters(twq, oracle, monkeypatch, M, K, N, r, G):
+    """decode_kernel.cu with the K range of stage 1 split over the whole grid (DecodeParams.ncl_k > 1): cluster-level
+    partials of H meet in the workspace behind a grid-wide barrier.  Forced on for shapes the oracle finishes quickly;
+    the same workspace serves three calls in a row (the counter must come back to zero)."""
+    import torch
+    monkeypatch.setenv("TWQ_DEBUG_DECODE_GRIDK", "1")
+    need = twq.workspace_bytes(M, N, K, r, G)
+    assert need > 0
+    L = gen.make_layer(M, K, N, r, G, seed=5200 + M)
+    X, packed, _ = _upload(twq, L)
+    Xq, sx = twq.quantize_act(X, G)
+    ws = torch.zeros(need, dtype=torch.uint8, device="cuda")
+    ref = oracle.forward(L.X, L.Rq, L.sw, L.L1, L.L2, G, want_P=False)["Y"]
+    ys = [twq.dual_linear(X, Xq, sx, packed, twq.OUT_FP32, ws=ws) for _ in range(3)]
+    torch.cuda.synchronize()
+    for y in ys:
+        assert np.abs(y.cpu().numpy().astype(np.float64) - ref).max() / np.abs(ref).max() <= TOL
+        assert (y == ys[0]).all(), "not deterministic across calls"
+    assert int(ws[:4].view(torch.int32).item()) == 0, "barrier counter not left at zero"
+    monkeypatch.setenv("TWQ_DEBUG_DECODE_GRIDK", "0")
+    assert twq.workspace_bytes(M, N, K, r, G) == 0
+    y0 = twq.dual_linear(X, Xq, sx, packed, twq.OUT_FP32)
+    assert np.abs(y0.cpu().numpy().astype(np.float64) - ref).max() / np.abs(ref).max() <= TOL
+
+
 def test_decode_kernel_strides_fp16_output_no_workspace(twq, oracle):
     """M <= 16 runs the register-resident decode kernel: no scratch, padded Y rows untouched, repeatable."""
     import torch
