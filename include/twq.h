@@ -111,9 +111,13 @@ size_t twq_workspace_bytes(int M, int N, int K, int r, int G);
  *   Y      [M,ldy]          out, dtype ydt (ldy >= N elements)
  *   ws, ws_bytes            scratch of at least twq_workspace_bytes(...) bytes, 256-byte aligned (may be
  *                           NULL when that is 0).  It holds split-K partial sums and tile counters for
- *                           calls with few output tiles (16 < M, roughly M*N < 1.5 M outputs); calls with
- *                           M <= 16 and prefill-shaped calls need none.  The caller zero-fills it ONCE after allocation; every
- *                           call leaves the counters zero again, so it can be reused without clearing.
+ *                           calls with few output tiles (16 < M, roughly M*N < 1.5 M outputs), and, for
+ *                           M <= 16 on layers with a large low-rank factor (K*r above ~1.3 M elements),
+ *                           the per-cluster partial sums of H and a barrier counter; other calls with
+ *                           M <= 16 and prefill-shaped calls need none.  The caller zero-fills it ONCE
+ *                           after allocation; every call leaves the counters zero again, so it can be
+ *                           reused without clearing -- by calls on ONE stream at a time (two calls that
+ *                           share a workspace must not run concurrently).
  *   dbg_P  [M,K/G,N] int32  NULL, or receives the integer group accumulators P taken from the
  *                           same tensor-core path that feeds Y (parity evidence; slows the call)
  */
