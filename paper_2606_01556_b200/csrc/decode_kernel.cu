@@ -474,7 +474,15 @@ __global__ void __launch_bounds__(kDecThreads, 1) decode_dual_linear_kernel(cons
                 for (int i = threadIdx.x; i < p.M * jc; i += kDecThreads) {
                     const int m = i / jc, j = rank * jc + (i - m * jc);
                     float s = 0.0f;
-                    for (int c = 0; c < p.ncl_k; ++c) s += __ldcg(p.ws_h + (static_cast<size_t>(c) * 16 + m) * r + j);
+                    const float* src = p.ws_h + static_cast<size_t>(m) * r + j;
+                    for (int c0 = 0; c0 < p.ncl_k; c0 += 8) {      // eight loads in flight, summed in cluster order
+                        float v[8];
+#pragma unroll
+                        for (int q = 0; q < 8; ++q)
+                            v[q] = c0 + q < p.ncl_k ? __ldcg(src + static_cast<size_t>(c0 + q) * 16 * r) : 0.0f;
+#pragma unroll
+                        for (int q = 0; q < 8; ++q) s += v[q];
+                    }
                     s = fminf(fmaxf(s, -65504.0f), 65504.0f);
                     const __half hv = __float2half_rn(s);
                     const uint32_t dsta = smem_u32(sH + m * hstride + j);
