@@ -44,6 +44,14 @@ WORKLOADS = {
     "c3_down_m2048": ("config3_mlp", dict(which="down", M=2048), "LLaMA3-8B down K=14336 N=4096 r=128 G=128 M=2048"),
     "c3_gateup_m2048_r256": ("config3_mlp", dict(which="gate_up", M=2048, r=256), "LLaMA3-8B gate/up r=256 M=2048"),
     "c1_tiny": ("config1_tiny", dict(), "tiny M=8 K=256 N=512 r=16 G=64"),
+    # configs 4 / 5 (rank 256): not in the default sweep; DESIGN.md section 10 quotes them
+    "c4_gateup_m4096": ("config4_qwen", dict(which="gate_up", M=4096), "Qwen3-32B gate/up K=5120 N=25600 r=256 M=4096"),
+    "c4_down_m4096": ("config4_qwen", dict(which="down", M=4096), "Qwen3-32B down K=25600 N=5120 r=256 M=4096"),
+    "c4_down_m1": ("config4_qwen", dict(which="down", M=1), "Qwen3-32B down K=25600 N=5120 r=256 M=1"),
+    "c4_attn_m64": ("config4_qwen", dict(which="attn", M=64), "Qwen3-32B attention K=5120 N=5120 r=256 M=64"),
+    "c5_gateup_m2048": ("config5_llama70b", dict(which="gate_up", M=2048), "LLaMA3-70B gate/up K=8192 N=28672 r=256 M=2048"),
+    "c5_down_m1": ("config5_llama70b", dict(which="down", M=1), "LLaMA3-70B down K=28672 N=8192 r=256 M=1"),
+    "c5_qproj_m16": ("config5_llama70b", dict(which="q", M=16), "LLaMA3-70B q_proj K=8192 N=8192 r=256 M=16"),
 }
 DEFAULT_WORKLOAD = "c2_qproj_m16"
 DEFAULT_SWEEP = ["c2_qproj_m1", "c2_qproj_m16", "c2_qproj_m128", "c3_gateup_m2048", "c3_down_m2048",
