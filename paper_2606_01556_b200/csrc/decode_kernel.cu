@@ -674,7 +674,7 @@ int decode_cluster_capacity(int cs, int num_sms) {
         }
         cudaGetLastError();
     }
-    if (n <= 0) n = cs == 2 ? num_sms / 2 : (cs == 4 ? (num_sms / 4) * 7 / 8 : (cs == 8 ? (num_sms / 8) * 7 / 8 : 0));
+    if (n <= 0) n = cs == 2 ? num_sms / 2 : (cs == 4 ? (num_sms / 4) * 7 / 8 : (cs == 8 ? (num_sms / 8) * 7 / 8 : (num_sms / 16) * 7 / 8));
     if (n > num_sms / cs) n = num_sms / cs;
     cache[cs] = n;
     return n;
