@@ -47,6 +47,34 @@ def test_packed_bytes_accounts_for_every_section(lib):
         assert twq.packed_bytes(*bad) == 0, bad
 
 
+def test_algorithmic_bytes_pinned_to_paper_L86():
+    """bench.py's byte accounting (binding.algorithmic_bytes) against the two storage ratios PAPER.md L86
+    prints (tests/golden/paper_L86_storage_ratios.txt): the FP16 low-rank bytes are what the function adds when r goes
+    from 0 to r, and the 4-bit residual bytes are what remains of the r = 0 weights once the FP16 group scales are taken
+    out.  Also the activation-side terms, one by one (differences in M / out_bytes / with_quantizer)."""
+    from paper_2606_01556_b200.binding import algorithmic_bytes as ab
+    G = 128
+    with open(os.path.join(ROOT, "tests", "golden", "paper_L86_storage_ratios.txt")) as f:
+        rows = [ln.split() for ln in f if ln.strip() and not ln.startswith("#")]
+    assert len(rows) == 2
+    for m, n, r, pct in rows:
+        K, N, r, pct = int(m), int(n), int(r), float(pct)
+        # weight-side bytes = the M -> 0 limit: take two M values and extrapolate linearly
+        w_r = 2 * ab(1, N, K, r, G) - ab(2, N, K, r, G)
+        w_0 = 2 * ab(1, N, K, 0, G) - ab(2, N, K, 0, G)
+        lowrank = w_r - w_0
+        residual = w_0 - 2 * N * (K // G)                       # FP16 scales, one per group and channel (L193)
+        assert residual == N * K // 2
+        assert abs(100.0 * lowrank / residual - pct) < 1e-9
+    # per-token terms at q_proj: X (bf16, only when r > 0), Xq (4 bit), sx (fp32 per group), Y
+    N = K = 4096
+    per_tok = ab(2, N, K, 128, G) - ab(1, N, K, 128, G)
+    assert per_tok == 2 * K + K // 2 + 4 * (K // G) + 2 * N
+    assert ab(2, N, K, 0, G) - ab(1, N, K, 0, G) == K // 2 + 4 * (K // G) + 2 * N
+    assert ab(1, N, K, 128, G, out_bytes=4) - ab(1, N, K, 128, G) == 2 * N
+    assert ab(3, N, K, 128, G, with_quantizer=True) - ab(3, N, K, 128, G) == 3 * (2 * K + K // 2 + 4 * (K // G))
+
+
 def test_workspace_rule(lib):
     import paper_2606_01556_b200 as twq
     assert twq.workspace_bytes(2048, 14336, 4096, 128, 128) == 0      # prefill: tiles fill the GPU, no split

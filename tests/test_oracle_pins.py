@@ -208,6 +208,30 @@ def test_forward_additivity_and_transposition_sensitivity(oracle):
     assert np.abs(res).max() > 1e-3 and np.abs(lr).max() > 1e-3
 
 
+def test_forward_row_subset_is_rows_of_the_full_call(oracle):
+    """The `rows != NULL` path of twq_oracle_forward (oracle/twq_oracle.c, the path every M >= 2048 parity
+    test relies on): rows [4, 1] of a 6-row layer, Y and P, are exactly rows 4 and 1 of the full call --
+    through forward() and through forward_from_quantized(); the full call itself is pinned by the brute-force
+    and library tests above.  An out-of-order, repeated row and the empty tail (ragged last row) are included."""
+    L = gen.make_layer(6, 256, 48, 16, 64, seed=25, with_tinv=True)
+    full = oracle.forward(L.X, L.Rq, L.sw, L.L1, L.L2, L.G, tinv=L.tinv, want_P=True)
+    for rows in ([4, 1], [5], [0, 5, 5, 2]):
+        sub = oracle.forward(L.X, L.Rq, L.sw, L.L1, L.L2, L.G, tinv=L.tinv, rows=rows, want_P=True)
+        assert sub["Y"].shape == (len(rows), L.N) and sub["P"].shape == (len(rows), L.ng, L.N)
+        for i, m in enumerate(rows):
+            assert (sub["Y"][i] == full["Y"][m]).all()          # same FP64 operations in the same order: bit-equal
+            assert (sub["P"][i] == full["P"][m]).all()
+        # the quantizer outputs are always whole (rows only selects what steps 5-8 evaluate)
+        assert (sub["Xq"] == full["Xq"]).all() and (sub["sx"] == full["sx"]).all()
+        Y2, P2 = oracle.forward_from_quantized(L.X, full["Xq"], full["sx"], oracle.pack_nibbles(L.Rq), L.sw, L.L1, L.L2,
+                                               L.G, rows=rows, want_P=True)
+        assert (Y2 == sub["Y"]).all() and (P2 == sub["P"]).all()
+    # rank 0 through the same path
+    r0 = oracle.forward(L.X, L.Rq, L.sw, None, None, L.G, rows=[4, 1])["Y"]
+    f0 = oracle.forward(L.X, L.Rq, L.sw, None, None, L.G)["Y"]
+    assert (r0[0] == f0[4]).all() and (r0[1] == f0[1]).all()
+
+
 def test_scale_fold_constant_and_pow2_exact(oracle):
     """Constant scales factor out; power-of-two scales and small integers make Y exactly representable."""
     rng = np.random.default_rng(7)
