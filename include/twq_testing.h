@@ -1,0 +1,46 @@
+/*
+ * twq_testing.h -- hooks for the test-suite and the bench harness.  NOT part of the product ABI (include/twq.h):
+ * nothing here changes what a call computes, only which launch plan the planner picks, so that small test shapes
+ * can reach the code paths that production shapes take (CTA pairs, unsplit tiles, forced cluster sizes), and a way
+ * to read the plan back.  The planner never reads the environment.
+ */
+#ifndef TWQ_TESTING_H_
+#define TWQ_TESTING_H_
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* Bits of the process-wide planner override word (0 = production behaviour). */
+#define TWQ_PLAN_NO_SPLIT      1u    /* tcgen05 kernel: no K split for shapes with few output tiles */
+#define TWQ_PLAN_NO_PAIR       2u    /* tcgen05 kernel: no CTA pairs (cta_group::2) */
+#define TWQ_PLAN_NO_YSTAGE     4u    /* tcgen05 kernel: finished tiles are stored from registers, no staged TMA store */
+#define TWQ_PLAN_NO_ALIAS2     8u    /* tcgen05 kernel: the stage-1 ring may not overlay the L2T tile */
+#define TWQ_PLAN_NO_DECODE     16u   /* small batches go to the tcgen05 kernel as well */
+#define TWQ_PLAN_FUSED_CS(c)   (((unsigned)(c) & 15u) << 8)    /* forced cluster size of the tcgen05 kernel */
+#define TWQ_PLAN_DECODE_CS(c)  (((unsigned)(c) & 31u) << 12)   /* forced cluster size of the small-batch kernel */
+
+void twq_testing_set_plan_flags(unsigned flags);
+unsigned twq_testing_get_plan_flags(void);
+
+/* Fields written by twq_testing_describe_plan (ints). */
+enum {
+    TWQ_PLAN_KERNEL = 0,       /* 0 = small-batch (decode) kernel, 1 = tcgen05 kernel */
+    TWQ_PLAN_CLUSTER,          /* CTAs per cluster */
+    TWQ_PLAN_GRID,             /* CTAs */
+    TWQ_PLAN_TILE_TOKENS,      /* tokens per tile (padded tokens for the small-batch kernel) */
+    TWQ_PLAN_SPLITS,           /* K splits */
+    TWQ_PLAN_PAIR,             /* 1 = CTA pairs */
+    TWQ_PLAN_SMEM,             /* dynamic shared memory, bytes */
+    TWQ_PLAN_RING,             /* ring depth of the packed-operand pipeline */
+    TWQ_PLAN_CHUNKS,           /* small-batch kernel: ring chunks per call; tcgen05 kernel: work units */
+    TWQ_PLAN_FIELDS
+};
+/* The launch plan twq_dual_linear would use for this shape on the current device (or the no-device defaults).
+ * Writes up to n_out ints; returns the number of fields, or -1 for an invalid shape. */
+int twq_testing_describe_plan(int M, int N, int K, int r, int G, int* out, int n_out);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TWQ_TESTING_H_ */

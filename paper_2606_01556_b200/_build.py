@@ -14,7 +14,8 @@ CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libtwq.so")
 SOURCES = ["twq_api.cu", "quantize_act.cu", "pack_weights.cu", "fused_kernel.cu", "decode_kernel.cu", "fused_inst_tn16.cu",
            "fused_inst_tn32.cu", "fused_inst_tn64.cu", "fused_inst_tn128.cu", "fused_inst_tn128p.cu"]
-HEADERS = ["sm100_ptx.cuh", "fused_kernel.h", "fused_kernel.cuh", "packed_layout.h", os.path.join("..", "..", "include", "twq.h")]
+HEADERS = ["sm100_ptx.cuh", "fused_kernel.h", "fused_kernel.cuh", "packed_layout.h", os.path.join("..", "..", "include", "twq.h"),
+           os.path.join("..", "..", "include", "twq_testing.h")]
 # No --use_fast_math: the quantizer's FP32 op order is part of the specification.
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xptxas", "-v", "--fmad=true"]

@@ -17,6 +17,20 @@ EXPORTS = ("twq_status_string", "twq_packed_bytes", "twq_pack_weights", "twq_qua
            "twq_workspace_bytes", "twq_dual_linear", "twq_last_launch_count")
 
 
+TESTING_EXPORTS = ("twq_testing_set_plan_flags", "twq_testing_get_plan_flags", "twq_testing_describe_plan")
+# include/twq_testing.h: planner overrides for tests
+PLAN_NO_SPLIT, PLAN_NO_PAIR, PLAN_NO_YSTAGE, PLAN_NO_ALIAS2, PLAN_NO_DECODE = 1, 2, 4, 8, 16
+_PLAN_FIELDS = ("kernel", "cluster", "grid", "tile_tokens", "splits", "pair", "smem", "ring", "chunks")
+
+
+def plan_fused_cs(c: int) -> int:
+    return (c & 15) << 8
+
+
+def plan_decode_cs(c: int) -> int:
+    return (c & 31) << 12
+
+
 class TwqError(RuntimeError):
     def __init__(self, code: int, where: str):
         super().__init__(f"{where}: {_STATUS.get(code, code)}")
@@ -56,6 +70,13 @@ def load_library(build_if_missing: bool = True):
     lib.twq_dual_linear.argtypes = [vp, i, vp, vp, vp, i, i, i, i, i, vp, i, i, vp, sz, vp, vp]
     lib.twq_last_launch_count.restype = i
     lib.twq_last_launch_count.argtypes = []
+    # testing hooks (include/twq_testing.h): not part of the product ABI
+    lib.twq_testing_set_plan_flags.restype = None
+    lib.twq_testing_set_plan_flags.argtypes = [ctypes.c_uint]
+    lib.twq_testing_get_plan_flags.restype = ctypes.c_uint
+    lib.twq_testing_get_plan_flags.argtypes = []
+    lib.twq_testing_describe_plan.restype = i
+    lib.twq_testing_describe_plan.argtypes = [i, i, i, i, i, ctypes.POINTER(ctypes.c_int), i]
     _lib = lib
     return lib
 
@@ -84,6 +105,22 @@ def workspace_bytes(M: int, N: int, K: int, r: int, G: int) -> int:
 
 def last_launch_count() -> int:
     return int(load_library().twq_last_launch_count())
+
+
+def testing_set_plan_flags(flags: int) -> None:
+    """include/twq_testing.h: process-wide planner overrides (0 = production)."""
+    load_library().twq_testing_set_plan_flags(flags)
+
+
+def testing_describe_plan(M: int, N: int, K: int, r: int, G: int) -> dict:
+    """The launch plan twq_dual_linear would use: kernel ('decode' / 'tcgen05'), cluster, grid, ..."""
+    out = (ctypes.c_int * len(_PLAN_FIELDS))()
+    n = load_library().twq_testing_describe_plan(M, N, K, r, G, out, len(_PLAN_FIELDS))
+    if n < 0:
+        raise TwqError(1, "twq_testing_describe_plan")
+    d = dict(zip(_PLAN_FIELDS, [int(v) for v in out]))
+    d["kernel"] = "decode" if d["kernel"] == 0 else "tcgen05"
+    return d
 
 
 @dataclasses.dataclass

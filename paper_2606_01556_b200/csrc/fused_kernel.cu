@@ -1,7 +1,5 @@
 // fused_kernel.cu -- launch planning and dispatch for the fused dual-branch kernel
 // (kernel template: fused_kernel.cuh; instantiations: fused_inst_*.cu).  Host arithmetic only.
-#include <stdlib.h>
-
 #include "fused_kernel.cuh"
 
 namespace twq {
@@ -17,13 +15,17 @@ int round_up(int x, int a) { return (x + a - 1) / a * a; }
 // with a conservative table when no device is present (planning on a CPU-only box).
 int cluster_capacity(int cs, int num_sms) {
     if (cs <= 1) return num_sms;
-    static int cache[9] = {0, 0, 0, 0, 0, 0, 0, 0, 0};
-    if (cache[cs] > 0) return cache[cs];
-    int n = max_active_clusters_inst<128, 128, false>(cs, num_sms);
+    constexpr int kMaxDevices = 64;
+    static int cache[kMaxDevices][9] = {};                 // per device; idempotent values
+    int dev = 0;
+    const bool have_dev = cudaGetDevice(&dev) == cudaSuccess && dev >= 0 && dev < kMaxDevices - 1;
+    if (!have_dev) { cudaGetLastError(); dev = kMaxDevices - 1; }
+    if (cache[dev][cs] > 0) return cache[dev][cs];
+    int n = have_dev ? max_active_clusters_inst<128, 128, false>(cs, num_sms) : 0;
     if (n <= 0) n = cs == 2 ? num_sms / 2 : (cs == 4 ? (num_sms / 4) * 7 / 8 : (num_sms / 8) * 7 / 8);
     if (n > num_sms / cs) n = num_sms / cs;
     if (n < 1) n = 1;
-    cache[cs] = n;
+    cache[dev][cs] = n;
     return n;
 }
 
@@ -67,8 +69,9 @@ static bool make_plan_tn(int TN, int M, int N, int K, int r, int G, int num_sms,
             }
         }
     }
-    if (const char* e = getenv("TWQ_DEBUG_FUSED_CS")) {   // debugging aid: force the cluster size
-        const int c = atoi(e);
+    const unsigned flags = plan_flags();                  // test overrides (include/twq_testing.h); 0 in production
+    {
+        const int c = static_cast<int>((flags >> kPlanFusedCsShift) & 15u);
         if (r > 0 && (c == 1 || c == 2 || c == 4 || c == 8) && pl.n_tiles % c == 0) pl.cs = c;
     }
     pl.n_blocks = pl.n_tiles / pl.cs;
@@ -76,8 +79,8 @@ static bool make_plan_tn(int TN, int M, int N, int K, int r, int G, int num_sms,
     // K splits when the output tiles alone cannot fill the machine (decode-shaped M)
     const long long tiles = static_cast<long long>(pl.n_tiles) * pl.m_tiles;
     int s = 1;
-    // TWQ_DEBUG_NO_SPLIT: testing aid -- small shapes then take the unsplit path (and CTA pairs) of large ones
-    if (tiles < (3 * num_sms) / 4 && getenv("TWQ_DEBUG_NO_SPLIT") == nullptr) {
+    // kPlanNoSplit: testing aid -- small shapes then take the unsplit path (and CTA pairs) of large ones
+    if (tiles < (3 * num_sms) / 4 && !(flags & kPlanNoSplit)) {
         s = static_cast<int>(static_cast<long long>(max_clusters) * pl.cs / tiles);
         if (s > 16) s = 16;
         if (s > ng) s = ng;
@@ -97,7 +100,7 @@ static bool make_plan_tn(int TN, int M, int N, int K, int r, int G, int num_sms,
     const int nrb = (r + 127) / 128, nkb = (r + 63) / 64;
     const int hbytes = nkb * TN * 128, l2bytes = nkb * kL1Chunk;
     // CTA pairs: prefill tiles in an even cluster without K splits; each CTA then expands half of the token rows
-    pl.pair = (TN == 128 && pl.cs >= 2 && pl.splits == 1 && getenv("TWQ_DEBUG_NO_PAIR") == nullptr) ? 1 : 0;
+    pl.pair = (TN == 128 && pl.cs >= 2 && pl.splits == 1 && !(flags & kPlanNoPair)) ? 1 : 0;
     const int xr = pl.pair ? TN / 2 : TN;
     const int ub = xr * G, pb = kTileN * (G / 2) + xr * (G / 2);
     const int s1b = TN * 128 + nrb * kL1Chunk;
@@ -108,7 +111,7 @@ static bool make_plan_tn(int TN, int M, int N, int K, int r, int G, int num_sms,
     // swizzled halves of 64 channels; taken only where it fits beside a packed ring of at least 6 (pairs) / 4 stages.
     // The caller clears the flag for FP32 outputs and row pitches that are not a multiple of 16 bytes.
     const int ybytes = TN * kTileN * 2;
-    pl.ystage = (TN == 128 && pl.splits == 1 && getenv("TWQ_DEBUG_NO_YSTAGE") == nullptr) ? 1 : 0;
+    pl.ystage = (TN == 128 && pl.splits == 1 && !(flags & kPlanNoYStage)) ? 1 : 0;
     pl.nsu = kMaxNSU;
     pl.nsp = (TN <= 32 || pl.pair) ? kMaxNSP : 4;   // a pair's packed stage is 12 KB: the ring can be twice as deep
     pl.ns1 = r > 0 ? (TN <= 32 ? 3 : 2) : 0;
@@ -128,7 +131,7 @@ static bool make_plan_tn(int TN, int M, int N, int K, int r, int G, int num_sms,
         else if (total(pl) > budget) pl.nsp = q.nsp;
     }
     if (total(pl) > budget) { pl.alias = 1; pl.ns1 = r > 0 ? 3 : 0; }
-    if (total(pl) > budget && r > 0 && getenv("TWQ_DEBUG_NO_ALIAS2") == nullptr) {
+    if (total(pl) > budget && r > 0 && !(flags & kPlanNoAlias2)) {
         // Rank-256 buffers beside a 128-token tile: the stage-1 ring and the FP32 partial of H overlay the L2T tile as
         // well as the residual rings.  L2T is dead whenever stage 1 runs: its stage-2 MMAs were issued at the start
         // of the previous tile, whose residual MMAs (B_RESID) the producer waits for before the first stage-1 load,

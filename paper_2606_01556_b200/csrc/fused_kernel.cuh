@@ -309,7 +309,7 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
                     TWQ_TR(0, trn, 2);
                     const uint32_t st = sP_a + sp * p_stage_bytes;
                     mbar_arrive_expect_tx_a(TWQ_BAR(B_PFULL + sp), p_stage_bytes);
-                    tma_load_2d_a(st, &tmW, TWQ_BAR(B_PFULL + sp), c0, t.n0);
+                    tma_load_4d_a(st, &tmW, TWQ_BAR(B_PFULL + sp), 0, 0, g, t.n0 >> 3);   // 16 blocks of (8 channels x G/2 bytes)
                     if (!waited) { pdl_wait(); waited = true; }               // Xq comes from the quantizer
                     tma_load_2d_a(st + C::kWB, &tmXq, TWQ_BAR(B_PFULL + sp), c0, t.m0 + (kPair ? (rank & 1) * C::kXR : 0));
                     if (++sp == pl.nsp) { sp = 0; php ^= 1; }
@@ -688,10 +688,11 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
             const Unit t = decode_unit(p, u, rank);
             const int n = t.n0 + row;
             const bool n_ok = n < p.N;
-            const float* swp = p.swT + (n_ok ? n : 0);
+            // FP16 group scales, tiled [N/8][ng][8]: channel n of group g at ((n >> 3) * ng + g) * 8 + (n & 7)
+            const __half* swp = p.sw16 + (n_ok ? (static_cast<size_t>(n >> 3) * p.ng * 8 + (n & 7)) : 0);
             // weight scales two groups ahead of use
-            float sw0 = n_ok ? __ldg(swp + static_cast<size_t>(t.g_begin) * p.N) : 0.0f;
-            float sw1 = (n_ok && t.g_begin + 1 < t.g_end) ? __ldg(swp + static_cast<size_t>(t.g_begin + 1) * p.N) : 0.0f;
+            float sw0 = n_ok ? __half2float(__ldg(swp + static_cast<size_t>(t.g_begin) * 8)) : 0.0f;
+            float sw1 = (n_ok && t.g_begin + 1 < t.g_end) ? __half2float(__ldg(swp + static_cast<size_t>(t.g_begin + 1) * 8)) : 0.0f;
             if (r > 0 && t.ctx != cur_ctx) {
                 cur_ctx = t.ctx;
                 int kc0, kc1;
@@ -817,7 +818,7 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
             for (int g = t.g_begin; g < t.g_end; ++g, ++itp) {
                 const float swn = sw0;
                 sw0 = sw1;
-                sw1 = (n_ok && g + 2 < t.g_end) ? __ldg(swp + static_cast<size_t>(g + 2) * p.N) : 0.0f;
+                sw1 = (n_ok && g + 2 < t.g_end) ? __half2float(__ldg(swp + static_cast<size_t>(g + 2) * 8)) : 0.0f;
                 const float cm = __fmul_rn(12582912.0f, swn);   // exact: sw has an 11-bit significand
                 const uint64_t sw2 = pack_f2(swn, swn), ncm2 = pack_f2(-cm, -cm);
 #ifdef TWQ_TRACE
@@ -1096,10 +1097,15 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
         __syncthreads();
         if (threadIdx.x == 0) {
             atomicAdd(ctr, 1u);
-            unsigned seen;
+            // the launch is cooperative (every CTA of the grid is resident), so the wait is bounded; a protocol bug
+            // becomes a trap (reported as a launch failure), not a hung device
+            unsigned seen, spins = 0;
             do {
                 asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(seen) : "l"(ctr) : "memory");
-                if (seen < static_cast<unsigned>(pl.splits)) __nanosleep(64);
+                if (seen < static_cast<unsigned>(pl.splits)) {
+                    __nanosleep(64);
+                    if (++spins > (1u << 24)) __trap();
+                }
             } while (seen < static_cast<unsigned>(pl.splits));
             __threadfence();
         }
@@ -1156,18 +1162,22 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
 template <int TN, int G, bool kDbg, bool kPair = false>
 cudaError_t launch_fused_inst(const FusedMaps& maps, const FusedParams& p, cudaStream_t stream) {
     auto kern = fused_dual_linear_kernel<TN, G, kDbg, kPair>;
-    static int attr_smem = 0;
-    if (attr_smem < p.plan.smem_bytes) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxDynSmem);
+    constexpr int kMaxDevices = 64;
+    static bool attr_done[kMaxDevices] = {};      // function attributes are per device
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= kMaxDevices || !attr_done[dev]) {
+        e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, kMaxDynSmem);
         if (e != cudaSuccess) return e;
-        attr_smem = kMaxDynSmem;
+        if (dev >= 0 && dev < kMaxDevices) attr_done[dev] = true;
     }
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(static_cast<unsigned>(p.plan.nclusters * p.plan.cs));
     cfg.blockDim = dim3(kThreads);
     cfg.dynamicSmemBytes = static_cast<size_t>(p.plan.smem_bytes);
     cfg.stream = stream;
-    cudaLaunchAttribute attrs[2];
+    cudaLaunchAttribute attrs[3];
     int na = 0;
     if (p.plan.cs > 1) {
         attrs[na].id = cudaLaunchAttributeClusterDimension;
@@ -1176,9 +1186,17 @@ cudaError_t launch_fused_inst(const FusedMaps& maps, const FusedParams& p, cudaS
         attrs[na].val.clusterDim.z = 1;
         ++na;
     }
-    attrs[na].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-    attrs[na].val.programmaticStreamSerializationAllowed = 1;
-    ++na;
+    if (p.plan.splits > 1) {
+        // The split-K fix-up waits for the other CTAs of its tile: a cooperative launch makes the driver guarantee
+        // that the whole grid is co-resident (or refuse the launch) whatever else runs on the device.
+        attrs[na].id = cudaLaunchAttributeCooperative;
+        attrs[na].val.cooperative = 1;
+        ++na;
+    } else {
+        attrs[na].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        attrs[na].val.programmaticStreamSerializationAllowed = 1;
+        ++na;
+    }
     cfg.attrs = attrs;
     cfg.numAttrs = static_cast<unsigned>(na);
     return cudaLaunchKernelEx(&cfg, kern, maps.W, maps.Xq, maps.X, maps.L1T, maps.L2T, maps.Y, p);

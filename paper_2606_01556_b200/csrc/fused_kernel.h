@@ -3,6 +3,7 @@
 #pragma once
 #include <cuda.h>
 #include <cuda_runtime.h>
+#include <cuda_fp16.h>
 #include <stdint.h>
 
 namespace twq {
@@ -30,7 +31,7 @@ struct FusedParams {
     int M, N, K, r, ng;
     int ldy, ydt;            // ydt: 0 bf16, 1 fp16, 2 fp32
     const float* sx;         // [M][ng] activation group scales
-    const float* swT;        // [ng][N] weight group scales (FP32, transposed)
+    const __half* sw16;      // [N/8][ng][8] weight group scales (FP16, tiled like R4)
     void* Y;                 // [M][ldy]
     int32_t* dbgP;           // NULL or [M][ng][N]
     float* ws_part;          // split-K partials [splits][M][N] (splits > 1 only)
@@ -43,32 +44,47 @@ struct FusedMaps {
 };
 
 
-// Decode-shaped calls (M <= 16): parameters and plan of decode_kernel.cu (host-computed).
+// Small-batch calls (M <= kDecodeMaxM): parameters and plan of decode_kernel.cu (host-computed).
+constexpr int kDecodeMaxM = 32;
 struct DecodeParams {
     int M, N, K, r, ng;
     int ldx, ldy, ydt;       // ydt: 0 bf16, 1 fp16, 2 fp32
-    int n_tiles;             // N / 16
+    int n_tiles;             // N / 8 (8-channel tiles)
     int cs, grid;            // CTAs per cluster, CTAs in the grid (a multiple of cs)
-    int T, P;                // 16-channel tiles per CTA, K-parts per tile
-    int off_res, off_hpart, off_h, off_ylr, off_sx, off_xs, smem_bytes;
-    int ncl_k;               // > 1: stage 1 splits K over ALL ncl_k clusters (L1T read once per call); partials meet in ws_h
-    float* ws_h;             // [ncl_k][16][r] FP32 cluster-level partials of H (caller's workspace)
-    unsigned* ws_ctr;        // grid barrier counter (zero between calls)
-    const uint8_t* R4;       // [N][K/2]
-    const float* swT;        // [ng][N]
-    const void* L1T;         // [r][K] f16
+    int mt, mp;              // 16-token MMA tiles, padded tokens (16 * mt)
+    int lrw;                 // warps running the low-rank chain (0 when r == 0); the other compute warps stream the residual
+    int tmax;                // most 8-channel tiles any CTA owns
+    int gc, nchunks, nslots; // residual ring: K-groups per chunk, chunks per call, ring depth
+    int slot_bytes, xq_off;  // bytes of one ring slot; offset of the Xq box inside it
+    int sc, l1_slots;        // stage-1 ring: 32-wide K slabs per chunk, ring depth
+    int nu_max;              // most K slabs of stage 1 any CTA multiplies
+    int xs_stride;           // halves per token row of the staged FP16 X slice
+    int off_ring, off_l1, off_sw, off_xs, off_hpart, off_h, off_ylr, off_sx, off_res, off_bar, smem_bytes;
+    const uint8_t* R4;       // [N/8][ng][8][G/2]
+    const __half* sw16;      // [N/8][ng][8]
+    const void* L1D;         // [K/32][r][32] f16
     const void* L2T;         // [N][r] f16
     const void* X;           // [M][ldx] bf16
-    const uint8_t* Xq;       // [M][K/2]
     const float* sx;         // [M][ng]
     void* Y;
     int32_t* dbgP;
 };
 bool decode_make_plan(int M, int N, int K, int r, int G, int num_sms, DecodeParams* out);
-inline size_t decode_workspace_bytes(const DecodeParams& p) {
-    return p.ncl_k > 1 ? 256 + ((static_cast<size_t>(p.ncl_k) * 16 * p.r * sizeof(float) + 255) & ~static_cast<size_t>(255)) : 0;
-}
-cudaError_t launch_decode(const DecodeParams& p, int G, cudaStream_t stream);
+cudaError_t launch_decode(const CUtensorMap& tmXq, const DecodeParams& p, int G, cudaStream_t stream);
+
+// Planner overrides for tests (include/twq_testing.h, twq_testing_set_plan_flags): a process-wide word, never the
+// environment.  0 in production.
+enum : unsigned {
+    kPlanNoSplit = 1u,       // fused kernel: no K split for shapes with few tiles (small shapes then take the unsplit / CTA-pair path)
+    kPlanNoPair = 2u,        // fused kernel: no CTA pairs
+    kPlanNoYStage = 4u,      // fused kernel: finished tiles are stored from registers (no staged TMA store)
+    kPlanNoAlias2 = 8u,      // fused kernel: the stage-1 ring may not overlay the L2T tile
+    kPlanNoDecode = 16u,     // small-batch calls go to the tcgen05 kernel too
+    kPlanFusedCsShift = 8,   // bits 8..11: forced cluster size of the fused kernel (0 = planner's choice)
+    kPlanDecodeCsShift = 12, // bits 12..16: forced cluster size of the decode kernel (0 = planner's choice)
+};
+unsigned plan_flags();
+void set_plan_flags(unsigned f);
 
 // Fills `plan` for a shape; returns false if the shape cannot be planned (never for valid ABI shapes).
 bool fused_make_plan(int M, int N, int K, int r, int G, int num_sms, FusedPlan* plan);

@@ -1,11 +1,6 @@
 // pack_weights.cu -- offline re-layout of one layer's weights (step a0; PAPER.md L123:
 // all transforms and weight formats are "pre-processed offline").  Not on the timed path.
-//
-// Blob sections (each 256-byte aligned; offsets from packed_layout.h):
-//   R4   [N][K/2] u8    two INT4 codes per byte, low nibble = even k (two's complement)
-//   swT  [K/G][N] f32   group scales transposed, so an epilogue warp reads 32 consecutive n
-//   L1T  [r][K]   f16   L1 transposed (K-major A operand of the stage-1 MMA)
-//   L2T  [N][r]   f16   L2 transposed (K-major A operand of the stage-2 MMA, reduction over r)
+// Blob sections and their reasons: packed_layout.h.
 #include <cuda_fp16.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -14,8 +9,10 @@
 
 namespace twq {
 
-__global__ void pack_codes_kernel(const int8_t* __restrict__ Rq, uint8_t* __restrict__ R4, long long n_words) {
-    // one thread: 8 codes (8 bytes in) -> 4 bytes out
+// one thread: 8 codes of one row (8 bytes in) -> 4 bytes of the (n/8, g) block, row n%8
+__global__ void pack_codes_kernel(const int8_t* __restrict__ Rq, uint8_t* __restrict__ R4, int N, int K, int G) {
+    const long long n_words = static_cast<long long>(N) * (K / 8);
+    const int wpr = K / 8, ng = K / G;
     for (long long i = blockIdx.x * static_cast<long long>(blockDim.x) + threadIdx.x; i < n_words;
          i += static_cast<long long>(gridDim.x) * blockDim.x) {
         const uint2 v = __ldg(reinterpret_cast<const uint2*>(Rq) + i);
@@ -25,21 +22,20 @@ __global__ void pack_codes_kernel(const int8_t* __restrict__ Rq, uint8_t* __rest
             out |= ((v.x >> (8 * b)) & 0xFu) << (4 * b);
             out |= ((v.y >> (8 * b)) & 0xFu) << (16 + 4 * b);
         }
-        reinterpret_cast<uint32_t*>(R4)[i] = out;
+        const int n = static_cast<int>(i / wpr), k0 = static_cast<int>(i - static_cast<long long>(n) * wpr) * 8;
+        const int g = k0 / G, b0 = (k0 - g * G) >> 1;
+        const size_t o = (static_cast<size_t>(n >> 3) * ng + g) * (4 * static_cast<size_t>(G)) + (n & 7) * (G / 2) + b0;
+        *reinterpret_cast<uint32_t*>(R4 + o) = out;
     }
 }
 
-__global__ void pack_scales_kernel(const __half* __restrict__ sw, float* __restrict__ swT, int N, int ng) {
-    __shared__ float tile[32][33];
-    const int n0 = blockIdx.x * 32, g0 = blockIdx.y * 32;
-    for (int j = threadIdx.y; j < 32; j += blockDim.y) {
-        const int n = n0 + j, g = g0 + threadIdx.x;
-        if (n < N && g < ng) tile[j][threadIdx.x] = __half2float(sw[static_cast<size_t>(n) * ng + g]);
-    }
-    __syncthreads();
-    for (int j = threadIdx.y; j < 32; j += blockDim.y) {
-        const int g = g0 + j, n = n0 + threadIdx.x;
-        if (n < N && g < ng) swT[static_cast<size_t>(g) * N + n] = tile[threadIdx.x][j];
+// sw [N][ng] f16 -> sw16 [N/8][ng][8] f16
+__global__ void pack_scales_kernel(const __half* __restrict__ sw, __half* __restrict__ sw16, int N, int ng) {
+    const long long total = static_cast<long long>(N) * ng;
+    for (long long i = blockIdx.x * static_cast<long long>(blockDim.x) + threadIdx.x; i < total;
+         i += static_cast<long long>(gridDim.x) * blockDim.x) {
+        const int n = static_cast<int>(i / ng), g = static_cast<int>(i - static_cast<long long>(n) * ng);
+        sw16[(static_cast<size_t>(n >> 3) * ng + g) * 8 + (n & 7)] = sw[i];
     }
 }
 
@@ -58,6 +54,21 @@ __global__ void transpose16_kernel(const uint16_t* __restrict__ in, uint16_t* __
     }
 }
 
+// L1 [K][r] f16 -> L1D [K/32][r][32] f16 (a 32 x 32 tile transpose per block: both sides coalesced)
+__global__ void slab_l1_kernel(const uint16_t* __restrict__ L1, uint16_t* __restrict__ L1D, int K, int r) {
+    __shared__ uint16_t tile[32][34];
+    const int j0 = blockIdx.x * 32, k0 = blockIdx.y * 32;      // K % 32 == 0; r % 16 == 0
+    for (int kk = threadIdx.y; kk < 32; kk += blockDim.y) {
+        const int j = j0 + threadIdx.x;
+        if (j < r) tile[kk][threadIdx.x] = L1[static_cast<size_t>(k0 + kk) * r + j];
+    }
+    __syncthreads();
+    for (int jj = threadIdx.y; jj < 32; jj += blockDim.y) {
+        const int j = j0 + jj;
+        if (j < r) L1D[(static_cast<size_t>(k0 >> 5) * r + j) * 32 + threadIdx.x] = tile[threadIdx.x][jj];
+    }
+}
+
 cudaError_t launch_pack_weights(const int8_t* Rq, const void* sw, const void* L1, const void* L2, int N, int K, int r,
                                 int G, void* packed, cudaStream_t stream, int* launches) {
     const PackedLayout lay = packed_layout(N, K, r, G);
@@ -65,20 +76,25 @@ cudaError_t launch_pack_weights(const int8_t* Rq, const void* sw, const void* L1
     const long long n_words = static_cast<long long>(N) * K / 8;
     long long blocks = (n_words + 255) / 256;
     if (blocks > 148 * 32) blocks = 148 * 32;
-    pack_codes_kernel<<<static_cast<unsigned>(blocks), 256, 0, stream>>>(Rq, base + lay.off_r4, n_words);
+    pack_codes_kernel<<<static_cast<unsigned>(blocks), 256, 0, stream>>>(Rq, base + lay.off_r4, N, K, G);
     const int ng = K / G;
-    dim3 tb(32, 8);
-    pack_scales_kernel<<<dim3((N + 31) / 32, (ng + 31) / 32), tb, 0, stream>>>(
-        static_cast<const __half*>(sw), reinterpret_cast<float*>(base + lay.off_swT), N, ng);
+    long long sblocks = (static_cast<long long>(N) * ng + 255) / 256;
+    if (sblocks > 148 * 32) sblocks = 148 * 32;
+    pack_scales_kernel<<<static_cast<unsigned>(sblocks), 256, 0, stream>>>(
+        static_cast<const __half*>(sw), reinterpret_cast<__half*>(base + lay.off_sw16), N, ng);
     int n = 2;
     if (r > 0) {
+        dim3 tb(32, 8);
         // L1 [K][r] -> L1T [r][K]
         transpose16_kernel<<<dim3((r + 31) / 32, (K + 31) / 32), tb, 0, stream>>>(
             static_cast<const uint16_t*>(L1), reinterpret_cast<uint16_t*>(base + lay.off_l1t), K, r);
+        // L1 [K][r] -> L1D [K/32][r][32]
+        slab_l1_kernel<<<dim3((r + 31) / 32, K / 32), tb, 0, stream>>>(
+            static_cast<const uint16_t*>(L1), reinterpret_cast<uint16_t*>(base + lay.off_l1d), K, r);
         // L2 [r][N] -> L2T [N][r]
         transpose16_kernel<<<dim3((N + 31) / 32, (r + 31) / 32), tb, 0, stream>>>(
             static_cast<const uint16_t*>(L2), reinterpret_cast<uint16_t*>(base + lay.off_l2t), r, N);
-        n += 2;
+        n += 3;
     }
     if (launches) *launches = n;
     return cudaGetLastError();

@@ -1,17 +1,31 @@
 // twq_api.cu -- the C ABI declared in include/twq.h: argument validation (before any CUDA
-// call), TMA descriptor construction, launch configuration.  No compute lives here.
+// call), launch planning, TMA descriptors (cached), launch.  No compute lives here.
 #include <cuda.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
 #include <string.h>
 
+#include <atomic>
+
 #include "../../include/twq.h"
+#include "../../include/twq_testing.h"
 #include "fused_kernel.h"
 #include "packed_layout.h"
+
+namespace twq {
+
+namespace {
+std::atomic<unsigned> g_plan_flags{0u};
+}
+unsigned plan_flags() { return g_plan_flags.load(std::memory_order_relaxed); }
+void set_plan_flags(unsigned f) { g_plan_flags.store(f, std::memory_order_relaxed); }
+
+}  // namespace twq
 
 namespace {
 
 thread_local int g_last_launches = 0;
+constexpr int kMaxDevices = 64;
 
 bool aligned16(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 
@@ -24,64 +38,153 @@ bool shape_ok(int M, int N, int K, int r, int G) {
     return true;
 }
 
+// Per-device facts, looked up once per device (relaxed atomics: the values are idempotent).
+struct DevInfo {
+    std::atomic<int> sms{0};      // 0 = not asked yet
+    std::atomic<int> sm100{-1};   // -1 = not asked yet
+};
+DevInfo g_dev[kMaxDevices];
+
+int current_device() {
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) { cudaGetLastError(); return -1; }
+    return dev;
+}
+
 // SM count of the current device (148 on B200; also the planning default when no device is present,
 // so twq_workspace_bytes gives the same answer on a CPU-only box).
 int num_sms() {
-    static thread_local int cached = 0;
-    if (cached == 0) {
-        int dev = 0, n = 0;
-        if (cudaGetDevice(&dev) == cudaSuccess &&
-            cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && n > 0)
-            cached = n;
-        else
-            return 148;
+    const int dev = current_device();
+    if (dev < 0 || dev >= kMaxDevices) return 148;
+    int n = g_dev[dev].sms.load(std::memory_order_relaxed);
+    if (n == 0) {
+        if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) { cudaGetLastError(); return 148; }
+        g_dev[dev].sms.store(n, std::memory_order_relaxed);
     }
-    return cached;
+    return n;
+}
+
+bool device_is_sm100() {
+    const int dev = current_device();
+    if (dev < 0) return false;
+    if (dev >= kMaxDevices) {
+        int major = 0;
+        return cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev) == cudaSuccess && major == 10;
+    }
+    int v = g_dev[dev].sm100.load(std::memory_order_relaxed);
+    if (v < 0) {
+        int major = 0;
+        if (cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev) != cudaSuccess) { cudaGetLastError(); return false; }
+        v = major == 10 ? 1 : 0;
+        g_dev[dev].sm100.store(v, std::memory_order_relaxed);
+    }
+    return v == 1;
 }
 
 size_t ctr_bytes(const twq::FusedPlan& pl) {
     return twq::align256(static_cast<size_t>(pl.n_tiles) * pl.m_tiles * sizeof(unsigned));
 }
 
+// ------------------------------------------------------------------ the plan of a call, made once per call and cached
+struct CallPlan {
+    int dev, M, N, K, r, G;
+    unsigned flags;
+    bool valid, decode;
+    twq::DecodeParams dp;      // decode == true
+    twq::FusedPlan fp;         // decode == false
+    size_t ws_bytes;
+};
+
+const CallPlan* get_plan(int M, int N, int K, int r, int G) {
+    constexpr int kSlots = 16;
+    thread_local CallPlan cache[kSlots];
+    thread_local unsigned next = 0;
+    const int dev = current_device();
+    const unsigned flags = twq::plan_flags();
+    for (int i = 0; i < kSlots; ++i) {
+        const CallPlan& c = cache[i];
+        if (c.valid && c.dev == dev && c.M == M && c.N == N && c.K == K && c.r == r && c.G == G && c.flags == flags) return &c;
+    }
+    CallPlan c;
+    memset(&c, 0, sizeof(c));
+    c.dev = dev; c.M = M; c.N = N; c.K = K; c.r = r; c.G = G; c.flags = flags;
+    const int sms = num_sms();
+    if (twq::decode_make_plan(M, N, K, r, G, sms, &c.dp)) {
+        c.decode = true;
+        c.ws_bytes = 0;
+    } else {
+        if (!twq::fused_make_plan(M, N, K, r, G, sms, &c.fp)) return nullptr;
+        c.decode = false;
+        c.ws_bytes = c.fp.splits > 1 ? ctr_bytes(c.fp) + static_cast<size_t>(c.fp.splits) * M * N * sizeof(float) : 0;
+    }
+    c.valid = true;
+    CallPlan& slot = cache[next++ % kSlots];
+    slot = c;
+    return &slot;
+}
+
+// ------------------------------------------------------------------ TMA descriptors, cached by everything they encode
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
                                   const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
                                   CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
 
 EncodeTiledFn get_encode() {
-    static EncodeTiledFn fn = nullptr;
-    if (!fn) {
+    static std::atomic<EncodeTiledFn> fn{nullptr};
+    EncodeTiledFn f = fn.load(std::memory_order_relaxed);
+    if (!f) {
         void* p = nullptr;
         cudaDriverEntryPointQueryResult q;
         if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
-            q == cudaDriverEntryPointSuccess)
-            fn = reinterpret_cast<EncodeTiledFn>(p);
+            q == cudaDriverEntryPointSuccess) {
+            f = reinterpret_cast<EncodeTiledFn>(p);
+            fn.store(f, std::memory_order_relaxed);
+        }
     }
-    return fn;
+    return f;
 }
 
-// 2D row-major tensor [rows][inner] with a row pitch in bytes; box = [box_rows][box_inner].
-bool make_map(CUtensorMap* m, CUtensorMapDataType dt, int elem_bytes, const void* ptr, uint64_t inner, uint64_t rows,
-              uint64_t pitch_bytes, uint32_t box_inner, uint32_t box_rows, CUtensorMapSwizzle sw) {
+struct MapKey {
+    const void* ptr;
+    uint64_t dim[4];
+    uint64_t stride[3];      // bytes, dims 1..rank-1
+    uint32_t box[4];
+    int rank, dt, sw;
+};
+
+// Row-major tensor of `rank` dims (innermost first); a hit costs one 128-byte copy instead of a driver call.
+bool get_map(CUtensorMap* out, const MapKey& k) {
+    constexpr int kSlots = 128;
+    struct Entry { MapKey key; CUtensorMap map; bool valid; };
+    thread_local Entry cache[kSlots];
+    uint64_t h = reinterpret_cast<uintptr_t>(k.ptr) * 0x9E3779B97F4A7C15ull;
+    h ^= (k.dim[0] + 31 * k.dim[1] + 977 * k.dim[2] + 7919 * k.dim[3] + 104729ull * k.box[1] + 1299709ull * k.box[2] + k.sw) * 0xC2B2AE3D27D4EB4Full;
+    Entry& e = cache[(h >> 40) % kSlots];
+    if (e.valid && memcmp(&e.key, &k, sizeof(MapKey)) == 0) { *out = e.map; return true; }
     EncodeTiledFn enc = get_encode();
     if (!enc) return false;
-    cuuint64_t gdim[2] = {inner, rows};
-    cuuint64_t gstride[1] = {pitch_bytes};
-    cuuint32_t box[2] = {box_inner, box_rows};
-    cuuint32_t estr[2] = {1, 1};
-    (void)elem_bytes;
-    return enc(m, dt, 2, const_cast<void*>(ptr), gdim, gstride, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, sw,
-               CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+    cuuint64_t gdim[4], gstride[3];
+    cuuint32_t box[4], estr[4] = {1, 1, 1, 1};
+    for (int i = 0; i < 4; ++i) { gdim[i] = k.dim[i]; box[i] = k.box[i]; }
+    for (int i = 0; i < 3; ++i) gstride[i] = k.stride[i];
+    CUtensorMap m;
+    if (enc(&m, static_cast<CUtensorMapDataType>(k.dt), static_cast<cuuint32_t>(k.rank), const_cast<void*>(k.ptr), gdim,
+            gstride, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, static_cast<CUtensorMapSwizzle>(k.sw),
+            CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+        return false;
+    e.key = k; e.map = m; e.valid = true;
+    *out = m;
+    return true;
 }
 
-bool device_is_sm100() {
-    static thread_local int cached = -1;
-    if (cached < 0) {
-        int dev = 0, major = 0;
-        if (cudaGetDevice(&dev) != cudaSuccess) return false;
-        if (cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev) != cudaSuccess) return false;
-        cached = major == 10 ? 1 : 0;
-    }
-    return cached == 1;
+MapKey key2d(CUtensorMapDataType dt, const void* ptr, uint64_t inner, uint64_t rows, uint64_t pitch_bytes,
+             uint32_t box_inner, uint32_t box_rows, CUtensorMapSwizzle sw) {
+    MapKey k;
+    memset(&k, 0, sizeof(k));
+    k.ptr = ptr; k.rank = 2; k.dt = static_cast<int>(dt); k.sw = static_cast<int>(sw);
+    k.dim[0] = inner; k.dim[1] = rows;
+    k.stride[0] = pitch_bytes;
+    k.box[0] = box_inner; k.box[1] = box_rows;
+    return k;
 }
 
 }  // namespace
@@ -100,6 +203,29 @@ const char* twq_status_string(twq_status s) {
 }
 
 int twq_last_launch_count(void) { return g_last_launches; }
+
+void twq_testing_set_plan_flags(unsigned flags) { twq::set_plan_flags(flags); }
+unsigned twq_testing_get_plan_flags(void) { return twq::plan_flags(); }
+
+int twq_testing_describe_plan(int M, int N, int K, int r, int G, int* out, int n_out) {
+    if (!shape_ok(M, N, K, r, G) || !out) return -1;
+    const CallPlan* cp = get_plan(M, N, K, r, G);
+    if (!cp) return -1;
+    int v[TWQ_PLAN_FIELDS];
+    memset(v, 0, sizeof(v));
+    v[TWQ_PLAN_KERNEL] = cp->decode ? 0 : 1;
+    if (cp->decode) {
+        v[TWQ_PLAN_CLUSTER] = cp->dp.cs; v[TWQ_PLAN_GRID] = cp->dp.grid; v[TWQ_PLAN_TILE_TOKENS] = cp->dp.mp;
+        v[TWQ_PLAN_SPLITS] = 1; v[TWQ_PLAN_PAIR] = 0; v[TWQ_PLAN_SMEM] = cp->dp.smem_bytes;
+        v[TWQ_PLAN_RING] = cp->dp.nslots; v[TWQ_PLAN_CHUNKS] = cp->dp.nchunks;
+    } else {
+        v[TWQ_PLAN_CLUSTER] = cp->fp.cs; v[TWQ_PLAN_GRID] = cp->fp.nclusters * cp->fp.cs; v[TWQ_PLAN_TILE_TOKENS] = cp->fp.TN;
+        v[TWQ_PLAN_SPLITS] = cp->fp.splits; v[TWQ_PLAN_PAIR] = cp->fp.pair; v[TWQ_PLAN_SMEM] = cp->fp.smem_bytes;
+        v[TWQ_PLAN_RING] = cp->fp.nsp; v[TWQ_PLAN_CHUNKS] = cp->fp.units;
+    }
+    for (int i = 0; i < n_out && i < TWQ_PLAN_FIELDS; ++i) out[i] = v[i];
+    return TWQ_PLAN_FIELDS;
+}
 
 size_t twq_packed_bytes(int N, int K, int r, int G) {
     if (!shape_ok(1, N, K, r, G)) return 0;
@@ -139,12 +265,8 @@ twq_status twq_quantize_act(const void* X, int M, int K, int ldx, const float* t
 
 size_t twq_workspace_bytes(int M, int N, int K, int r, int G) {
     if (!shape_ok(M, N, K, r, G)) return 0;
-    twq::DecodeParams dp;
-    if (twq::decode_make_plan(M, N, K, r, G, num_sms(), &dp)) return twq::decode_workspace_bytes(dp);   // 0 for most
-    twq::FusedPlan pl;
-    if (!twq::fused_make_plan(M, N, K, r, G, num_sms(), &pl)) return 0;
-    if (pl.splits <= 1) return 0;
-    return ctr_bytes(pl) + static_cast<size_t>(pl.splits) * M * N * sizeof(float);
+    const CallPlan* cp = get_plan(M, N, K, r, G);
+    return cp ? cp->ws_bytes : 0;
 }
 
 twq_status twq_dual_linear(const void* X, int ldx, const uint8_t* Xq, const float* sx, const void* packed, int M,
@@ -160,65 +282,85 @@ twq_status twq_dual_linear(const void* X, int ldx, const uint8_t* Xq, const floa
     if (!aligned16(Xq) || !aligned16(sx) || !aligned16(Y) || (X && !aligned16(X)) ||
         (reinterpret_cast<uintptr_t>(packed) & 255u))
         return TWQ_ERR_INVALID_ARG;
-    const size_t need = twq_workspace_bytes(M, N, K, r, G);
+    const CallPlan* cp = get_plan(M, N, K, r, G);          // one plan per call (cached per shape)
+    if (!cp) return TWQ_ERR_UNSUPPORTED;
+    const size_t need = cp->ws_bytes;
     if (need > 0 && (!ws || ws_bytes < need)) return TWQ_ERR_WORKSPACE;
     if (need > 0 && (reinterpret_cast<uintptr_t>(ws) & 255u)) return TWQ_ERR_INVALID_ARG;
     if (!device_is_sm100()) return TWQ_ERR_UNSUPPORTED;
 
     const twq::PackedLayout lay = twq::packed_layout(N, K, r, G);
     const uint8_t* base = static_cast<const uint8_t*>(packed);
+    const int ng = K / G;
 
-    // decode-shaped calls (M <= 16): the register-resident kernel of decode_kernel.cu
-    twq::DecodeParams dp;
-    if (twq::decode_make_plan(M, N, K, r, G, num_sms(), &dp)) {
+    if (cp->decode) {
+        // small batches: the bulk-copy streaming kernel of decode_kernel.cu
+        twq::DecodeParams dp = cp->dp;
         dp.ldx = ldx; dp.ldy = ldy; dp.ydt = static_cast<int>(ydt);
         dp.R4 = base + lay.off_r4;
-        dp.swT = reinterpret_cast<const float*>(base + lay.off_swT);
-        dp.L1T = base + lay.off_l1t;
+        dp.sw16 = reinterpret_cast<const __half*>(base + lay.off_sw16);
+        dp.L1D = base + lay.off_l1d;
         dp.L2T = base + lay.off_l2t;
-        dp.X = X; dp.Xq = Xq; dp.sx = sx; dp.Y = Y; dp.dbgP = dbg_P;
-        dp.ws_ctr = static_cast<unsigned*>(ws);
-        dp.ws_h = dp.ncl_k > 1 ? reinterpret_cast<float*>(static_cast<uint8_t*>(ws) + 256) : nullptr;
-        if (twq::launch_decode(dp, G, static_cast<cudaStream_t>(stream)) != cudaSuccess) return TWQ_ERR_CUDA;
+        dp.X = X; dp.sx = sx; dp.Y = Y; dp.dbgP = dbg_P;
+        // Xq [M][K/2] as (G/2 bytes, K/G groups, M tokens); one box = gc groups of all (padded) tokens
+        MapKey k;
+        memset(&k, 0, sizeof(k));
+        k.ptr = Xq; k.rank = 3; k.dt = static_cast<int>(CU_TENSOR_MAP_DATA_TYPE_UINT8); k.sw = static_cast<int>(CU_TENSOR_MAP_SWIZZLE_NONE);
+        k.dim[0] = G / 2; k.dim[1] = ng; k.dim[2] = M;
+        k.stride[0] = G / 2; k.stride[1] = K / 2;
+        k.box[0] = G / 2; k.box[1] = dp.gc; k.box[2] = dp.mp;
+        CUtensorMap tmXq;
+        if (!get_map(&tmXq, k)) return TWQ_ERR_CUDA;
+        if (twq::launch_decode(tmXq, dp, G, static_cast<cudaStream_t>(stream)) != cudaSuccess) return TWQ_ERR_CUDA;
         g_last_launches = 1;
         return TWQ_OK;
     }
 
     twq::FusedParams p;
     memset(&p, 0, sizeof(p));
-    if (!twq::fused_make_plan(M, N, K, r, G, num_sms(), &p.plan)) return TWQ_ERR_UNSUPPORTED;
+    p.plan = cp->fp;
     const int TN = p.plan.TN;
     const int splits = p.plan.splits;
 
     twq::FusedMaps maps;
     memset(&maps, 0, sizeof(maps));
     bool ok = true;
-    // packed INT4 tiles: rows of G/2 bytes, swizzled so that one-row-per-thread reads are conflict-free
+    // packed INT4 tiles: rows of G/2 bytes, swizzled so that one-row-per-thread reads are conflict-free.
+    // Weights: R4 [N/8][ng][8][G/2]; one box = the (8 x G/2)-byte blocks of 16 consecutive tiles for one group
+    // = 128 channel rows x G/2 bytes in shared memory.
     const CUtensorMapSwizzle psw = G == 128 ? CU_TENSOR_MAP_SWIZZLE_64B : CU_TENSOR_MAP_SWIZZLE_32B;
-    ok &= make_map(&maps.W, CU_TENSOR_MAP_DATA_TYPE_UINT8, 1, base + lay.off_r4, K / 2, N, K / 2, G / 2, 128, psw);
-    ok &= make_map(&maps.Xq, CU_TENSOR_MAP_DATA_TYPE_UINT8, 1, Xq, K / 2, M, K / 2, G / 2, p.plan.pair ? TN / 2 : TN, psw);
+    {
+        MapKey k;
+        memset(&k, 0, sizeof(k));
+        k.ptr = base + lay.off_r4; k.rank = 4; k.dt = static_cast<int>(CU_TENSOR_MAP_DATA_TYPE_UINT8); k.sw = static_cast<int>(psw);
+        k.dim[0] = G / 2; k.dim[1] = 8; k.dim[2] = ng; k.dim[3] = N / 8;
+        k.stride[0] = G / 2; k.stride[1] = 4 * static_cast<uint64_t>(G); k.stride[2] = static_cast<uint64_t>(ng) * 4 * G;
+        k.box[0] = G / 2; k.box[1] = 8; k.box[2] = 1; k.box[3] = 16;
+        ok &= get_map(&maps.W, k);
+    }
+    ok &= get_map(&maps.Xq, key2d(CU_TENSOR_MAP_DATA_TYPE_UINT8, Xq, K / 2, M, K / 2, G / 2, p.plan.pair ? TN / 2 : TN, psw));
     if (r > 0) {
-        ok &= make_map(&maps.X, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, X, K, M, static_cast<uint64_t>(ldx) * 2, 64, TN,
-                       CU_TENSOR_MAP_SWIZZLE_128B);
-        ok &= make_map(&maps.L1T, CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 2, base + lay.off_l1t, K, r,
-                       static_cast<uint64_t>(K) * 2, 64, 128, CU_TENSOR_MAP_SWIZZLE_128B);
-        ok &= make_map(&maps.L2T, CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 2, base + lay.off_l2t, r, N,
-                       static_cast<uint64_t>(r) * 2, 64, 128, CU_TENSOR_MAP_SWIZZLE_128B);
+        ok &= get_map(&maps.X, key2d(CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, X, K, M, static_cast<uint64_t>(ldx) * 2, 64, TN,
+                                     CU_TENSOR_MAP_SWIZZLE_128B));
+        ok &= get_map(&maps.L1T, key2d(CU_TENSOR_MAP_DATA_TYPE_FLOAT16, base + lay.off_l1t, K, r,
+                                       static_cast<uint64_t>(K) * 2, 64, 128, CU_TENSOR_MAP_SWIZZLE_128B));
+        ok &= get_map(&maps.L2T, key2d(CU_TENSOR_MAP_DATA_TYPE_FLOAT16, base + lay.off_l2t, r, N,
+                                       static_cast<uint64_t>(r) * 2, 64, 128, CU_TENSOR_MAP_SWIZZLE_128B));
     }
     if (p.plan.ystage) {
         // asynchronous tile store: 16-bit outputs with a row pitch TMA accepts (a multiple of 16 bytes)
         if (static_cast<int>(ydt) <= 1 && (ldy & 7) == 0)
-            ok &= make_map(&maps.Y, CU_TENSOR_MAP_DATA_TYPE_UINT16, 2, Y, N, M, static_cast<uint64_t>(ldy) * 2, 64, TN,
-                           CU_TENSOR_MAP_SWIZZLE_128B);
+            ok &= get_map(&maps.Y, key2d(CU_TENSOR_MAP_DATA_TYPE_UINT16, Y, N, M, static_cast<uint64_t>(ldy) * 2, 64, TN,
+                                         CU_TENSOR_MAP_SWIZZLE_128B));
         else
             p.plan.ystage = 0;     // the kernel stores from registers (the staging bytes stay unused)
     }
     if (!ok) return TWQ_ERR_CUDA;
 
-    p.M = M; p.N = N; p.K = K; p.r = r; p.ng = K / G;
+    p.M = M; p.N = N; p.K = K; p.r = r; p.ng = ng;
     p.ldy = ldy; p.ydt = static_cast<int>(ydt);
     p.sx = sx;
-    p.swT = reinterpret_cast<const float*>(base + lay.off_swT);
+    p.sw16 = reinterpret_cast<const __half*>(base + lay.off_sw16);
     p.Y = Y;
     p.dbgP = dbg_P;
     p.ws_ctr = splits > 1 ? static_cast<unsigned*>(ws) : nullptr;

@@ -37,7 +37,7 @@ def test_packed_bytes_accounts_for_every_section(lib):
     import paper_2606_01556_b200 as twq
     N, K, r, G = 4096, 4096, 128, 128
     b = twq.packed_bytes(N, K, r, G)
-    sections = [N * K // 2, (K // G) * N * 4, r * K * 2, N * r * 2]
+    sections = [N * K // 2, (K // G) * N * 2, r * K * 2, r * K * 2, N * r * 2]   # R4, FP16 scales, L1T, L1 slabs, L2T
     assert b == sum((s + 255) & ~255 for s in sections)
     # 4-bit residual dominates: PAPER.md L86 ratio (2 r (m+n)) / (m n / 2) at r = 128 is 25 %
     assert abs((r * K * 2 + N * r * 2) / (N * K // 2) - 0.25) < 1e-12
@@ -75,13 +75,42 @@ def test_algorithmic_bytes_pinned_to_paper_L86():
     assert ab(3, N, K, 128, G, with_quantizer=True) - ab(3, N, K, 128, G) == 3 * (2 * K + K // 2 + 4 * (K // G))
 
 
+def test_testing_hooks_are_separate_from_the_product_abi(lib):
+    """include/twq_testing.h: planner overrides and plan read-back; exported, but not declared in twq.h."""
+    import paper_2606_01556_b200 as twq
+    from paper_2606_01556_b200.binding import TESTING_EXPORTS
+    hdr = open(os.path.join(ROOT, "include", "twq_testing.h")).read()
+    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+    assert set(re.findall(r"\b(twq_testing_[a-z_]+)\s*\(", hdr)) == set(TESTING_EXPORTS)
+    for n in TESTING_EXPORTS:
+        assert getattr(lib, n) is not None
+    assert "twq_testing" not in open(os.path.join(ROOT, "include", "twq.h")).read()
+    # no environment variable reaches the planner
+    for dirpath, _, files in os.walk(os.path.join(ROOT, "paper_2606_01556_b200", "csrc")):
+        for f in files:
+            if f.endswith((".cu", ".cuh", ".h")):
+                assert "getenv" not in open(os.path.join(dirpath, f)).read(), f
+    try:
+        base = twq.testing_describe_plan(300, 1024, 1024, 128, 128)
+        assert base["kernel"] == "tcgen05" and base["splits"] > 1
+        twq.testing_set_plan_flags(twq.PLAN_NO_SPLIT)
+        forced = twq.testing_describe_plan(300, 1024, 1024, 128, 128)
+        assert forced["splits"] == 1 and forced["pair"] == 1
+        assert twq.testing_describe_plan(16, 4096, 4096, 128, 128)["kernel"] == "decode"
+        twq.testing_set_plan_flags(twq.PLAN_NO_DECODE)
+        assert twq.testing_describe_plan(16, 4096, 4096, 128, 128)["kernel"] == "tcgen05"
+    finally:
+        twq.testing_set_plan_flags(0)
+
+
 def test_workspace_rule(lib):
     import paper_2606_01556_b200 as twq
     assert twq.workspace_bytes(2048, 14336, 4096, 128, 128) == 0      # prefill: tiles fill the GPU, no split
     assert twq.workspace_bytes(1, 4096, 4096, 128, 128) == 0           # decode kernel (M <= 16): no scratch
     assert twq.workspace_bytes(16, 4096, 4096, 128, 128) == 0
-    w = twq.workspace_bytes(32, 4096, 4096, 128, 128)                  # few tiles: split-K partials + counters
-    assert w > 0 and (w - 256) % (32 * 4096 * 4) == 0
+    assert twq.workspace_bytes(32, 4096, 4096, 128, 128) == 0          # small-batch kernel up to M = 32
+    w = twq.workspace_bytes(48, 4096, 4096, 128, 128)                  # few tiles: split-K partials + counters
+    assert w > 0 and (w - 256) % (48 * 4096 * 4) == 0
     assert twq.workspace_bytes(0, 4096, 4096, 128, 128) == 0           # invalid shape
 
 
@@ -104,7 +133,7 @@ def test_argument_validation_happens_before_cuda(lib):
     assert lib.twq_dual_linear(None, 256, p, p, p, 8, 512, 256, 16, 64, p, 0, 512, None, 0, None, None) == 1
     assert lib.twq_dual_linear(p, 256, p, p, p, 8, 512, 256, 16, 64, p, 7, 512, None, 0, None, None) == 1
     assert lib.twq_dual_linear(p, 256, p, p, p, 8, 512, 256, 16, 64, p, 0, 256, None, 0, None, None) == 1
-    assert lib.twq_dual_linear(p, 256, p, p, p, 24, 512, 256, 16, 64, p, 0, 512, None, 0, None, None) == 3
+    assert lib.twq_dual_linear(p, 256, p, p, p, 40, 512, 256, 16, 64, p, 0, 512, None, 0, None, None) == 3
     # valid arguments but no sm_100 device here -> UNSUPPORTED or CUDA error, never a crash, never OK
     import torch
     if not torch.cuda.is_available():

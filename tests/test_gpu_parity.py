@@ -26,6 +26,13 @@ def twq():
     return t
 
 
+@pytest.fixture
+def plan_flags(twq):
+    """Planner overrides of include/twq_testing.h for one test (reset to 0 afterwards)."""
+    yield twq.testing_set_plan_flags
+    twq.testing_set_plan_flags(0)
+
+
 def _dev(a, dtype=None):
     import torch
     t = torch.from_numpy(np.ascontiguousarray(a)).cuda()
@@ -125,11 +132,17 @@ def test_ragged_shapes(twq, oracle, M, K, N, r, G):
     (8, 2048, 528, 48, 128),     # r not a multiple of 32: half-empty last stage-2 step; N = 33 tiles
     (9, 1024, 272, 256, 128),    # two token tiles of the MMA (M > 8), rank 256: two j-tiles per warp
     (12, 640, 16, 0, 128),       # rank 0 in the decode kernel, fewer tiles than CTAs
-    (16, 7168, 1040, 128, 128),  # long K: items with more groups than pipeline slots, several ring rounds
+    (16, 7168, 1040, 128, 128),  # long K: more ring chunks than slots, several ring rounds
     (16, 512, 4112, 32, 64),     # many tiles per CTA, whole K in one part
+    (17, 384, 400, 48, 128),     # two 16-token MMA tiles, second almost empty
+    (32, 1024, 528, 256, 64),    # two full token tiles, rank 256, G = 64
+    (25, 2048, 2064, 128, 128),  # ragged second token tile, N = 258 tiles over the grid
+    (2, 256, 8192, 16, 128),     # many tiles per CTA; smallest rank
+    (4, 128, 16, 256, 128),      # one K-group, two tiles, rank 256 with most cluster ranks holding no K slab
 ])
 def test_decode_kernel_shapes(twq, oracle, M, K, N, r, G):
-    """M <= 16 takes the register-resident decode kernel (decode_kernel.cu); same bar as every other shape."""
+    """M <= 32 takes the bulk-copy streaming kernel (decode_kernel.cu); same bar as every other shape."""
+    assert twq.testing_describe_plan(M, N, K, r, G)["kernel"] == "decode"
     assert twq.workspace_bytes(M, N, K, r, G) == 0
     _check_layer(twq, oracle, gen.make_layer(M, K, N, r, G, seed=2000 + M + N, with_tinv=(M % 2 == 1)))
 
@@ -143,10 +156,12 @@ def test_decode_kernel_shapes(twq, oracle, M, K, N, r, G):
                                   # with a new token tile's stage 1 following tiles that used L2T
     (300, 512, 1280, 256, 64),    # the same overlay with G = 64 and a ragged token tile
 ])
-def test_fused_kernel_cta_pairs(twq, oracle, monkeypatch, M, K, N, r, G):
+def test_fused_kernel_cta_pairs(twq, oracle, plan_flags, M, K, N, r, G):
     """128-token tiles in an even cluster run as CTA pairs (cta_group::2, fused_kernel.cuh); same bar.
-    Shapes this small would split K instead; the planner's testing switch sends them down the unsplit path."""
-    monkeypatch.setenv("TWQ_DEBUG_NO_SPLIT", "1")
+    Shapes this small would split K instead; the planner's testing override sends them down the unsplit path."""
+    plan_flags(twq.PLAN_NO_SPLIT)
+    plan = twq.testing_describe_plan(M, N, K, r, G)
+    assert plan["kernel"] == "tcgen05" and plan["pair"] == 1 and plan["splits"] == 1
     assert twq.workspace_bytes(M, N, K, r, G) == 0
     rows = None if M * N * K <= 2 ** 29 else sorted(set(np.linspace(0, M - 1, 96).astype(int).tolist()))
     _check_layer(twq, oracle, gen.make_layer(M, K, N, r, G, seed=3000 + M, with_tinv=(M % 2 == 0)), rows=rows)
@@ -154,7 +169,7 @@ def test_fused_kernel_cta_pairs(twq, oracle, monkeypatch, M, K, N, r, G):
 
 @pytest.mark.parametrize("pad", [0, 8, 2, 1])
 @pytest.mark.parametrize("split,N", [(False, 1232), (False, 1200), (True, 1232)])
-def test_fused_kernel_store_paths(twq, oracle, monkeypatch, pad, split, N):
+def test_fused_kernel_store_paths(twq, oracle, plan_flags, pad, split, N):
     """Every store path of the fused kernel writes the same Y (fused_kernel.cuh, 'The store of a finished tile' in
     DESIGN.md 6.2): row pitch N + pad selects staged TMA tiles / 16-byte transposed stores (pad % 8 == 0), lane pairs
     (even pad) or element stores (odd pad); unsplit 128-token tiles (CTA pairs: 10 channel tiles) or the split-K
@@ -163,7 +178,7 @@ def test_fused_kernel_store_paths(twq, oracle, monkeypatch, pad, split, N):
     import torch
     M, K, r, G = 300, 512, 64, 128
     if not split:
-        monkeypatch.setenv("TWQ_DEBUG_NO_SPLIT", "1")
+        plan_flags(twq.PLAN_NO_SPLIT)
     L = gen.make_layer(M, K, N, r, G, seed=4100)
     X, packed, _ = _upload(twq, L)
     Xq, sx = twq.quantize_act(X, G)
@@ -180,19 +195,36 @@ def test_fused_kernel_store_paths(twq, oracle, monkeypatch, pad, split, N):
             assert (buf[:, N:] == -77.0).all(), "wrote beyond N"
 
 
-def test_rank0_is_plain_w4a4_and_zero_residual_is_lowrank(twq, oracle):
-    """north_star special cases, on the GPU path."""
+@pytest.mark.parametrize("M,flags,kernel,pair,split", [
+    (5, 0, "decode", 0, False),           # small-batch kernel, one token tile
+    (24, 0, "decode", 0, False),          # small-batch kernel, two token tiles
+    (40, 0, "tcgen05", 0, True),          # tcgen05 kernel, split-K path
+    (300, 1, "tcgen05", 1, False),        # tcgen05 kernel, CTA pairs (PLAN_NO_SPLIT)
+    (24, 16, "tcgen05", 0, True),         # small batch forced onto the tcgen05 kernel (PLAN_NO_DECODE)
+])
+def test_rank0_is_plain_w4a4_and_zero_residual_is_lowrank(twq, oracle, plan_flags, M, flags, kernel, pair, split):
+    """north_star special cases on every GPU path.  With R = 0 the output is the low-rank product alone, so an error
+    of that branch cannot hide under max|Yref| of the (much larger) residual branch."""
     import torch
-    L = gen.make_layer(24, 512, 256, 0, 128, seed=31)
+    plan_flags(flags)
+    K, N = 512, 512
+    plan = twq.testing_describe_plan(M, N, K, 64, 128)
+    assert plan["kernel"] == kernel and plan["pair"] == pair and (plan["splits"] > 1) == split, plan
+    L = gen.make_layer(M, K, N, 0, 128, seed=31)
     _check_layer(twq, oracle, L)
-    L = gen.make_layer(24, 512, 256, 64, 128, seed=32)
+    L = gen.make_layer(M, K, N, 64, 128, seed=32)
     L.Rq[:] = 0
     X, packed, _ = _upload(twq, L)
     Xq, sx = twq.quantize_act(X, L.G)
-    Y = twq.dual_linear(X, Xq, sx, packed, twq.OUT_FP32).cpu().numpy().astype(np.float64)
+    ws = None
+    need = twq.workspace_bytes(M, N, K, L.r, L.G)
+    if need:
+        ws = torch.zeros(need, dtype=torch.uint8, device="cuda")
+    Y = twq.dual_linear(X, Xq, sx, packed, twq.OUT_FP32, ws=ws).cpu().numpy().astype(np.float64)
     Xf = gen.bf16_bits_to_f32(L.X).astype(np.float64)
     ref = (Xf @ L.L1.astype(np.float64)) @ L.L2.astype(np.float64)      # FP64 BLAS, independent of the oracle
-    assert np.abs(Y - ref).max() / np.abs(ref).max() <= TOL
+    # H is rounded once to FP16 (reading R12): 2^-11 relative per term of the r-term sum
+    assert np.abs(Y - ref).max() / np.abs(ref).max() <= 1e-3
 
 
 def test_extreme_codes_hit_the_accumulator_bound(twq, oracle):
@@ -233,34 +265,29 @@ def test_exactly_representable_output_is_bit_exact(twq, oracle):
     assert (ref["Y"] == gen.bf16_bits_to_f32(oracle.round_bf16(ref["Y"])).astype(np.float64)).all()  # truly exact
 
 
-@pytest.mark.parametrize("M,K,N,r,G", [(1, 8192, 4096, 128, 128), (16, 8192, 2048, 256, 128), (5, 4096, 4096, 64, 64)])
-def test_decode_kernel_stage1_over_all_clusters(twq, oracle, monkeypatch, M, K, N, r, G):
-    """decode_kernel.cu with the K range of stage 1 split over the whole grid (DecodeParams.ncl_k > 1): cluster-level
-    partials of H meet in the workspace behind a grid-wide barrier.  Forced on for shapes the oracle finishes quickly;
-    the same workspace serves three calls in a row (the counter must come back to zero)."""
+@pytest.mark.parametrize("cs", [1, 2, 4, 8, 16])
+@pytest.mark.parametrize("M,K,N,r,G", [(1, 4096, 1024, 128, 128), (16, 2048, 2048, 256, 128), (20, 1024, 528, 64, 64)])
+def test_decode_kernel_every_cluster_size(twq, oracle, plan_flags, cs, M, K, N, r, G):
+    """decode_kernel.cu shares H = X*L1 inside a thread-block cluster: every cluster size the planner can pick
+    (16 on an idle B200) gives the same Y within the tolerance, repeatably, with no workspace."""
     import torch
-    monkeypatch.setenv("TWQ_DEBUG_DECODE_GRIDK", "1")
-    need = twq.workspace_bytes(M, N, K, r, G)
-    assert need > 0
+    plan_flags(twq.plan_decode_cs(cs))
+    plan = twq.testing_describe_plan(M, N, K, r, G)
+    assert plan["kernel"] == "decode" and plan["cluster"] == cs, plan
+    assert twq.workspace_bytes(M, N, K, r, G) == 0
     L = gen.make_layer(M, K, N, r, G, seed=5200 + M)
     X, packed, _ = _upload(twq, L)
     Xq, sx = twq.quantize_act(X, G)
-    ws = torch.zeros(need, dtype=torch.uint8, device="cuda")
     ref = oracle.forward(L.X, L.Rq, L.sw, L.L1, L.L2, G, want_P=False)["Y"]
-    ys = [twq.dual_linear(X, Xq, sx, packed, twq.OUT_FP32, ws=ws) for _ in range(3)]
+    ys = [twq.dual_linear(X, Xq, sx, packed, twq.OUT_FP32) for _ in range(3)]
     torch.cuda.synchronize()
     for y in ys:
         assert np.abs(y.cpu().numpy().astype(np.float64) - ref).max() / np.abs(ref).max() <= TOL
         assert (y == ys[0]).all(), "not deterministic across calls"
-    assert int(ws[:4].view(torch.int32).item()) == 0, "barrier counter not left at zero"
-    monkeypatch.setenv("TWQ_DEBUG_DECODE_GRIDK", "0")
-    assert twq.workspace_bytes(M, N, K, r, G) == 0
-    y0 = twq.dual_linear(X, Xq, sx, packed, twq.OUT_FP32)
-    assert np.abs(y0.cpu().numpy().astype(np.float64) - ref).max() / np.abs(ref).max() <= TOL
 
 
 def test_decode_kernel_strides_fp16_output_no_workspace(twq, oracle):
-    """M <= 16 runs the register-resident decode kernel: no scratch, padded Y rows untouched, repeatable."""
+    """Small batches run the bulk-copy streaming kernel: no scratch, padded Y rows untouched, repeatable."""
     import torch
     L = gen.make_layer(9, 512, 256, 32, 128, seed=41)
     X, packed, _ = _upload(twq, L)
@@ -280,11 +307,11 @@ def test_decode_kernel_strides_fp16_output_no_workspace(twq, oracle):
 
 def test_strides_fp16_output_and_workspace_reuse(twq, oracle):
     import torch
-    L = gen.make_layer(24, 512, 256, 32, 128, seed=41)
+    L = gen.make_layer(40, 512, 256, 32, 128, seed=41)
     X, packed, _ = _upload(twq, L)
     Xq, sx = twq.quantize_act(X, L.G)
     need = twq.workspace_bytes(L.M, L.N, L.K, L.r, L.G)
-    assert need > 0                                         # decode-shaped: split-K path
+    assert need > 0                                         # few output tiles: split-K path of the tcgen05 kernel
     ws = torch.zeros(need, dtype=torch.uint8, device="cuda")
     Ybig = torch.full((L.M, L.N + 64), 7.0, dtype=torch.float16, device="cuda")
     Yv = Ybig[:, :L.N]
@@ -302,7 +329,7 @@ def test_strides_fp16_output_and_workspace_reuse(twq, oracle):
 
 def test_errors_are_reported_not_thrown_by_cuda(twq):
     import torch
-    L = gen.make_layer(20, 256, 128, 0, 128, seed=5)
+    L = gen.make_layer(40, 256, 128, 0, 128, seed=5)
     X, packed, _ = _upload(twq, L)
     Xq, sx = twq.quantize_act(X, L.G)
     with pytest.raises(twq.TwqError):
