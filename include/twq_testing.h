@@ -40,6 +40,12 @@ enum {
  * Writes up to n_out ints; returns the number of fields, or -1 for an invalid shape. */
 int twq_testing_describe_plan(int M, int N, int K, int r, int G, int* out, int n_out);
 
+/* In-kernel timeline (csrc/trace.cuh).  Hands a device buffer of at least 16384 unsigned 64-bit words to the library;
+ * NULL switches the timeline off.  Returns 1 if this library was built with the timeline compiled in
+ * (`python -m paper_2606_01556_b200._build --trace` -> libtwq_trace.so), 0 if not (the product library: the call has
+ * no effect). */
+int twq_testing_set_trace_buffer(void* dev_buf);
+
 #ifdef __cplusplus
 }
 #endif

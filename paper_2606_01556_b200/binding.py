@@ -17,7 +17,8 @@ EXPORTS = ("twq_status_string", "twq_packed_bytes", "twq_pack_weights", "twq_qua
            "twq_workspace_bytes", "twq_dual_linear", "twq_last_launch_count")
 
 
-TESTING_EXPORTS = ("twq_testing_set_plan_flags", "twq_testing_get_plan_flags", "twq_testing_describe_plan")
+TESTING_EXPORTS = ("twq_testing_set_plan_flags", "twq_testing_get_plan_flags", "twq_testing_describe_plan",
+                   "twq_testing_set_trace_buffer")
 # include/twq_testing.h: planner overrides for tests
 PLAN_NO_SPLIT, PLAN_NO_PAIR, PLAN_NO_YSTAGE, PLAN_NO_ALIAS2, PLAN_NO_DECODE = 1, 2, 4, 8, 16
 _PLAN_FIELDS = ("kernel", "cluster", "grid", "tile_tokens", "splits", "pair", "smem", "ring", "chunks")
@@ -77,6 +78,8 @@ def load_library(build_if_missing: bool = True):
     lib.twq_testing_get_plan_flags.argtypes = []
     lib.twq_testing_describe_plan.restype = i
     lib.twq_testing_describe_plan.argtypes = [i, i, i, i, i, ctypes.POINTER(ctypes.c_int), i]
+    lib.twq_testing_set_trace_buffer.restype = i
+    lib.twq_testing_set_trace_buffer.argtypes = [vp]
     _lib = lib
     return lib
 
@@ -110,6 +113,11 @@ def last_launch_count() -> int:
 def testing_set_plan_flags(flags: int) -> None:
     """include/twq_testing.h: process-wide planner overrides (0 = production)."""
     load_library().twq_testing_set_plan_flags(flags)
+
+
+def testing_set_trace_buffer(buf) -> bool:
+    """csrc/trace.cuh: hand a CUDA uint64 tensor (>= 16384 words) or None; True if the timeline is compiled in."""
+    return bool(load_library().twq_testing_set_trace_buffer(_ptr(buf)))
 
 
 def testing_describe_plan(M: int, N: int, K: int, r: int, G: int) -> dict:

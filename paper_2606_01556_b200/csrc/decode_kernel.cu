@@ -9,18 +9,18 @@
 // Everything that does not depend on the activations is therefore in flight from the first instruction, as
 // asynchronous bulk copies (TMA, cp.async.bulk) into shared memory that complete on mbarriers:
 //
-//   warp 16      residual producer.  The CTA owns `ntile` consecutive 8-channel tiles; R4 is stored tile-major
+//   warp 18      residual producer.  The CTA owns `ntile` consecutive 8-channel tiles; R4 is stored tile-major
 //                ([N/8][K/G][8][G/2]), so the K-groups [c*gc, (c+1)*gc) of a tile are one contiguous range.  Chunk c
 //                of the ring = those ranges of all tiles (1-D bulk copies, issued BEFORE griddepcontrol.wait: weights
 //                do not depend on the previous kernel) + the same groups of Xq for all tokens (one 3-D tensor-map box,
 //                after the wait; rows beyond M are zero-filled by the TMA unit).
-//   warp 17      stage-1 producer: this cluster rank's K slice of L1 (slab layout [K/32][r][32]: one contiguous
+//   warp 19      stage-1 producer: this cluster rank's K slice of L1 (slab layout [K/32][r][32]: one contiguous
 //                range) through its own ring; also pulls the CTA's rows of L2T into L2.
 //   warps 0..lrw-1   the low-rank chain: X slice -> FP16 shared memory, H partial (FP16 warp MMA, FP32 accumulate),
 //                reduce-scatter of the FP32 partials and all-gather of the FP16 result through distributed shared
 //                memory (fixed order; mbarriers with cluster-scope release / acquire), then Ylr = H * L2T rows.
 //                H never leaves the chip (L177-179).
-//   warps lrw..15    the residual: per ring chunk, INT4 -> int8 (each code c becomes the byte 16*c: one shift / and
+//   warps lrw..17    the residual: per ring chunk, INT4 -> int8 (each code c becomes the byte 16*c: one shift / and
 //                per word, sign for free), warp-level int8 MMAs (activations are the 16-row operand, so a tile is 8
 //                channels), int32 = 256*P folded with both group scales in FP32.  When the CTA has fewer tiles than
 //                residual warps the K-groups of a tile are dealt round-robin to P warps and summed in fixed order.
@@ -36,17 +36,21 @@
 #include <cuda_fp16.h>
 #include <stdio.h>
 
+#include <type_traits>
+
 #include "fused_kernel.h"
 #include "sm100_ptx.cuh"
+#include "trace.cuh"
 
 namespace twq {
 
 namespace {
 
-constexpr int kDecWarps = 16;                       // compute warps
-constexpr int kDecThreads = (kDecWarps + 2) * 32;   // + the two producer warps
+constexpr int kDecWarps = 18;                       // compute warps (registers are allotted to warps in fours: 20 warps
+                                                    // cost the same 96 registers per thread as 18 would)
+constexpr int kDecThreads = (kDecWarps + 2) * 32;   // + the producer warp and a spare
 constexpr int kMaxSlots = 8, kMaxL1Slots = 4;
-constexpr int kTPW = 3;                             // 8-channel tiles one residual warp can own
+constexpr int kTB = 3;                              // tiles whose MMA chains a residual warp interleaves
 constexpr int kJT = 8;                              // 8-wide j tiles of H one low-rank warp can own
 constexpr int kDecSmemMax = 232448 - 1024;
 
@@ -160,6 +164,12 @@ decode_dual_linear_kernel(const __grid_constant__ CUtensorMap tmXq, const __grid
     const int gid = lane >> 2, tid4 = lane & 3;
     const int r = p.r, ng = p.ng, cs = p.cs, lrw = p.lrw;
     const int nrw = kDecWarps - lrw;
+    constexpr int kTPW = MT == 1 ? 6 : 3;       // 8-channel tiles one residual warp can own (its accumulators)
+    // Warp roles by id: [0, nrw) residual, [nrw, 18) low-rank chain, 18 spare, 19 producer.  The scheduler of an SM
+    // sub-partition favours HIGHER warp ids: the dependent low-rank chain and the producer must not queue behind the
+    // residual warps (with the chain in warps 0-3 every step of it waited for an issue slot; in-kernel timeline, r02).
+    const bool is_lr = warp >= nrw && warp < kDecWarps;
+    const int lw = warp - nrw;                  // index among the low-rank warps
     const int rank = cs > 1 ? static_cast<int>(cluster_ctarank()) : 0;
     // 8-channel tiles of this CTA: an even split of the n_tiles over the grid
     const int tile0 = static_cast<int>(static_cast<long long>(blockIdx.x) * p.n_tiles / gridDim.x);
@@ -170,12 +180,17 @@ decode_dual_linear_kernel(const __grid_constant__ CUtensorMap tmXq, const __grid
     const int nu = r > 0 ? static_cast<int>(static_cast<long long>(units) * (rank + 1) / cs) - u0 : 0;
     const int nl1 = (nu + p.sc - 1) / p.sc;                 // stage-1 ring chunks
     const int slab_bytes = r * 64;
-    // K-parts per tile: with fewer tiles than residual warps the groups of a tile are dealt to P warps
-    int P = ntile > 0 ? nrw / ntile : 1;
+    // Residual warps form a (tile group x K part) grid: TG groups of at most kTPW tiles, P = nrw / TG warps per group,
+    // warp `part` of a group taking the K-groups g = part (mod P).  A warp thus expands the activation fragments of a
+    // K-group once for all its tiles, and its tiles are independent MMA chains.
+    const int TG = ntile > 0 ? (ntile + kTPW - 1) / kTPW : 1;
+    const int tpg = (ntile + TG - 1) / TG;      // tiles per group
+    int P = nrw / TG;
     P = max(1, min(P, ng));
     const int nloc = p.tmax * 8;
     const int hstride = r + 8;
 
+    TWQ_DSTAMP(0);
     const uint32_t bar0 = smem_u32(dsm + p.off_bar);
 #define DBAR(i) (bar0 + 8u * static_cast<uint32_t>(i))
     if (threadIdx.x == 0) {
@@ -191,66 +206,99 @@ decode_dual_linear_kernel(const __grid_constant__ CUtensorMap tmXq, const __grid
     // everyone else before exit; it costs nothing on the way in.
     if (cs > 1) cluster_arrive_relaxed();
     pdl_launch_dependents();
+    TWQ_DSTAMP(1);
 
-    if (warp == kDecWarps) {
-        // ================================================================ residual producer
-        if (lane == 0 && ntile > 0) {
-            const uint64_t pol = policy_evict_first();          // streamed once
-            const uint32_t ring = smem_u32(dsm + p.off_ring);
-            const uint8_t* src0 = p.R4 + static_cast<size_t>(tile0) * ng * kBlk;
-            const uint32_t xq_bytes = static_cast<uint32_t>(p.gc) * kMp * (G / 2);   // a full box, zero-filled beyond M / ng
-            const int first = min(p.nslots, p.nchunks);
-            const uint32_t sw_bytes = static_cast<uint32_t>(ntile) * ng * 16;        // this CTA's FP16 group scales
-            auto issue_w = [&](int c, int slot) {
-                const int g0 = c * p.gc, gcnt = min(p.gc, ng - g0);
-                mbar_arrive_expect_tx_a(DBAR(D_FULL + slot),
-                                        static_cast<uint32_t>(ntile) * gcnt * kBlk + xq_bytes + (c == 0 ? sw_bytes : 0u));
-                if (c == 0)   // the scales ride on the first chunk's barrier: every residual warp waits for it first
-                    bulk_load_1d_a(smem_u32(dsm + p.off_sw), p.sw16 + static_cast<size_t>(tile0) * ng * 8, sw_bytes,
-                                   DBAR(D_FULL + slot), policy_evict_first());
-                for (int t = 0; t < ntile; ++t)
-                    bulk_load_1d_a(ring + slot * p.slot_bytes + t * (p.gc * kBlk),
-                                   src0 + (static_cast<size_t>(t) * ng + g0) * kBlk, static_cast<uint32_t>(gcnt) * kBlk,
-                                   DBAR(D_FULL + slot), pol);
-            };
-            for (int c = 0; c < first; ++c) issue_w(c, c);       // weights do not depend on the previous kernel
-            pdl_wait();                                          // Xq does (twq_quantize_act)
-            for (int c = 0; c < first; ++c)
-                tma_load_3d_a(ring + c * p.slot_bytes + p.xq_off, &tmXq, DBAR(D_FULL + c), 0, c * p.gc, 0);
-            int slot = 0, lap = 1;
-            for (int c = first; c < p.nchunks; ++c) {
-                mbar_wait_a(DBAR(D_EMPTY + slot), (lap - 1) & 1);
-                issue_w(c, slot);
-                tma_load_3d_a(ring + slot * p.slot_bytes + p.xq_off, &tmXq, DBAR(D_FULL + slot), 0, c * p.gc, 0);
-                if (++slot == p.nslots) { slot = 0; ++lap; }
-            }
-        }
-    } else if (warp == kDecWarps + 1) {
-        // ================================================================ stage-1 producer
-        if (lane == 0 && r > 0) {
-            const uint64_t pol = policy_evict_last();            // every cluster reads all of L1: keep it in L2
-            const uint32_t l1ring = smem_u32(dsm + p.off_l1);
-            const uint8_t* src = static_cast<const uint8_t*>(p.L1D) + static_cast<size_t>(u0) * slab_bytes;
-            int slot = 0, lap = 0;
-            for (int i = 0; i < nl1; ++i) {
-                if (lap > 0) mbar_wait_a(DBAR(D_L1EMPTY + slot), (lap - 1) & 1);
-                const int cnt = min(p.sc, nu - i * p.sc);
-                mbar_arrive_expect_tx_a(DBAR(D_L1FULL + slot), static_cast<uint32_t>(cnt) * slab_bytes);
-                bulk_load_1d_a(l1ring + slot * (p.sc * slab_bytes), src + static_cast<size_t>(i) * p.sc * slab_bytes,
-                               static_cast<uint32_t>(cnt) * slab_bytes, DBAR(D_L1FULL + slot), pol);
-                if (++slot == p.l1_slots) { slot = 0; ++lap; }
-                if (i == p.l1_slots - 1 && ntile > 0)   // stage 2 reads this CTA's rows of L2T straight from L2
-                    bulk_prefetch_l2(static_cast<const uint8_t*>(p.L2T) + static_cast<size_t>(tile0) * 8 * r * 2,
-                                     static_cast<uint32_t>(ntile) * 8 * r * 2);
-            }
-            if (nl1 < p.l1_slots && ntile > 0)
+    if (warp == kDecWarps + 1) {
+        // ================================================================ producer warp
+        // One bulk copy occupies its issuing thread for as long as the copy engine needs for the copies queued before
+        // it (~60 GB/s per SM with the whole grid streaming; in-kernel timeline, r02), so (a) the copies of a lap are
+        // dealt to the 32 lanes, and (b) the order of issue is the order of need: the stage-1 slice of L1 (the dependent
+        // chain X*L1 -> exchange -> H*L2 is the critical path) before the residual stream.
+        const uint32_t l1ring = smem_u32(dsm + p.off_l1);
+        const uint8_t* l1src = static_cast<const uint8_t*>(p.L1D) + static_cast<size_t>(u0) * slab_bytes;
+        const uint64_t pol_keep = policy_evict_last();           // every cluster reads all of L1: keep it in L2
+        const uint64_t pol = policy_evict_first();               // the residual is streamed once
+        auto copy_l1 = [&](int i, int slot) {
+            const int cnt = min(p.sc, nu - i * p.sc);
+            mbar_arrive_expect_tx_a(DBAR(D_L1FULL + slot), static_cast<uint32_t>(cnt) * slab_bytes);
+            bulk_load_1d_a(l1ring + slot * (p.sc * slab_bytes), l1src + static_cast<size_t>(i) * p.sc * slab_bytes,
+                           static_cast<uint32_t>(cnt) * slab_bytes, DBAR(D_L1FULL + slot), pol_keep);
+        };
+        const int l1_first = r > 0 ? min(p.l1_slots, nl1) : 0;
+        if (lane < l1_first) copy_l1(lane, lane);                // first lap of the stage-1 ring: one lane per chunk
+        __syncwarp();
+        const uint32_t ring = smem_u32(dsm + p.off_ring);
+        const uint8_t* src0 = p.R4 + static_cast<size_t>(tile0) * ng * kBlk;
+        const uint32_t xq_bytes = static_cast<uint32_t>(p.gc) * kMp * (G / 2);   // a full box, zero-filled beyond M / ng
+        const uint32_t sw_bytes = static_cast<uint32_t>(ntile) * ng * 16;        // this CTA's FP16 group scales
+        const int first = ntile > 0 ? min(p.nslots, p.nchunks) : 0;
+        auto arm = [&](int c, int slot) {
+            const int gcnt = min(p.gc, ng - c * p.gc);
+            mbar_arrive_expect_tx_a(DBAR(D_FULL + slot),
+                                    static_cast<uint32_t>(ntile) * gcnt * kBlk + xq_bytes + (c == 0 ? sw_bytes : 0u));
+        };
+        auto copy_w = [&](int c, int slot, int t) {
+            const int g0 = c * p.gc, gcnt = min(p.gc, ng - g0);
+            bulk_load_1d_a(ring + slot * p.slot_bytes + t * (p.gc * kBlk), src0 + (static_cast<size_t>(t) * ng + g0) * kBlk,
+                           static_cast<uint32_t>(gcnt) * kBlk, DBAR(D_FULL + slot), pol);
+        };
+        if (lane == 0)
+            for (int c = 0; c < first; ++c) arm(c, c);
+        __syncwarp();
+        // weights do not depend on the previous kernel: the whole first lap goes out before griddepcontrol.wait
+        for (int i = lane; i < first * ntile; i += 32) copy_w(i / ntile, i / ntile, i % ntile);
+        if (lane == 31 && ntile > 0) {
+            // the scales ride on the first chunk's barrier (every residual warp waits for it first); stage 2 reads this
+            // CTA's rows of L2T straight from L2
+            bulk_load_1d_a(smem_u32(dsm + p.off_sw), p.sw16 + static_cast<size_t>(tile0) * ng * 8, sw_bytes, DBAR(D_FULL), pol);
+            if (r > 0)
                 bulk_prefetch_l2(static_cast<const uint8_t*>(p.L2T) + static_cast<size_t>(tile0) * 8 * r * 2,
                                  static_cast<uint32_t>(ntile) * 8 * r * 2);
         }
-    } else if (warp < lrw) {
+        TWQ_DSTAMP(2);
+        pdl_wait();                                              // Xq comes from twq_quantize_act
+        TWQ_DSTAMP(3);
+        if (lane < first)
+            tma_load_3d_a(ring + lane * p.slot_bytes + p.xq_off, &tmXq, DBAR(D_FULL + lane), 0, lane * p.gc, 0);
+        TWQ_DSTAMP(4);
+        // later laps of both rings (long K / many tiles only): lane 0 refills stage-1 chunks, the warp refills residual chunks
+        {
+            int s1 = 0, lap1 = 1, i1n = l1_first;                // stage-1 ring
+            int slot = 0, lap = 1, c = first;                    // residual ring
+            while (i1n < nl1 || (ntile > 0 && c < p.nchunks)) {
+                // stage-1 refills never wait for residual consumers and vice versa: poll both, act on what is free
+                if (i1n < nl1) {
+                    bool ok = false;
+                    if (lane == 0) ok = mbar_try_wait_a(DBAR(D_L1EMPTY + s1), (lap1 - 1) & 1);
+                    ok = __shfl_sync(0xffffffffu, ok ? 1 : 0, 0) != 0;
+                    if (ok) {
+                        if (lane == 0) copy_l1(i1n, s1);
+                        ++i1n;
+                        if (++s1 == p.l1_slots) { s1 = 0; ++lap1; }
+                    }
+                }
+                if (ntile > 0 && c < p.nchunks) {
+                    bool ok = false;
+                    if (lane == 0) ok = mbar_try_wait_a(DBAR(D_EMPTY + slot), (lap - 1) & 1);
+                    ok = __shfl_sync(0xffffffffu, ok ? 1 : 0, 0) != 0;
+                    if (ok) {
+                        if (lane == 0) arm(c, slot);
+                        __syncwarp();
+                        for (int t = lane; t < ntile; t += 32) copy_w(c, slot, t);
+                        if (lane == 31) tma_load_3d_a(ring + slot * p.slot_bytes + p.xq_off, &tmXq, DBAR(D_FULL + slot), 0, c * p.gc, 0);
+                        ++c;
+                        if (++slot == p.nslots) { slot = 0; ++lap; }
+                    }
+                }
+            }
+        }
+    } else if (warp == kDecWarps) {
+        // spare warp (registers are allotted to warps in fours)
+    } else if (is_lr) {
         // ================================================================ low-rank chain
-        const int lrt = threadIdx.x, nlr = lrw * 32;
+        const int lrt = threadIdx.x - nrw * 32, nlr = lrw * 32;
         pdl_wait();                                              // X comes from the previous kernel of the stream
+        TWQ_DSTAMP(2);
         {
             // X slice (tokens x 32*nu k, BF16 -> FP16) into shared memory, four 16-byte loads in flight per thread
             const uint16_t* X = static_cast<const uint16_t*>(p.X);
@@ -278,6 +326,7 @@ decode_dual_linear_kernel(const __grid_constant__ CUtensorMap tmXq, const __grid
             }
         }
         named_bar_sync(1, nlr);
+        TWQ_DSTAMP(3);
         // ---- stage 1: partial H of this CTA's K slice; warp w owns the j tiles w, w + lrw, ...
         const int njt = r >> 3;
         float d[kJT][MT][4];
@@ -291,39 +340,49 @@ decode_dual_linear_kernel(const __grid_constant__ CUtensorMap tmXq, const __grid
             const uint32_t l1ring = smem_u32(dsm + p.off_l1);
             const uint32_t xs0 = smem_u32(sXs) + (gid * p.xs_stride + tid4 * 8) * 2;
             int slot = 0, lap = 0;
+            TWQ_DCLK(0);
             for (int i = 0; i < nl1; ++i) {
                 mbar_wait_a(DBAR(D_L1FULL + slot), lap & 1);
+                if (i < 4) TWQ_DCLK(1 + 2 * i);
                 const uint32_t base = l1ring + slot * (p.sc * slab_bytes) + (gid * 64 + tid4 * 16);
                 const int cnt = min(p.sc, nu - i * p.sc);
                 for (int s = 0; s < cnt; ++s) {
                     const int us = i * p.sc + s;
+                    // all fragments of the slab first, then the MMAs interleaved over the j tiles: the warp issues in
+                    // order, so a load placed between two dependent MMAs would expose its latency and theirs in turn
                     uint4 a[MT][2];
+                    uint4 l[kJT];
 #pragma unroll
                     for (int t = 0; t < MT; ++t) {
                         a[t][0] = lds_v4(xs0 + ((t * 16) * p.xs_stride + us * 32) * 2);
                         a[t][1] = lds_v4(xs0 + ((t * 16 + 8) * p.xs_stride + us * 32) * 2);
                     }
 #pragma unroll
-                    for (int q = 0; q < kJT; ++q) {
-                        const int jt = warp + q * lrw;
-                        if (jt < njt) {                          // warp-uniform
-                            const uint4 l = lds_v4(base + (s * r + jt * 8) * 64);
+                    for (int q = 0; q < kJT; ++q)
+                        if (lw + q * lrw < njt) l[q] = lds_v4(base + (s * r + (lw + q * lrw) * 8) * 64);
 #pragma unroll
-                            for (int t = 0; t < MT; ++t) {
-                                hmma_16816(d[q][t], a[t][0].x, a[t][1].x, a[t][0].y, a[t][1].y, l.x, l.y);
-                                hmma_16816(d[q][t], a[t][0].z, a[t][1].z, a[t][0].w, a[t][1].w, l.z, l.w);
-                            }
+                    for (int q = 0; q < kJT; ++q)
+                        if (lw + q * lrw < njt) {              // warp-uniform
+#pragma unroll
+                            for (int t = 0; t < MT; ++t) hmma_16816(d[q][t], a[t][0].x, a[t][1].x, a[t][0].y, a[t][1].y, l[q].x, l[q].y);
                         }
-                    }
+#pragma unroll
+                    for (int q = 0; q < kJT; ++q)
+                        if (lw + q * lrw < njt) {
+#pragma unroll
+                            for (int t = 0; t < MT; ++t) hmma_16816(d[q][t], a[t][0].z, a[t][1].z, a[t][0].w, a[t][1].w, l[q].z, l[q].w);
+                        }
                 }
                 __syncwarp();
+                if (i < 4) TWQ_DCLK(2 + 2 * i);
                 if (lane == 0) mbar_arrive_a(DBAR(D_L1EMPTY + slot));
                 if (++slot == p.l1_slots) { slot = 0; ++lap; }
             }
         }
+        TWQ_DSTAMP(4);
 #pragma unroll
         for (int q = 0; q < kJT; ++q) {
-            const int jt = warp + q * lrw;
+            const int jt = lw + q * lrw;
             if (jt < njt) {
                 const int j = jt * 8 + tid4 * 2;
 #pragma unroll
@@ -343,32 +402,40 @@ decode_dual_linear_kernel(const __grid_constant__ CUtensorMap tmXq, const __grid
             for (int js = 0; js < kL2; ++js)
                 l2v[js] = (js * 32 + tid4 * 8 < r) ? ldg_nc(lrow + js * 64) : make_uint4(0, 0, 0, 0);
         };
-        if (warp < ntile) load_l2(warp);
+        if (lw < ntile) load_l2(lw);
         named_bar_sync(1, nlr);                                  // this CTA's partial is complete in shared memory
+        TWQ_DSTAMP(5);
         // ---- H = sum of the cluster's partials (fixed order), FP16, in every CTA's shared memory
         if (cs > 1) {
             cluster_wait();                                      // every peer's mbarriers are initialised
-            if (warp == 0 && lane < cs) mbar_arrive_remote(mapa_u32(DBAR(D_X1), static_cast<uint32_t>(lane)));
+            TWQ_DSTAMP(6);
+            if (lw == 0 && lane < cs) mbar_arrive_remote(mapa_u32(DBAR(D_X1), static_cast<uint32_t>(lane)));
             mbar_wait_cluster_a(DBAR(D_X1), 0);                  // every CTA's FP32 partial is visible
+            TWQ_DSTAMP(7);
+            // A thread owns one (token, column) element of this CTA's r/cs columns: the cs remote loads of its partials
+            // go out together (a warp's 32 lanes read 32 consecutive floats of ONE peer per instruction -- one remote
+            // transaction; one lane per peer was 16x the transactions and 6 us), are summed in rank order, and the FP16
+            // result is stored into every peer.
             const int jc = r / cs;
+            TWQ_DCLK(10);
             for (int e = lrt; e < p.M * jc; e += nlr) {
                 const int m = e / jc, j = rank * jc + (e - m * jc);
                 const uint32_t src = smem_u32(sHpart + m * r + j);
-                float s = 0.0f;
-                for (int pr = 0; pr < cs; pr += 8) {             // eight remote loads in flight, summed in rank order
-                    float v[8];
+                float v[16];
 #pragma unroll
-                    for (int q = 0; q < 8; ++q) v[q] = pr + q < cs ? ld_dsmem_f(mapa_u32(src, pr + q)) : 0.0f;
+                for (int q = 0; q < 16; ++q) v[q] = q < cs ? ld_dsmem_f(mapa_u32(src, q)) : 0.0f;
+                float sum = 0.0f;
 #pragma unroll
-                    for (int q = 0; q < 8; ++q) s += v[q];
-                }
-                s = fminf(fmaxf(s, -65504.0f), 65504.0f);
-                const __half hv = __float2half_rn(s);
+                for (int q = 0; q < 16; ++q) sum += v[q];
+                sum = fminf(fmaxf(sum, -65504.0f), 65504.0f);
+                const __half hv = __float2half_rn(sum);
                 const uint32_t dsta = smem_u32(sH + m * hstride + j);
                 for (int pr = 0; pr < cs; ++pr) st_dsmem_u16(mapa_u32(dsta, pr), *reinterpret_cast<const uint16_t*>(&hv));
             }
+            TWQ_DCLK(11);
+            TWQ_DSTAMP(8);
             named_bar_sync(1, nlr);
-            if (warp == 0 && lane < cs) mbar_arrive_remote(mapa_u32(DBAR(D_X2), static_cast<uint32_t>(lane)));
+            if (lw == 0 && lane < cs) mbar_arrive_remote(mapa_u32(DBAR(D_X2), static_cast<uint32_t>(lane)));
             mbar_wait_cluster_a(DBAR(D_X2), 0);                  // every CTA's columns of H have arrived (and nobody reads
                                                                  // this CTA's partial any more)
         } else {
@@ -379,9 +446,10 @@ decode_dual_linear_kernel(const __grid_constant__ CUtensorMap tmXq, const __grid
             }
             named_bar_sync(1, nlr);
         }
+        TWQ_DSTAMP(9);
         // ---- stage 2: Ylr[m, n] = sum_j H[m,j] * L2T[n,j] for this CTA's tiles
-        for (int t = warp; t < ntile; t += lrw) {
-            if (t != warp) load_l2(t);
+        for (int t = lw; t < ntile; t += lrw) {
+            if (t != lw) load_l2(t);
             float d2[MT][4];
 #pragma unroll
             for (int mt = 0; mt < MT; ++mt)
@@ -410,91 +478,114 @@ decode_dual_linear_kernel(const __grid_constant__ CUtensorMap tmXq, const __grid
                 *reinterpret_cast<float2*>(sYlr + (mt * 16 + gid + 8) * nloc + nl) = make_float2(d2[mt][2], d2[mt][3]);
             }
         }
+        TWQ_DSTAMP(10);
     } else {
         // ================================================================ residual warps
-        const int rw = warp - lrw;
-        const int tw = rw / P, part = rw - tw * P;
-        // tiles of this warp: with P == 1 tiles tw, tw + nrw, ...; otherwise the single tile tw (if it exists)
-        int ntw = 0;
-        if (P == 1) { for (int t = tw; t < ntile && ntw < kTPW; t += nrw) ++ntw; }
-        else if (tw < ntile) ntw = 1;
+        const int rw = warp;
+        const int tg = rw / P, part = rw - tg * P;
+        const int t_lo = tg * tpg;                               // this warp's tiles: [t_lo, t_lo + ntw)
+        const int ntw = tg < TG ? min(tpg, ntile - t_lo) : 0;
         pdl_wait();                                              // sx comes from twq_quantize_act
+        TWQ_DSTAMP(2);
         for (int i = rw * 32 + lane; i < kMp * ng; i += nrw * 32) {
             const int g = i / kMp, m = i - g * kMp;
             sSx[i] = m < p.M ? ldg_f32(p.sx + static_cast<size_t>(m) * ng + g) * 0x1p-8f : 0.0f;   // MMA operands are 16*code
         }
         named_bar_sync(2, nrw * 32);
-        float acc[kTPW][MT][4];
-#pragma unroll
-        for (int i = 0; i < kTPW; ++i)
-#pragma unroll
-            for (int t = 0; t < MT; ++t)
-#pragma unroll
-                for (int e = 0; e < 4; ++e) acc[i][t][e] = 0.0f;
-        const uint32_t ring = smem_u32(dsm + p.off_ring);
-        const uint32_t sw_a = smem_u32(dsm + p.off_sw) + tid4 * 4;
-        const uint32_t sx_a = smem_u32(sSx) + gid * 4;
+        TWQ_DSTAMP(3);
         if (ntile > 0) {
+            const uint32_t ring = smem_u32(dsm + p.off_ring);
+            const uint32_t sw_a = smem_u32(dsm + p.off_sw) + tid4 * 4;
+            const uint32_t sx_a = smem_u32(sSx) + gid * 4;
+            float acc[kTPW][MT][4];
+#pragma unroll
+            for (int i = 0; i < kTPW; ++i)
+#pragma unroll
+                for (int t = 0; t < MT; ++t)
+#pragma unroll
+                    for (int e = 0; e < 4; ++e) acc[i][t][e] = 0.0f;
             int slot = 0, lap = 0;
+#pragma unroll 1
             for (int c = 0; c < p.nchunks; ++c) {
                 mbar_wait_a(DBAR(D_FULL + slot), lap & 1);
+                if (c < 6) TWQ_DSTAMP(4 + 2 * c);
                 if (ntw > 0) {
                     const int g0 = c * p.gc, gcnt = min(p.gc, ng - g0);
-                    const uint32_t wbase = ring + slot * p.slot_bytes + gid * (G / 2) + tid4 * (kW * 4);
+                    const uint32_t wbase = ring + slot * p.slot_bytes + t_lo * (p.gc * kBlk) + gid * (G / 2) + tid4 * (kW * 4);
                     const uint32_t xbase = ring + slot * p.slot_bytes + p.xq_off + (gid * p.gc) * (G / 2) + tid4 * (kW * 4);
                     int gl = part - g0 % P;
                     if (gl < 0) gl += P;
+#pragma unroll 1
                     for (; gl < gcnt; gl += P) {
                         const int g = g0 + gl;
-                        // activation fragments of tokens gid / gid + 8 (per 16-token tile) and their scales
-                        uint32_t xa[MT][2][kW];
+                        // activation fragments of the K-group, expanded once for all tiles of the warp
+                        uint32_t ax[MT][kW][4];
                         float sxa[MT][2];
 #pragma unroll
                         for (int mt = 0; mt < MT; ++mt) {
-                            lds_words<kW>(xa[mt][0], xbase + ((mt * 16) * p.gc + gl) * (G / 2));
-                            lds_words<kW>(xa[mt][1], xbase + ((mt * 16 + 8) * p.gc + gl) * (G / 2));
+                            uint32_t x0[kW], x1[kW];
+                            lds_words<kW>(x0, xbase + ((mt * 16) * p.gc + gl) * (G / 2));
+                            lds_words<kW>(x1, xbase + ((mt * 16 + 8) * p.gc + gl) * (G / 2));
                             sxa[mt][0] = __uint_as_float(lds_u32(sx_a + (g * kMp + mt * 16) * 4));
                             sxa[mt][1] = __uint_as_float(lds_u32(sx_a + (g * kMp + mt * 16 + 8) * 4));
+#pragma unroll
+                            for (int w = 0; w < kW; ++w) {
+                                ax[mt][w][0] = d_lo16(x0[w]); ax[mt][w][1] = d_lo16(x1[w]);
+                                ax[mt][w][2] = d_hi16(x0[w]); ax[mt][w][3] = d_hi16(x1[w]);
+                            }
                         }
 #pragma unroll
-                        for (int i = 0; i < kTPW; ++i) {
-                            if (i < ntw) {                       // warp-uniform
-                                const int t = tw + i * nrw;
-                                uint32_t wt[kW];
-                                lds_words<kW>(wt, wbase + t * (p.gc * kBlk) + gl * kBlk);
-                                const uint32_t swh = lds_u32(sw_a + (t * ng + g) * 16);
-                                const float2 sw2 = __half22float2(*reinterpret_cast<const __half2*>(&swh));
-                                int dd[MT][4];
+                        for (int ib = 0; ib < kTPW; ib += kTB) {
+                            if (ib < ntw) {                      // warp-uniform
+                                // up to kTB tiles at a time: loads first, then their MMA chains interleaved
+                                uint32_t wt[kTB][kW];
+                                uint32_t swh[kTB];
+                                int dd[kTB][MT][4];
 #pragma unroll
-                                for (int mt = 0; mt < MT; ++mt)
-#pragma unroll
-                                    for (int e = 0; e < 4; ++e) dd[mt][e] = 0;
-#pragma unroll
-                                for (int w = 0; w < kW; ++w) {   // one K-step of 32 codes per packed word
-                                    const uint32_t b0 = d_lo16(wt[w]), b1 = d_hi16(wt[w]);
+                                for (int b = 0; b < kTB; ++b) {
+                                    const int i = min(ib + b, ntw - 1);   // a missing tile repeats the last one (its result is dropped)
+                                    lds_words<kW>(wt[b], wbase + i * (p.gc * kBlk) + gl * kBlk);
+                                    swh[b] = lds_u32(sw_a + ((t_lo + i) * ng + g) * 16);
 #pragma unroll
                                     for (int mt = 0; mt < MT; ++mt)
-                                        imma_16832(dd[mt], d_lo16(xa[mt][0][w]), d_lo16(xa[mt][1][w]), d_hi16(xa[mt][0][w]),
-                                                   d_hi16(xa[mt][1][w]), b0, b1);
+#pragma unroll
+                                        for (int e = 0; e < 4; ++e) dd[b][mt][e] = 0;
+                                }
+#pragma unroll
+                                for (int w = 0; w < kW; ++w) {   // one K-step of 32 codes per packed word
+#pragma unroll
+                                    for (int b = 0; b < kTB; ++b) {
+                                        const uint32_t b0 = d_lo16(wt[b][w]), b1 = d_hi16(wt[b][w]);
+#pragma unroll
+                                        for (int mt = 0; mt < MT; ++mt)
+                                            imma_16832(dd[b][mt], ax[mt][w][0], ax[mt][w][1], ax[mt][w][2], ax[mt][w][3], b0, b1);
+                                    }
                                 }
                                 // dd = 256 * P (exact); fold both scales in FP32 (sx already carries 2^-8)
 #pragma unroll
-                                for (int mt = 0; mt < MT; ++mt) {
-                                    acc[i][mt][0] = fmaf(__fmul_rn(static_cast<float>(dd[mt][0]), sw2.x), sxa[mt][0], acc[i][mt][0]);
-                                    acc[i][mt][1] = fmaf(__fmul_rn(static_cast<float>(dd[mt][1]), sw2.y), sxa[mt][0], acc[i][mt][1]);
-                                    acc[i][mt][2] = fmaf(__fmul_rn(static_cast<float>(dd[mt][2]), sw2.x), sxa[mt][1], acc[i][mt][2]);
-                                    acc[i][mt][3] = fmaf(__fmul_rn(static_cast<float>(dd[mt][3]), sw2.y), sxa[mt][1], acc[i][mt][3]);
-                                    if (kDbg) {
-                                        if (p.dbgP != nullptr) {
-                                            const int n = (tile0 + t) * 8 + tid4 * 2;
-                                            const int m0 = mt * 16 + gid;
-                                            if (m0 < p.M) {
-                                                p.dbgP[(static_cast<size_t>(m0) * ng + g) * p.N + n] = dd[mt][0] >> 8;
-                                                p.dbgP[(static_cast<size_t>(m0) * ng + g) * p.N + n + 1] = dd[mt][1] >> 8;
-                                            }
-                                            if (m0 + 8 < p.M) {
-                                                p.dbgP[(static_cast<size_t>(m0 + 8) * ng + g) * p.N + n] = dd[mt][2] >> 8;
-                                                p.dbgP[(static_cast<size_t>(m0 + 8) * ng + g) * p.N + n + 1] = dd[mt][3] >> 8;
+                                for (int b = 0; b < kTB; ++b) {
+                                    if (ib + b < ntw) {          // warp-uniform
+                                        const float2 sw2 = __half22float2(*reinterpret_cast<const __half2*>(&swh[b]));
+#pragma unroll
+                                        for (int mt = 0; mt < MT; ++mt) {
+                                            float (&a)[4] = acc[ib + b][mt];
+                                            a[0] = fmaf(__fmul_rn(static_cast<float>(dd[b][mt][0]), sw2.x), sxa[mt][0], a[0]);
+                                            a[1] = fmaf(__fmul_rn(static_cast<float>(dd[b][mt][1]), sw2.y), sxa[mt][0], a[1]);
+                                            a[2] = fmaf(__fmul_rn(static_cast<float>(dd[b][mt][2]), sw2.x), sxa[mt][1], a[2]);
+                                            a[3] = fmaf(__fmul_rn(static_cast<float>(dd[b][mt][3]), sw2.y), sxa[mt][1], a[3]);
+                                            if (kDbg) {
+                                                if (p.dbgP != nullptr) {
+                                                    const int n = (tile0 + t_lo + ib + b) * 8 + tid4 * 2;
+                                                    const int m0 = mt * 16 + gid;
+                                                    if (m0 < p.M) {
+                                                        p.dbgP[(static_cast<size_t>(m0) * ng + g) * p.N + n] = dd[b][mt][0] >> 8;
+                                                        p.dbgP[(static_cast<size_t>(m0) * ng + g) * p.N + n + 1] = dd[b][mt][1] >> 8;
+                                                    }
+                                                    if (m0 + 8 < p.M) {
+                                                        p.dbgP[(static_cast<size_t>(m0 + 8) * ng + g) * p.N + n] = dd[b][mt][2] >> 8;
+                                                        p.dbgP[(static_cast<size_t>(m0 + 8) * ng + g) * p.N + n + 1] = dd[b][mt][3] >> 8;
+                                                    }
+                                                }
                                             }
                                         }
                                     }
@@ -504,27 +595,31 @@ decode_dual_linear_kernel(const __grid_constant__ CUtensorMap tmXq, const __grid
                     }
                 }
                 __syncwarp();
+                if (c < 6) TWQ_DSTAMP(5 + 2 * c);
                 if (lane == 0) mbar_arrive_a(DBAR(D_EMPTY + slot));
                 if (++slot == p.nslots) { slot = 0; ++lap; }
             }
-        }
-        // this warp's partial tiles: [tile * P + part][token][8 channels]
+            // this warp's partial tiles: [tile * P + part][token][8 channels], parked in the ring, which every residual
+            // warp has finished reading (all chunks have landed and been consumed)
+            named_bar_sync(2, nrw * 32);
 #pragma unroll
-        for (int i = 0; i < kTPW; ++i) {
-            if (i < ntw) {
-                const int t = tw + i * nrw;
-                float* dst = sRes + static_cast<size_t>(t * P + part) * kMp * 8 + tid4 * 2;
+            for (int i = 0; i < kTPW; ++i) {
+                if (i < ntw) {
+                    float* dst = sRes + static_cast<size_t>((t_lo + i) * P + part) * kMp * 8 + tid4 * 2;
 #pragma unroll
-                for (int mt = 0; mt < MT; ++mt) {
-                    *reinterpret_cast<float2*>(dst + (mt * 16 + gid) * 8) = make_float2(acc[i][mt][0], acc[i][mt][1]);
-                    *reinterpret_cast<float2*>(dst + (mt * 16 + gid + 8) * 8) = make_float2(acc[i][mt][2], acc[i][mt][3]);
+                    for (int mt = 0; mt < MT; ++mt) {
+                        *reinterpret_cast<float2*>(dst + (mt * 16 + gid) * 8) = make_float2(acc[i][mt][0], acc[i][mt][1]);
+                        *reinterpret_cast<float2*>(dst + (mt * 16 + gid + 8) * 8) = make_float2(acc[i][mt][2], acc[i][mt][3]);
+                    }
                 }
             }
         }
     }
 
     // ---------------------------------------------------------------- single epilogue: sum the K-parts, add Ylr, one store
+    TWQ_DSTAMP(27);
     __syncthreads();
+    TWQ_DSTAMP(28);
     if (warp < kDecWarps) {
         const int ncl = ntile * 8;
         for (int i = threadIdx.x; i < ncl * p.M; i += kDecWarps * 32) {
@@ -539,7 +634,8 @@ decode_dual_linear_kernel(const __grid_constant__ CUtensorMap tmXq, const __grid
             else static_cast<float*>(p.Y)[o] = y;
         }
     }
-    if (cs > 1 && !(warp < lrw)) cluster_wait();   // completes this thread's half of the split barrier (long since released)
+    TWQ_DSTAMP(29);
+    if (cs > 1 && !is_lr) cluster_wait();   // completes this thread's half of the split barrier (long since released)
 #undef DBAR
 }
 
@@ -659,7 +755,8 @@ bool decode_make_plan(int M, int N, int K, int r, int G, int num_sms, DecodePara
     if (nclusters < 1) nclusters = 1;
     p.grid = nclusters * p.cs;
     p.tmax = (p.n_tiles + p.grid - 1) / p.grid;
-    if (p.tmax > kTPW * nrw) return false;
+    const int kTPWh = p.mt == 1 ? 6 : 3;                      // tiles per residual warp (kernel: kTPW)
+    if (p.tmax > kTPWh * nrw) return false;
     // ---- shared-memory plan
     const int kBlk = 4 * G;
     p.nu_max = r > 0 ? ((K >> 5) + p.cs - 1) / p.cs : 0;
@@ -669,7 +766,6 @@ bool decode_make_plan(int M, int N, int K, int r, int G, int num_sms, DecodePara
     p.off_bar = o; o += round_up_i(D_COUNT * 8, 128);
     p.off_sw = o; o += round_up_i(p.tmax * p.ng * 16, 128);
     p.off_sx = o; o += round_up_i(p.ng * p.mp * 4, 128);
-    p.off_res = o; o += round_up_i((p.tmax > nrw ? p.tmax : nrw) * p.mp * 8 * 4, 128);
     p.off_ylr = o; o += r > 0 ? round_up_i(p.mp * p.tmax * 8 * 4, 128) : 0;
     p.off_hpart = o; o += r > 0 ? round_up_i(p.mp * r * 4, 128) : 0;
     p.off_h = o; o += r > 0 ? round_up_i(p.mp * (r + 8) * 2, 128) : 0;
@@ -704,7 +800,13 @@ bool decode_make_plan(int M, int N, int K, int r, int G, int num_sms, DecodePara
     if (p.nslots > kMaxSlots) p.nslots = kMaxSlots;
     if (p.nslots > p.nchunks) p.nslots = p.nchunks;
     if (p.nslots < (p.nchunks > 1 ? 2 : 1)) return false;
-    o += p.nslots * p.slot_bytes;
+    // The K-part partial sums ([tile * P + part][token][8 channels], at most min(tmax, kTPW) * nrw of them) are parked in
+    // the ring once every chunk has been consumed.
+    const int res_bytes = (p.tmax < kTPWh ? p.tmax : kTPWh) * nrw * p.mp * 8 * 4;
+    p.off_res = p.off_ring;
+    const int ring_bytes = p.nslots * p.slot_bytes;
+    if (res_bytes > ring_bytes && res_bytes > budget) return false;
+    o += ring_bytes > res_bytes ? ring_bytes : res_bytes;
     p.smem_bytes = o + 1024;                                  // alignment slack of the dynamic base
     if (p.smem_bytes > kDecSmemMax) return false;
     *out = p;

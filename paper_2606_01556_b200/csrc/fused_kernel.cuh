@@ -62,6 +62,7 @@
 
 #include "fused_kernel.h"
 #include "sm100_ptx.cuh"
+#include "trace.cuh"
 
 namespace twq {
 
@@ -141,18 +142,6 @@ __device__ __forceinline__ uint32_t packed_chunk_offset(uint32_t row, uint32_t c
 
 // uses of P buffer b among the first q uses of the rotation
 __device__ __forceinline__ int buf_uses(int q, int b) { return (q + kNB - 1 - b) / kNB; }
-
-#ifdef TWQ_TRACE
-// Debug timeline: CTA 0 records (tag, clock64) per role.  Built only into the trace library.
-__device__ unsigned long long g_twq_trace[4 * 4096];
-#define TWQ_TR(role, n, tag)                                                                      \
-    do {                                                                                          \
-        if (blockIdx.x == 0 && (n) < 4096) g_twq_trace[(role) * 4096 + (n)++] =                   \
-            (static_cast<unsigned long long>(tag) << 48) | (static_cast<unsigned long long>(clock64()) & 0xFFFFFFFFFFFFull); \
-    } while (0)
-#else
-#define TWQ_TR(role, n, tag) do { } while (0)
-#endif
 
 struct Unit {
     int n0, m0, g_begin, g_end, ctx, ks;
@@ -690,9 +679,11 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
             const bool n_ok = n < p.N;
             // FP16 group scales, tiled [N/8][ng][8]: channel n of group g at ((n >> 3) * ng + g) * 8 + (n & 7)
             const __half* swp = p.sw16 + (n_ok ? (static_cast<size_t>(n >> 3) * p.ng * 8 + (n & 7)) : 0);
-            // weight scales two groups ahead of use
-            float sw0 = n_ok ? __half2float(__ldg(swp + static_cast<size_t>(t.g_begin) * 8)) : 0.0f;
-            float sw1 = (n_ok && t.g_begin + 1 < t.g_end) ? __half2float(__ldg(swp + static_cast<size_t>(t.g_begin + 1) * 8)) : 0.0f;
+            // weight scales two groups ahead of use; the raw FP16 bits wait in the registers and are converted at use
+            // (a conversion right behind the load would make the warp wait for the load it just issued)
+            const unsigned short* swu = reinterpret_cast<const unsigned short*>(swp);
+            unsigned short sw0 = n_ok ? __ldg(swu + static_cast<size_t>(t.g_begin) * 8) : static_cast<unsigned short>(0);
+            unsigned short sw1 = (n_ok && t.g_begin + 1 < t.g_end) ? __ldg(swu + static_cast<size_t>(t.g_begin + 1) * 8) : static_cast<unsigned short>(0);
             if (r > 0 && t.ctx != cur_ctx) {
                 cur_ctx = t.ctx;
                 int kc0, kc1;
@@ -816,9 +807,9 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
             }
 
             for (int g = t.g_begin; g < t.g_end; ++g, ++itp) {
-                const float swn = sw0;
+                const float swn = __half2float(__ushort_as_half(sw0));
                 sw0 = sw1;
-                sw1 = (n_ok && g + 2 < t.g_end) ? __half2float(__ldg(swp + static_cast<size_t>(g + 2) * 8)) : 0.0f;
+                sw1 = (n_ok && g + 2 < t.g_end) ? __ldg(swu + static_cast<size_t>(g + 2) * 8) : static_cast<unsigned short>(0);
                 const float cm = __fmul_rn(12582912.0f, swn);   // exact: sw has an 11-bit significand
                 const uint64_t sw2 = pack_f2(swn, swn), ncm2 = pack_f2(-cm, -cm);
 #ifdef TWQ_TRACE

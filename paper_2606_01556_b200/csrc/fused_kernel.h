@@ -36,6 +36,7 @@ struct FusedParams {
     int32_t* dbgP;           // NULL or [M][ng][N]
     float* ws_part;          // split-K partials [splits][M][N] (splits > 1 only)
     unsigned* ws_ctr;        // split-K tile counters [m_tiles][n_tiles], zero between calls
+    unsigned long long* trace;   // NULL, or the timeline buffer of a -DTWQ_TRACE build (trace.cuh)
     FusedPlan plan;
 };
 
@@ -68,6 +69,7 @@ struct DecodeParams {
     const float* sx;         // [M][ng]
     void* Y;
     int32_t* dbgP;
+    unsigned long long* trace;   // NULL, or the timeline buffer of a -DTWQ_TRACE build (trace.cuh)
 };
 bool decode_make_plan(int M, int N, int K, int r, int G, int num_sms, DecodeParams* out);
 cudaError_t launch_decode(const CUtensorMap& tmXq, const DecodeParams& p, int G, cudaStream_t stream);
@@ -85,6 +87,7 @@ enum : unsigned {
 };
 unsigned plan_flags();
 void set_plan_flags(unsigned f);
+unsigned long long* trace_buffer();   // set by twq_testing_set_trace_buffer; only read by -DTWQ_TRACE builds
 
 // Fills `plan` for a shape; returns false if the shape cannot be planned (never for valid ABI shapes).
 bool fused_make_plan(int M, int N, int K, int r, int G, int num_sms, FusedPlan* plan);

@@ -16,7 +16,10 @@ namespace twq {
 
 namespace {
 std::atomic<unsigned> g_plan_flags{0u};
+std::atomic<unsigned long long*> g_trace{nullptr};
 }
+unsigned long long* trace_buffer() { return g_trace.load(std::memory_order_relaxed); }
+void g_trace_store(unsigned long long* p) { g_trace.store(p, std::memory_order_relaxed); }
 unsigned plan_flags() { return g_plan_flags.load(std::memory_order_relaxed); }
 void set_plan_flags(unsigned f) { g_plan_flags.store(f, std::memory_order_relaxed); }
 
@@ -206,6 +209,14 @@ int twq_last_launch_count(void) { return g_last_launches; }
 
 void twq_testing_set_plan_flags(unsigned flags) { twq::set_plan_flags(flags); }
 unsigned twq_testing_get_plan_flags(void) { return twq::plan_flags(); }
+int twq_testing_set_trace_buffer(void* dev_buf) {
+    twq::g_trace_store(static_cast<unsigned long long*>(dev_buf));
+#ifdef TWQ_TRACE
+    return 1;
+#else
+    return 0;
+#endif
+}
 
 int twq_testing_describe_plan(int M, int N, int K, int r, int G, int* out, int n_out) {
     if (!shape_ok(M, N, K, r, G) || !out) return -1;
@@ -302,6 +313,7 @@ twq_status twq_dual_linear(const void* X, int ldx, const uint8_t* Xq, const floa
         dp.L1D = base + lay.off_l1d;
         dp.L2T = base + lay.off_l2t;
         dp.X = X; dp.sx = sx; dp.Y = Y; dp.dbgP = dbg_P;
+        dp.trace = twq::trace_buffer();
         // Xq [M][K/2] as (G/2 bytes, K/G groups, M tokens); one box = gc groups of all (padded) tokens
         MapKey k;
         memset(&k, 0, sizeof(k));
@@ -363,6 +375,7 @@ twq_status twq_dual_linear(const void* X, int ldx, const uint8_t* Xq, const floa
     p.sw16 = reinterpret_cast<const __half*>(base + lay.off_sw16);
     p.Y = Y;
     p.dbgP = dbg_P;
+    p.trace = twq::trace_buffer();
     p.ws_ctr = splits > 1 ? static_cast<unsigned*>(ws) : nullptr;
     p.ws_part = splits > 1 ? reinterpret_cast<float*>(static_cast<uint8_t*>(ws) + ctr_bytes(p.plan)) : nullptr;
     if (twq::launch_fused(maps, p, G, static_cast<cudaStream_t>(stream)) != cudaSuccess) return TWQ_ERR_CUDA;
