@@ -172,12 +172,13 @@ decode_dual_linear_kernel(const __grid_constant__ CUtensorMap tmXq, const __grid
     const int lw = warp - nrw;                  // index among the low-rank warps
     const int rank = cs > 1 ? static_cast<int>(cluster_ctarank()) : 0;
     // 8-channel tiles of this CTA: an even split of the n_tiles over the grid
-    const int tile0 = static_cast<int>(static_cast<long long>(blockIdx.x) * p.n_tiles / gridDim.x);
-    const int ntile = static_cast<int>(static_cast<long long>(blockIdx.x + 1) * p.n_tiles / gridDim.x) - tile0;
+    // (32-bit arithmetic: n_tiles * grid < 2^31 for every shape the planner accepts; a 64-bit division is ~100 instructions)
+    const int tile0 = static_cast<int>(blockIdx.x * static_cast<unsigned>(p.n_tiles) / gridDim.x);
+    const int ntile = static_cast<int>((blockIdx.x + 1u) * static_cast<unsigned>(p.n_tiles) / gridDim.x) - tile0;
     // stage-1 K slice of this cluster rank, in 32-wide slabs
     const int units = p.K >> 5;
-    const int u0 = static_cast<int>(static_cast<long long>(units) * rank / cs);
-    const int nu = r > 0 ? static_cast<int>(static_cast<long long>(units) * (rank + 1) / cs) - u0 : 0;
+    const int u0 = static_cast<int>(static_cast<unsigned>(units) * static_cast<unsigned>(rank) / static_cast<unsigned>(cs));
+    const int nu = r > 0 ? static_cast<int>(static_cast<unsigned>(units) * static_cast<unsigned>(rank + 1) / static_cast<unsigned>(cs)) - u0 : 0;
     const int nl1 = (nu + p.sc - 1) / p.sc;                 // stage-1 ring chunks
     const int slab_bytes = r * 64;
     // Residual warps form a (tile group x K part) grid: TG groups of at most kTPW tiles, P = nrw / TG warps per group,
@@ -304,16 +305,21 @@ decode_dual_linear_kernel(const __grid_constant__ CUtensorMap tmXq, const __grid
             const uint16_t* X = static_cast<const uint16_t*>(p.X);
             const int chunks = nu * 4;                           // 16-byte chunks per token row
             const int total = kMp * chunks;
+            // element i = (token i / chunks, chunk i % chunks): one division per thread, then (token, chunk) advance by
+            // the constant (nlr / chunks, nlr % chunks) with a carry
+            int m = chunks > 0 ? lrt / chunks : 0, cq = lrt - m * chunks;
+            const int dm = chunks > 0 ? nlr / chunks : 0, dc = nlr - dm * chunks;
             for (int i0 = lrt; i0 < total; i0 += 4 * nlr) {
                 uint4 v[4];
                 int mm[4], cc[4];
 #pragma unroll
                 for (int q = 0; q < 4; ++q) {
-                    const int i = i0 + q * nlr;
-                    mm[q] = i / chunks; cc[q] = i - mm[q] * chunks;
+                    mm[q] = m; cc[q] = cq;
                     v[q] = make_uint4(0, 0, 0, 0);
-                    if (i < total && mm[q] < p.M)
-                        v[q] = ldg_v4(X + static_cast<size_t>(mm[q]) * p.ldx + u0 * 32 + cc[q] * 8);
+                    if (i0 + q * nlr < total && m < p.M)
+                        v[q] = ldg_v4(X + static_cast<size_t>(m) * p.ldx + u0 * 32 + cq * 8);
+                    m += dm; cq += dc;
+                    if (cq >= chunks) { cq -= chunks; ++m; }
                 }
 #pragma unroll
                 for (int q = 0; q < 4; ++q) {
@@ -327,71 +333,81 @@ decode_dual_linear_kernel(const __grid_constant__ CUtensorMap tmXq, const __grid
         }
         named_bar_sync(1, nlr);
         TWQ_DSTAMP(3);
-        // ---- stage 1: partial H of this CTA's K slice; warp w owns the j tiles w, w + lrw, ...
+        // ---- stage 1: partial H of this CTA's K slice; low-rank warp lw owns the j tiles lw, lw + lrw, ...
+        // The chain is latency-bound and runs one warp per scheduler, so the loop must be tight: the body is instantiated
+        // for NQ = 1 / 2 / 4 / 8 j tiles per warp with no guard inside (a missing j tile repeats the last one and is
+        // dropped at the write-out), fragment addresses are hoisted and advance by constants, all fragments of a slab
+        // are loaded before its MMAs, and the MMAs are interleaved over the j tiles (with per-load address arithmetic
+        // and guards the same loop took 1200 cycles per slab; in-kernel timeline, r02).
         const int njt = r >> 3;
-        float d[kJT][MT][4];
+        const int nq_need = njt > lw ? (njt - lw + lrw - 1) / lrw : 0;          // j tiles of this warp
+        auto stage1 = [&](auto nq_c) {
+            constexpr int NQ = decltype(nq_c)::value;
+            float d[NQ][MT][4];
 #pragma unroll
-        for (int q = 0; q < kJT; ++q)
+            for (int q = 0; q < NQ; ++q)
 #pragma unroll
-            for (int t = 0; t < MT; ++t)
+                for (int t = 0; t < MT; ++t)
 #pragma unroll
-                for (int e = 0; e < 4; ++e) d[q][t][e] = 0.0f;
-        {
-            const uint32_t l1ring = smem_u32(dsm + p.off_l1);
-            const uint32_t xs0 = smem_u32(sXs) + (gid * p.xs_stride + tid4 * 8) * 2;
+                    for (int e = 0; e < 4; ++e) d[q][t][e] = 0.0f;
+            const uint32_t l1lane = smem_u32(dsm + p.off_l1) + gid * 64 + tid4 * 16;
+            uint32_t loff[NQ];
+#pragma unroll
+            for (int q = 0; q < NQ; ++q) loff[q] = static_cast<uint32_t>(min(lw + q * lrw, max(njt - 1, 0))) * 512u;
+            uint32_t xs_a = smem_u32(sXs) + (gid * p.xs_stride + tid4 * 8) * 2;   // advances 64 bytes per slab
+            const uint32_t xrow8 = 8u * p.xs_stride * 2u;
+            const uint32_t chunk_bytes = static_cast<uint32_t>(p.sc) * slab_bytes;
             int slot = 0, lap = 0;
+            uint32_t slot_a = 0;
             TWQ_DCLK(0);
+#pragma unroll 1
             for (int i = 0; i < nl1; ++i) {
                 mbar_wait_a(DBAR(D_L1FULL + slot), lap & 1);
-                if (i < 4) TWQ_DCLK(1 + 2 * i);
-                const uint32_t base = l1ring + slot * (p.sc * slab_bytes) + (gid * 64 + tid4 * 16);
                 const int cnt = min(p.sc, nu - i * p.sc);
-                for (int s = 0; s < cnt; ++s) {
-                    const int us = i * p.sc + s;
-                    // all fragments of the slab first, then the MMAs interleaved over the j tiles: the warp issues in
-                    // order, so a load placed between two dependent MMAs would expose its latency and theirs in turn
+                uint32_t la = l1lane + slot_a;
+#pragma unroll 2
+                for (int sl = 0; sl < cnt; ++sl, la += slab_bytes, xs_a += 64) {
                     uint4 a[MT][2];
-                    uint4 l[kJT];
+                    uint4 l[NQ];
 #pragma unroll
                     for (int t = 0; t < MT; ++t) {
-                        a[t][0] = lds_v4(xs0 + ((t * 16) * p.xs_stride + us * 32) * 2);
-                        a[t][1] = lds_v4(xs0 + ((t * 16 + 8) * p.xs_stride + us * 32) * 2);
+                        a[t][0] = lds_v4(xs_a + t * 2 * xrow8);
+                        a[t][1] = lds_v4(xs_a + t * 2 * xrow8 + xrow8);
                     }
 #pragma unroll
-                    for (int q = 0; q < kJT; ++q)
-                        if (lw + q * lrw < njt) l[q] = lds_v4(base + (s * r + (lw + q * lrw) * 8) * 64);
+                    for (int q = 0; q < NQ; ++q) l[q] = lds_v4(la + loff[q]);
 #pragma unroll
-                    for (int q = 0; q < kJT; ++q)
-                        if (lw + q * lrw < njt) {              // warp-uniform
+                    for (int q = 0; q < NQ; ++q)
 #pragma unroll
-                            for (int t = 0; t < MT; ++t) hmma_16816(d[q][t], a[t][0].x, a[t][1].x, a[t][0].y, a[t][1].y, l[q].x, l[q].y);
-                        }
+                        for (int t = 0; t < MT; ++t) hmma_16816(d[q][t], a[t][0].x, a[t][1].x, a[t][0].y, a[t][1].y, l[q].x, l[q].y);
 #pragma unroll
-                    for (int q = 0; q < kJT; ++q)
-                        if (lw + q * lrw < njt) {
+                    for (int q = 0; q < NQ; ++q)
 #pragma unroll
-                            for (int t = 0; t < MT; ++t) hmma_16816(d[q][t], a[t][0].z, a[t][1].z, a[t][0].w, a[t][1].w, l[q].z, l[q].w);
-                        }
+                        for (int t = 0; t < MT; ++t) hmma_16816(d[q][t], a[t][0].z, a[t][1].z, a[t][0].w, a[t][1].w, l[q].z, l[q].w);
                 }
                 __syncwarp();
-                if (i < 4) TWQ_DCLK(2 + 2 * i);
                 if (lane == 0) mbar_arrive_a(DBAR(D_L1EMPTY + slot));
-                if (++slot == p.l1_slots) { slot = 0; ++lap; }
+                slot_a += chunk_bytes;
+                if (++slot == p.l1_slots) { slot = 0; slot_a = 0; ++lap; }
             }
-        }
-        TWQ_DSTAMP(4);
+            TWQ_DSTAMP(4);
 #pragma unroll
-        for (int q = 0; q < kJT; ++q) {
-            const int jt = lw + q * lrw;
-            if (jt < njt) {
-                const int j = jt * 8 + tid4 * 2;
+            for (int q = 0; q < NQ; ++q) {
+                const int jt = lw + q * lrw;
+                if (jt < njt) {
+                    const int j = jt * 8 + tid4 * 2;
 #pragma unroll
-                for (int t = 0; t < MT; ++t) {
-                    *reinterpret_cast<float2*>(sHpart + (t * 16 + gid) * r + j) = make_float2(d[q][t][0], d[q][t][1]);
-                    *reinterpret_cast<float2*>(sHpart + (t * 16 + gid + 8) * r + j) = make_float2(d[q][t][2], d[q][t][3]);
+                    for (int t = 0; t < MT; ++t) {
+                        *reinterpret_cast<float2*>(sHpart + (t * 16 + gid) * r + j) = make_float2(d[q][t][0], d[q][t][1]);
+                        *reinterpret_cast<float2*>(sHpart + (t * 16 + gid + 8) * r + j) = make_float2(d[q][t][2], d[q][t][3]);
+                    }
                 }
             }
-        }
+        };
+        if (nq_need <= 1) stage1(std::integral_constant<int, 1>{});
+        else if (nq_need == 2) stage1(std::integral_constant<int, 2>{});
+        else if (nq_need <= 4) stage1(std::integral_constant<int, 4>{});
+        else stage1(std::integral_constant<int, kJT>{});
         // stage-2 operand of this warp's first tile (L2T rows, L2-resident by now), ahead of the exchange
         constexpr int kL2 = 8;                                   // 32-wide j steps (r <= 256)
         uint4 l2v[kL2];
@@ -494,9 +510,29 @@ decode_dual_linear_kernel(const __grid_constant__ CUtensorMap tmXq, const __grid
         named_bar_sync(2, nrw * 32);
         TWQ_DSTAMP(3);
         if (ntile > 0) {
+            // The loop is issue-bound (ncu r02a: 38 K warp instructions per CTA, most of them address arithmetic), so
+            // everything that does not change per K-group is hoisted: per-tile offsets are registers, the four running
+            // addresses advance by constants.
             const uint32_t ring = smem_u32(dsm + p.off_ring);
-            const uint32_t sw_a = smem_u32(dsm + p.off_sw) + tid4 * 4;
+            const uint32_t tstride = static_cast<uint32_t>(p.gc) * kBlk;          // bytes between tiles inside a slot
+            const uint32_t lane_w = ring + t_lo * tstride + gid * (G / 2) + tid4 * (kW * 4);
+            const uint32_t lane_x = ring + p.xq_off + (gid * p.gc) * (G / 2) + tid4 * (kW * 4);
+            const uint32_t x8 = 8u * p.gc * (G / 2);                              // token gid -> gid + 8 inside the Xq box
+            const uint32_t sw_a = smem_u32(dsm + p.off_sw) + tid4 * 4 + static_cast<uint32_t>(t_lo) * ng * 16;
             const uint32_t sx_a = smem_u32(sSx) + gid * 4;
+            // The warp's tiles are worked in batches of kTB interleaved MMA chains; with more than kTB tiles they are split
+            // evenly over two batches (4 -> 2 + 2, 5 -> 3 + 2): accumulator slot i holds tile tix(i); empty slots are skipped.
+            const int nb0 = ntw > kTB ? (ntw + 1) / 2 : ntw;                      // tiles of the first batch
+            auto tix = [&](int i) { return i < kTB ? i : nb0 + (i - kTB); };      // accumulator slot -> tile of the warp
+            auto slot_on = [&](int i) { return i < kTB ? i < nb0 : nb0 + (i - kTB) < ntw; };
+            uint32_t toff[kTPW], swoff[kTPW];
+#pragma unroll
+            for (int i = 0; i < kTPW; ++i) {
+                const int ii = slot_on(i) ? tix(i) : 0;
+                toff[i] = ii * tstride;
+                swoff[i] = static_cast<uint32_t>(ii) * ng * 16;
+            }
+            const uint32_t step_w = P * kBlk, step_x = P * (G / 2), step_sx = P * kMp * 4, step_sw = P * 16;
             float acc[kTPW][MT][4];
 #pragma unroll
             for (int i = 0; i < kTPW; ++i)
@@ -505,29 +541,31 @@ decode_dual_linear_kernel(const __grid_constant__ CUtensorMap tmXq, const __grid
 #pragma unroll
                     for (int e = 0; e < 4; ++e) acc[i][t][e] = 0.0f;
             int slot = 0, lap = 0;
+            uint32_t slot_a = 0;                      // slot * slot_bytes
+            int gl = part;                            // next K-group of this warp, relative to the current chunk
+            int g = part;                             // the same, absolute
 #pragma unroll 1
             for (int c = 0; c < p.nchunks; ++c) {
                 mbar_wait_a(DBAR(D_FULL + slot), lap & 1);
                 if (c < 6) TWQ_DSTAMP(4 + 2 * c);
+                const int gcnt = min(p.gc, ng - c * p.gc);
                 if (ntw > 0) {
-                    const int g0 = c * p.gc, gcnt = min(p.gc, ng - g0);
-                    const uint32_t wbase = ring + slot * p.slot_bytes + t_lo * (p.gc * kBlk) + gid * (G / 2) + tid4 * (kW * 4);
-                    const uint32_t xbase = ring + slot * p.slot_bytes + p.xq_off + (gid * p.gc) * (G / 2) + tid4 * (kW * 4);
-                    int gl = part - g0 % P;
-                    if (gl < 0) gl += P;
+                    uint32_t wa = lane_w + slot_a + gl * kBlk;
+                    uint32_t xa = lane_x + slot_a + gl * (G / 2);
+                    uint32_t sxp = sx_a + g * (kMp * 4);
+                    uint32_t swp = sw_a + g * 16;
 #pragma unroll 1
-                    for (; gl < gcnt; gl += P) {
-                        const int g = g0 + gl;
+                    for (; gl < gcnt; gl += P, g += P, wa += step_w, xa += step_x, sxp += step_sx, swp += step_sw) {
                         // activation fragments of the K-group, expanded once for all tiles of the warp
                         uint32_t ax[MT][kW][4];
                         float sxa[MT][2];
 #pragma unroll
                         for (int mt = 0; mt < MT; ++mt) {
                             uint32_t x0[kW], x1[kW];
-                            lds_words<kW>(x0, xbase + ((mt * 16) * p.gc + gl) * (G / 2));
-                            lds_words<kW>(x1, xbase + ((mt * 16 + 8) * p.gc + gl) * (G / 2));
-                            sxa[mt][0] = __uint_as_float(lds_u32(sx_a + (g * kMp + mt * 16) * 4));
-                            sxa[mt][1] = __uint_as_float(lds_u32(sx_a + (g * kMp + mt * 16 + 8) * 4));
+                            lds_words<kW>(x0, xa + mt * 2 * x8);
+                            lds_words<kW>(x1, xa + mt * 2 * x8 + x8);
+                            sxa[mt][0] = __uint_as_float(lds_u32(sxp + mt * 64));
+                            sxa[mt][1] = __uint_as_float(lds_u32(sxp + mt * 64 + 32));
 #pragma unroll
                             for (int w = 0; w < kW; ++w) {
                                 ax[mt][w][0] = d_lo16(x0[w]); ax[mt][w][1] = d_lo16(x1[w]);
@@ -536,16 +574,17 @@ decode_dual_linear_kernel(const __grid_constant__ CUtensorMap tmXq, const __grid
                         }
 #pragma unroll
                         for (int ib = 0; ib < kTPW; ib += kTB) {
-                            if (ib < ntw) {                      // warp-uniform
+                            if (slot_on(ib)) {                   // warp-uniform
                                 // up to kTB tiles at a time: loads first, then their MMA chains interleaved
                                 uint32_t wt[kTB][kW];
                                 uint32_t swh[kTB];
                                 int dd[kTB][MT][4];
 #pragma unroll
                                 for (int b = 0; b < kTB; ++b) {
-                                    const int i = min(ib + b, ntw - 1);   // a missing tile repeats the last one (its result is dropped)
-                                    lds_words<kW>(wt[b], wbase + i * (p.gc * kBlk) + gl * kBlk);
-                                    swh[b] = lds_u32(sw_a + ((t_lo + i) * ng + g) * 16);
+                                    if (b == 0 || slot_on(ib + b)) {
+                                        lds_words<kW>(wt[b], wa + toff[ib + b]);
+                                        swh[b] = lds_u32(swp + swoff[ib + b]);
+                                    }
 #pragma unroll
                                     for (int mt = 0; mt < MT; ++mt)
 #pragma unroll
@@ -555,27 +594,33 @@ decode_dual_linear_kernel(const __grid_constant__ CUtensorMap tmXq, const __grid
                                 for (int w = 0; w < kW; ++w) {   // one K-step of 32 codes per packed word
 #pragma unroll
                                     for (int b = 0; b < kTB; ++b) {
-                                        const uint32_t b0 = d_lo16(wt[b][w]), b1 = d_hi16(wt[b][w]);
+                                        if (b == 0 || slot_on(ib + b)) {
+                                            const uint32_t b0 = d_lo16(wt[b][w]), b1 = d_hi16(wt[b][w]);
 #pragma unroll
-                                        for (int mt = 0; mt < MT; ++mt)
-                                            imma_16832(dd[b][mt], ax[mt][w][0], ax[mt][w][1], ax[mt][w][2], ax[mt][w][3], b0, b1);
+                                            for (int mt = 0; mt < MT; ++mt)
+                                                imma_16832(dd[b][mt], ax[mt][w][0], ax[mt][w][1], ax[mt][w][2], ax[mt][w][3], b0, b1);
+                                        }
                                     }
                                 }
-                                // dd = 256 * P (exact); fold both scales in FP32 (sx already carries 2^-8)
+                                // dd = 256 * P (exact); fold both scales in FP32 (sx already carries 2^-8): two packed
+                                // f32x2 operations per token row instead of four scalar ones
 #pragma unroll
                                 for (int b = 0; b < kTB; ++b) {
-                                    if (ib + b < ntw) {          // warp-uniform
+                                    if (slot_on(ib + b)) {       // warp-uniform
                                         const float2 sw2 = __half22float2(*reinterpret_cast<const __half2*>(&swh[b]));
+                                        const uint64_t swp2 = pack_f2(sw2.x, sw2.y);
 #pragma unroll
                                         for (int mt = 0; mt < MT; ++mt) {
                                             float (&a)[4] = acc[ib + b][mt];
-                                            a[0] = fmaf(__fmul_rn(static_cast<float>(dd[b][mt][0]), sw2.x), sxa[mt][0], a[0]);
-                                            a[1] = fmaf(__fmul_rn(static_cast<float>(dd[b][mt][1]), sw2.y), sxa[mt][0], a[1]);
-                                            a[2] = fmaf(__fmul_rn(static_cast<float>(dd[b][mt][2]), sw2.x), sxa[mt][1], a[2]);
-                                            a[3] = fmaf(__fmul_rn(static_cast<float>(dd[b][mt][3]), sw2.y), sxa[mt][1], a[3]);
+                                            const uint64_t t01 = fma2(pack_f2(static_cast<float>(dd[b][mt][0]), static_cast<float>(dd[b][mt][1])), swp2, 0ull);
+                                            const uint64_t t23 = fma2(pack_f2(static_cast<float>(dd[b][mt][2]), static_cast<float>(dd[b][mt][3])), swp2, 0ull);
+                                            const uint64_t a01 = fma2(t01, pack_f2(sxa[mt][0], sxa[mt][0]), pack_f2(a[0], a[1]));
+                                            const uint64_t a23 = fma2(t23, pack_f2(sxa[mt][1], sxa[mt][1]), pack_f2(a[2], a[3]));
+                                            unpack_f2(a01, a[0], a[1]);
+                                            unpack_f2(a23, a[2], a[3]);
                                             if (kDbg) {
                                                 if (p.dbgP != nullptr) {
-                                                    const int n = (tile0 + t_lo + ib + b) * 8 + tid4 * 2;
+                                                    const int n = (tile0 + t_lo + tix(ib + b)) * 8 + tid4 * 2;
                                                     const int m0 = mt * 16 + gid;
                                                     if (m0 < p.M) {
                                                         p.dbgP[(static_cast<size_t>(m0) * ng + g) * p.N + n] = dd[b][mt][0] >> 8;
@@ -594,18 +639,20 @@ decode_dual_linear_kernel(const __grid_constant__ CUtensorMap tmXq, const __grid
                         }
                     }
                 }
+                gl -= gcnt;                           // the warp's next group, relative to the next chunk
                 __syncwarp();
                 if (c < 6) TWQ_DSTAMP(5 + 2 * c);
                 if (lane == 0) mbar_arrive_a(DBAR(D_EMPTY + slot));
-                if (++slot == p.nslots) { slot = 0; ++lap; }
+                slot_a += p.slot_bytes;
+                if (++slot == p.nslots) { slot = 0; slot_a = 0; ++lap; }
             }
             // this warp's partial tiles: [tile * P + part][token][8 channels], parked in the ring, which every residual
             // warp has finished reading (all chunks have landed and been consumed)
             named_bar_sync(2, nrw * 32);
 #pragma unroll
             for (int i = 0; i < kTPW; ++i) {
-                if (i < ntw) {
-                    float* dst = sRes + static_cast<size_t>((t_lo + i) * P + part) * kMp * 8 + tid4 * 2;
+                if (slot_on(i)) {
+                    float* dst = sRes + static_cast<size_t>((t_lo + tix(i)) * P + part) * kMp * 8 + tid4 * 2;
 #pragma unroll
                     for (int mt = 0; mt < MT; ++mt) {
                         *reinterpret_cast<float2*>(dst + (mt * 16 + gid) * 8) = make_float2(acc[i][mt][0], acc[i][mt][1]);
@@ -621,17 +668,47 @@ decode_dual_linear_kernel(const __grid_constant__ CUtensorMap tmXq, const __grid
     __syncthreads();
     TWQ_DSTAMP(28);
     if (warp < kDecWarps) {
-        const int ncl = ntile * 8;
-        for (int i = threadIdx.x; i < ncl * p.M; i += kDecWarps * 32) {
-            const int m = i / ncl, nl = i - m * ncl;
-            const int t = nl >> 3, ch = nl & 7;
-            float y = 0.0f;
-            for (int pp = 0; pp < P; ++pp) y += sRes[(static_cast<size_t>(t * P + pp) * kMp + m) * 8 + ch];
-            if (r > 0) y += sYlr[m * nloc + nl];
+        // a thread owns four consecutive channels of one token: the P partial tiles are read as 16-byte vectors (all
+        // loads independent), summed in part order, Ylr added, one rounding, one store
+        const int nq4 = ntile * 2;                               // 4-channel quads of this CTA
+        for (int i = threadIdx.x; i < nq4 * p.M; i += kDecWarps * 32) {
+            const int m = i / nq4, q4 = i - m * nq4;
+            const int t = q4 >> 1, ch = (q4 & 1) * 4;
+            const float* src = sRes + (static_cast<size_t>(t * P) * kMp + m) * 8 + ch;
+            float4 y = make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll 4
+            for (int pp = 0; pp < P; ++pp) {
+                const float4 v = *reinterpret_cast<const float4*>(src + static_cast<size_t>(pp) * kMp * 8);
+                y.x += v.x; y.y += v.y; y.z += v.z; y.w += v.w;
+            }
+            const int nl = q4 * 4;
+            if (r > 0) {
+                const float4 v = *reinterpret_cast<const float4*>(sYlr + m * nloc + nl);
+                y.x += v.x; y.y += v.y; y.z += v.z; y.w += v.w;
+            }
             const size_t o = static_cast<size_t>(m) * p.ldy + tile0 * 8 + nl;
-            if (p.ydt == 0) static_cast<__nv_bfloat16*>(p.Y)[o] = __float2bfloat16_rn(y);
-            else if (p.ydt == 1) static_cast<__half*>(p.Y)[o] = __float2half_rn(y);
-            else static_cast<float*>(p.Y)[o] = y;
+            const float yv[4] = {y.x, y.y, y.z, y.w};
+            if (p.ydt == 2) {
+                if ((p.ldy & 3) == 0) *reinterpret_cast<float4*>(static_cast<float*>(p.Y) + o) = y;
+                else
+#pragma unroll
+                    for (int e = 0; e < 4; ++e) static_cast<float*>(p.Y)[o + e] = yv[e];
+            } else {
+                uint2 w;
+                if (p.ydt == 0) {
+                    const __nv_bfloat162 a = __floats2bfloat162_rn(y.x, y.y), c = __floats2bfloat162_rn(y.z, y.w);
+                    w = make_uint2(*reinterpret_cast<const uint32_t*>(&a), *reinterpret_cast<const uint32_t*>(&c));
+                } else {
+                    const __half2 a = __floats2half2_rn(y.x, y.y), c = __floats2half2_rn(y.z, y.w);
+                    w = make_uint2(*reinterpret_cast<const uint32_t*>(&a), *reinterpret_cast<const uint32_t*>(&c));
+                }
+                if ((p.ldy & 3) == 0) *reinterpret_cast<uint2*>(static_cast<uint8_t*>(p.Y) + o * 2) = w;
+                else {
+                    uint16_t* yp = static_cast<uint16_t*>(p.Y) + o;
+                    yp[0] = static_cast<uint16_t>(w.x); yp[1] = static_cast<uint16_t>(w.x >> 16);
+                    yp[2] = static_cast<uint16_t>(w.y); yp[3] = static_cast<uint16_t>(w.y >> 16);
+                }
+            }
         }
     }
     TWQ_DSTAMP(29);
