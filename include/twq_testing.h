@@ -40,6 +40,11 @@ enum {
  * Writes up to n_out ints; returns the number of fields, or -1 for an invalid shape. */
 int twq_testing_describe_plan(int M, int N, int K, int r, int G, int* out, int n_out);
 
+/* Measured dense int8 tensor rate in TOP/s: an MMA-only loop of tcgen05.mma kind::i8 (128 x 128 x 32) on every SM
+ * (csrc/peak_i8.cu), best of `reps` launches of iters x 8 MMAs per SM.  SYNCHRONISES the stream.  Negative on failure.
+ * bench.py prints it next to the 2 x BF16 figure that the prefill roofline uses. */
+float twq_testing_measure_i8_tops(int iters, int reps, void* stream);
+
 /* In-kernel timeline (csrc/trace.cuh).  Hands a device buffer of at least 16384 unsigned 64-bit words to the library;
  * NULL switches the timeline off.  Returns 1 if this library was built with the timeline compiled in
  * (`python -m paper_2606_01556_b200._build --trace` -> libtwq_trace.so), 0 if not (the product library: the call has

@@ -18,7 +18,7 @@ EXPORTS = ("twq_status_string", "twq_packed_bytes", "twq_pack_weights", "twq_qua
 
 
 TESTING_EXPORTS = ("twq_testing_set_plan_flags", "twq_testing_get_plan_flags", "twq_testing_describe_plan",
-                   "twq_testing_set_trace_buffer")
+                   "twq_testing_set_trace_buffer", "twq_testing_measure_i8_tops")
 # include/twq_testing.h: planner overrides for tests
 PLAN_NO_SPLIT, PLAN_NO_PAIR, PLAN_NO_YSTAGE, PLAN_NO_ALIAS2, PLAN_NO_DECODE = 1, 2, 4, 8, 16
 _PLAN_FIELDS = ("kernel", "cluster", "grid", "tile_tokens", "splits", "pair", "smem", "ring", "chunks")
@@ -80,6 +80,8 @@ def load_library(build_if_missing: bool = True):
     lib.twq_testing_describe_plan.argtypes = [i, i, i, i, i, ctypes.POINTER(ctypes.c_int), i]
     lib.twq_testing_set_trace_buffer.restype = i
     lib.twq_testing_set_trace_buffer.argtypes = [vp]
+    lib.twq_testing_measure_i8_tops.restype = ctypes.c_float
+    lib.twq_testing_measure_i8_tops.argtypes = [i, i, vp]
     _lib = lib
     return lib
 
@@ -118,6 +120,11 @@ def testing_set_plan_flags(flags: int) -> None:
 def testing_set_trace_buffer(buf) -> bool:
     """csrc/trace.cuh: hand a CUDA uint64 tensor (>= 16384 words) or None; True if the timeline is compiled in."""
     return bool(load_library().twq_testing_set_trace_buffer(_ptr(buf)))
+
+
+def testing_measure_i8_tops(iters: int = 4096, reps: int = 5) -> float:
+    """csrc/peak_i8.cu: measured tcgen05 kind::i8 rate in TOP/s (synchronises)."""
+    return float(load_library().twq_testing_measure_i8_tops(iters, reps, _stream()))
 
 
 def testing_describe_plan(M: int, N: int, K: int, r: int, G: int) -> dict:

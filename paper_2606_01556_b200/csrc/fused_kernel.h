@@ -87,6 +87,7 @@ enum : unsigned {
 };
 unsigned plan_flags();
 void set_plan_flags(unsigned f);
+float measure_i8_tops(int iters, int reps, cudaStream_t stream);   // peak_i8.cu (bench measurement aid)
 unsigned long long* trace_buffer();   // set by twq_testing_set_trace_buffer; only read by -DTWQ_TRACE builds
 
 // Fills `plan` for a shape; returns false if the shape cannot be planned (never for valid ABI shapes).

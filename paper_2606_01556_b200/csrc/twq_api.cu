@@ -218,6 +218,11 @@ int twq_testing_set_trace_buffer(void* dev_buf) {
 #endif
 }
 
+float twq_testing_measure_i8_tops(int iters, int reps, void* stream) {
+    if (iters < 1 || reps < 1 || !device_is_sm100()) return -1.0f;
+    return twq::measure_i8_tops(iters, reps, static_cast<cudaStream_t>(stream));
+}
+
 int twq_testing_describe_plan(int M, int N, int K, int r, int G, int* out, int n_out) {
     if (!shape_ok(M, N, K, r, G) || !out) return -1;
     const CallPlan* cp = get_plan(M, N, K, r, G);

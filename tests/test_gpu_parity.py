@@ -53,25 +53,29 @@ def _bits(t):
 
 
 def _check_layer(twq, oracle, L, rows=None, check_P=True):
-    """Full pipeline on L; compare every output (or the given token rows) with the oracle."""
+    """Full pipeline on L; compare every output (or the given token rows) with the oracle.  The integer accumulators are
+    dumped for the whole call (dbg_P [M, ng, N] lives in HBM only) and the sampled rows are gathered on the device."""
     import torch
     X, packed, tinv = _upload(twq, L)
     Xq, sx = twq.quantize_act(X, L.G, tinv)
     dbg = torch.zeros((L.M, L.ng, L.N), dtype=torch.int32, device="cuda") if check_P else None
-    Y32 = twq.dual_linear(X, Xq, sx, packed, twq.OUT_FP32, dbg_P=dbg)
-    Y16 = twq.dual_linear(X, Xq, sx, packed, twq.OUT_BF16)
+    need = twq.workspace_bytes(L.M, L.N, L.K, L.r, L.G)
+    ws = torch.zeros(need, dtype=torch.uint8, device="cuda") if need else None
+    Y32 = twq.dual_linear(X, Xq, sx, packed, twq.OUT_FP32, dbg_P=dbg, ws=ws)
+    Y16 = twq.dual_linear(X, Xq, sx, packed, twq.OUT_BF16, ws=ws)
     torch.cuda.synchronize()
     ref = oracle.forward(L.X, L.Rq, L.sw, L.L1 if L.r else None, L.L2 if L.r else None, L.G, tinv=L.tinv,
                          rows=rows, want_P=check_P)
     assert (Xq.cpu().numpy() == ref["Xq"]).all(), "codes"
     assert (sx.cpu().numpy() == ref["sx"]).all(), "scales"
-    sel = slice(None) if rows is None else rows
+    sel = slice(None) if rows is None else torch.tensor(rows, device="cuda")
     if check_P:
-        assert (dbg.cpu().numpy()[sel].astype(np.int64) == ref["P"]).all(), "integer accumulators"
-    y = Y32.cpu().numpy().astype(np.float64)[sel]
+        assert (dbg[sel].cpu().numpy().astype(np.int64) == ref["P"]).all(), "integer accumulators"
+        del dbg
+    y = Y32[sel].cpu().numpy().astype(np.float64)
     err = np.abs(y - ref["Y"]).max() / np.abs(ref["Y"]).max()
     assert err <= TOL, err
-    assert (_bits(Y16) == _bits(Y32.to(torch.bfloat16))).all(), "BF16 != rne(Y32)"
+    assert torch.equal(Y16.view(torch.int16), Y32.to(torch.bfloat16).view(torch.int16)), "BF16 != rne(Y32)"
     return err
 
 
@@ -351,7 +355,7 @@ def _sample_rows(M, n):
     return sorted(set(np.linspace(0, M - 1, n).astype(int).tolist()))
 
 
-@pytest.mark.parametrize("which,r", [("gate_up", 128), ("down", 128), ("gate_up", 256)])
+@pytest.mark.parametrize("which,r", [("gate_up", 128), ("down", 128), ("gate_up", 256), ("down", 256)])
 def test_config3_mlp_prefill_sampled(twq, oracle, which, r):
     """Full size, the launch configuration bench.py times; 64 token rows (all N, all groups) are compared."""
     L = gen.config3_mlp(which, M=2048, r=r)
@@ -370,20 +374,26 @@ def test_config3_every_row_of_one_ntile(twq, oracle):
     assert np.abs(Y32[:, n0:n1] - ref).max() / np.abs(ref).max() <= TOL
 
 
-@pytest.mark.parametrize("which,M,nrows", [("attn", 64, None), ("gate_up", 1, None), ("down", 1, None),
-                                           ("attn", 4096, 24)])
+@pytest.mark.parametrize("which,M,nrows", [
+    ("attn", 64, None), ("gate_up", 1, None), ("down", 1, None),
+    ("gate_up", 64, 32), ("down", 64, 16),                       # M = 64 on the wide and the deep layer
+    ("attn", 4096, 24), ("gate_up", 4096, 24), ("down", 4096, 16),   # the largest M of configs[3], every layer
+])
 def test_config4_qwen(twq, oracle, which, M, nrows):
+    """configs[3] (Qwen3-32B shapes, r = 256) at M in {1, 64, 4096}: full size, the launch configuration bench.py
+    times; sampled token rows x all N x all groups, INCLUDING the integer accumulators."""
     L = gen.config4_qwen(which, M)
-    _check_layer(twq, oracle, L, rows=None if nrows is None else _sample_rows(M, nrows), check_P=(M <= 64))
+    _check_layer(twq, oracle, L, rows=None if nrows is None else _sample_rows(M, nrows))
 
 
-@pytest.mark.parametrize("which,M", [("q", 1), ("k", 8), ("down", 16), ("gate_up", 2)])
-def test_config5_llama70b(twq, oracle, which, M):
-    _check_layer(twq, oracle, gen.config5_llama70b(which, M), check_P=(which != "gate_up"))
-
-
-def test_config5_llama70b_largest_prefill_sampled(twq, oracle):
-    """configs[4] at its largest layer and a prefill batch: gate/up K = 8192, N = 28672, r = 256, M = 2048 (the
-    rank-256 buffers force the 64-token tile); 24 token rows x all N are compared, without the P dump (60 GB)."""
-    L = gen.config5_llama70b("gate_up", 2048)
-    _check_layer(twq, oracle, L, rows=_sample_rows(2048, 24), check_P=False)
+@pytest.mark.parametrize("which,M,nrows", [
+    ("q", 1, None), ("k", 8, None), ("down", 16, None), ("gate_up", 2, None), ("o", 4, None), ("v", 16, None),
+    ("v", 32, None),                                             # M = 32: two token tiles of the small-batch kernel
+    ("o", 2048, 24), ("down", 2048, 16), ("gate_up", 2048, 24),  # prefill on the square, the deep and the wide layer
+    ("q", 8192, 24), ("gate_up", 8192, 16),                      # the top of the "M = 1..8192" sweep
+])
+def test_config5_llama70b(twq, oracle, which, M, nrows):
+    """configs[4] (LLaMA3-70B decoder-block linear set, r = 256) from M = 1 to M = 8192, full size; sampled token
+    rows x all N x all groups for the prefill batches, INCLUDING the integer accumulators."""
+    L = gen.config5_llama70b(which, M)
+    _check_layer(twq, oracle, L, rows=None if nrows is None else _sample_rows(M, nrows))
