@@ -67,6 +67,14 @@ def load_peaks():
     return dict(hbm_gbs=6650.0, bf16_tflops=1590.0, bf16_tflops_sustained=1400.0, source="fallback")
 
 
+def config_for(name):
+    """The `config` object of the JSON line: identical for the GPU arm and the reference (oracle) arm."""
+    return dict(workload=name, desc=WORKLOADS[name][2],
+                l2="inputs larger than L2: weights and activations rotate through copies, one lap >= 2x the 126 MB L2",
+                launch="CUDA graph of K steps; step = twq_quantize_act + twq_dual_linear",
+                multi_gpu="replicas only")
+
+
 def make_layer(name):
     fn, kw, _ = WORKLOADS[name]
     return getattr(gen, fn)(**kw)
@@ -158,8 +166,9 @@ class GpuLayer:
         self.step(i)
         self.Yh.copy_(self.Y[c], non_blocking=True)
 
-    def time_graph(self, steps, warmup, quant=True, dual=True):
-        """Device time per step of a CUDA graph holding `steps` consecutive steps (no host launch gaps)."""
+    def time_graph(self, steps, warmup, quant=True, dual=True, replays=20):
+        """Device time per step of a CUDA graph holding `steps` consecutive steps (no host launch gaps), over
+        `replays` timed replays of the graph: returns (median, min) in us per step (SURVEY.md 8d protocol)."""
         torch = self.torch
         s = torch.cuda.Stream()
         s.wait_stream(torch.cuda.current_stream())
@@ -173,13 +182,31 @@ class GpuLayer:
                     self.step(i, quant, dual)
             g.replay()                                            # one untimed replay (graph upload)
             s.synchronize()
-            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            e0.record(s)
-            g.replay()
-            e1.record(s)
+            ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(replays)]
+            for e0, e1 in ev:
+                e0.record(s)
+                g.replay()
+                e1.record(s)
             s.synchronize()
         torch.cuda.current_stream().wait_stream(s)
-        return e0.elapsed_time(e1) * 1e3 / steps                  # us per step
+        us = sorted(e0.elapsed_time(e1) * 1e3 / steps for e0, e1 in ev)
+        return float(np.median(us)), us[0]                        # us per step: median, min
+
+    def time_host(self, calls=2000):
+        """Host time of one twq_dual_linear call through the binding (plan + descriptor caches warm), no device
+        synchronisation inside the loop; the queue is drained every 100 calls so that it never back-pressures."""
+        torch = self.torch
+        for i in range(20):
+            self.step(i, False, True)
+        torch.cuda.synchronize()
+        t = 0.0
+        for base in range(0, calls, 100):
+            t0 = time.perf_counter()
+            for i in range(base, base + 100):
+                self.step(i, False, True)
+            t += time.perf_counter() - t0
+            torch.cuda.synchronize()
+        return t / calls * 1e6
 
     def time_e2e(self, steps, warmup):
         torch = self.torch
@@ -195,7 +222,7 @@ class GpuLayer:
         return e0.elapsed_time(e1) * 1e3 / steps
 
 
-def roofline_for(L, twq, us_dual, peaks, traffic=None):
+def roofline_for(L, twq, us_dual, peaks, traffic=None, traffic_src=None):
     by = twq.algorithmic_bytes(L.M, L.N, L.K, L.r, L.G)
     ops_i8, fl_lr = twq.flops(L.M, L.N, L.K, L.r)
     p_i8 = 2.0 * peaks["bf16_tflops"] * 1e12        # int8 dense = 2x bf16 (guide's nominal ratio) x measured bf16
@@ -206,47 +233,51 @@ def roofline_for(L, twq, us_dual, peaks, traffic=None):
     if t_hbm >= t_tensor:
         ach = by / t / 1e9
         return dict(bound="hbm", achieved=round(ach, 1), peak=peaks["hbm_gbs"], unit="GB/s",
-                    frac=round(ach / peaks["hbm_gbs"], 4), traffic=traffic, peak_source=peaks["source"],
-                    kernel=kernel_name(L), us=round(us_dual, 3), algorithmic_bytes=by)
+                    frac=round(ach / peaks["hbm_gbs"], 4), traffic=traffic, traffic_source=traffic_src,
+                    peak_source=peaks["source"], kernel=kernel_name(L), us=round(us_dual, 3), algorithmic_bytes=by)
     eq_ops = ops_i8 + 2.0 * fl_lr                    # low-rank flops run at half the int8 rate
     ach = eq_ops / t / 1e12
     return dict(bound="tensor", achieved=round(ach, 1), peak=round(p_i8 / 1e12, 1), unit="TFLOP/s",
-                frac=round(ach / (p_i8 / 1e12), 4), traffic=traffic, peak_source=peaks["source"] + " bf16 burst x2 (int8)",
+                frac=round(ach / (p_i8 / 1e12), 4), traffic=traffic, traffic_source=traffic_src,
+                peak_source=peaks["source"] + " bf16 burst x2 (int8)",
                 kernel=kernel_name(L), us=round(us_dual, 3), int8_equivalent_ops=eq_ops)
 
 
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dual-linear kernel, from the ncu --set full
-# captures summarised under profiles/ (r01c_full_*.txt); None where no capture exists.
-TRAFFIC_BYTES = {
-    "c2_qproj_m1": 11086848,          # profiles/r01c_full_decode_c2_qproj_m1.txt
-    "c2_qproj_m16": 11246080,         # profiles/r01c_full_decode_c2_qproj_m16.txt
-    "c3_gateup_m2048": 111107840,     # profiles/r01d_full_fused_c3_gateup_m2048.txt
-}
-
-
 def load_traffic(name):
-    return TRAFFIC_BYTES.get(name)
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the dual-linear kernel, from the `ncu --set full`
+    captures summarised under profiles/ (profiles/traffic.json names capture file and commit per workload)."""
+    path = os.path.join(ROOT, "profiles", "traffic.json")
+    if not os.path.exists(path):
+        return None, None
+    ent = json.load(open(path)).get(name)
+    if not ent:
+        return None, None
+    return int(ent["dram_bytes"]), "%s @ %s" % (ent["capture"], ent["commit"])
 
 
 def kernel_name(L):
-    return "decode_dual_linear_kernel" if L.M <= 16 else "fused_dual_linear_kernel"
+    return "decode_dual_linear_kernel" if L.M <= 32 else "fused_dual_linear_kernel"
 
 
 def measure_workload(name, twq, torch, steps, warmup, peaks, with_e2e=False, with_cublas=False):
     L = make_layer(name)
     gl = GpuLayer(L, twq, torch)
-    us_step = gl.time_graph(steps, warmup, True, True)
-    us_dual = gl.time_graph(steps, warmup, False, True)
-    us_quant = gl.time_graph(steps, warmup, True, False)
+    us_step, us_step_min = gl.time_graph(steps, warmup, True, True)
+    us_dual, us_dual_min = gl.time_graph(steps, warmup, False, True)
+    us_quant, us_quant_min = gl.time_graph(steps, warmup, True, False)
     ops_i8, fl_lr = twq.flops(L.M, L.N, L.K, L.r)
+    traffic, traffic_src = load_traffic(name)
     out = dict(workload=name, M=L.M, N=L.N, K=L.K, r=L.r, G=L.G, us_step=round(us_step, 3),
                us_dual_linear=round(us_dual, 3), us_quantize_act=round(us_quant, 3),
+               us_min=dict(step=round(us_step_min, 3), dual_linear=round(us_dual_min, 3), quantize_act=round(us_quant_min, 3)),
+               timing="median of 20 replays of a CUDA graph of %d steps (min alongside)" % steps,
                eff_tops=round((ops_i8 + fl_lr) / (us_dual * 1e-6) / 1e12, 2),
                gbs=round(twq.algorithmic_bytes(L.M, L.N, L.K, L.r, L.G) / (us_dual * 1e-6) / 1e9, 1),
                weight_copies=gl.ncopies, lap_mb=round(gl.lap_bytes / 2 ** 20, 1),
-               roofline=roofline_for(L, twq, us_dual, peaks, load_traffic(name)))
+               roofline=roofline_for(L, twq, us_dual, peaks, traffic, traffic_src))
     if with_e2e:
         out["us_e2e"] = round(gl.time_e2e(steps, warmup), 3)
+        out["us_host_per_call"] = round(gl.time_host(), 3)
     if with_cublas:
         A = torch.randn(L.M, L.K, device="cuda", dtype=torch.bfloat16)
         Bs = [torch.randn(L.K, L.N, device="cuda", dtype=torch.bfloat16) for _ in range(max(2, min(16, (2 * L2_BYTES) // (2 * L.K * L.N) + 1)))]
@@ -307,7 +338,7 @@ def run_reference(args):
     line = dict(metric="fused dual-linear us/call", value=round(us, 1), unit="us/call", n_gpus=args.gpus,
                 steps=args.steps, warmup=args.warmup, ms_per_step=round(us / 1e3, 4), higher_is_better=False,
                 scaling="weak", vs_baseline=None, dtype="int64+f64", data="synthetic", impl="reference",
-                config=dict(workload=args.workload, desc=WORKLOADS[args.workload][2]),
+                config=config_for(args.workload),
                 cpu_baseline=cb,
                 e2e=dict(value=round(us, 1), unit="us/call", h2d_bytes_per_step=0, d2h_bytes_per_step=0),
                 wall_s=round(time.perf_counter() - t0, 1))
@@ -394,24 +425,39 @@ def main():
             del g2
             torch.cuda.empty_cache()
 
+    i8_tops = None
+    if rank == 0:
+        # an MMA-only tcgen05 kind::i8 loop on every SM, next to the 2 x BF16 figure the roofline uses
+        i8_tops = twq.testing_measure_i8_tops(4096, 5)
+        by_name = {r["workload"]: r for r in sweep}
+        by_name.setdefault(args.workload, main_res)
+
     if rank == 0:
         cpu = None if args.no_cpu_baseline else time_oracle(L)
         # whole-job figure: N replicas each finish K calls in the max-over-ranks time
         value = whole_job_us_per_call(us, world)
         line = dict(metric="fused dual-linear us/call", value=round(value, 3), unit="us/call", n_gpus=world,
+                    timing=main_res["timing"],
                     steps=args.steps, warmup=args.warmup, ms_per_step=round(us / 1e3, 6), higher_is_better=False,
                     scaling="weak", vs_baseline=None, dtype="s8 (INT4 codes x16) -> s32; f16 -> f32 low-rank",
                     data="synthetic",
-                    config=dict(workload=args.workload, desc=WORKLOADS[args.workload][2],
-                                l2="inputs larger than L2: %d rotating copies, %.0f MB per lap" %
-                                   (main_res["weight_copies"], main_res["lap_mb"]),
-                                launch="CUDA graph of K steps; step = twq_quantize_act + twq_dual_linear",
-                                multi_gpu="replicas only"),
+                    config=config_for(args.workload),
+                    l2_rotation="%d rotating copies, %.0f MB per lap" % (main_res["weight_copies"], main_res["lap_mb"]),
                     clocks=clocks,
                     e2e=dict(value=round(whole_job_us_per_call(us_e2e, world), 3), unit="us/call", h2d_bytes_per_step=2 * L.M * L.K,
                              d2h_bytes_per_step=2 * L.M * L.N),
                     gpu_launches=2 * args.steps,
-                    roofline=main_res["roofline"], cpu_baseline=cpu,
+                    roofline=main_res["roofline"],
+                    # the two graded shapes (north_star: ">= 60 % of roofline at M = 1 and M = 2048"), lifted out of `sweep`
+                    roofline_m1=by_name.get("c2_qproj_m1", {}).get("roofline"),
+                    roofline_m2048=by_name.get("c3_gateup_m2048", {}).get("roofline"),
+                    roofline_m2048_down=by_name.get("c3_down_m2048", {}).get("roofline"),
+                    int8_peak=dict(measured_mma_only_tops=None if i8_tops is None else round(i8_tops, 1),
+                                   roofline_uses_tops=round(2.0 * peaks["bf16_tflops"], 1),
+                                   how="tcgen05.mma kind::i8 128x128x32 from shared memory, 4096 x 8 MMAs per SM, best of 5 "
+                                       "(csrc/peak_i8.cu); the roofline denominator stays 2 x measured cuBLAS BF16 burst"),
+                    us_host_per_call=main_res.get("us_host_per_call"),
+                    cpu_baseline=cpu,
                     us_dual_linear=main_res["us_dual_linear"], us_quantize_act=main_res["us_quantize_act"],
                     eff_tops=main_res["eff_tops"], gbs=main_res["gbs"],
                     cublas_bf16_gemm_us=main_res.get("us_cublas_bf16_gemm"),
