@@ -196,7 +196,7 @@ class GpuLayer:
         """Host time of one twq_dual_linear call through the binding (plan + descriptor caches warm), no device
         synchronisation inside the loop; the queue is drained every 100 calls so that it never back-pressures."""
         torch = self.torch
-        for i in range(20):
+        for i in range(max(20, self.ncopies)):                   # every rotating copy has its descriptors cached
             self.step(i, False, True)
         torch.cuda.synchronize()
         t = 0.0
@@ -210,7 +210,7 @@ class GpuLayer:
 
     def time_e2e(self, steps, warmup):
         torch = self.torch
-        for i in range(warmup):
+        for i in range(max(warmup, self.ncopies)):               # every rotating copy has its descriptors cached
             self.e2e_step(i)
         torch.cuda.synchronize()
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
