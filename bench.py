@@ -39,11 +39,16 @@ WORKLOADS = {
     # name: (generator, kwargs, description)
     "c2_qproj_m1": ("config2_qproj", dict(M=1), "LLaMA3-8B q_proj K=4096 N=4096 r=128 G=128 M=1"),
     "c2_qproj_m16": ("config2_qproj", dict(M=16), "LLaMA3-8B q_proj K=4096 N=4096 r=128 G=128 M=16"),
+    "c2_qproj_m32": ("config2_qproj", dict(M=32), "LLaMA3-8B q_proj K=4096 N=4096 r=128 G=128 M=32"),
+    "c2_qproj_m64": ("config2_qproj", dict(M=64), "LLaMA3-8B q_proj K=4096 N=4096 r=128 G=128 M=64"),
     "c2_qproj_m128": ("config2_qproj", dict(M=128), "LLaMA3-8B q_proj K=4096 N=4096 r=128 G=128 M=128"),
     "c3_gateup_m2048": ("config3_mlp", dict(which="gate_up", M=2048), "LLaMA3-8B gate/up K=4096 N=14336 r=128 G=128 M=2048"),
     "c3_down_m2048": ("config3_mlp", dict(which="down", M=2048), "LLaMA3-8B down K=14336 N=4096 r=128 G=128 M=2048"),
     "c3_gateup_m2048_r256": ("config3_mlp", dict(which="gate_up", M=2048, r=256), "LLaMA3-8B gate/up r=256 M=2048"),
     "c1_tiny": ("config1_tiny", dict(), "tiny M=8 K=256 N=512 r=16 G=64"),
+    # rank 0 (plain W4A4): what the residual stream alone costs
+    "c2_qproj_m1_r0": ("config2_qproj", dict(M=1, r=0), "LLaMA3-8B q_proj K=4096 N=4096 r=0 G=128 M=1"),
+    "c2_qproj_m16_r0": ("config2_qproj", dict(M=16, r=0), "LLaMA3-8B q_proj K=4096 N=4096 r=0 G=128 M=16"),
     # configs 4 / 5 (rank 256): not in the default sweep; DESIGN.md section 10 quotes them
     "c4_gateup_m4096": ("config4_qwen", dict(which="gate_up", M=4096), "Qwen3-32B gate/up K=5120 N=25600 r=256 M=4096"),
     "c4_down_m4096": ("config4_qwen", dict(which="down", M=4096), "Qwen3-32B down K=25600 N=5120 r=256 M=4096"),

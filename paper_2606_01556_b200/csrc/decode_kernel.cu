@@ -246,6 +246,7 @@ decode_dual_linear_kernel(const __grid_constant__ CUtensorMap tmXq, const __grid
         if (lane == 0)
             for (int c = 0; c < first; ++c) arm(c, c);
         __syncwarp();
+        asm volatile("bar.arrive 3, 64;" ::: "memory");          // the barriers are armed: the activation-side warp may issue
         // weights do not depend on the previous kernel: the whole first lap goes out before griddepcontrol.wait
         for (int i = lane; i < first * ntile; i += 32) copy_w(i / ntile, i / ntile, i % ntile);
         if (lane == 31 && ntile > 0) {
@@ -257,11 +258,8 @@ decode_dual_linear_kernel(const __grid_constant__ CUtensorMap tmXq, const __grid
                                  static_cast<uint32_t>(ntile) * 8 * r * 2);
         }
         TWQ_DSTAMP(2);
-        pdl_wait();                                              // Xq comes from twq_quantize_act
+        pdl_wait();                                              // later laps carry Xq boxes (twq_quantize_act's output)
         TWQ_DSTAMP(3);
-        if (lane < first)
-            tma_load_3d_a(ring + lane * p.slot_bytes + p.xq_off, &tmXq, DBAR(D_FULL + lane), 0, lane * p.gc, 0);
-        TWQ_DSTAMP(4);
         // later laps of both rings (long K / many tiles only): lane 0 refills stage-1 chunks, the warp refills residual chunks
         {
             int s1 = 0, lap1 = 1, i1n = l1_first;                // stage-1 ring
@@ -294,7 +292,18 @@ decode_dual_linear_kernel(const __grid_constant__ CUtensorMap tmXq, const __grid
             }
         }
     } else if (warp == kDecWarps) {
-        // spare warp (registers are allotted to warps in fours)
+        // ================================================================ activation-side producer
+        // The Xq boxes of the first lap.  They must wait for the previous kernel (twq_quantize_act), the weights need not:
+        // issued from the producer warp behind the weight copies they were the LAST bytes of every chunk to land (the
+        // copy engine works in order) and no chunk was complete before 2.4 us; from their own warp they go out as soon
+        // as the previous kernel is done and land first.
+        named_bar_sync(3, 64);                                   // the chunk barriers are armed
+        pdl_wait();
+        const int first = ntile > 0 ? min(p.nslots, p.nchunks) : 0;
+        if (lane < first)
+            tma_load_3d_a(smem_u32(dsm + p.off_ring) + lane * p.slot_bytes + p.xq_off, &tmXq, DBAR(D_FULL + lane), 0,
+                          lane * p.gc, 0);
+        TWQ_DSTAMP(4);
     } else if (is_lr) {
         // ================================================================ low-rank chain
         const int lrt = threadIdx.x - nrw * 32, nlr = lrw * 32;
@@ -304,7 +313,7 @@ decode_dual_linear_kernel(const __grid_constant__ CUtensorMap tmXq, const __grid
             // X slice (tokens x 32*nu k, BF16 -> FP16) into shared memory, four 16-byte loads in flight per thread
             const uint16_t* X = static_cast<const uint16_t*>(p.X);
             const int chunks = nu * 4;                           // 16-byte chunks per token row
-            const int total = kMp * chunks;
+            const int total = p.xrows * chunks;
             // element i = (token i / chunks, chunk i % chunks): one division per thread, then (token, chunk) advance by
             // the constant (nlr / chunks, nlr % chunks) with a carry
             int m = chunks > 0 ? lrt / chunks : 0, cq = lrt - m * chunks;
@@ -355,7 +364,8 @@ decode_dual_linear_kernel(const __grid_constant__ CUtensorMap tmXq, const __grid
 #pragma unroll
             for (int q = 0; q < NQ; ++q) loff[q] = static_cast<uint32_t>(min(lw + q * lrw, max(njt - 1, 0))) * 512u;
             uint32_t xs_a = smem_u32(sXs) + (gid * p.xs_stride + tid4 * 8) * 2;   // advances 64 bytes per slab
-            const uint32_t xrow8 = 8u * p.xs_stride * 2u;
+            // with at most 8 tokens only rows 0..7 are staged: the gid + 8 fragment re-reads row gid (its output rows are dropped)
+            const uint32_t xrow8 = p.xrows > 8 ? 8u * p.xs_stride * 2u : 0u;
             const uint32_t chunk_bytes = static_cast<uint32_t>(p.sc) * slab_bytes;
             int slot = 0, lap = 0;
             uint32_t slot_a = 0;
@@ -846,7 +856,8 @@ bool decode_make_plan(int M, int N, int K, int r, int G, int num_sms, DecodePara
     p.off_ylr = o; o += r > 0 ? round_up_i(p.mp * p.tmax * 8 * 4, 128) : 0;
     p.off_hpart = o; o += r > 0 ? round_up_i(p.mp * r * 4, 128) : 0;
     p.off_h = o; o += r > 0 ? round_up_i(p.mp * (r + 8) * 2, 128) : 0;
-    p.off_xs = o; o += r > 0 ? round_up_i(p.mp * p.xs_stride * 2, 128) : 0;
+    p.xrows = M <= 8 ? 8 : p.mp;                              // token rows of the staged X slice
+    p.off_xs = o; o += r > 0 ? round_up_i(p.xrows * p.xs_stride * 2, 128) : 0;
     // stage-1 ring: chunks of ~16 KB of L1 slabs
     p.sc = 1; p.l1_slots = 1;
     if (r > 0) {

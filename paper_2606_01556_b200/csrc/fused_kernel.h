@@ -60,6 +60,7 @@ struct DecodeParams {
     int sc, l1_slots;        // stage-1 ring: 32-wide K slabs per chunk, ring depth
     int nu_max;              // most K slabs of stage 1 any CTA multiplies
     int xs_stride;           // halves per token row of the staged FP16 X slice
+    int xrows;               // token rows staged (8 when M <= 8, else mp)
     int off_ring, off_l1, off_sw, off_xs, off_hpart, off_h, off_ylr, off_sx, off_res, off_bar, smem_bytes;
     const uint8_t* R4;       // [N/8][ng][8][G/2]
     const __half* sw16;      // [N/8][ng][8]
