@@ -22,6 +22,20 @@
  *   - Non-finite inputs give unspecified values, never a fault.
  *   - There is no CPU fallback: without an sm_100 device the compute entry points
  *     return TWQ_ERR_UNSUPPORTED / TWQ_ERR_CUDA.
+ *   - One device per call: the current CUDA device (cudaSetDevice) at the time of the call.  Per-device facts and
+ *     function attributes are cached per device; plans and TMA descriptors are cached per host thread.  Calls from
+ *     several host threads are safe as long as two calls that share a workspace do not run concurrently.
+ *
+ * Stream-ordering contract (programmatic dependent launch)
+ *   twq_quantize_act and twq_dual_linear are launched with the programmatic-stream-serialization attribute: a
+ *   kernel may START while its stream predecessor is still running.  What each kernel does before / after its
+ *   griddepcontrol.wait (= "the predecessor has completed and its writes are visible"):
+ *     before the wait : reads of `packed` only (weights, scales, low-rank factors).  `packed` must therefore not be
+ *                       written by the kernel that immediately precedes the call in the stream (pack once, offline).
+ *     after the wait  : every read of X, Xq, sx and every write of Y, dbg_P, ws.  A predecessor -- a kernel of this
+ *                       library or the caller's own, PDL-aware or not -- may produce X / Xq / sx up to its last
+ *                       instruction.
+ *   twq_quantize_act waits for its predecessor before it touches memory and only then lets its successor start.
  */
 #ifndef TWQ_H_
 #define TWQ_H_
@@ -55,9 +69,9 @@ const char* twq_status_string(twq_status s);
 /* ---------------------------------------------------------------------------
  * twq_packed_bytes -- size in bytes of the opaque kernel-native weight blob that
  * twq_pack_weights writes for one layer (0 if the shape is invalid).
- * Contents ("pre-processed offline"; L193 groups of G along K):
- * 4-bit residual codes [N,K/2], FP32 group scales transposed [K/G,N], L1^T [r,K]
- * FP16, L2^T [N,r] FP16; each section 256-byte aligned.
+ * Contents ("pre-processed offline"; L193 groups of G along K), each section 256-byte aligned:
+ * 4-bit residual codes tiled [N/8][K/G][8][G/2] (N*K/2 bytes), FP16 group scales tiled the same way [N/8][K/G][8],
+ * L1^T [r,K] FP16 (tcgen05 kernel), L1 in 32-wide K slabs [K/32][r][32] FP16 (small-batch kernel), L2^T [N,r] FP16.
  */
 size_t twq_packed_bytes(int N, int K, int r, int G);
 
@@ -104,20 +118,25 @@ size_t twq_workspace_bytes(int M, int N, int K, int r, int G);
  *   residual : P[m,g,n] = sum_{k in g} qx[m,k]*qw[n,k]   exact int32   (Eq. 2; L177)
  *              Yres     = sum_g sx[m,g]*sw[n,g]*P[m,g,n]  FP32          (L181 "folds the scale factors")
  *   low-rank : H = X*L1 (FP32 accumulate, kept on chip), Ylr = H*L2    (Eq. 3; L177-179)
+ *              The 16-bit tensor-core product needs one operand format and L1 is FP16, so X (BF16) is rewritten to
+ *              FP16 on chip: exact for 2^-14 <= |x| <= 65504, SATURATING at +-65504 above, and losing bits below
+ *              2^-14 (flush to zero below 2^-24).  H is rounded once to FP16 (saturating) as the operand of the
+ *              second product (readings R2, R12).  The residual branch reads X through Xq / sx only.
  *   epilogue : Y = round_out(Yres + Ylr), one store                    (L181)
  *   X      [M,ldx] bf16     raw activations (read by the low-rank branch; may be NULL iff r == 0)
  *   Xq,sx                   outputs of twq_quantize_act for the same X
  *   packed                  blob written by twq_pack_weights for (N,K,r,G)
  *   Y      [M,ldy]          out, dtype ydt (ldy >= N elements)
  *   ws, ws_bytes            scratch of at least twq_workspace_bytes(...) bytes, 256-byte aligned (may be
- *                           NULL when that is 0).  It holds split-K partial sums and tile counters for
- *                           calls with few output tiles (16 < M, roughly M*N < 1.5 M outputs), and, for
- *                           M <= 16 on layers with a large low-rank factor (K*r above ~1.3 M elements),
- *                           the per-cluster partial sums of H and a barrier counter; other calls with
- *                           M <= 16 and prefill-shaped calls need none.  The caller zero-fills it ONCE
- *                           after allocation; every call leaves the counters zero again, so it can be
+ *                           NULL when that is 0).  Only calls with few output tiles beyond the small-batch
+ *                           kernel (32 < M, roughly M*N < 1.5 M outputs) need it: split-K partial sums of Y
+ *                           and tile counters.  Small batches (M <= 32) and prefill-shaped calls need none,
+ *                           and the on-chip intermediate H never passes through it.  The caller zero-fills it
+ *                           ONCE after allocation; every call leaves the counters zero again, so it can be
  *                           reused without clearing -- by calls on ONE stream at a time (two calls that
- *                           share a workspace must not run concurrently).
+ *                           share a workspace must not run concurrently).  Calls that use a workspace are
+ *                           launched cooperatively (their CTAs wait for one another): the driver refuses the
+ *                           launch (TWQ_ERR_CUDA) rather than let it hang if the grid cannot be co-resident.
  *   dbg_P  [M,K/G,N] int32  NULL, or receives the integer group accumulators P taken from the
  *                           same tensor-core path that feeds Y (parity evidence; slows the call)
  */

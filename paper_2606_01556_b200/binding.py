@@ -181,6 +181,23 @@ def quantize_act(X: torch.Tensor, G: int, tinv=None, out=None, stream=None):
     return Xq, sx
 
 
+_ws_cache = {}
+
+
+def _cached_workspace(need: int, device, stream):
+    """One zero-initialised workspace per (device, stream), grown on demand and zeroed ON that stream: the library
+    leaves its counters at zero after every call, so the buffer is reused without clearing, and no memset is
+    queued between a call and its stream predecessor."""
+    s = torch.cuda.current_stream(device) if stream is None else stream
+    key = (device.index if device.index is not None else torch.cuda.current_device(), s.cuda_stream)
+    buf = _ws_cache.get(key)
+    if buf is None or buf.numel() < need:
+        with torch.cuda.stream(s):
+            buf = torch.zeros(need, dtype=torch.uint8, device=device)
+        _ws_cache[key] = buf
+    return buf
+
+
 def dual_linear(X, Xq, sx, packed: PackedLayer, out_dtype: int = OUT_BF16, Y=None, ws=None, dbg_P=None,
                 stream=None):
     """twq_dual_linear.  Returns Y [M,N] in out_dtype.  `ws` must be a zero-initialised uint8 tensor of at
@@ -191,7 +208,7 @@ def dual_linear(X, Xq, sx, packed: PackedLayer, out_dtype: int = OUT_BF16, Y=Non
         Y = torch.empty((M, N), dtype=_OUT_TORCH.get(out_dtype, torch.bfloat16), device=Xq.device)
     need = workspace_bytes(M, N, K, r, G)
     if need and ws is None:
-        ws = torch.zeros(need, dtype=torch.uint8, device=Xq.device)
+        ws = _cached_workspace(need, Xq.device, stream)
     ldx = X.stride(0) if X is not None else K
     code = load_library().twq_dual_linear(_ptr(X) if r else None, ldx, _ptr(Xq), _ptr(sx), _ptr(packed.blob),
                                           M, N, K, r, G, _ptr(Y), out_dtype, Y.stride(0), _ptr(ws),

@@ -497,12 +497,14 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
         bool fx_ok = false;
         auto fetch_sx = [&](const float* src, int left) {
             if (fx_ok && left >= 8 && (reinterpret_cast<uintptr_t>(src) & 15u) == 0) {
-                const float4 a = __ldg(reinterpret_cast<const float4*>(src)), c = __ldg(reinterpret_cast<const float4*>(src) + 1);
+                // sx is written by the stream predecessor, which may still have been running when this kernel started
+                // (programmatic dependent launch): coherent loads, not the read-only (.nc) path
+                const float4 a = __ldcg(reinterpret_cast<const float4*>(src)), c = __ldcg(reinterpret_cast<const float4*>(src) + 1);
                 sxv[0] = a.x; sxv[1] = a.y; sxv[2] = a.z; sxv[3] = a.w;
                 sxv[4] = c.x; sxv[5] = c.y; sxv[6] = c.z; sxv[7] = c.w;
             } else {
 #pragma unroll
-                for (int j = 0; j < 8; ++j) sxv[j] = (fx_ok && j < left) ? __ldg(src + j) : 0.0f;
+                for (int j = 0; j < 8; ++j) sxv[j] = (fx_ok && j < left) ? __ldcg(src + j) : 0.0f;
             }
         };
         {

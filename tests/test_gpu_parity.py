@@ -231,6 +231,35 @@ def test_rank0_is_plain_w4a4_and_zero_residual_is_lowrank(twq, oracle, plan_flag
     assert np.abs(Y - ref).max() / np.abs(ref).max() <= 1e-3
 
 
+@pytest.mark.parametrize("M,flags", [(7, 0), (20, 0), (40, 0), (300, 1)])
+def test_lowrank_fp16_rewrite_saturates_as_documented(twq, oracle, plan_flags, M, flags):
+    """include/twq.h: the low-rank branch rewrites X (BF16) to FP16 on chip -- exact in [2^-14, 65504], saturating
+    above.  With R = 0 the output is that branch alone: it must equal the FP64 product of the CLAMPED activations
+    (values beyond +-65504 saturate; values below 2^-14 only lose bits far under the tolerance).  Every kernel path."""
+    import torch
+    plan_flags(flags)
+    K, N, r, G = 512, 512, 32, 128
+    L = gen.make_layer(M, K, N, r, G, seed=77, lr_sigma=0.002)
+    L.Rq[:] = 0
+    x = gen.bf16_bits_to_f32(L.X).copy()
+    x[:, 5] = 3.0e5                      # beyond FP16 range
+    x[:, 17] = -1.0e6
+    x[:, 40] = 2.0 ** -20                # FP16 subnormal
+    x[:, 41] = 2.0 ** -30                # flushes to zero
+    L.X = gen.f32_to_bf16_bits(x)
+    X, packed, _ = _upload(twq, L)
+    Xq, sx = twq.quantize_act(X, G)
+    need = twq.workspace_bytes(M, N, K, r, G)
+    ws = torch.zeros(need, dtype=torch.uint8, device="cuda") if need else None
+    Y = twq.dual_linear(X, Xq, sx, packed, twq.OUT_FP32, ws=ws).cpu().numpy().astype(np.float64)
+    xc = np.clip(gen.bf16_bits_to_f32(L.X).astype(np.float64), -65504.0, 65504.0)
+    ref = (xc @ L.L1.astype(np.float64)) @ L.L2.astype(np.float64)
+    assert np.isfinite(Y).all()
+    assert np.abs(Y - ref).max() / np.abs(ref).max() <= 1e-3
+    unclamped = (gen.bf16_bits_to_f32(L.X).astype(np.float64) @ L.L1.astype(np.float64)) @ L.L2.astype(np.float64)
+    assert np.abs(unclamped - ref).max() / np.abs(ref).max() > 0.1      # the clamp is what the kernel computes, not X itself
+
+
 def test_extreme_codes_hit_the_accumulator_bound(twq, oracle):
     """|P| = 7*8*G exactly and sign extension of -8."""
     import torch
