@@ -261,7 +261,7 @@ def load_traffic(name):
 
 
 def kernel_name(L):
-    return "decode_dual_linear_kernel" if L.M <= 32 else "fused_dual_linear_kernel"
+    return "decode_dual_linear_kernel" if L.M <= 64 else "fused_dual_linear_kernel"
 
 
 def measure_workload(name, twq, torch, steps, warmup, peaks, with_e2e=False, with_cublas=False):

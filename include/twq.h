@@ -129,8 +129,8 @@ size_t twq_workspace_bytes(int M, int N, int K, int r, int G);
  *   Y      [M,ldy]          out, dtype ydt (ldy >= N elements)
  *   ws, ws_bytes            scratch of at least twq_workspace_bytes(...) bytes, 256-byte aligned (may be
  *                           NULL when that is 0).  Only calls with few output tiles beyond the small-batch
- *                           kernel (32 < M, roughly M*N < 1.5 M outputs) need it: split-K partial sums of Y
- *                           and tile counters.  Small batches (M <= 32) and prefill-shaped calls need none,
+ *                           kernel (64 < M, roughly M*N < 1.5 M outputs) need it: split-K partial sums of Y
+ *                           and tile counters.  Small batches (M <= 64) and prefill-shaped calls need none,
  *                           and the on-chip intermediate H never passes through it.  The caller zero-fills it
  *                           ONCE after allocation; every call leaves the counters zero again, so it can be
  *                           reused without clearing -- by calls on ONE stream at a time (two calls that

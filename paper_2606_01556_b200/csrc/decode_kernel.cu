@@ -164,7 +164,7 @@ decode_dual_linear_kernel(const __grid_constant__ CUtensorMap tmXq, const __grid
     const int gid = lane >> 2, tid4 = lane & 3;
     const int r = p.r, ng = p.ng, cs = p.cs, lrw = p.lrw;
     const int nrw = kDecWarps - lrw;
-    constexpr int kTPW = MT == 1 ? 6 : 3;       // 8-channel tiles one residual warp can own (its accumulators)
+    constexpr int kTPW = MT == 1 ? 6 : (MT == 2 ? 3 : 2);   // 8-channel tiles one residual warp can own (its accumulators)
     // Warp roles by id: [0, nrw) residual, [nrw, 18) low-rank chain, 18 spare, 19 producer.  The scheduler of an SM
     // sub-partition favours HIGHER warp ids: the dependent low-rank chain and the producer must not queue behind the
     // residual warps (with the chain in warps 0-3 every step of it waited for an issue slot; in-kernel timeline, r02).
@@ -416,8 +416,8 @@ decode_dual_linear_kernel(const __grid_constant__ CUtensorMap tmXq, const __grid
         };
         if (nq_need <= 1) stage1(std::integral_constant<int, 1>{});
         else if (nq_need == 2) stage1(std::integral_constant<int, 2>{});
-        else if (nq_need <= 4) stage1(std::integral_constant<int, 4>{});
-        else stage1(std::integral_constant<int, kJT>{});
+        else if (nq_need <= 4 || MT == 4) stage1(std::integral_constant<int, 4>{});   // MT == 4 runs 8 low-rank warps: r / 64 <= 4
+        else stage1(std::integral_constant<int, MT == 4 ? 4 : kJT>{});
         // stage-2 operand of this warp's first tile (L2T rows, L2-resident by now), ahead of the exchange
         constexpr int kL2 = 8;                                   // 32-wide j steps (r <= 256)
         uint4 l2v[kL2];
@@ -566,6 +566,68 @@ decode_dual_linear_kernel(const __grid_constant__ CUtensorMap tmXq, const __grid
                     uint32_t swp = sw_a + g * 16;
 #pragma unroll 1
                     for (; gl < gcnt; gl += P, g += P, wa += step_w, xa += step_x, sxp += step_sx, swp += step_sw) {
+                        if constexpr (MT >= 2) {
+                            // Several 16-token tiles: the warp's tiles (kTPW <= kTB) are one batch whose weight fragments are
+                            // loaded once per K-group; the token tiles are walked inside, each expanding its own activation
+                            // fragments (16 registers at a time instead of 16 * MT).
+                            uint32_t wt[kTPW][kW];
+                            uint32_t swh[kTPW];
+#pragma unroll
+                            for (int b = 0; b < kTPW; ++b) {
+                                if (b == 0 || slot_on(b)) {
+                                    lds_words<kW>(wt[b], wa + toff[b]);
+                                    swh[b] = lds_u32(swp + swoff[b]);
+                                }
+                            }
+#pragma unroll
+                            for (int mt = 0; mt < MT; ++mt) {
+                                uint32_t x0[kW], x1[kW];
+                                lds_words<kW>(x0, xa + mt * 2 * x8);
+                                lds_words<kW>(x1, xa + mt * 2 * x8 + x8);
+                                const float sx0 = __uint_as_float(lds_u32(sxp + mt * 64));
+                                const float sx1 = __uint_as_float(lds_u32(sxp + mt * 64 + 32));
+                                int dd[kTPW][4];
+#pragma unroll
+                                for (int b = 0; b < kTPW; ++b)
+#pragma unroll
+                                    for (int e = 0; e < 4; ++e) dd[b][e] = 0;
+#pragma unroll
+                                for (int w = 0; w < kW; ++w) {
+                                    const uint32_t a0 = d_lo16(x0[w]), a1 = d_lo16(x1[w]), a2 = d_hi16(x0[w]), a3 = d_hi16(x1[w]);
+#pragma unroll
+                                    for (int b = 0; b < kTPW; ++b)
+                                        if (b == 0 || slot_on(b)) imma_16832(dd[b], a0, a1, a2, a3, d_lo16(wt[b][w]), d_hi16(wt[b][w]));
+                                }
+#pragma unroll
+                                for (int b = 0; b < kTPW; ++b) {
+                                    if (slot_on(b)) {
+                                        const float2 sw2 = __half22float2(*reinterpret_cast<const __half2*>(&swh[b]));
+                                        const uint64_t swp2 = pack_f2(sw2.x, sw2.y);
+                                        float (&a)[4] = acc[b][mt];
+                                        const uint64_t t01 = fma2(pack_f2(static_cast<float>(dd[b][0]), static_cast<float>(dd[b][1])), swp2, 0ull);
+                                        const uint64_t t23 = fma2(pack_f2(static_cast<float>(dd[b][2]), static_cast<float>(dd[b][3])), swp2, 0ull);
+                                        const uint64_t a01 = fma2(t01, pack_f2(sx0, sx0), pack_f2(a[0], a[1]));
+                                        const uint64_t a23 = fma2(t23, pack_f2(sx1, sx1), pack_f2(a[2], a[3]));
+                                        unpack_f2(a01, a[0], a[1]);
+                                        unpack_f2(a23, a[2], a[3]);
+                                        if (kDbg) {
+                                            if (p.dbgP != nullptr) {
+                                                const int n = (tile0 + t_lo + tix(b)) * 8 + tid4 * 2;
+                                                const int m0 = mt * 16 + gid;
+                                                if (m0 < p.M) {
+                                                    p.dbgP[(static_cast<size_t>(m0) * ng + g) * p.N + n] = dd[b][0] >> 8;
+                                                    p.dbgP[(static_cast<size_t>(m0) * ng + g) * p.N + n + 1] = dd[b][1] >> 8;
+                                                }
+                                                if (m0 + 8 < p.M) {
+                                                    p.dbgP[(static_cast<size_t>(m0 + 8) * ng + g) * p.N + n] = dd[b][2] >> 8;
+                                                    p.dbgP[(static_cast<size_t>(m0 + 8) * ng + g) * p.N + n + 1] = dd[b][3] >> 8;
+                                                }
+                                            }
+                                        }
+                                    }
+                                }
+                            }
+                        } else {
                         // activation fragments of the K-group, expanded once for all tiles of the warp
                         uint32_t ax[MT][kW][4];
                         float sxa[MT][2];
@@ -646,6 +708,7 @@ decode_dual_linear_kernel(const __grid_constant__ CUtensorMap tmXq, const __grid
                                     }
                                 }
                             }
+                        }
                         }
                     }
                 }
@@ -813,9 +876,9 @@ bool decode_make_plan(int M, int N, int K, int r, int G, int num_sms, DecodePara
     DecodeParams p = {};
     p.M = M; p.N = N; p.K = K; p.r = r; p.ng = K / G;
     p.n_tiles = N / 8;
-    p.mt = M <= 16 ? 1 : 2;
+    p.mt = M <= 16 ? 1 : (M <= 32 ? 2 : 4);
     p.mp = 16 * p.mt;
-    p.lrw = r > 0 ? 4 : 0;
+    p.lrw = r > 0 ? (p.mt == 4 ? 8 : 4) : 0;              // more token tiles: stage 1 / stage 2 over eight warps
     const int nrw = kDecWarps - p.lrw;
     // cluster size: H is shared by the cluster and every cluster streams all of L1 (K*r*2 bytes) from L2, so the
     // largest cluster that still covers 70 % of the SMs wins; otherwise the size covering the most SMs
@@ -842,7 +905,7 @@ bool decode_make_plan(int M, int N, int K, int r, int G, int num_sms, DecodePara
     if (nclusters < 1) nclusters = 1;
     p.grid = nclusters * p.cs;
     p.tmax = (p.n_tiles + p.grid - 1) / p.grid;
-    const int kTPWh = p.mt == 1 ? 6 : 3;                      // tiles per residual warp (kernel: kTPW)
+    const int kTPWh = p.mt == 1 ? 6 : (p.mt == 2 ? 3 : 2);    // tiles per residual warp (kernel: kTPW)
     if (p.tmax > kTPWh * nrw) return false;
     // ---- shared-memory plan
     const int kBlk = 4 * G;
@@ -865,7 +928,8 @@ bool decode_make_plan(int M, int N, int K, int r, int G, int num_sms, DecodePara
         if (p.sc < 1) p.sc = 1;
         if (p.sc > p.nu_max) p.sc = p.nu_max > 0 ? p.nu_max : 1;
         const int chunks = (p.nu_max + p.sc - 1) / p.sc;
-        p.l1_slots = chunks < kMaxL1Slots ? (chunks > 0 ? chunks : 1) : kMaxL1Slots;
+        const int max_l1 = p.mt == 4 ? 2 : kMaxL1Slots;       // 64 tokens: the X slice and the H partial take the room
+        p.l1_slots = chunks < max_l1 ? (chunks > 0 ? chunks : 1) : max_l1;
         p.off_l1 = o; o += p.l1_slots * p.sc * r * 64;
     } else {
         p.off_l1 = o;
@@ -905,7 +969,7 @@ cudaError_t launch_decode(const CUtensorMap& tmXq, const DecodeParams& p, int G,
     const bool dbg = p.dbgP != nullptr;
 #define TWQ_DCASE(g, m)                                                                   \
     if (G == g && p.mt == m) return dbg ? decode_launch_inst<g, m, true>(tmXq, p, stream) : decode_launch_inst<g, m, false>(tmXq, p, stream);
-    TWQ_DCASE(128, 1) TWQ_DCASE(128, 2) TWQ_DCASE(64, 1) TWQ_DCASE(64, 2)
+    TWQ_DCASE(128, 1) TWQ_DCASE(128, 2) TWQ_DCASE(128, 4) TWQ_DCASE(64, 1) TWQ_DCASE(64, 2) TWQ_DCASE(64, 4)
 #undef TWQ_DCASE
     return cudaErrorInvalidValue;
 }

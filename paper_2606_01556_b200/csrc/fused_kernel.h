@@ -46,7 +46,7 @@ struct FusedMaps {
 
 
 // Small-batch calls (M <= kDecodeMaxM): parameters and plan of decode_kernel.cu (host-computed).
-constexpr int kDecodeMaxM = 32;
+constexpr int kDecodeMaxM = 64;
 struct DecodeParams {
     int M, N, K, r, ng;
     int ldx, ldy, ydt;       // ydt: 0 bf16, 1 fp16, 2 fp32

@@ -108,9 +108,9 @@ def test_workspace_rule(lib):
     assert twq.workspace_bytes(2048, 14336, 4096, 128, 128) == 0      # prefill: tiles fill the GPU, no split
     assert twq.workspace_bytes(1, 4096, 4096, 128, 128) == 0           # decode kernel (M <= 16): no scratch
     assert twq.workspace_bytes(16, 4096, 4096, 128, 128) == 0
-    assert twq.workspace_bytes(32, 4096, 4096, 128, 128) == 0          # small-batch kernel up to M = 32
-    w = twq.workspace_bytes(48, 4096, 4096, 128, 128)                  # few tiles: split-K partials + counters
-    assert w > 0 and (w - 256) % (48 * 4096 * 4) == 0
+    assert twq.workspace_bytes(64, 4096, 4096, 128, 128) == 0          # small-batch kernel up to M = 64
+    w = twq.workspace_bytes(80, 4096, 4096, 128, 128)                  # few tiles: split-K partials + counters
+    assert w > 0 and (w - 256) % (80 * 4096 * 4) == 0
     assert twq.workspace_bytes(0, 4096, 4096, 128, 128) == 0           # invalid shape
 
 
@@ -133,7 +133,7 @@ def test_argument_validation_happens_before_cuda(lib):
     assert lib.twq_dual_linear(None, 256, p, p, p, 8, 512, 256, 16, 64, p, 0, 512, None, 0, None, None) == 1
     assert lib.twq_dual_linear(p, 256, p, p, p, 8, 512, 256, 16, 64, p, 7, 512, None, 0, None, None) == 1
     assert lib.twq_dual_linear(p, 256, p, p, p, 8, 512, 256, 16, 64, p, 0, 256, None, 0, None, None) == 1
-    assert lib.twq_dual_linear(p, 256, p, p, p, 40, 512, 256, 16, 64, p, 0, 512, None, 0, None, None) == 3
+    assert lib.twq_dual_linear(p, 256, p, p, p, 72, 512, 256, 16, 64, p, 0, 512, None, 0, None, None) == 3
     # valid arguments but no sm_100 device here -> UNSUPPORTED or CUDA error, never a crash, never OK
     import torch
     if not torch.cuda.is_available():

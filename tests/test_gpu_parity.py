@@ -143,9 +143,13 @@ def test_ragged_shapes(twq, oracle, M, K, N, r, G):
     (25, 2048, 2064, 128, 128),  # ragged second token tile, N = 258 tiles over the grid
     (2, 256, 8192, 16, 128),     # many tiles per CTA; smallest rank
     (4, 128, 16, 256, 128),      # one K-group, two tiles, rank 256 with most cluster ranks holding no K slab
+    (33, 512, 272, 256, 64),     # four 16-token MMA tiles, the third almost empty, the fourth empty; rank 256
+    (64, 2048, 1040, 128, 128),  # four full token tiles
+    (50, 1024, 4112, 48, 128),   # ragged fourth token tile, many tiles per CTA
+    (40, 640, 16, 0, 128),       # rank 0 with four token tiles
 ])
 def test_decode_kernel_shapes(twq, oracle, M, K, N, r, G):
-    """M <= 32 takes the bulk-copy streaming kernel (decode_kernel.cu); same bar as every other shape."""
+    """M <= 64 takes the bulk-copy streaming kernel (decode_kernel.cu); same bar as every other shape."""
     assert twq.testing_describe_plan(M, N, K, r, G)["kernel"] == "decode"
     assert twq.workspace_bytes(M, N, K, r, G) == 0
     _check_layer(twq, oracle, gen.make_layer(M, K, N, r, G, seed=2000 + M + N, with_tinv=(M % 2 == 1)))
@@ -202,7 +206,8 @@ def test_fused_kernel_store_paths(twq, oracle, plan_flags, pad, split, N):
 @pytest.mark.parametrize("M,flags,kernel,pair,split", [
     (5, 0, "decode", 0, False),           # small-batch kernel, one token tile
     (24, 0, "decode", 0, False),          # small-batch kernel, two token tiles
-    (40, 0, "tcgen05", 0, True),          # tcgen05 kernel, split-K path
+    (40, 0, "decode", 0, False),          # small-batch kernel, four token tiles
+    (72, 0, "tcgen05", 0, True),          # tcgen05 kernel, split-K path
     (300, 1, "tcgen05", 1, False),        # tcgen05 kernel, CTA pairs (PLAN_NO_SPLIT)
     (24, 16, "tcgen05", 0, True),         # small batch forced onto the tcgen05 kernel (PLAN_NO_DECODE)
 ])
@@ -231,7 +236,7 @@ def test_rank0_is_plain_w4a4_and_zero_residual_is_lowrank(twq, oracle, plan_flag
     assert np.abs(Y - ref).max() / np.abs(ref).max() <= 1e-3
 
 
-@pytest.mark.parametrize("M,flags", [(7, 0), (20, 0), (40, 0), (300, 1)])
+@pytest.mark.parametrize("M,flags", [(7, 0), (20, 0), (40, 0), (72, 0), (300, 1)])
 def test_lowrank_fp16_rewrite_saturates_as_documented(twq, oracle, plan_flags, M, flags):
     """include/twq.h: the low-rank branch rewrites X (BF16) to FP16 on chip -- exact in [2^-14, 65504], saturating
     above.  With R = 0 the output is that branch alone: it must equal the FP64 product of the CLAMPED activations
@@ -299,7 +304,8 @@ def test_exactly_representable_output_is_bit_exact(twq, oracle):
 
 
 @pytest.mark.parametrize("cs", [1, 2, 4, 8, 16])
-@pytest.mark.parametrize("M,K,N,r,G", [(1, 4096, 1024, 128, 128), (16, 2048, 2048, 256, 128), (20, 1024, 528, 64, 64)])
+@pytest.mark.parametrize("M,K,N,r,G", [(1, 4096, 1024, 128, 128), (16, 2048, 2048, 256, 128), (20, 1024, 528, 64, 64),
+                                       (56, 512, 528, 128, 128)])
 def test_decode_kernel_every_cluster_size(twq, oracle, plan_flags, cs, M, K, N, r, G):
     """decode_kernel.cu shares H = X*L1 inside a thread-block cluster: every cluster size the planner can pick
     (16 on an idle B200) gives the same Y within the tolerance, repeatably, with no workspace."""
@@ -340,7 +346,7 @@ def test_decode_kernel_strides_fp16_output_no_workspace(twq, oracle):
 
 def test_strides_fp16_output_and_workspace_reuse(twq, oracle):
     import torch
-    L = gen.make_layer(40, 512, 256, 32, 128, seed=41)
+    L = gen.make_layer(72, 512, 256, 32, 128, seed=41)
     X, packed, _ = _upload(twq, L)
     Xq, sx = twq.quantize_act(X, L.G)
     need = twq.workspace_bytes(L.M, L.N, L.K, L.r, L.G)
@@ -362,7 +368,7 @@ def test_strides_fp16_output_and_workspace_reuse(twq, oracle):
 
 def test_errors_are_reported_not_thrown_by_cuda(twq):
     import torch
-    L = gen.make_layer(40, 256, 128, 0, 128, seed=5)
+    L = gen.make_layer(72, 256, 128, 0, 128, seed=5)
     X, packed, _ = _upload(twq, L)
     Xq, sx = twq.quantize_act(X, L.G)
     with pytest.raises(twq.TwqError):
@@ -417,7 +423,7 @@ def test_config4_qwen(twq, oracle, which, M, nrows):
 
 @pytest.mark.parametrize("which,M,nrows", [
     ("q", 1, None), ("k", 8, None), ("down", 16, None), ("gate_up", 2, None), ("o", 4, None), ("v", 16, None),
-    ("v", 32, None),                                             # M = 32: two token tiles of the small-batch kernel
+    ("v", 32, None), ("k", 64, None),                            # M = 32 / 64: two / four token tiles of the small-batch kernel
     ("o", 2048, 24), ("down", 2048, 16), ("gate_up", 2048, 24),  # prefill on the square, the deep and the wide layer
     ("q", 8192, 24), ("gate_up", 8192, 16),                      # the top of the "M = 1..8192" sweep
 ])
