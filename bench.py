@@ -152,6 +152,8 @@ class GpuLayer:
         self.Y = [torch.empty((L.M, L.N), dtype=torch.bfloat16, device=dev) for _ in range(self.ncopies)]
         need = twq.workspace_bytes(L.M, L.N, L.K, L.r, L.G)
         self.ws = torch.zeros(max(need, 256), dtype=torch.uint8, device=dev) if need else None
+        need_x = twq.workspace_bytes_x(L.M, L.N, L.K, L.r, L.G)
+        self.ws_x = torch.zeros(max(need_x, 256), dtype=torch.uint8, device=dev) if need_x else None
         self.Yh = torch.empty((L.M, L.N), dtype=torch.bfloat16).pin_memory()
         self.lap_bytes = per_copy * self.ncopies
         del Rq, sw, L1, L2
@@ -165,13 +167,18 @@ class GpuLayer:
             self.twq.dual_linear(self.X[c], self.Xq[c], self.sx[c], self.packed[c], self.twq.OUT_BF16, Y=self.Y[c],
                                  ws=self.ws)
 
+    def step_x(self, i):
+        """The whole hot path through twq_dual_linear_x (one launch for M <= 64 where the plan fits)."""
+        c = i % self.ncopies
+        self.twq.dual_linear_x(self.X[c], self.packed[c], None, self.twq.OUT_BF16, Y=self.Y[c], ws=self.ws_x)
+
     def e2e_step(self, i):
         c = i % self.ncopies
         self.X[c].copy_(self.Xh, non_blocking=True)
         self.step(i)
         self.Yh.copy_(self.Y[c], non_blocking=True)
 
-    def time_graph(self, steps, warmup, quant=True, dual=True, replays=20):
+    def time_graph(self, steps, warmup, quant=True, dual=True, replays=20, fused=False):
         """Device time per step of a CUDA graph holding `steps` consecutive steps (no host launch gaps), over
         `replays` timed replays of the graph: returns (median, min) in us per step (SURVEY.md 8d protocol)."""
         torch = self.torch
@@ -180,11 +187,16 @@ class GpuLayer:
         with torch.cuda.stream(s):
             for i in range(max(warmup, self.ncopies)):           # every Xq/sx copy is valid before dual-only timing
                 self.step(i, True, True)
+                if fused:
+                    self.step_x(i)
             s.synchronize()
             g = torch.cuda.CUDAGraph()
             with torch.cuda.graph(g, stream=s):
                 for i in range(steps):
-                    self.step(i, quant, dual)
+                    if fused:
+                        self.step_x(i)
+                    else:
+                        self.step(i, quant, dual)
             g.replay()                                            # one untimed replay (graph upload)
             s.synchronize()
             ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(replays)]
@@ -270,11 +282,12 @@ def measure_workload(name, twq, torch, steps, warmup, peaks, with_e2e=False, wit
     us_step, us_step_min = gl.time_graph(steps, warmup, True, True)
     us_dual, us_dual_min = gl.time_graph(steps, warmup, False, True)
     us_quant, us_quant_min = gl.time_graph(steps, warmup, True, False)
+    us_x, us_x_min = gl.time_graph(steps, warmup, fused=True)   # the same step through twq_dual_linear_x
     ops_i8, fl_lr = twq.flops(L.M, L.N, L.K, L.r)
     traffic, traffic_src = load_traffic(name)
     out = dict(workload=name, M=L.M, N=L.N, K=L.K, r=L.r, G=L.G, us_step=round(us_step, 3),
-               us_dual_linear=round(us_dual, 3), us_quantize_act=round(us_quant, 3),
-               us_min=dict(step=round(us_step_min, 3), dual_linear=round(us_dual_min, 3), quantize_act=round(us_quant_min, 3)),
+               us_dual_linear=round(us_dual, 3), us_quantize_act=round(us_quant, 3), us_step_dual_linear_x=round(us_x, 3),
+               us_min=dict(step=round(us_step_min, 3), step_dual_linear_x=round(us_x_min, 3), dual_linear=round(us_dual_min, 3), quantize_act=round(us_quant_min, 3)),
                timing="median of 20 replays of a CUDA graph of %d steps (min alongside)" % steps,
                eff_tops=round((ops_i8 + fl_lr) / (us_dual * 1e-6) / 1e12, 2),
                gbs=round(twq.algorithmic_bytes(L.M, L.N, L.K, L.r, L.G) / (us_dual * 1e-6) / 1e9, 1),

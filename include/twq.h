@@ -145,7 +145,30 @@ twq_status twq_dual_linear(const void* X, int ldx, const uint8_t* Xq, const floa
                            void* Y, twq_out_dtype ydt, int ldy,
                            void* ws, size_t ws_bytes, int32_t* dbg_P, void* stream);
 
-/* Number of kernel launches the last successful twq_dual_linear / twq_quantize_act /
+/* ---------------------------------------------------------------------------
+ * twq_dual_linear_x -- the whole hot path (steps a1-a7) from the raw activations: quantizer + fused layer.
+ * the kernel "quantizes the input activation tile once and reuses it for both components"; here the
+ * quantized tile is produced once per thread-block cluster and reused by every CTA and channel tile of the call.
+ *   M <= 64 (the small-batch kernel, when its shared-memory plan fits): ONE kernel launch; codes and scales never
+ *     leave the chip unless Xq_out / sx_out ask for a copy.  Same FP32 operation order as twq_quantize_act: the codes
+ *     and scales (and therefore P and Y) are bit-identical to the two-call path.
+ *   otherwise: twq_quantize_act followed by twq_dual_linear (two launches), the quantizer's outputs going to
+ *     Xq_out / sx_out if given, else to the front of the workspace.
+ *   X      [M,ldx] bf16     raw activations (required)
+ *   tinv   [K] fp32         diagonal of the activation-side transform, or NULL for identity
+ *   Xq_out [M,K/2] u8       NULL, or receives the packed codes;  sx_out [M,K/G] fp32: NULL, or receives the scales
+ *   ws, ws_bytes            at least twq_workspace_bytes_x(...) bytes, 256-byte aligned, zero-filled once (as for
+ *                           twq_dual_linear); 0 bytes for the one-launch shapes
+ * Other arguments, stream ordering and errors as for twq_dual_linear.
+ */
+size_t twq_workspace_bytes_x(int M, int N, int K, int r, int G);
+twq_status twq_dual_linear_x(const void* X, int ldx, const float* tinv, const void* packed,
+                             int M, int N, int K, int r, int G,
+                             void* Y, twq_out_dtype ydt, int ldy,
+                             void* ws, size_t ws_bytes, uint8_t* Xq_out, float* sx_out,
+                             int32_t* dbg_P, void* stream);
+
+/* Number of kernel launches the last successful twq_dual_linear(_x) / twq_quantize_act /
  * twq_pack_weights call on this thread issued (bench.py's gpu_launches accounting). */
 int twq_last_launch_count(void);
 

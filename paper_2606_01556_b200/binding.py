@@ -14,7 +14,7 @@ _STATUS = {0: "TWQ_OK", 1: "TWQ_ERR_INVALID_ARG", 2: "TWQ_ERR_UNSUPPORTED", 3: "
 _OUT_TORCH = {OUT_BF16: torch.bfloat16, OUT_FP16: torch.float16, OUT_FP32: torch.float32}
 
 EXPORTS = ("twq_status_string", "twq_packed_bytes", "twq_pack_weights", "twq_quantize_act",
-           "twq_workspace_bytes", "twq_dual_linear", "twq_last_launch_count")
+           "twq_workspace_bytes", "twq_dual_linear", "twq_workspace_bytes_x", "twq_dual_linear_x", "twq_last_launch_count")
 
 
 TESTING_EXPORTS = ("twq_testing_set_plan_flags", "twq_testing_get_plan_flags", "twq_testing_describe_plan",
@@ -69,6 +69,10 @@ def load_library(build_if_missing: bool = True):
     lib.twq_workspace_bytes.argtypes = [i, i, i, i, i]
     lib.twq_dual_linear.restype = i
     lib.twq_dual_linear.argtypes = [vp, i, vp, vp, vp, i, i, i, i, i, vp, i, i, vp, sz, vp, vp]
+    lib.twq_workspace_bytes_x.restype = sz
+    lib.twq_workspace_bytes_x.argtypes = [i, i, i, i, i]
+    lib.twq_dual_linear_x.restype = i
+    lib.twq_dual_linear_x.argtypes = [vp, i, vp, vp, i, i, i, i, i, vp, i, i, vp, sz, vp, vp, vp, vp]
     lib.twq_last_launch_count.restype = i
     lib.twq_last_launch_count.argtypes = []
     # testing hooks (include/twq_testing.h): not part of the product ABI
@@ -214,6 +218,28 @@ def dual_linear(X, Xq, sx, packed: PackedLayer, out_dtype: int = OUT_BF16, Y=Non
                                           M, N, K, r, G, _ptr(Y), out_dtype, Y.stride(0), _ptr(ws),
                                           0 if ws is None else ws.numel(), _ptr(dbg_P), _stream(stream))
     _check(code, "twq_dual_linear")
+    return Y
+
+
+def workspace_bytes_x(M: int, N: int, K: int, r: int, G: int) -> int:
+    return int(load_library().twq_workspace_bytes_x(M, N, K, r, G))
+
+
+def dual_linear_x(X, packed: PackedLayer, tinv=None, out_dtype: int = OUT_BF16, Y=None, ws=None, Xq_out=None,
+                  sx_out=None, dbg_P=None, stream=None):
+    """twq_dual_linear_x: the whole hot path from raw activations (one launch for M <= 64 where the plan fits)."""
+    M = X.shape[0]
+    N, K, r, G = packed.N, packed.K, packed.r, packed.G
+    assert X.dtype == torch.bfloat16 and X.stride(1) == 1 and X.shape[1] == K
+    if Y is None:
+        Y = torch.empty((M, N), dtype=_OUT_TORCH.get(out_dtype, torch.bfloat16), device=X.device)
+    need = workspace_bytes_x(M, N, K, r, G)
+    if need and ws is None:
+        ws = _cached_workspace(need, X.device, stream)
+    code = load_library().twq_dual_linear_x(_ptr(X), X.stride(0), _ptr(tinv), _ptr(packed.blob), M, N, K, r, G,
+                                            _ptr(Y), out_dtype, Y.stride(0), _ptr(ws), 0 if ws is None else ws.numel(),
+                                            _ptr(Xq_out), _ptr(sx_out), _ptr(dbg_P), _stream(stream))
+    _check(code, "twq_dual_linear_x")
     return Y
 
 

@@ -55,7 +55,7 @@ constexpr int kJT = 8;                              // 8-wide j tiles of H one l
 constexpr int kDecSmemMax = 232448 - 1024;
 
 enum : int { D_FULL = 0, D_EMPTY = D_FULL + kMaxSlots, D_L1FULL = D_EMPTY + kMaxSlots, D_L1EMPTY = D_L1FULL + kMaxL1Slots,
-             D_X1 = D_L1EMPTY + kMaxL1Slots, D_X2, D_COUNT };
+             D_X1 = D_L1EMPTY + kMaxL1Slots, D_X2, D_XQ, D_COUNT };
 
 __device__ __forceinline__ uint32_t d_lo16(uint32_t w) { return (w << 4) & 0xF0F0F0F0u; }  // 16*code, even k
 __device__ __forceinline__ uint32_t d_hi16(uint32_t w) { return w & 0xF0F0F0F0u; }         // 16*code, odd k
@@ -127,6 +127,9 @@ __device__ __forceinline__ float ld_dsmem_f(uint32_t cluster_addr) {
 __device__ __forceinline__ void st_dsmem_u16(uint32_t cluster_addr, uint16_t v) {
     asm volatile("st.shared::cluster.u16 [%0], %1;" ::"r"(cluster_addr), "h"(v) : "memory");
 }
+__device__ __forceinline__ void st_dsmem_u32(uint32_t cluster_addr, uint32_t v) {
+    asm volatile("st.shared::cluster.u32 [%0], %1;" ::"r"(cluster_addr), "r"(v) : "memory");
+}
 __device__ __forceinline__ void cluster_arrive_relaxed() { asm volatile("barrier.cluster.arrive.relaxed.aligned;" ::: "memory"); }
 __device__ __forceinline__ void cluster_wait() { asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory"); }
 
@@ -143,7 +146,9 @@ __device__ __forceinline__ void lds_words(uint32_t (&dst)[kW], uint32_t a) {
 
 }  // namespace
 
-template <int G, int MT, bool kDbg>
+// kQ: the activation quantizer (steps a1-a2) runs inside this kernel: every cluster rank quantizes 1/cs of the K-groups of
+// all tokens and the cluster all-gathers codes and scales through distributed shared memory (twq_dual_linear_x).
+template <int G, int MT, bool kDbg, bool kQ>
 __global__ void __launch_bounds__(kDecThreads, 1)
 decode_dual_linear_kernel(const __grid_constant__ CUtensorMap tmXq, const __grid_constant__ DecodeParams p) {
     extern __shared__ uint8_t dsm_raw[];
@@ -200,6 +205,7 @@ decode_dual_linear_kernel(const __grid_constant__ CUtensorMap tmXq, const __grid
         for (int i = 0; i < kMaxL1Slots; ++i) { mbar_init(&bars[D_L1FULL + i], 1); mbar_init(&bars[D_L1EMPTY + i], lrw > 0 ? lrw : 1); }
         mbar_init(&bars[D_X1], cs);
         mbar_init(&bars[D_X2], cs);
+        mbar_init(&bars[D_XQ], cs);
         fence_mbar_init();
     }
     __syncthreads();
@@ -230,7 +236,7 @@ decode_dual_linear_kernel(const __grid_constant__ CUtensorMap tmXq, const __grid
         __syncwarp();
         const uint32_t ring = smem_u32(dsm + p.off_ring);
         const uint8_t* src0 = p.R4 + static_cast<size_t>(tile0) * ng * kBlk;
-        const uint32_t xq_bytes = static_cast<uint32_t>(p.gc) * kMp * (G / 2);   // a full box, zero-filled beyond M / ng
+        const uint32_t xq_bytes = kQ ? 0u : static_cast<uint32_t>(p.gc) * kMp * (G / 2);   // a full box, zero-filled beyond M / ng
         const uint32_t sw_bytes = static_cast<uint32_t>(ntile) * ng * 16;        // this CTA's FP16 group scales
         const int first = ntile > 0 ? min(p.nslots, p.nchunks) : 0;
         auto arm = [&](int c, int slot) {
@@ -284,7 +290,7 @@ decode_dual_linear_kernel(const __grid_constant__ CUtensorMap tmXq, const __grid
                         if (lane == 0) arm(c, slot);
                         __syncwarp();
                         for (int t = lane; t < ntile; t += 32) copy_w(c, slot, t);
-                        if (lane == 31) tma_load_3d_a(ring + slot * p.slot_bytes + p.xq_off, &tmXq, DBAR(D_FULL + slot), 0, c * p.gc, 0);
+                        if (!kQ && lane == 31) tma_load_3d_a(ring + slot * p.slot_bytes + p.xq_off, &tmXq, DBAR(D_FULL + slot), 0, c * p.gc, 0);
                         ++c;
                         if (++slot == p.nslots) { slot = 0; ++lap; }
                     }
@@ -299,7 +305,7 @@ decode_dual_linear_kernel(const __grid_constant__ CUtensorMap tmXq, const __grid
         // as the previous kernel is done and land first.
         named_bar_sync(3, 64);                                   // the chunk barriers are armed
         pdl_wait();
-        const int first = ntile > 0 ? min(p.nslots, p.nchunks) : 0;
+        const int first = (!kQ && ntile > 0) ? min(p.nslots, p.nchunks) : 0;
         if (lane < first)
             tma_load_3d_a(smem_u32(dsm + p.off_ring) + lane * p.slot_bytes + p.xq_off, &tmXq, DBAR(D_FULL + lane), 0,
                           lane * p.gc, 0);
@@ -511,13 +517,89 @@ decode_dual_linear_kernel(const __grid_constant__ CUtensorMap tmXq, const __grid
         const int tg = rw / P, part = rw - tg * P;
         const int t_lo = tg * tpg;                               // this warp's tiles: [t_lo, t_lo + ntw)
         const int ntw = tg < TG ? min(tpg, ntile - t_lo) : 0;
-        pdl_wait();                                              // sx comes from twq_quantize_act
+        pdl_wait();                                              // sx (or X) comes from the previous kernel of the stream
         TWQ_DSTAMP(2);
-        for (int i = rw * 32 + lane; i < kMp * ng; i += nrw * 32) {
-            const int g = i / kMp, m = i - g * kMp;
-            sSx[i] = m < p.M ? ldg_f32(p.sx + static_cast<size_t>(m) * ng + g) * 0x1p-8f : 0.0f;   // MMA operands are 16*code
+        if constexpr (kQ) {
+            // ---- steps a1-a2 inside the kernel (Eq. 1; the FP32 operation order of
+            // include/twq.h, bit for bit the codes and scales twq_quantize_act writes).  Cluster rank q quantizes the
+            // K-groups [ng*q/cs, ng*(q+1)/cs) of every token and stores codes and scales into EVERY peer's shared memory
+            // ([g][token][G/2], the layout the MMA fragments read without bank conflicts): the activation tile is
+            // quantized once per cluster and reused by all its CTAs and tiles (L179).
+            uint8_t* sXq = dsm + p.off_xq;
+            constexpr int kLPI = G / 8;                          // lanes per (token, group): 8 elements each
+            constexpr int kIPW = 32 / kLPI;                      // (token, group) items per warp pass
+            // rows beyond M are written by nobody: codes 0, scale 0
+            for (int i = rw * 32 + lane; i < ng * kMp * (G / 8); i += nrw * 32)
+                if ((i / (G / 8)) % kMp >= p.M) reinterpret_cast<uint32_t*>(sXq)[i] = 0u;
+            for (int i = rw * 32 + lane; i < ng * kMp; i += nrw * 32)
+                if (i % kMp >= p.M) sSx[i] = 0.0f;
+            const int gq0 = static_cast<int>(static_cast<unsigned>(ng) * rank / cs);
+            const int ngq = static_cast<int>(static_cast<unsigned>(ng) * (rank + 1) / cs) - gq0;
+            const int items = p.M * ngq;
+            const int li = lane % kLPI, sub = lane / kLPI;
+            const uint16_t* X = static_cast<const uint16_t*>(p.X);
+            if (cs > 1) cluster_wait();                          // every CTA of the cluster is running (its shared memory exists)
+            for (int base = rw * kIPW; base < items; base += nrw * kIPW) {
+                const int it = base + sub;
+                const bool on = it < items;                      // whole items are on or off: the shuffles below stay inside one
+                const int m = on ? it / ngq : 0, g = gq0 + (on ? it - (it / ngq) * ngq : 0);
+                float x[8];
+#pragma unroll
+                for (int i = 0; i < 8; ++i) x[i] = 0.0f;
+                if (on) {
+                    const uint4 v = ldg_v4(X + static_cast<size_t>(m) * p.ldx + g * G + li * 8);
+                    const uint32_t w[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+                    for (int i = 0; i < 4; ++i) {
+                        x[2 * i] = __uint_as_float(w[i] << 16);              // BF16 -> FP32, exact
+                        x[2 * i + 1] = __uint_as_float(w[i] & 0xFFFF0000u);
+                    }
+                    if (p.tinv != nullptr) {
+                        const float4 t0 = __ldg(reinterpret_cast<const float4*>(p.tinv + g * G + li * 8));
+                        const float4 t1 = __ldg(reinterpret_cast<const float4*>(p.tinv + g * G + li * 8) + 1);
+                        x[0] = __fmul_rn(x[0], t0.x); x[1] = __fmul_rn(x[1], t0.y); x[2] = __fmul_rn(x[2], t0.z); x[3] = __fmul_rn(x[3], t0.w);
+                        x[4] = __fmul_rn(x[4], t1.x); x[5] = __fmul_rn(x[5], t1.y); x[6] = __fmul_rn(x[6], t1.z); x[7] = __fmul_rn(x[7], t1.w);
+                    }
+                }
+                float amax = 0.0f;
+#pragma unroll
+                for (int i = 0; i < 8; ++i) amax = fmaxf(amax, fabsf(x[i]));
+#pragma unroll
+                for (int d = kLPI / 2; d >= 1; d >>= 1) amax = fmaxf(amax, __shfl_xor_sync(0xffffffffu, amax, d));
+                const float sc = __fdiv_rn(fmaxf(amax, 0x1p-30f), 7.0f);
+                const float inv = __fdiv_rn(1.0f, sc);
+                uint32_t pk = 0u;
+#pragma unroll
+                for (int i = 0; i < 8; ++i) {
+                    int q = __float2int_rn(__fmul_rn(x[i], inv));            // round-half-to-even
+                    q = max(-7, min(7, q));
+                    pk |= (static_cast<uint32_t>(q) & 0xFu) << (4 * i);      // low nibble = even k
+                }
+                if (on) {
+                    const uint32_t qa = smem_u32(sXq + (g * kMp + m) * (G / 2) + li * 4);
+                    for (int pr = 0; pr < cs; ++pr) st_dsmem_u32(mapa_u32(qa, pr), pk);
+                    if (li == 0) {
+                        const uint32_t sa = smem_u32(sSx + g * kMp + m);
+                        const uint32_t sv = __float_as_uint(sc * 0x1p-8f);   // MMA operands are 16*code
+                        for (int pr = 0; pr < cs; ++pr) st_dsmem_u32(mapa_u32(sa, pr), sv);
+                        if (p.sx_out != nullptr) p.sx_out[static_cast<size_t>(m) * ng + g] = sc;
+                    }
+                    if (p.xq_out != nullptr)
+                        *reinterpret_cast<uint32_t*>(p.xq_out + static_cast<size_t>(m) * (p.K >> 1) + g * (G / 2) + li * 4) = pk;
+                }
+            }
+            named_bar_sync(2, nrw * 32);                         // this CTA's share is stored (everywhere)
+            if (cs > 1) {
+                if (rw == 0 && lane < cs) mbar_arrive_remote(mapa_u32(DBAR(D_XQ), static_cast<uint32_t>(lane)));
+                mbar_wait_cluster_a(DBAR(D_XQ), 0);              // every rank's share has arrived here
+            }
+        } else {
+            for (int i = rw * 32 + lane; i < kMp * ng; i += nrw * 32) {
+                const int g = i / kMp, m = i - g * kMp;
+                sSx[i] = m < p.M ? ldg_f32(p.sx + static_cast<size_t>(m) * ng + g) * 0x1p-8f : 0.0f;   // MMA operands are 16*code
+            }
+            named_bar_sync(2, nrw * 32);
         }
-        named_bar_sync(2, nrw * 32);
         TWQ_DSTAMP(3);
         if (ntile > 0) {
             // The loop is issue-bound (ncu r02a: 38 K warp instructions per CTA, most of them address arithmetic), so
@@ -526,8 +608,10 @@ decode_dual_linear_kernel(const __grid_constant__ CUtensorMap tmXq, const __grid
             const uint32_t ring = smem_u32(dsm + p.off_ring);
             const uint32_t tstride = static_cast<uint32_t>(p.gc) * kBlk;          // bytes between tiles inside a slot
             const uint32_t lane_w = ring + t_lo * tstride + gid * (G / 2) + tid4 * (kW * 4);
-            const uint32_t lane_x = ring + p.xq_off + (gid * p.gc) * (G / 2) + tid4 * (kW * 4);
-            const uint32_t x8 = 8u * p.gc * (G / 2);                              // token gid -> gid + 8 inside the Xq box
+            // activation codes: the Xq box of the ring slot ([token][gc][G/2]), or the resident tile the in-kernel quantizer fills ([g][token][G/2])
+            const uint32_t lane_x = kQ ? smem_u32(dsm + p.off_xq) + gid * (G / 2) + tid4 * (kW * 4)
+                                       : ring + p.xq_off + (gid * p.gc) * (G / 2) + tid4 * (kW * 4);
+            const uint32_t x8 = kQ ? 8u * (G / 2) : 8u * p.gc * (G / 2);          // token gid -> gid + 8
             const uint32_t sw_a = smem_u32(dsm + p.off_sw) + tid4 * 4 + static_cast<uint32_t>(t_lo) * ng * 16;
             const uint32_t sx_a = smem_u32(sSx) + gid * 4;
             // The warp's tiles are worked in batches of kTB interleaved MMA chains; with more than kTB tiles they are split
@@ -542,7 +626,7 @@ decode_dual_linear_kernel(const __grid_constant__ CUtensorMap tmXq, const __grid
                 toff[i] = ii * tstride;
                 swoff[i] = static_cast<uint32_t>(ii) * ng * 16;
             }
-            const uint32_t step_w = P * kBlk, step_x = P * (G / 2), step_sx = P * kMp * 4, step_sw = P * 16;
+            const uint32_t step_w = P * kBlk, step_x = kQ ? P * kMp * (G / 2) : P * (G / 2), step_sx = P * kMp * 4, step_sw = P * 16;
             float acc[kTPW][MT][4];
 #pragma unroll
             for (int i = 0; i < kTPW; ++i)
@@ -561,7 +645,7 @@ decode_dual_linear_kernel(const __grid_constant__ CUtensorMap tmXq, const __grid
                 const int gcnt = min(p.gc, ng - c * p.gc);
                 if (ntw > 0) {
                     uint32_t wa = lane_w + slot_a + gl * kBlk;
-                    uint32_t xa = lane_x + slot_a + gl * (G / 2);
+                    uint32_t xa = kQ ? lane_x + g * (kMp * (G / 2)) : lane_x + slot_a + gl * (G / 2);
                     uint32_t sxp = sx_a + g * (kMp * 4);
                     uint32_t swp = sw_a + g * 16;
 #pragma unroll 1
@@ -785,7 +869,7 @@ decode_dual_linear_kernel(const __grid_constant__ CUtensorMap tmXq, const __grid
         }
     }
     TWQ_DSTAMP(29);
-    if (cs > 1 && !is_lr) cluster_wait();   // completes this thread's half of the split barrier (long since released)
+    if (cs > 1 && !is_lr && !(kQ && warp < nrw)) cluster_wait();   // completes this thread's half of the split barrier (long since released)
 #undef DBAR
 }
 
@@ -794,9 +878,9 @@ namespace {
 
 constexpr int kMaxDevices = 64;
 
-template <int G, int MT, bool kDbg>
+template <int G, int MT, bool kDbg, bool kQ>
 cudaError_t decode_launch_inst(const CUtensorMap& tmXq, const DecodeParams& p, cudaStream_t stream) {
-    auto kern = decode_dual_linear_kernel<G, MT, kDbg>;
+    auto kern = decode_dual_linear_kernel<G, MT, kDbg, kQ>;
     static bool attr_done[kMaxDevices] = {};       // function attributes are per device
     int dev = 0;
     cudaError_t e = cudaGetDevice(&dev);
@@ -840,7 +924,7 @@ int decode_cluster_capacity(int cs, int num_sms) {
     if (cache[dev][cs] > 0) return cache[dev][cs];
     int n = 0;
     if (have_dev) {
-        auto kern = decode_dual_linear_kernel<128, 1, false>;
+        auto kern = decode_dual_linear_kernel<128, 1, false, false>;
         if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, kDecSmemMax) == cudaSuccess &&
             cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1) == cudaSuccess) {
             cudaLaunchConfig_t cfg = {};
@@ -870,7 +954,7 @@ int round_up_i(int x, int a) { return (x + a - 1) / a * a; }
 }  // namespace
 
 // Fills the decode plan; false when the shape is outside this kernel's domain (the tcgen05 kernel takes it).
-bool decode_make_plan(int M, int N, int K, int r, int G, int num_sms, DecodeParams* out) {
+bool decode_make_plan(int M, int N, int K, int r, int G, int num_sms, bool quant, DecodeParams* out) {
     if (M < 1 || M > kDecodeMaxM || (G != 64 && G != 128) || K % G != 0 || N % 16 != 0 || r % 16 != 0 || r > 256) return false;
     if (plan_flags() & kPlanNoDecode) return false;
     DecodeParams p = {};
@@ -883,12 +967,13 @@ bool decode_make_plan(int M, int N, int K, int r, int G, int num_sms, DecodePara
     // cluster size: H is shared by the cluster and every cluster streams all of L1 (K*r*2 bytes) from L2, so the
     // largest cluster that still covers 70 % of the SMs wins; otherwise the size covering the most SMs
     p.cs = 1;
+    p.quant = quant ? 1 : 0;
     int cap = num_sms;
-    if (r > 0) {
+    if (r > 0 || quant) {                                     // the in-kernel quantizer shares its work across the cluster too
         int best = 0;
         bool done = false;
         for (int c = 16; c >= 1 && !done; c >>= 1) {
-            if (r % c != 0) continue;
+            if (r % c != 0) continue;                         // (r == 0 divides everything)
             const int n = decode_cluster_capacity(c, num_sms);
             if (n * c > best) { best = n * c; p.cs = c; cap = n; }
             if (n * c * 10 >= num_sms * 7) done = true;
@@ -916,6 +1001,7 @@ bool decode_make_plan(int M, int N, int K, int r, int G, int num_sms, DecodePara
     p.off_bar = o; o += round_up_i(D_COUNT * 8, 128);
     p.off_sw = o; o += round_up_i(p.tmax * p.ng * 16, 128);
     p.off_sx = o; o += round_up_i(p.ng * p.mp * 4, 128);
+    p.off_xq = o; o += quant ? round_up_i(p.ng * p.mp * (G / 2), 128) : 0;   // resident codes [g][token][G/2] of the in-kernel quantizer
     p.off_ylr = o; o += r > 0 ? round_up_i(p.mp * p.tmax * 8 * 4, 128) : 0;
     p.off_hpart = o; o += r > 0 ? round_up_i(p.mp * r * 4, 128) : 0;
     p.off_h = o; o += r > 0 ? round_up_i(p.mp * (r + 8) * 2, 128) : 0;
@@ -939,7 +1025,7 @@ bool decode_make_plan(int M, int N, int K, int r, int G, int num_sms, DecodePara
     // residual ring: chunk = gc K-groups of every tile of the CTA + the same groups of Xq for all (padded) tokens.
     // About four chunks per call where everything fits (consumers start on the first quarter, the tail after the last
     // byte is a quarter of the work), at most ~40 KB per slot otherwise.
-    const int per_g = p.tmax * kBlk + p.mp * (G / 2);
+    const int per_g = p.tmax * kBlk + (quant ? 0 : p.mp * (G / 2));
     const int budget = kDecSmemMax - 1024 - o;
     p.gc = (p.ng + 3) / 4;
     while (p.gc > 1 && p.gc * per_g > 40 * 1024) p.gc = (p.gc + 1) / 2;
@@ -968,7 +1054,10 @@ bool decode_make_plan(int M, int N, int K, int r, int G, int num_sms, DecodePara
 cudaError_t launch_decode(const CUtensorMap& tmXq, const DecodeParams& p, int G, cudaStream_t stream) {
     const bool dbg = p.dbgP != nullptr;
 #define TWQ_DCASE(g, m)                                                                   \
-    if (G == g && p.mt == m) return dbg ? decode_launch_inst<g, m, true>(tmXq, p, stream) : decode_launch_inst<g, m, false>(tmXq, p, stream);
+    if (G == g && p.mt == m) {                                                            \
+        if (p.quant) return dbg ? decode_launch_inst<g, m, true, true>(tmXq, p, stream) : decode_launch_inst<g, m, false, true>(tmXq, p, stream); \
+        return dbg ? decode_launch_inst<g, m, true, false>(tmXq, p, stream) : decode_launch_inst<g, m, false, false>(tmXq, p, stream);        \
+    }
     TWQ_DCASE(128, 1) TWQ_DCASE(128, 2) TWQ_DCASE(128, 4) TWQ_DCASE(64, 1) TWQ_DCASE(64, 2) TWQ_DCASE(64, 4)
 #undef TWQ_DCASE
     return cudaErrorInvalidValue;

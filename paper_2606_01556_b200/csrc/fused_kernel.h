@@ -61,7 +61,11 @@ struct DecodeParams {
     int nu_max;              // most K slabs of stage 1 any CTA multiplies
     int xs_stride;           // halves per token row of the staged FP16 X slice
     int xrows;               // token rows staged (8 when M <= 8, else mp)
-    int off_ring, off_l1, off_sw, off_xs, off_hpart, off_h, off_ylr, off_sx, off_res, off_bar, smem_bytes;
+    int off_ring, off_l1, off_sw, off_xs, off_hpart, off_h, off_ylr, off_sx, off_xq, off_res, off_bar, smem_bytes;
+    int quant;               // 1: the activation quantizer runs inside the kernel (twq_dual_linear_x)
+    const float* tinv;       // quant: [K] diagonal transform or NULL
+    uint8_t* xq_out;         // quant: NULL, or [M][K/2] copy of the codes (parity evidence)
+    float* sx_out;           // quant: NULL, or [M][K/G] copy of the scales
     const uint8_t* R4;       // [N/8][ng][8][G/2]
     const __half* sw16;      // [N/8][ng][8]
     const void* L1D;         // [K/32][r][32] f16
@@ -72,7 +76,7 @@ struct DecodeParams {
     int32_t* dbgP;
     unsigned long long* trace;   // NULL, or the timeline buffer of a -DTWQ_TRACE build (trace.cuh)
 };
-bool decode_make_plan(int M, int N, int K, int r, int G, int num_sms, DecodeParams* out);
+bool decode_make_plan(int M, int N, int K, int r, int G, int num_sms, bool quant, DecodeParams* out);
 cudaError_t launch_decode(const CUtensorMap& tmXq, const DecodeParams& p, int G, cudaStream_t stream);
 
 // Planner overrides for tests (include/twq_testing.h, twq_testing_set_plan_flags): a process-wide word, never the

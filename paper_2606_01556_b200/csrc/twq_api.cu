@@ -92,13 +92,14 @@ size_t ctr_bytes(const twq::FusedPlan& pl) {
 struct CallPlan {
     int dev, M, N, K, r, G;
     unsigned flags;
+    bool quant;                // planned for twq_dual_linear_x (in-kernel quantizer): only small-batch plans exist
     bool valid, decode;
     twq::DecodeParams dp;      // decode == true
     twq::FusedPlan fp;         // decode == false
     size_t ws_bytes;
 };
 
-const CallPlan* get_plan(int M, int N, int K, int r, int G) {
+const CallPlan* get_plan(int M, int N, int K, int r, int G, bool quant = false) {
     constexpr int kSlots = 16;
     thread_local CallPlan cache[kSlots];
     thread_local unsigned next = 0;
@@ -106,14 +107,19 @@ const CallPlan* get_plan(int M, int N, int K, int r, int G) {
     const unsigned flags = twq::plan_flags();
     for (int i = 0; i < kSlots; ++i) {
         const CallPlan& c = cache[i];
-        if (c.valid && c.dev == dev && c.M == M && c.N == N && c.K == K && c.r == r && c.G == G && c.flags == flags) return &c;
+        if (c.valid && c.dev == dev && c.M == M && c.N == N && c.K == K && c.r == r && c.G == G && c.flags == flags &&
+            c.quant == quant)
+            return c.decode || !quant ? &c : nullptr;
     }
     CallPlan c;
     memset(&c, 0, sizeof(c));
-    c.dev = dev; c.M = M; c.N = N; c.K = K; c.r = r; c.G = G; c.flags = flags;
+    c.dev = dev; c.M = M; c.N = N; c.K = K; c.r = r; c.G = G; c.flags = flags; c.quant = quant;
     const int sms = num_sms();
-    if (twq::decode_make_plan(M, N, K, r, G, sms, &c.dp)) {
+    if (twq::decode_make_plan(M, N, K, r, G, sms, quant, &c.dp)) {
         c.decode = true;
+        c.ws_bytes = 0;
+    } else if (quant) {
+        c.decode = false;                                      // remembered: no one-launch plan for this shape
         c.ws_bytes = 0;
     } else {
         if (!twq::fused_make_plan(M, N, K, r, G, sms, &c.fp)) return nullptr;
@@ -123,7 +129,7 @@ const CallPlan* get_plan(int M, int N, int K, int r, int G) {
     c.valid = true;
     CallPlan& slot = cache[next++ % kSlots];
     slot = c;
-    return &slot;
+    return slot.decode || !quant ? &slot : nullptr;
 }
 
 // ------------------------------------------------------------------ TMA descriptors, cached by everything they encode
@@ -385,6 +391,64 @@ twq_status twq_dual_linear(const void* X, int ldx, const uint8_t* Xq, const floa
     p.ws_part = splits > 1 ? reinterpret_cast<float*>(static_cast<uint8_t*>(ws) + ctr_bytes(p.plan)) : nullptr;
     if (twq::launch_fused(maps, p, G, static_cast<cudaStream_t>(stream)) != cudaSuccess) return TWQ_ERR_CUDA;
     g_last_launches = 1;
+    return TWQ_OK;
+}
+
+// Scratch for twq_dual_linear_x: nothing where the one-launch plan exists, otherwise room for the quantizer's outputs
+// (codes, scales; each 256-byte aligned) in front of what twq_dual_linear itself needs.
+size_t twq_workspace_bytes_x(int M, int N, int K, int r, int G) {
+    if (!shape_ok(M, N, K, r, G)) return 0;
+    if (get_plan(M, N, K, r, G, true)) return 0;
+    return twq::align256(static_cast<size_t>(M) * (K / 2)) + twq::align256(static_cast<size_t>(M) * (K / G) * sizeof(float)) +
+           twq_workspace_bytes(M, N, K, r, G);
+}
+
+twq_status twq_dual_linear_x(const void* X, int ldx, const float* tinv, const void* packed, int M, int N, int K, int r,
+                             int G, void* Y, twq_out_dtype ydt, int ldy, void* ws, size_t ws_bytes, uint8_t* Xq_out,
+                             float* sx_out, int32_t* dbg_P, void* stream) {
+    g_last_launches = 0;
+    if (!shape_ok(M, N, K, r, G)) return TWQ_ERR_INVALID_ARG;
+    if (!X || !packed || !Y) return TWQ_ERR_INVALID_ARG;
+    if (ydt != TWQ_OUT_BF16 && ydt != TWQ_OUT_FP16 && ydt != TWQ_OUT_FP32) return TWQ_ERR_INVALID_ARG;
+    if (ldy < N || ldx < K || ldx % 8 != 0) return TWQ_ERR_INVALID_ARG;
+    if (!aligned16(X) || !aligned16(Y) || (tinv && !aligned16(tinv)) || (Xq_out && !aligned16(Xq_out)) ||
+        (sx_out && !aligned16(sx_out)) || (reinterpret_cast<uintptr_t>(packed) & 255u))
+        return TWQ_ERR_INVALID_ARG;
+    const size_t need = twq_workspace_bytes_x(M, N, K, r, G);
+    if (need > 0 && (!ws || ws_bytes < need)) return TWQ_ERR_WORKSPACE;
+    if (need > 0 && (reinterpret_cast<uintptr_t>(ws) & 255u)) return TWQ_ERR_INVALID_ARG;
+    if (!device_is_sm100()) return TWQ_ERR_UNSUPPORTED;
+    if (const CallPlan* cp = get_plan(M, N, K, r, G, true)) {
+        // small batches: quantizer, both branches and the epilogue in ONE launch
+        const twq::PackedLayout lay = twq::packed_layout(N, K, r, G);
+        const uint8_t* base = static_cast<const uint8_t*>(packed);
+        twq::DecodeParams dp = cp->dp;
+        dp.ldx = ldx; dp.ldy = ldy; dp.ydt = static_cast<int>(ydt);
+        dp.R4 = base + lay.off_r4;
+        dp.sw16 = reinterpret_cast<const __half*>(base + lay.off_sw16);
+        dp.L1D = base + lay.off_l1d;
+        dp.L2T = base + lay.off_l2t;
+        dp.X = X; dp.sx = nullptr; dp.Y = Y; dp.dbgP = dbg_P;
+        dp.tinv = tinv; dp.xq_out = Xq_out; dp.sx_out = sx_out;
+        dp.trace = twq::trace_buffer();
+        CUtensorMap none;
+        memset(&none, 0, sizeof(none));                       // the one-launch kernel issues no tensor-map copy
+        if (twq::launch_decode(none, dp, G, static_cast<cudaStream_t>(stream)) != cudaSuccess) return TWQ_ERR_CUDA;
+        g_last_launches = 1;
+        return TWQ_OK;
+    }
+    // larger batches: the stand-alone quantizer into the workspace (or the caller's buffers), then the fused layer
+    uint8_t* w = static_cast<uint8_t*>(ws);
+    uint8_t* xq = Xq_out ? Xq_out : w;
+    w += twq::align256(static_cast<size_t>(M) * (K / 2));
+    float* sx = sx_out ? sx_out : reinterpret_cast<float*>(w);
+    w += twq::align256(static_cast<size_t>(M) * (K / G) * sizeof(float));
+    const size_t used = static_cast<size_t>(w - static_cast<uint8_t*>(ws));
+    twq_status st = twq_quantize_act(X, M, K, ldx, tinv, G, xq, sx, stream);
+    if (st != TWQ_OK) return st;
+    st = twq_dual_linear(X, ldx, xq, sx, packed, M, N, K, r, G, Y, ydt, ldy, w, ws_bytes - used, dbg_P, stream);
+    if (st != TWQ_OK) return st;
+    g_last_launches = 2;
     return TWQ_OK;
 }
 

@@ -380,6 +380,73 @@ def test_errors_are_reported_not_thrown_by_cuda(twq):
     assert e.value.code == 3
 
 
+# ------------------------------------------------------------------------------ the whole hot path in one call
+@pytest.mark.parametrize("M,K,N,r,G,with_tinv", [
+    (1, 128, 16, 0, 128, False),      # smallest problem, rank 0 (no low-rank warps), one group
+    (3, 192, 48, 16, 64, True),       # G = 64, three groups over the cluster ranks (most ranks quantize nothing)
+    (8, 2048, 528, 48, 128, False),
+    (16, 4096, 4096, 128, 128, True), # configs[1] at the headline M, diagonal transform
+    (1, 4096, 4096, 128, 128, False),
+    (25, 2048, 2064, 128, 128, True), # two token tiles, ragged
+    (64, 2048, 1040, 128, 128, False),# four token tiles
+    (50, 1024, 4112, 0, 128, True),   # rank 0 with many tiles
+    (12, 8192, 1024, 256, 128, False),# configs[4] k / v shape
+])
+def test_dual_linear_x_one_launch(twq, oracle, M, K, N, r, G, with_tinv):
+    """twq_dual_linear_x at M <= 64: quantizer, both branches and the epilogue in ONE launch.  The codes and scales it
+    produces on chip (copied out through Xq_out / sx_out) and the integer accumulators are bit-identical to the oracle,
+    and Y is bit-identical to the two-call path wherever both use the same grid (same arithmetic, same order)."""
+    import torch
+    L = gen.make_layer(M, K, N, r, G, seed=7000 + M + N, with_tinv=with_tinv)
+    X, packed, tinv = _upload(twq, L)
+    assert twq.workspace_bytes_x(M, N, K, r, G) == 0
+    Xq_o = torch.full((M, K // 2), 0x55, dtype=torch.uint8, device="cuda")
+    sx_o = torch.full((M, K // G), -1.0, dtype=torch.float32, device="cuda")
+    dbg = torch.zeros((M, L.ng, N), dtype=torch.int32, device="cuda")
+    Y32 = twq.dual_linear_x(X, packed, tinv, twq.OUT_FP32, Xq_out=Xq_o, sx_out=sx_o, dbg_P=dbg)
+    assert twq.last_launch_count() == 1
+    Y16 = twq.dual_linear_x(X, packed, tinv, twq.OUT_BF16)
+    torch.cuda.synchronize()
+    ref = oracle.forward(L.X, L.Rq, L.sw, L.L1 if r else None, L.L2 if r else None, G, tinv=L.tinv, want_P=True)
+    assert (Xq_o.cpu().numpy() == ref["Xq"]).all(), "codes"
+    assert (sx_o.cpu().numpy() == ref["sx"]).all(), "scales"
+    assert (dbg.cpu().numpy().astype(np.int64) == ref["P"]).all(), "integer accumulators"
+    err = np.abs(Y32.cpu().numpy().astype(np.float64) - ref["Y"]).max() / np.abs(ref["Y"]).max()
+    assert err <= TOL, err
+    assert torch.equal(Y16.view(torch.int16), Y32.to(torch.bfloat16).view(torch.int16)), "BF16 != rne(Y32)"
+    Xq, sx = twq.quantize_act(X, G, tinv)
+    Y2 = twq.dual_linear(X, Xq, sx, packed, twq.OUT_FP32)
+    if r > 0:      # same grid, same K-parts, same order of every sum: bit-identical
+        assert torch.equal(Y2, Y32), "one-launch path differs from quantize_act + dual_linear"
+    else:          # rank 0: the one-launch call still runs clusters (they share the quantizer), the two-call path does not
+        assert (Y2 - Y32).abs().max().item() <= 1e-5 * float(np.abs(ref["Y"]).max())
+
+
+@pytest.mark.parametrize("M,K,N,r,G", [(80, 512, 384, 32, 128), (300, 1024, 1024, 128, 128)])
+def test_dual_linear_x_larger_batches_use_the_workspace(twq, oracle, M, K, N, r, G):
+    """Beyond the small-batch kernel twq_dual_linear_x runs the stand-alone quantizer into the workspace, then the fused
+    layer: two launches, same results; the caller's Xq_out / sx_out are used instead of the workspace when given."""
+    import torch
+    L = gen.make_layer(M, K, N, r, G, seed=7100 + M, with_tinv=True)
+    X, packed, tinv = _upload(twq, L)
+    need = twq.workspace_bytes_x(M, N, K, r, G)
+    assert need >= M * K // 2 + 4 * M * (K // G)
+    ws = torch.zeros(need, dtype=torch.uint8, device="cuda")
+    Y = twq.dual_linear_x(X, packed, tinv, twq.OUT_FP32, ws=ws)
+    assert twq.last_launch_count() == 2
+    sx_o = torch.empty((M, K // G), dtype=torch.float32, device="cuda")
+    Xq_o = torch.empty((M, K // 2), dtype=torch.uint8, device="cuda")
+    Yb = twq.dual_linear_x(X, packed, tinv, twq.OUT_FP32, ws=ws, Xq_out=Xq_o, sx_out=sx_o)
+    torch.cuda.synchronize()
+    ref = oracle.forward(L.X, L.Rq, L.sw, L.L1, L.L2, G, tinv=L.tinv)
+    assert (Xq_o.cpu().numpy() == ref["Xq"]).all() and (sx_o.cpu().numpy() == ref["sx"]).all()
+    assert torch.equal(Y, Yb)
+    assert np.abs(Y.cpu().numpy().astype(np.float64) - ref["Y"]).max() / np.abs(ref["Y"]).max() <= TOL
+    with pytest.raises(twq.TwqError) as e:
+        twq.dual_linear_x(X, packed, tinv, twq.OUT_FP32, ws=torch.zeros(256, dtype=torch.uint8, device="cuda"))
+    assert e.value.code == 3
+
+
 # ------------------------------------------------------------------------------ BASELINE.json configs
 @pytest.mark.parametrize("M", [1, 16, 128])
 def test_config2_qproj(twq, oracle, M):
