@@ -477,6 +477,9 @@ def main():
                     us_host_per_call=main_res.get("us_host_per_call"),
                     cpu_baseline=cpu,
                     us_dual_linear=main_res["us_dual_linear"], us_quantize_act=main_res["us_quantize_act"],
+                    # the same step through twq_dual_linear_x (one launch for M <= 64): reported beside `value`, which stays the
+                    # two-call step that BASELINE.json's subsystems name (twq_quantize_act + twq_dual_linear)
+                    us_step_dual_linear_x=main_res["us_step_dual_linear_x"],
                     eff_tops=main_res["eff_tops"], gbs=main_res["gbs"],
                     cublas_bf16_gemm_us=main_res.get("us_cublas_bf16_gemm"),
                     paper_context="paper: up to 1.8x over FP16 TensorRT-LLM end to end on RTX 4090 / L20 (PAPER.md L232)",
