@@ -34,6 +34,8 @@ enum {
     TWQ_PLAN_SMEM,             /* dynamic shared memory, bytes */
     TWQ_PLAN_RING,             /* ring depth of the packed-operand pipeline */
     TWQ_PLAN_CHUNKS,           /* small-batch kernel: ring chunks per call; tcgen05 kernel: work units */
+    TWQ_PLAN_S1RING,           /* depth of the stage-1 (X, L1) ring */
+    TWQ_PLAN_ALIAS,            /* tcgen05 kernel: 1 / 2 = the stage-1 ring overlays the residual rings (/ and the L2T tile) */
     TWQ_PLAN_FIELDS
 };
 /* The launch plan twq_dual_linear would use for this shape on the current device (or the no-device defaults).

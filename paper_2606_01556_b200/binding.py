@@ -21,7 +21,7 @@ TESTING_EXPORTS = ("twq_testing_set_plan_flags", "twq_testing_get_plan_flags", "
                    "twq_testing_set_trace_buffer", "twq_testing_measure_i8_tops")
 # include/twq_testing.h: planner overrides for tests
 PLAN_NO_SPLIT, PLAN_NO_PAIR, PLAN_NO_YSTAGE, PLAN_NO_ALIAS2, PLAN_NO_DECODE = 1, 2, 4, 8, 16
-_PLAN_FIELDS = ("kernel", "cluster", "grid", "tile_tokens", "splits", "pair", "smem", "ring", "chunks")
+_PLAN_FIELDS = ("kernel", "cluster", "grid", "tile_tokens", "splits", "pair", "smem", "ring", "chunks", "s1_ring", "alias")
 
 
 def plan_fused_cs(c: int) -> int:

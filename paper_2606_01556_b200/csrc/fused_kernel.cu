@@ -131,6 +131,9 @@ static bool make_plan_tn(int TN, int M, int N, int K, int r, int G, int num_sms,
         else if (total(pl) > budget) pl.nsp = q.nsp;
     }
     if (total(pl) > budget) { pl.alias = 1; pl.ns1 = r > 0 ? 3 : 0; }
+    // split-K calls run ONE unit per cluster, so the overlay of the stage-1 ring on the residual rings never makes a
+    // tile wait for its predecessor: take it, and with it the deepest stage-1 ring
+    if (pl.splits > 1 && r > 0 && pl.alias == 0) { pl.alias = 1; pl.ns1 = kMaxNS1; }
     if (total(pl) > budget && r > 0 && !(flags & kPlanNoAlias2)) {
         // Rank-256 buffers beside a 128-token tile: the stage-1 ring and the FP32 partial of H overlay the L2T tile as
         // well as the residual rings.  L2T is dead whenever stage 1 runs: its stage-2 MMAs were issued at the start
@@ -141,6 +144,15 @@ static bool make_plan_tn(int TN, int M, int N, int K, int r, int G, int num_sms,
         q.ystage = 0;
         while (total(q) > budget && q.nsp > 4) --q.nsp;
         if (total(q) <= budget) pl = q;
+    }
+    // a deeper stage-1 ring wherever it costs nothing (it overlays the residual rings) or still fits: every chunk of the
+    // stage-1 chain is a round trip to L2 / HBM, and with two stages in flight the chain ran at one round trip per chunk
+    // (in-kernel timeline at M = 128, r02: 2600 cycles per 64-wide chunk, 11 of the call's 29 us)
+    while (r > 0 && pl.ns1 < kMaxNS1) {
+        FusedPlan q = pl;
+        ++q.ns1;
+        if (total(q) > budget) break;
+        pl = q;
     }
     while (total(pl) > budget && pl.nsp > 2) --pl.nsp;
     while (total(pl) > budget && pl.nsu > 2) --pl.nsu;

@@ -192,6 +192,7 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
     uint64_t* bars = reinterpret_cast<uint64_t*>(smem + pl.off_bar);
     uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + B_COUNT);
 
+    TWQ_TG(0);
     const int warp = threadIdx.x >> 5;
     const int lane = threadIdx.x & 31;
     const int r = p.r;
@@ -249,6 +250,7 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
 #define TWQ_LBAR(i) (lbar0 + 8u * static_cast<uint32_t>(i))
     const bool leader = !kPair || (rank & 1) == 0;
     pdl_launch_dependents();          // the next kernel may start its own prologue / weight prefetch
+    TWQ_TG(1);
 
     if (warp >= kCtlWarp0) {
         reg_dec<kRegsCtl>();
@@ -672,6 +674,7 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
             }
         }
         pdl_wait();                          // Y / workspace writes must follow the previous kernel
+        TWQ_TG(2);
 
         int itp = 0, ctx_n = 0, cur_ctx = -1;
         int b = 0, pb = 0;                   // next P buffer / parity of its use count (same rotation as the MMA issuer)
@@ -692,6 +695,7 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
                 s1_range<G>(p, t, rank, kc0, kc1);
                 const bool has_s1 = kc0 < kc1;
                 mbar_wait(&bars[B_HFULL], ctx_n & 1, 40);
+                TWQ_TG(12);
                 tc_fence_after();
                 if (active) {
                     for (int rb = 0; rb < nrb; ++rb) {
@@ -731,6 +735,7 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
                 }
                 tc_fence_before();
                 __syncwarp();
+                TWQ_TG(13);
                 if (lane == 0) {
                     mbar_arrive(&bars[B_HDRAINED]);
                     if (kPair) mbar_arrive_remote_relaxed(TWQ_LBAR(B_HDRAINED2));
@@ -739,17 +744,30 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
                     // ---- reduce-scatter the FP32 partials, all-gather the FP16 result (DSMEM)
                     if (lane < cs) mbar_arrive_remote(mapa_u32(smem_u32(&bars[B_X1]), lane));
                     mbar_wait_cluster(&bars[B_X1], ctx_n & 1, 41);
+                    TWQ_TG(14);
                     const int jcs = r >> 3;                     // 8-wide column chunks of H
                     const int total = TN * jcs;
                     for (int i = rank + cs * et; i < total; i += cs * 256) {
                         const int m = i / jcs, jc = i - m * jcs;
                         const uint32_t src = smem_u32(sHpart + m * r + jc * 8);
                         float s[8] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
-                        for (int pr = 0; pr < cs; ++pr) {       // fixed order: every CTA sees identical H
-                            const uint32_t a = mapa_u32(src, pr);
-                            const float4 x0 = ld_dsmem_f4(a), x1 = ld_dsmem_f4(a + 16);
+                        // the remote loads of two peers in flight together (one at a time was a chain of cs round trips per
+                        // element: 6400 cycles of the split-K call at M = 128, r02); fixed order: every CTA sees identical H
+                        // the CTA's own partial is read with plain shared loads: distributed shared memory moves ~20 bytes per
+                        // cycle, and through it the own half cost as much as the peer's
+                        const float* own = sHpart + m * r + jc * 8;
+                        for (int pr = 0; pr < cs; pr += 2) {
+                            const int p1 = pr + 1 < cs ? pr + 1 : pr;
+                            const uint32_t a0 = mapa_u32(src, pr), a1 = mapa_u32(src, p1);
+                            const float4 x0 = pr == rank ? *reinterpret_cast<const float4*>(own) : ld_dsmem_f4(a0);
+                            const float4 x1 = pr == rank ? *reinterpret_cast<const float4*>(own + 4) : ld_dsmem_f4(a0 + 16);
+                            float4 y0 = p1 == rank ? *reinterpret_cast<const float4*>(own) : ld_dsmem_f4(a1);
+                            float4 y1 = p1 == rank ? *reinterpret_cast<const float4*>(own + 4) : ld_dsmem_f4(a1 + 16);
+                            if (pr + 1 >= cs) { y0 = make_float4(0.f, 0.f, 0.f, 0.f); y1 = y0; }
                             s[0] += x0.x; s[1] += x0.y; s[2] += x0.z; s[3] += x0.w;
                             s[4] += x1.x; s[5] += x1.y; s[6] += x1.z; s[7] += x1.w;
+                            s[0] += y0.x; s[1] += y0.y; s[2] += y0.z; s[3] += y0.w;
+                            s[4] += y1.x; s[5] += y1.y; s[6] += y1.z; s[7] += y1.w;
                         }
                         uint32_t hw[4];
 #pragma unroll
@@ -759,9 +777,14 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
                             const __half2 h2 = __floats2half2_rn(lo, hi);
                             hw[e] = *reinterpret_cast<const uint32_t*>(&h2);
                         }
-                        const uint32_t dst = smem_u32(sH + (jc >> 3) * (TN * 128) + swizzled_chunk_offset<128>(m, jc & 7));
-                        for (int pr = 0; pr < cs; ++pr) st_dsmem_u4(mapa_u32(dst, pr), make_uint4(hw[0], hw[1], hw[2], hw[3]));
+                        uint8_t* dloc = sH + (jc >> 3) * (TN * 128) + swizzled_chunk_offset<128>(m, jc & 7);
+                        const uint32_t dst = smem_u32(dloc);
+                        for (int pr = 0; pr < cs; ++pr) {
+                            if (pr == rank) *reinterpret_cast<uint4*>(dloc) = make_uint4(hw[0], hw[1], hw[2], hw[3]);
+                            else st_dsmem_u4(mapa_u32(dst, pr), make_uint4(hw[0], hw[1], hw[2], hw[3]));
+                        }
                     }
+                    TWQ_TG(15);
                     fence_proxy_async_all();
                     __syncwarp();
                     if (lane < cs) mbar_arrive_remote(mapa_u32(smem_u32(&bars[B_X2]), lane));
@@ -770,6 +793,7 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
                 fence_proxy_async_smem();
                 __syncwarp();
                 if (lane == 0) mbar_arrive(&bars[B_HREADY]);
+                TWQ_TG(3);
                 ++ctx_n;
             }
 
@@ -1066,12 +1090,14 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
             if (trw) TWQ_TR(3, trn, 6);
 #endif
         }
+        TWQ_TG(4);
         if (y_pending) bulk_wait_all0();     // the staged tiles are in global memory before the CTA goes away
     }
 
     // ---------------------------------------------------------------- teardown
     tc_fence_before();
     __syncthreads();
+    TWQ_TG(5);
     if (kPair) cluster_sync_all();   // the leader's MMAs write the peer's TMEM: both CTAs are done before either frees
     if (warp == kCtlWarp0 + 2) {
         tc_fence_after();
@@ -1103,6 +1129,7 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
             __threadfence();
         }
         __syncthreads();
+        TWQ_TG(6);
         {
             const int rows = min(TN, p.M - t.m0);
             const int r0 = rows * t.ks / pl.splits, r1 = rows * (t.ks + 1) / pl.splits;
@@ -1112,9 +1139,17 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
                 const int mm = t.m0 + r0 + idx / (kTileN / 4), nn = t.n0 + (idx % (kTileN / 4)) * 4;
                 if (nn >= p.N) continue;
                 float4 y = make_float4(0.f, 0.f, 0.f, 0.f);
-                for (int z = 0; z < pl.splits; ++z) {
-                    const float4 v = __ldcg(reinterpret_cast<const float4*>(p.ws_part + (static_cast<size_t>(z) * p.M + mm) * p.N + nn));
-                    y.x += v.x; y.y += v.y; y.z += v.z; y.w += v.w;
+                // the loads of all splits in flight together (four at a time), the sum in split order
+                for (int z0 = 0; z0 < pl.splits; z0 += 4) {
+                    float4 v[4];
+#pragma unroll
+                    for (int q = 0; q < 4; ++q)
+                        v[q] = z0 + q < pl.splits
+                                   ? __ldcg(reinterpret_cast<const float4*>(p.ws_part + (static_cast<size_t>(z0 + q) * p.M + mm) * p.N + nn))
+                                   : make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+                    for (int q = 0; q < 4; ++q) { y.x += v[q].x; y.y += v[q].y; y.z += v[q].z; y.w += v[q].w; }
+                    if (z0 == 0 && idx == threadIdx.x) TWQ_TG(11);
                 }
                 const size_t o = static_cast<size_t>(mm) * p.ldy + nn;
                 if (p.ydt == 2 && (p.ldy & 3) == 0) {
@@ -1140,13 +1175,17 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
                 }
             }
         }
+        TWQ_TG(9);
         __syncthreads();
+        TWQ_TG(10);
         if (threadIdx.x == 0) {
             const unsigned prev = atomicAdd(ctr, 1u);
             if (prev == static_cast<unsigned>(2 * pl.splits - 1)) atomicExch(ctr, 0u);
         }
     }
+    TWQ_TG(7);
     if (cs > 1) cluster_sync_all();   // no CTA exits while a peer may still touch its shared memory
+    TWQ_TG(8);
 }
 
 

@@ -6,7 +6,8 @@
 //   decode kernel : TWQ_DSTAMP(k) -- lane 0 of every warp of CTA 0 and of CTA grid/2 stores %globaltimer (ns) at
 //                   buffer[((cta_sel * 20 + warp) * 64) + k], k < 32;
 //                   TWQ_DCLK(k) stores clock64 (SM cycles) at slot 32 + k of the same row.
-//   tcgen05 kernel: TWQ_TR(role, n, tag) -- CTA 0 appends (tag << 48 | clock64) to buffer[role * 4096 + n++], four roles.
+//   tcgen05 kernel: TWQ_TR(role, n, tag) -- CTA 0 appends (tag << 48 | clock64) to buffer[role * 4096 + n++], four roles;
+//                   TWQ_TG(k) -- whole-kernel milestones (clock64) of CTA 0 at buffer[4 * 4096 - 64 + k].
 #pragma once
 
 #ifdef TWQ_TRACE
@@ -31,7 +32,14 @@
             p.trace[(role) * 4096 + (n)++] = (static_cast<unsigned long long>(tag) << 48) |              \
                                              (static_cast<unsigned long long>(clock64()) & 0xFFFFFFFFFFFFull); \
     } while (0)
+/* tcgen05 kernel, whole-kernel milestones: thread 256 (first epilogue thread) of CTA 0 stores clock64 at buffer[4 * 4096 - 64 + k] */
+#define TWQ_TG(k)                                                                                        \
+    do {                                                                                                 \
+        if (p.trace != nullptr && blockIdx.x == 0 && threadIdx.x == 256)                                 \
+            p.trace[4 * 4096 - 64 + (k)] = static_cast<unsigned long long>(clock64());                   \
+    } while (0)
 #else
+#define TWQ_TG(k) do { } while (0)
 #define TWQ_DSTAMP(k) do { } while (0)
 #define TWQ_DCLK(k) do { } while (0)
 #define TWQ_TR(role, n, tag) do { } while (0)

@@ -240,10 +240,12 @@ int twq_testing_describe_plan(int M, int N, int K, int r, int G, int* out, int n
         v[TWQ_PLAN_CLUSTER] = cp->dp.cs; v[TWQ_PLAN_GRID] = cp->dp.grid; v[TWQ_PLAN_TILE_TOKENS] = cp->dp.mp;
         v[TWQ_PLAN_SPLITS] = 1; v[TWQ_PLAN_PAIR] = 0; v[TWQ_PLAN_SMEM] = cp->dp.smem_bytes;
         v[TWQ_PLAN_RING] = cp->dp.nslots; v[TWQ_PLAN_CHUNKS] = cp->dp.nchunks;
+        v[TWQ_PLAN_S1RING] = cp->dp.l1_slots; v[TWQ_PLAN_ALIAS] = 0;
     } else {
         v[TWQ_PLAN_CLUSTER] = cp->fp.cs; v[TWQ_PLAN_GRID] = cp->fp.nclusters * cp->fp.cs; v[TWQ_PLAN_TILE_TOKENS] = cp->fp.TN;
         v[TWQ_PLAN_SPLITS] = cp->fp.splits; v[TWQ_PLAN_PAIR] = cp->fp.pair; v[TWQ_PLAN_SMEM] = cp->fp.smem_bytes;
         v[TWQ_PLAN_RING] = cp->fp.nsp; v[TWQ_PLAN_CHUNKS] = cp->fp.units;
+        v[TWQ_PLAN_S1RING] = cp->fp.ns1; v[TWQ_PLAN_ALIAS] = cp->fp.alias;
     }
     for (int i = 0; i < n_out && i < TWQ_PLAN_FIELDS; ++i) out[i] = v[i];
     return TWQ_PLAN_FIELDS;
