@@ -110,6 +110,21 @@ def make_layer(M: int, K: int, N: int, r: int, G: int, *, seed: int,
     return LayerInputs(M, K, N, r, G, Xb, Rq, sw, L1, L2, tinv)
 
 
+def make_q4_lowrank(K: int, N: int, r: int, G: int, *, seed: int):
+    """4-bit low-rank factors for the paper's own branch: codes uniform on [-8,7]
+    with FP16 group scales, like the residual.  U codes [r,K] with scales [r,K/G] (groups along K); V codes [N,r] with
+    scales [N,r/Gr], Gr = r for r <= 128 else 128 (groups along r).  Scale ranges are chosen so that the dequantized
+    factors have about the N(0, 0.02) magnitude of the FP16 factors of configs 2-5 (code std 4.6 x 0.0043).
+    Draw order: U codes, su, V codes, sv.  No method arithmetic."""
+    rng = np.random.Generator(np.random.PCG64(seed))
+    Gr = r if r <= 128 else 128
+    Uq = rng.integers(-8, 8, size=(r, K), dtype=np.int8)
+    su = rng.uniform(0.003, 0.006, size=(r, K // G)).astype(np.float32).astype(np.float16)
+    Vq = rng.integers(-8, 8, size=(N, r), dtype=np.int8)
+    sv = rng.uniform(0.003, 0.006, size=(N, r // Gr)).astype(np.float32).astype(np.float16)
+    return Uq, su, Vq, sv
+
+
 # --------------------------------------------------------------------------
 # BASELINE.json configs
 # --------------------------------------------------------------------------

@@ -144,6 +144,57 @@ def forward(X_bf16, Rq, sw, L1, L2, G: int, tinv=None, rows=None, want_P: bool =
     return out
 
 
+def lowrank_group(r: int) -> int:
+    """Group size of the re-quantized intermediate H along r (reading R18): r for r <= 128, else 128."""
+    return r if r <= 128 else 128
+
+
+def forward_q4lr_from_quantized(Xq, sx, R4, sw, U4, su, V4, sv, G: int, rows=None, want_H: bool = False):
+    """NEXT-1, steps on given quantizer outputs: both low-rank factors 4-bit, H re-quantized on the
+    fly.  U4 [r,K/2], su fp16 [r,K/G], V4 [N,r/2], sv fp16 [N,r/Gr].  Returns Y [nrows,N] (and dict(H, QH, sH))."""
+    Xq = np.ascontiguousarray(Xq, dtype=np.uint8)
+    sx = np.ascontiguousarray(sx, dtype=np.float32)
+    R4 = np.ascontiguousarray(R4, dtype=np.uint8)
+    sw = np.ascontiguousarray(sw, dtype=np.float16)
+    U4 = np.ascontiguousarray(U4, dtype=np.uint8)
+    su = np.ascontiguousarray(su, dtype=np.float16)
+    V4 = np.ascontiguousarray(V4, dtype=np.uint8)
+    sv = np.ascontiguousarray(sv, dtype=np.float16)
+    M, K2 = Xq.shape
+    K, N, r = 2 * K2, R4.shape[0], U4.shape[0]
+    ng, Gr = K // G, lowrank_group(U4.shape[0])
+    assert r % Gr == 0 and U4.shape == (r, K2) and su.shape == (r, ng) and V4.shape == (N, r // 2) and sv.shape == (N, r // Gr)
+    rows_a = None if rows is None else np.ascontiguousarray(rows, dtype=np.int32)
+    nrows = M if rows is None else len(rows_a)
+    Y = np.empty((nrows, N), np.float64)
+    H = np.empty((nrows, r), np.float64) if want_H else None
+    QH = np.empty((nrows, r), np.int8) if want_H else None
+    sH = np.empty((nrows, r // Gr), np.float32) if want_H else None
+    _load().twq_oracle_forward_q4lr(_p(Xq, ctypes.c_uint8), _p(sx, ctypes.c_float), _p(R4, ctypes.c_uint8),
+                                    _p(sw.view(np.uint16), ctypes.c_uint16), _p(U4, ctypes.c_uint8),
+                                    _p(su.view(np.uint16), ctypes.c_uint16), _p(V4, ctypes.c_uint8),
+                                    _p(sv.view(np.uint16), ctypes.c_uint16), M, N, K, r, G, Gr,
+                                    _p(rows_a, ctypes.c_int32), nrows, _p(Y, ctypes.c_double), _p(H, ctypes.c_double),
+                                    _p(QH, ctypes.c_int8), _p(sH, ctypes.c_float))
+    return (Y, dict(H=H, QH=QH, sH=sH)) if want_H else Y
+
+
+def forward_q4lr(X_bf16, Rq, sw, Uq, su, Vq, sv, G: int, tinv=None, rows=None, want_H: bool = False):
+    """NEXT-1, the whole path: quantize X, pack every code tensor, run both 4-bit branches, merge.
+    Uq int8 [r,K], Vq int8 [N,r] codes in [-8,7].  Returns dict(q, Xq, sx, Y [, H, QH, sH])."""
+    q, sx = quantize_act(X_bf16, G, tinv)
+    Xq = pack_nibbles(q)
+    res = forward_q4lr_from_quantized(Xq, sx, pack_nibbles(Rq), sw, pack_nibbles(Uq), su, pack_nibbles(Vq), sv, G,
+                                      rows=rows, want_H=want_H)
+    out = dict(q=q, Xq=Xq, sx=sx)
+    if want_H:
+        out["Y"] = res[0]
+        out.update(res[1])
+    else:
+        out["Y"] = res
+    return out
+
+
 def round_bf16(Y: np.ndarray) -> np.ndarray:
     """FP64 -> BF16 bits with one round-to-nearest-even (reading R11)."""
     Y = np.ascontiguousarray(Y, dtype=np.float64)

@@ -26,7 +26,9 @@
  * bound, sign / power-of-two scaling invariances, nibble bijection, brute
  * force with python Fractions, numpy int64 matmul for P, numpy FP64 matmul for
  * the low-rank branch, r=0 and R=0 special cases, additivity, storage ratios
- * of PAPER.md L86.  The paper prints no worked numerical example, so the
+ * of PAPER.md L86; twq_oracle_forward_q4lr (NEXT-1, the paper's 4-bit low-rank branch): library
+ * integer matmul + explicit fold for H, numpy FP32 restatement of the re-quantizer, exact closed form,
+ * zero-factor reduction, round-trip bound.  The paper prints no worked numerical example, so the
  * readings R5 (rounding mode), R8 (op order), R9 (zero group), R10 (nibble
  * order) are "parity unpinned" BY THE PAPER and fixed by DESIGN.md.
  */
@@ -205,6 +207,97 @@ void twq_oracle_forward(const uint16_t* X, int ldx, const uint8_t* Xq, const flo
     free(H);
     free(qx);
     free(qw);
+}
+
+/* ---- NEXT-1: the paper's own, fully 4-bit low-rank branch -------
+ * PAPER.md L177-181 (section 4.3 "Fused two-stage low-rank pipeline", "On-the-fly scaling with a
+ * single epilogue"), Eq. 4: Q(X)[Q(U)Q(V) + Q(R)].  Both low-rank factors are 4-bit with group
+ * scales (L193) and the branch consumes the QUANTIZED activation ("quantizes the input activation
+ * tile once and reuses it for both components", L179):
+ *   P1[m,g,j] = sum_{k in g} qx[m,k] * qu[j,k]                exact int64 (first 4-bit GEMM, "int32 accumulation")
+ *   H[m,j]    = sum_g sx[m,g] * su[j,g] * P1[m,g,j]           FP64 (the value of the INT32 accumulators with their scales)
+ *   on-the-fly re-quantization (L181: "estimating an intermediate scale s_H from the INT32 accumulator and
+ *   re-quantizing on the fly"); readings R18 / R19: the quantizer of Eq. 1 (L43-47) on float32(H), one
+ *   scale per token and per group of Gr consecutive j (Gr = r for r <= 128, else 128), same FP32 operation order
+ *   as the activation quantizer:
+ *     a = max(max_{j in h} |H32[m,j]|, 2^-30);  sH[m,h] = a / 7.0f;  inv = 1.0f / sH;
+ *     QH[m,j] = clamp(rint(H32[m,j] * inv), -7, 7)
+ *   P2[m,h,n] = sum_{j in h} QH[m,j] * qv[n,j]                exact int64 (second 4-bit GEMM)
+ *   Ylr[m,n]  = sum_h sH[m,h] * sv[n,h] * P2[m,h,n]           FP64
+ *   Y         = Yres + Ylr                                    (single epilogue, L181)
+ * U4 [r][K/2] and V4 [N][r/2] are nibble-packed like R4; su [r][K/G], sv [N][r/Gr] are FP16 bit patterns.
+ * Optional outputs: H_out [nrows][r] (FP64), QH_out [nrows][r], sH_out [nrows][r/Gr].
+ */
+void twq_oracle_forward_q4lr(const uint8_t* Xq, const float* sx, const uint8_t* R4, const uint16_t* sw,
+                             const uint8_t* U4, const uint16_t* su, const uint8_t* V4, const uint16_t* sv,
+                             int M, int N, int K, int r, int G, int Gr, const int* rows, int nrows,
+                             double* Y, double* H_out, int8_t* QH_out, float* sH_out) {
+    int ng = K / G, nh = r / Gr;
+    (void)M;
+    int8_t* qw = (int8_t*)malloc((size_t)N * K);
+    int8_t* qu = (int8_t*)malloc((size_t)r * K);
+    int8_t* qv = (int8_t*)malloc((size_t)N * r);
+    twq_oracle_unpack_nibbles(R4, N, K, qw);
+    twq_oracle_unpack_nibbles(U4, r, K, qu);
+    twq_oracle_unpack_nibbles(V4, N, r, qv);
+    int8_t* qx = (int8_t*)malloc((size_t)K);
+    double* H = (double*)malloc(sizeof(double) * (size_t)r);
+    int8_t* QH = (int8_t*)malloc((size_t)r);
+    float* sH = (float*)malloc(sizeof(float) * (size_t)nh);
+    for (int i = 0; i < nrows; ++i) {
+        int m = rows ? rows[i] : i;
+        twq_oracle_unpack_nibbles(Xq + (size_t)m * (K / 2), 1, K, qx);
+        /* first 4-bit GEMM + its scales */
+        for (int j = 0; j < r; ++j) {
+            double h = 0.0;
+            for (int g = 0; g < ng; ++g) {
+                int64_t acc = 0;
+                for (int k = g * G; k < (g + 1) * G; ++k) acc += (int64_t)qx[k] * (int64_t)qu[(size_t)j * K + k];
+                h += (double)sx[(size_t)m * ng + g] * fp16_to_f64(su[(size_t)j * ng + g]) * (double)acc;
+            }
+            H[j] = h;
+            if (H_out) H_out[(size_t)i * r + j] = h;
+        }
+        /* on-the-fly re-quantization of H (Eq. 1 on float32(H), groups of Gr along r) */
+        for (int h = 0; h < nh; ++h) {
+            volatile float amax = 0.0f;
+            for (int j = h * Gr; j < (h + 1) * Gr; ++j) {
+                float a = fabsf((float)H[j]);
+                if (a > amax) amax = a;
+            }
+            float amax_c = amax > 0x1p-30f ? amax : 0x1p-30f;
+            volatile float s = amax_c / 7.0f;
+            volatile float inv = 1.0f / s;
+            sH[h] = s;
+            if (sH_out) sH_out[(size_t)i * nh + h] = s;
+            for (int j = h * Gr; j < (h + 1) * Gr; ++j) {
+                volatile float scaled = (float)H[j] * inv;
+                int qi = (int)nearbyintf(scaled);
+                if (qi > 7) qi = 7;
+                if (qi < -7) qi = -7;
+                QH[j] = (int8_t)qi;
+                if (QH_out) QH_out[(size_t)i * r + j] = (int8_t)qi;
+            }
+        }
+#pragma omp parallel for schedule(static)
+        for (int n = 0; n < N; ++n) {
+            double yres = 0.0;
+            for (int g = 0; g < ng; ++g) {
+                int64_t acc = 0;
+                for (int k = g * G; k < (g + 1) * G; ++k)
+                    acc += (int64_t)qx[k] * (int64_t)qw[(size_t)n * K + k];
+                yres += (double)sx[(size_t)m * ng + g] * fp16_to_f64(sw[(size_t)n * ng + g]) * (double)acc;
+            }
+            double ylr = 0.0;
+            for (int h = 0; h < nh; ++h) {
+                int64_t acc = 0;
+                for (int j = h * Gr; j < (h + 1) * Gr; ++j) acc += (int64_t)QH[j] * (int64_t)qv[(size_t)n * r + j];
+                ylr += (double)sH[h] * fp16_to_f64(sv[(size_t)n * nh + h]) * (double)acc;
+            }
+            Y[(size_t)i * N + n] = yres + ylr;
+        }
+    }
+    free(sH); free(QH); free(H); free(qx); free(qv); free(qu); free(qw);
 }
 
 /* ---- output rounding: FP64 -> BF16 with ONE round-to-nearest-even ----------

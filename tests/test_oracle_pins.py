@@ -232,6 +232,138 @@ def test_forward_row_subset_is_rows_of_the_full_call(oracle):
     assert (r0[0] == f0[4]).all() and (r0[1] == f0[1]).all()
 
 
+# --------------------------------------------------------------------------- NEXT-1: 4-bit low-rank branch
+def _q4lr_case(M, K, N, r, G, seed):
+    L = gen.make_layer(M, K, N, 0, G, seed=seed)
+    Uq, su, Vq, sv = gen.make_q4_lowrank(K, N, r, G, seed=seed + 1000)
+    return L, Uq, su, Vq, sv
+
+
+def _np_requant(H, Gr):
+    """numpy-float32 restatement of Eq. 1 (L43-47) on float32(H), groups of Gr along r (readings R18 / R19)."""
+    M, r = H.shape
+    h32 = H.astype(np.float32).reshape(M, r // Gr, Gr)
+    amax = np.maximum(np.abs(h32).max(axis=2), np.float32(2.0 ** -30))
+    s = (amax / np.float32(7.0)).astype(np.float32)
+    inv = (np.float32(1.0) / s).astype(np.float32)
+    q = np.clip(np.rint((h32 * inv[:, :, None]).astype(np.float32)), -7, 7).astype(np.int8)
+    return q.reshape(M, r), s
+
+
+@pytest.mark.parametrize("r,G", [(32, 64), (128, 128), (256, 64)])
+def test_q4lr_stage_by_stage_library_restatement(oracle, r, G):
+    """H by library integer matmul per group + explicit scale fold; QH / sH by the numpy
+    quantizer restatement; Ylr by a second integer matmul per r-group; Yres = the pinned rank-0 forward()."""
+    M, K, N = 5, 512, 48
+    L, Uq, su, Vq, sv = _q4lr_case(M, K, N, r, G, 31 + r)
+    out = oracle.forward_q4lr(L.X, L.Rq, L.sw, Uq, su, Vq, sv, G, want_H=True)
+    q, sx = out["q"].astype(np.int64), out["sx"].astype(np.float64)
+    ng, Gr = K // G, oracle.lowrank_group(r)
+    H = np.zeros((M, r))
+    for g in range(ng):
+        P1 = q[:, g * G:(g + 1) * G] @ Uq[:, g * G:(g + 1) * G].astype(np.int64).T        # [M, r] exact
+        H += sx[:, g:g + 1] * su[:, g].astype(np.float64)[None, :] * P1
+    assert np.allclose(out["H"], H, rtol=1e-13, atol=1e-300)
+    QH, sH = _np_requant(out["H"], Gr)
+    assert (out["sH"] == sH).all() and (out["QH"] == QH).all()
+    assert np.abs(out["QH"]).max() == 7                          # every group's largest element lands on +-7
+    Ylr = np.zeros((M, N))
+    for h in range(r // Gr):
+        P2 = QH[:, h * Gr:(h + 1) * Gr].astype(np.int64) @ Vq[:, h * Gr:(h + 1) * Gr].astype(np.int64).T
+        Ylr += sH[:, h:h + 1].astype(np.float64) * sv[:, h].astype(np.float64)[None, :] * P2
+    yres = oracle.forward(L.X, L.Rq, L.sw, None, None, G)["Y"]
+    assert np.allclose(out["Y"], yres + Ylr, rtol=1e-12, atol=1e-12)
+    assert np.abs(Ylr).max() > 0.05 * np.abs(yres).max()        # the branch is not negligible in this case
+
+
+def test_q4lr_bruteforce_fractions(oracle):
+    """Exact rational arithmetic on a tiny case, given the oracle's own QH / sH (pinned above)."""
+    M, K, N, r, G = 2, 128, 6, 16, 64
+    L, Uq, su, Vq, sv = _q4lr_case(M, K, N, r, G, 33)
+    out = oracle.forward_q4lr(L.X, L.Rq, L.sw, Uq, su, Vq, sv, G, want_H=True)
+    q, sx = out["q"], out["sx"]
+    for m in range(M):
+        Hm = []
+        for j in range(r):
+            h = Fraction(0)
+            for g in range(K // G):
+                acc = sum(int(q[m, k]) * int(Uq[j, k]) for k in range(g * G, (g + 1) * G))
+                h += Fraction(float(sx[m, g])) * Fraction(float(su[j, g])) * acc
+            Hm.append(h)
+            assert abs(out["H"][m, j] - float(h)) <= 1e-13 * abs(float(h)) + 1e-300
+        for n in range(N):
+            y = Fraction(0)
+            for g in range(K // G):
+                acc = sum(int(q[m, k]) * int(L.Rq[n, k]) for k in range(g * G, (g + 1) * G))
+                y += Fraction(float(sx[m, g])) * Fraction(float(L.sw[n, g])) * acc
+            acc = sum(int(out["QH"][m, j]) * int(Vq[n, j]) for j in range(r))
+            y += Fraction(float(out["sH"][m, 0])) * Fraction(float(sv[n, 0])) * acc
+            assert abs(out["Y"][m, n] - float(y)) <= 1e-12 * max(1.0, abs(float(y)))
+
+
+def test_q4lr_exactly_representable_closed_form(oracle):
+    """Closed form: X = one-hot rows of value 7 (so sx = 1, q = 7 e_k) and su = 1 give H[m,:] = 7 * Uq[:,k_m]; with
+    Uq in [-6,6] except one row of 7s, max|H| = 49, so sH = 7 and QH = Uq[:,k_m] exactly, and
+    Ylr[m,n] = 7 * sv * sum_j Uq[j,k_m] * Vq[n,j]: an integer matmul times a power of two."""
+    K, N, r, G = 128, 8, 16, 64
+    rng = np.random.default_rng(5)
+    Uq = rng.integers(-6, 7, size=(r, K), dtype=np.int8)
+    Uq[0, :] = 7                                                     # every column's amax is 7
+    Vq = rng.integers(-8, 8, size=(N, r), dtype=np.int8)
+    su = np.ones((r, K // G), np.float16)
+    sv = np.full((N, 1), 0.25, np.float16)
+    ks = [3, 64, 127]
+    X = np.zeros((len(ks), K), np.float32)
+    for m, k in enumerate(ks):
+        X[m, k] = 7.0
+    Rq0 = np.zeros((N, K), np.int8)
+    sw = np.ones((N, K // G), np.float16)
+    out = oracle.forward_q4lr(bf16(X), Rq0, sw, Uq, su, Vq, sv, G, want_H=True)
+    for m, k in enumerate(ks):
+        assert (out["H"][m] == 7.0 * Uq[:, k]).all()
+        assert out["sH"][m, 0] == 7.0 and (out["QH"][m] == Uq[:, k]).all()
+        ref = 7.0 * 0.25 * (Vq.astype(np.int64) @ Uq[:, k].astype(np.int64))
+        assert (out["Y"][m] == ref).all()
+
+
+def test_q4lr_reductions_and_sensitivity(oracle):
+    """Zero U -> H = 0 -> QH = 0 -> Y = the residual alone (the pinned rank-0 forward); zero V likewise; zero residual
+    -> Y = Ylr alone and Y(res) + Y(lr) = Y(both); swapping the roles of the two r-groups of V changes the result
+    (a wrong group index in the second GEMM's scales fails here)."""
+    M, K, N, r, G = 3, 256, 24, 256, 64
+    L, Uq, su, Vq, sv = _q4lr_case(M, K, N, r, G, 35)
+    yres = oracle.forward(L.X, L.Rq, L.sw, None, None, G)["Y"]
+    y0 = oracle.forward_q4lr(L.X, L.Rq, L.sw, np.zeros_like(Uq), su, Vq, sv, G, want_H=True)
+    assert (y0["QH"] == 0).all() and (y0["sH"] == np.float32(2.0 ** -30) / np.float32(7.0)).all()
+    assert (y0["Y"] == yres).all()
+    assert (oracle.forward_q4lr(L.X, L.Rq, L.sw, Uq, su, np.zeros_like(Vq), sv, G)["Y"] == yres).all()
+    both = oracle.forward_q4lr(L.X, L.Rq, L.sw, Uq, su, Vq, sv, G)["Y"]
+    lr = oracle.forward_q4lr(L.X, np.zeros_like(L.Rq), L.sw, Uq, su, Vq, sv, G)["Y"]
+    assert np.allclose(both, yres + lr, rtol=1e-12, atol=1e-12)
+    sv_sw = sv[:, ::-1].copy()
+    assert not np.allclose(oracle.forward_q4lr(L.X, L.Rq, L.sw, Uq, su, Vq, sv_sw, G)["Y"], both, rtol=1e-6)
+    rows = [2, 0]
+    sub = oracle.forward_q4lr(L.X, L.Rq, L.sw, Uq, su, Vq, sv, G, rows=rows)["Y"]
+    assert (sub == both[rows]).all()
+
+
+def test_q4lr_requantization_error_bound(oracle):
+    """The re-quantized branch stays within the quantizer's half-step bound of the un-requantized product
+    H . deq(V): |Ylr - sum_j H[m,j] sv qv| <= sum_h (sH/2)(1 + 2^-22) sum_{j in h} |sv qv|."""
+    M, K, N, r, G = 4, 512, 32, 256, 128
+    L, Uq, su, Vq, sv = _q4lr_case(M, K, N, r, G, 37)
+    out = oracle.forward_q4lr(L.X, np.zeros_like(L.Rq), L.sw, Uq, su, Vq, sv, G, want_H=True)
+    Gr = oracle.lowrank_group(r)
+    dv = Vq.astype(np.float64) * np.repeat(sv.astype(np.float64), Gr, axis=1)            # [N, r]
+    exact = out["H"] @ dv.T
+    bound = np.zeros((M, N))
+    for h in range(r // Gr):
+        bound += 0.5 * (1 + 2.0 ** -22) * out["sH"][:, h:h + 1].astype(np.float64) * np.abs(dv[:, h * Gr:(h + 1) * Gr]).sum(axis=1)[None, :]
+    err = np.abs(out["Y"] - exact)
+    assert (err <= bound).all()
+    assert err.max() > 0.02 * bound.max()                      # and the bound is not vacuous
+
+
 def test_scale_fold_constant_and_pow2_exact(oracle):
     """Constant scales factor out; power-of-two scales and small integers make Y exactly representable."""
     rng = np.random.default_rng(7)
