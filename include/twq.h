@@ -168,6 +168,48 @@ twq_status twq_dual_linear_x(const void* X, int ldx, const float* tinv, const vo
                              void* ws, size_t ws_bytes, uint8_t* Xq_out, float* sx_out,
                              int32_t* dbg_P, void* stream);
 
+/* ---------------------------------------------------------------------------
+ * The paper's own, fully 4-bit low-rank branch (section 4.3, Eq. 4):
+ *     Y = Q(X) [ Q(U) Q(V) + Q(R) ],   U = L1^T and V = L2^T both 4-bit with group scales.
+ *   stage 1  : H[m,j]  = sum_g sx[m,g]*su[j,g]*P1[m,g,j],  P1 = sum_{k in g} qx[m,k]*qu[j,k] (exact int32).  The branch
+ *              multiplies the SAME quantized activation tile as the residual (L179); H is summed in FP32 and never
+ *              leaves the chip (L177-179).
+ *   re-quantization on the fly (L181: "estimating an intermediate scale s_H from the INT32 accumulator and re-quantizing
+ *              on the fly"): one scale per token and per group of gr consecutive rank indices, gr = r for r <= 128,
+ *              else 128 (so r <= 128 or r == 256).  The quantizer of Eq. 1 in the FP32 operation order of
+ *              twq_quantize_act:  s_H = max(amax|H|, 2^-30) / 7;  Q_H = clamp(rint(H * (1 / s_H)), -7, 7), packed
+ *              4-bit in shared memory.
+ *   stage 2  : Ylr[m,n] = sum_h s_H[m,h]*sv[n,h]*P2[m,h,n],  P2 = sum_{j in h} Q_H[m,j]*qv[n,j] (exact int32)
+ *   epilogue : Y = round_out(Yres + Ylr), one store (L181); Yres as in twq_dual_linear.
+ * DESIGN.md readings R18-R22.  The quantizer, both branches and the epilogue are ONE launch per slab of at most 64 tokens
+ * (32 or 16 where the quantized activation tile of 64 tokens does not fit in shared memory: K > 4096 roughly).  Larger M:
+ * consecutive slabs, one launch each; a tcgen05 path for prefill-shaped M is not written yet.
+ *
+ * twq_pack_weights_q4lr -- offline re-layout (step a0) into an opaque blob of twq_packed_bytes_q4lr(N,K,r,G) bytes:
+ *   Rq  [N,K] int8, sw [N,K/G] fp16   the residual, as for twq_pack_weights
+ *   Uq  [r,K] int8 codes in [-8,7],  su [r,K/G] fp16     groups of G along K
+ *   Vq  [N,r] int8 codes in [-8,7],  sv [N,r/gr] fp16    groups of gr along r
+ *   r: a multiple of 16 in [16,128], or 256.  All pointers device, 16-byte aligned; packed 256-byte aligned.
+ *
+ * twq_dual_linear_q4lr_x -- the whole path from the raw activations.
+ *   X, ldx, tinv, Y, ydt, ldy, Xq_out, sx_out, dbg_P    as for twq_dual_linear_x (no workspace is ever needed)
+ *   packed                  blob written by twq_pack_weights_q4lr for (N,K,r,G)
+ *   dbg_H  [M,r] fp32       NULL, or receives H as the re-quantizer saw it
+ *   dbg_QH [M,r] int8       NULL, or receives the codes Q_H;  dbg_sH [M,r/gr] fp32: NULL, or receives s_H
+ *                           (parity evidence taken from the path that feeds Y; slows the call)
+ * Returns TWQ_ERR_UNSUPPORTED when even a 16-token slab's shared-memory plan does not fit (K / G > ~200 groups).
+ * Stream ordering and the other errors as for twq_dual_linear.
+ */
+size_t twq_packed_bytes_q4lr(int N, int K, int r, int G);
+twq_status twq_pack_weights_q4lr(const int8_t* Rq, const void* sw, const int8_t* Uq, const void* su,
+                                 const int8_t* Vq, const void* sv, int N, int K, int r, int G,
+                                 void* packed, size_t packed_bytes, void* stream);
+twq_status twq_dual_linear_q4lr_x(const void* X, int ldx, const float* tinv, const void* packed,
+                                  int M, int N, int K, int r, int G,
+                                  void* Y, twq_out_dtype ydt, int ldy,
+                                  uint8_t* Xq_out, float* sx_out, int32_t* dbg_P,
+                                  float* dbg_H, int8_t* dbg_QH, float* dbg_sH, void* stream);
+
 /* Number of kernel launches the last successful twq_dual_linear(_x) / twq_quantize_act /
  * twq_pack_weights call on this thread issued (bench.py's gpu_launches accounting). */
 int twq_last_launch_count(void);

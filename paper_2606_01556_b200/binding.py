@@ -14,7 +14,8 @@ _STATUS = {0: "TWQ_OK", 1: "TWQ_ERR_INVALID_ARG", 2: "TWQ_ERR_UNSUPPORTED", 3: "
 _OUT_TORCH = {OUT_BF16: torch.bfloat16, OUT_FP16: torch.float16, OUT_FP32: torch.float32}
 
 EXPORTS = ("twq_status_string", "twq_packed_bytes", "twq_pack_weights", "twq_quantize_act",
-           "twq_workspace_bytes", "twq_dual_linear", "twq_workspace_bytes_x", "twq_dual_linear_x", "twq_last_launch_count")
+           "twq_workspace_bytes", "twq_dual_linear", "twq_workspace_bytes_x", "twq_dual_linear_x", "twq_last_launch_count",
+           "twq_packed_bytes_q4lr", "twq_pack_weights_q4lr", "twq_dual_linear_q4lr_x")
 
 
 TESTING_EXPORTS = ("twq_testing_set_plan_flags", "twq_testing_get_plan_flags", "twq_testing_describe_plan",
@@ -75,6 +76,12 @@ def load_library(build_if_missing: bool = True):
     lib.twq_dual_linear_x.argtypes = [vp, i, vp, vp, i, i, i, i, i, vp, i, i, vp, sz, vp, vp, vp, vp]
     lib.twq_last_launch_count.restype = i
     lib.twq_last_launch_count.argtypes = []
+    lib.twq_packed_bytes_q4lr.restype = sz
+    lib.twq_packed_bytes_q4lr.argtypes = [i, i, i, i]
+    lib.twq_pack_weights_q4lr.restype = i
+    lib.twq_pack_weights_q4lr.argtypes = [vp, vp, vp, vp, vp, vp, i, i, i, i, vp, sz, vp]
+    lib.twq_dual_linear_q4lr_x.restype = i
+    lib.twq_dual_linear_q4lr_x.argtypes = [vp, i, vp, vp, i, i, i, i, i, vp, i, i, vp, vp, vp, vp, vp, vp, vp]
     # testing hooks (include/twq_testing.h): not part of the product ABI
     lib.twq_testing_set_plan_flags.restype = None
     lib.twq_testing_set_plan_flags.argtypes = [ctypes.c_uint]
@@ -241,6 +248,55 @@ def dual_linear_x(X, packed: PackedLayer, tinv=None, out_dtype: int = OUT_BF16, 
                                             _ptr(Xq_out), _ptr(sx_out), _ptr(dbg_P), _stream(stream))
     _check(code, "twq_dual_linear_x")
     return Y
+
+
+# ---- the paper's 4-bit low-rank branch (include/twq.h: twq_*_q4lr) ----
+def lowrank_group(r: int) -> int:
+    """Group of the re-quantized H along r (include/twq.h): r for r <= 128, else 128."""
+    return r if r <= 128 else 128
+
+
+def pack_weights_q4lr(Rq, sw, Uq, su, Vq, sv, G: int, stream=None) -> PackedLayer:
+    """twq_pack_weights_q4lr.  Rq int8 [N,K], sw fp16 [N,K/G], Uq int8 [r,K], su fp16 [r,K/G], Vq int8 [N,r],
+    sv fp16 [N,r/gr] (device, contiguous)."""
+    N, K = Rq.shape
+    r = int(Uq.shape[0])
+    nbytes = int(load_library().twq_packed_bytes_q4lr(N, K, r, G))
+    if nbytes == 0:
+        raise TwqError(1, "twq_packed_bytes_q4lr")
+    for t, dt in ((Rq, torch.int8), (Uq, torch.int8), (Vq, torch.int8), (sw, torch.float16), (su, torch.float16), (sv, torch.float16)):
+        assert t.dtype == dt and t.is_contiguous()
+    assert tuple(Uq.shape) == (r, K) and tuple(su.shape) == (r, K // G) and tuple(Vq.shape) == (N, r)
+    assert tuple(sv.shape) == (N, r // lowrank_group(r))
+    blob = torch.empty(nbytes, dtype=torch.uint8, device=Rq.device)
+    code = load_library().twq_pack_weights_q4lr(_ptr(Rq), _ptr(sw), _ptr(Uq), _ptr(su), _ptr(Vq), _ptr(sv), N, K, r, G,
+                                                _ptr(blob), nbytes, _stream(stream))
+    _check(code, "twq_pack_weights_q4lr")
+    return PackedLayer(blob, N, K, r, G)
+
+
+def dual_linear_q4lr_x(X, packed: PackedLayer, tinv=None, out_dtype: int = OUT_BF16, Y=None, Xq_out=None, sx_out=None,
+                       dbg_P=None, dbg_H=None, dbg_QH=None, dbg_sH=None, stream=None):
+    """twq_dual_linear_q4lr_x: quantizer, 4-bit residual, 4-bit two-stage low-rank branch with on-the-fly
+    re-quantization of H, one epilogue; one launch per slab of at most 64 tokens.  `packed` from pack_weights_q4lr."""
+    M = X.shape[0]
+    N, K, r, G = packed.N, packed.K, packed.r, packed.G
+    assert X.dtype == torch.bfloat16 and X.stride(1) == 1 and X.shape[1] == K
+    if Y is None:
+        Y = torch.empty((M, N), dtype=_OUT_TORCH.get(out_dtype, torch.bfloat16), device=X.device)
+    code = load_library().twq_dual_linear_q4lr_x(_ptr(X), X.stride(0), _ptr(tinv), _ptr(packed.blob), M, N, K, r, G,
+                                                 _ptr(Y), out_dtype, Y.stride(0), _ptr(Xq_out), _ptr(sx_out), _ptr(dbg_P),
+                                                 _ptr(dbg_H), _ptr(dbg_QH), _ptr(dbg_sH), _stream(stream))
+    _check(code, "twq_dual_linear_q4lr_x")
+    return Y
+
+
+def algorithmic_bytes_q4lr(M: int, N: int, K: int, r: int, G: int, out_bytes: int = 2) -> int:
+    """Bytes one twq_dual_linear_q4lr_x call must move: packed residual and its scales, both 4-bit factors and their
+    scales (4 bits per element + one FP16 scale per group), X read once, Y written once."""
+    ng, gr = K // G, lowrank_group(r)
+    w = N * K // 2 + 2 * N * ng + r * K // 2 + 2 * r * ng + N * r // 2 + 2 * N * (r // gr)
+    return w + 2 * M * K + out_bytes * M * N
 
 
 # ---- accounting used by bench.py (SURVEY.md section 8d; PAPER.md L86 byte arithmetic) ----

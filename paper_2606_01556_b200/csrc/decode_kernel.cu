@@ -146,11 +146,19 @@ __device__ __forceinline__ void lds_words(uint32_t (&dst)[kW], uint32_t a) {
 
 }  // namespace
 
-// kQ: the activation quantizer (steps a1-a2) runs inside this kernel: every cluster rank quantizes 1/cs of the K-groups of
-// all tokens and the cluster all-gathers codes and scales through distributed shared memory (twq_dual_linear_x).
-template <int G, int MT, bool kDbg, bool kQ>
+// kMode >= 1 (kQ): the activation quantizer (steps a1-a2) runs inside this kernel: every cluster rank quantizes 1/cs of the
+// K-groups of all tokens and the cluster all-gathers codes and scales through distributed shared memory (twq_dual_linear_x).
+// kMode == 2 (kL4): in addition the low-rank branch is the paper's own 4-bit pipeline (R18-R22):
+//   stage 1   H partial = sum over this rank's K-groups of sx*su*(qx . qu): the SAME quantized activation tile the residual
+//             uses (L179), int8 warp MMAs on 16*code like the residual, against the U section of the q4lr blob;
+//   exchange  FP32 sum in rank order, FP32 H to every peer;
+//   re-quantization on the fly (L181): per token and group of gr rank indices, s_H = max(amax, 2^-30)/7 and packed 4-bit
+//             Q_H in shared memory, in the activation quantizer's FP32 operation order;
+//   stage 2   Ylr = sum_h s_H*sv*(Q_H . qv): a second int8 MMA against the V section, folded into the same epilogue.
+template <int G, int MT, bool kDbg, int kMode>
 __global__ void __launch_bounds__(kDecThreads, 1)
 decode_dual_linear_kernel(const __grid_constant__ CUtensorMap tmXq, const __grid_constant__ DecodeParams p) {
+    constexpr bool kQ = kMode >= 1, kL4 = kMode == 2;
     extern __shared__ uint8_t dsm_raw[];
     // 1024-byte aligned base; the same offset in every CTA of the cluster (DSMEM addresses are formed from local ones)
     uint8_t* dsm = dsm_raw + ((1024u - (smem_u32(dsm_raw) & 1023u)) & 1023u);
@@ -181,11 +189,11 @@ decode_dual_linear_kernel(const __grid_constant__ CUtensorMap tmXq, const __grid
     const int tile0 = static_cast<int>(blockIdx.x * static_cast<unsigned>(p.n_tiles) / gridDim.x);
     const int ntile = static_cast<int>((blockIdx.x + 1u) * static_cast<unsigned>(p.n_tiles) / gridDim.x) - tile0;
     // stage-1 K slice of this cluster rank, in 32-wide slabs
-    const int units = p.K >> 5;
+    const int units = kL4 ? ng : (p.K >> 5);                // q4lr: the unit of the stage-1 slice is one K-group of U
     const int u0 = static_cast<int>(static_cast<unsigned>(units) * static_cast<unsigned>(rank) / static_cast<unsigned>(cs));
     const int nu = r > 0 ? static_cast<int>(static_cast<unsigned>(units) * static_cast<unsigned>(rank + 1) / static_cast<unsigned>(cs)) - u0 : 0;
     const int nl1 = (nu + p.sc - 1) / p.sc;                 // stage-1 ring chunks
-    const int slab_bytes = r * 64;
+    const int slab_bytes = kL4 ? r * (G / 2) + r * 2 : r * 64;
     // Residual warps form a (tile group x K part) grid: TG groups of at most kTPW tiles, P = nrw / TG warps per group,
     // warp `part` of a group taking the K-groups g = part (mod P).  A warp thus expands the activation fragments of a
     // K-group once for all its tiles, and its tiles are independent MMA chains.
@@ -259,9 +267,10 @@ decode_dual_linear_kernel(const __grid_constant__ CUtensorMap tmXq, const __grid
             // the scales ride on the first chunk's barrier (every residual warp waits for it first); stage 2 reads this
             // CTA's rows of L2T straight from L2
             bulk_load_1d_a(smem_u32(dsm + p.off_sw), p.sw16 + static_cast<size_t>(tile0) * ng * 8, sw_bytes, DBAR(D_FULL), pol);
-            if (r > 0)
-                bulk_prefetch_l2(static_cast<const uint8_t*>(p.L2T) + static_cast<size_t>(tile0) * 8 * r * 2,
-                                 static_cast<uint32_t>(ntile) * 8 * r * 2);
+            if (r > 0) {
+                const uint32_t trow = kL4 ? static_cast<uint32_t>(p.nh) * 8 * (p.grs / 2) : 8u * r * 2;   // bytes of a tile's stage-2 operand
+                bulk_prefetch_l2(static_cast<const uint8_t*>(p.L2T) + static_cast<size_t>(tile0) * trow, static_cast<uint32_t>(ntile) * trow);
+            }
         }
         TWQ_DSTAMP(2);
         pdl_wait();                                              // later laps carry Xq boxes (twq_quantize_act's output)
@@ -315,7 +324,16 @@ decode_dual_linear_kernel(const __grid_constant__ CUtensorMap tmXq, const __grid
         const int lrt = threadIdx.x - nrw * 32, nlr = lrw * 32;
         pdl_wait();                                              // X comes from the previous kernel of the stream
         TWQ_DSTAMP(2);
-        {
+        uint8_t* sQH = dsm + p.off_qh;                           // q4lr: packed Q_H [nh][kMp][grs/2]
+        float* sSH = reinterpret_cast<float*>(dsm + p.off_sh);   // q4lr: s_H * 2^-8 [nh][kMp]
+        float* sH32 = reinterpret_cast<float*>(dsm + p.off_h);   // q4lr: FP32 H [kMp][r]
+        if constexpr (kL4) {
+            // Q_H rows beyond M and the padding beyond gr codes are zero codes; nothing else to stage: stage 1 multiplies the
+            // quantized activation tile, and this rank's K-groups of it are the ones this CTA quantized itself
+            for (int i = lrt; i < p.nh * kMp * (p.grs / 8); i += nlr) reinterpret_cast<uint32_t*>(sQH)[i] = 0u;
+            for (int i = lrt; i < p.nh * kMp; i += nlr) sSH[i] = 0.0f;
+            asm volatile("bar.sync 4, %0;" ::"r"((nrw + lrw) * 32) : "memory");   // this CTA's share of Xq / sx is in shared memory
+        } else {
             // X slice (tokens x 32*nu k, BF16 -> FP16) into shared memory, four 16-byte loads in flight per thread
             const uint16_t* X = static_cast<const uint16_t*>(p.X);
             const int chunks = nu * 4;                           // 16-byte chunks per token row
@@ -420,10 +438,109 @@ decode_dual_linear_kernel(const __grid_constant__ CUtensorMap tmXq, const __grid
                 }
             }
         };
-        if (nq_need <= 1) stage1(std::integral_constant<int, 1>{});
-        else if (nq_need == 2) stage1(std::integral_constant<int, 2>{});
-        else if (nq_need <= 4 || MT == 4) stage1(std::integral_constant<int, 4>{});   // MT == 4 runs 8 low-rank warps: r / 64 <= 4
-        else stage1(std::integral_constant<int, MT == 4 ? 4 : kJT>{});
+        // ---- q4lr stage 1: the same loop shape on int8 MMAs.  A j tile of one K-group of U is 8 rows x G/2 bytes, exactly a
+        // block of R4, and the activation fragments are the residual's: codes from the resident tile [g][token][G/2], scales
+        // (with 2^-8 for the two 16*code operands) from sSx.  j tiles go in batches of at most four (registers).
+        auto stage1q = [&](auto nq_c) {
+            constexpr int NQ = decltype(nq_c)::value;
+            constexpr int QB = NQ < 4 ? NQ : 4;
+            float d[NQ][MT][4];
+#pragma unroll
+            for (int q = 0; q < NQ; ++q)
+#pragma unroll
+                for (int t = 0; t < MT; ++t)
+#pragma unroll
+                    for (int e = 0; e < 4; ++e) d[q][t][e] = 0.0f;
+            const uint32_t ulane = smem_u32(dsm + p.off_l1) + gid * (G / 2) + tid4 * (kW * 4);
+            const uint32_t sulane = smem_u32(dsm + p.off_l1) + r * (G / 2) + tid4 * 4;
+            uint32_t uoff[NQ], soff[NQ];
+#pragma unroll
+            for (int q = 0; q < NQ; ++q) {
+                const uint32_t jt = static_cast<uint32_t>(min(lw + q * lrw, max(njt - 1, 0)));
+                uoff[q] = jt * kBlk;
+                soff[q] = jt * 16u;
+            }
+            uint32_t xa = smem_u32(dsm + p.off_xq) + gid * (G / 2) + tid4 * (kW * 4) + u0 * (kMp * (G / 2));
+            uint32_t sxp = smem_u32(sSx) + gid * 4 + u0 * (kMp * 4);
+            constexpr uint32_t x8 = 8u * (G / 2);
+            const uint32_t chunk_bytes = static_cast<uint32_t>(p.sc) * slab_bytes;
+            int slot = 0, lap = 0;
+            uint32_t slot_a = 0;
+#pragma unroll 1
+            for (int i = 0; i < nl1; ++i) {
+                mbar_wait_a(DBAR(D_L1FULL + slot), lap & 1);
+                const int cnt = min(p.sc, nu - i * p.sc);
+                uint32_t la = slot_a;
+#pragma unroll 1
+                for (int sl = 0; sl < cnt; ++sl, la += slab_bytes, xa += kMp * (G / 2), sxp += kMp * 4) {
+#pragma unroll
+                    for (int qb = 0; qb < NQ; qb += QB) {
+                        uint32_t wt[QB][kW], suh[QB];
+#pragma unroll
+                        for (int b = 0; b < QB; ++b) {
+                            lds_words<kW>(wt[b], ulane + la + uoff[qb + b]);
+                            suh[b] = lds_u32(sulane + la + soff[qb + b]);
+                        }
+#pragma unroll
+                        for (int mt = 0; mt < MT; ++mt) {
+                            uint32_t x0[kW], x1[kW];
+                            lds_words<kW>(x0, xa + mt * 2 * x8);
+                            lds_words<kW>(x1, xa + mt * 2 * x8 + x8);
+                            const float sx0 = __uint_as_float(lds_u32(sxp + mt * 64));
+                            const float sx1 = __uint_as_float(lds_u32(sxp + mt * 64 + 32));
+                            int dd[QB][4];
+#pragma unroll
+                            for (int b = 0; b < QB; ++b)
+#pragma unroll
+                                for (int e = 0; e < 4; ++e) dd[b][e] = 0;
+#pragma unroll
+                            for (int w = 0; w < kW; ++w) {
+                                const uint32_t a0 = d_lo16(x0[w]), a1 = d_lo16(x1[w]), a2 = d_hi16(x0[w]), a3 = d_hi16(x1[w]);
+#pragma unroll
+                                for (int b = 0; b < QB; ++b) imma_16832(dd[b], a0, a1, a2, a3, d_lo16(wt[b][w]), d_hi16(wt[b][w]));
+                            }
+#pragma unroll
+                            for (int b = 0; b < QB; ++b) {
+                                const float2 su2 = __half22float2(*reinterpret_cast<const __half2*>(&suh[b]));
+                                float (&a)[4] = d[qb + b][mt];
+                                a[0] = fmaf(static_cast<float>(dd[b][0]) * su2.x, sx0, a[0]);
+                                a[1] = fmaf(static_cast<float>(dd[b][1]) * su2.y, sx0, a[1]);
+                                a[2] = fmaf(static_cast<float>(dd[b][2]) * su2.x, sx1, a[2]);
+                                a[3] = fmaf(static_cast<float>(dd[b][3]) * su2.y, sx1, a[3]);
+                            }
+                        }
+                    }
+                }
+                __syncwarp();
+                if (lane == 0) mbar_arrive_a(DBAR(D_L1EMPTY + slot));
+                slot_a += chunk_bytes;
+                if (++slot == p.l1_slots) { slot = 0; slot_a = 0; ++lap; }
+            }
+            TWQ_DSTAMP(4);
+#pragma unroll
+            for (int q = 0; q < NQ; ++q) {
+                const int jt = lw + q * lrw;
+                if (jt < njt) {
+                    const int j = jt * 8 + tid4 * 2;
+#pragma unroll
+                    for (int t = 0; t < MT; ++t) {
+                        *reinterpret_cast<float2*>(sHpart + (t * 16 + gid) * r + j) = make_float2(d[q][t][0], d[q][t][1]);
+                        *reinterpret_cast<float2*>(sHpart + (t * 16 + gid + 8) * r + j) = make_float2(d[q][t][2], d[q][t][3]);
+                    }
+                }
+            }
+        };
+        if constexpr (kL4) {
+            if (nq_need <= 1) stage1q(std::integral_constant<int, 1>{});
+            else if (nq_need == 2) stage1q(std::integral_constant<int, 2>{});
+            else if (nq_need <= 4 || MT == 4) stage1q(std::integral_constant<int, 4>{});
+            else stage1q(std::integral_constant<int, MT == 4 ? 4 : kJT>{});
+        } else {
+            if (nq_need <= 1) stage1(std::integral_constant<int, 1>{});
+            else if (nq_need == 2) stage1(std::integral_constant<int, 2>{});
+            else if (nq_need <= 4 || MT == 4) stage1(std::integral_constant<int, 4>{});   // MT == 4 runs 8 low-rank warps: r / 64 <= 4
+            else stage1(std::integral_constant<int, MT == 4 ? 4 : kJT>{});
+        }
         // stage-2 operand of this warp's first tile (L2T rows, L2-resident by now), ahead of the exchange
         constexpr int kL2 = 8;                                   // 32-wide j steps (r <= 256)
         uint4 l2v[kL2];
@@ -434,7 +551,23 @@ decode_dual_linear_kernel(const __grid_constant__ CUtensorMap tmXq, const __grid
             for (int js = 0; js < kL2; ++js)
                 l2v[js] = (js * 32 + tid4 * 8 < r) ? ldg_nc(lrow + js * 64) : make_uint4(0, 0, 0, 0);
         };
-        if (lw < ntile) load_l2(lw);
+        // q4lr: this thread's words of the V rows of a tile (row gid, grs/8 bytes from tid4 * grs/8) and the tile's scales
+        const int kWr = p.grs >> 5, vrow = p.grs >> 1;
+        uint32_t vv[2][4], svh[2];
+        auto load_v = [&](int t) {
+            const uint8_t* vb = static_cast<const uint8_t*>(p.L2T) + static_cast<size_t>(tile0 + t) * p.nh * 8 * vrow + gid * vrow + tid4 * (kWr * 4);
+#pragma unroll
+            for (int h = 0; h < 2; ++h) {
+#pragma unroll
+                for (int w = 0; w < 4; ++w)
+                    vv[h][w] = (h < p.nh && w < kWr) ? __ldg(reinterpret_cast<const uint32_t*>(vb + h * 8 * vrow) + w) : 0u;
+                svh[h] = h < p.nh ? __ldg(reinterpret_cast<const uint32_t*>(p.sv16 + (static_cast<size_t>(tile0 + t) * p.nh + h) * 8) + tid4) : 0u;
+            }
+        };
+        if (lw < ntile) {
+            if constexpr (kL4) load_v(lw);
+            else load_l2(lw);
+        }
         named_bar_sync(1, nlr);                                  // this CTA's partial is complete in shared memory
         TWQ_DSTAMP(5);
         // ---- H = sum of the cluster's partials (fixed order), FP16, in every CTA's shared memory
@@ -459,10 +592,15 @@ decode_dual_linear_kernel(const __grid_constant__ CUtensorMap tmXq, const __grid
                 float sum = 0.0f;
 #pragma unroll
                 for (int q = 0; q < 16; ++q) sum += v[q];
-                sum = fminf(fmaxf(sum, -65504.0f), 65504.0f);
-                const __half hv = __float2half_rn(sum);
-                const uint32_t dsta = smem_u32(sH + m * hstride + j);
-                for (int pr = 0; pr < cs; ++pr) st_dsmem_u16(mapa_u32(dsta, pr), *reinterpret_cast<const uint16_t*>(&hv));
+                if constexpr (kL4) {
+                    const uint32_t dsta = smem_u32(sH32 + m * r + j);
+                    for (int pr = 0; pr < cs; ++pr) st_dsmem_u32(mapa_u32(dsta, pr), __float_as_uint(sum));
+                } else {
+                    sum = fminf(fmaxf(sum, -65504.0f), 65504.0f);
+                    const __half hv = __float2half_rn(sum);
+                    const uint32_t dsta = smem_u32(sH + m * hstride + j);
+                    for (int pr = 0; pr < cs; ++pr) st_dsmem_u16(mapa_u32(dsta, pr), *reinterpret_cast<const uint16_t*>(&hv));
+                }
             }
             TWQ_DCLK(11);
             TWQ_DSTAMP(8);
@@ -473,20 +611,100 @@ decode_dual_linear_kernel(const __grid_constant__ CUtensorMap tmXq, const __grid
         } else {
             for (int i = lrt; i < p.M * r; i += nlr) {
                 const int m = i / r, j = i - m * r;
-                const float s = fminf(fmaxf(sHpart[i], -65504.0f), 65504.0f);
-                sH[m * hstride + j] = __float2half_rn(s);
+                if constexpr (kL4) {
+                    sH32[i] = sHpart[i];
+                } else {
+                    const float s = fminf(fmaxf(sHpart[i], -65504.0f), 65504.0f);
+                    sH[m * hstride + j] = __float2half_rn(s);
+                }
+            }
+            named_bar_sync(1, nlr);
+        }
+        if constexpr (kL4) {
+            // ---- re-quantization of H on the fly (Eq. 1 L43-47 on the FP32 H, R18 / R19): eight lanes
+            // per (token, r-group), gr/8 consecutive elements each; every CTA does this for all of H (2 K elements at most)
+            const int e = p.gr >> 3, items = p.M * p.nh;
+            const int li = lane & 7, sub = lane >> 3;
+            for (int base = lw * 4; base < items; base += lrw * 4) {
+                const int it = base + sub;
+                const bool on = it < items;
+                const int m = on ? it / p.nh : 0, h = on ? it - m * p.nh : 0;
+                const float* hp = sH32 + m * r + h * p.gr + li * e;
+                float amax = 0.0f;
+                if (on)
+                    for (int i = 0; i < e; ++i) amax = fmaxf(amax, fabsf(hp[i]));
+                amax = fmaxf(amax, __shfl_xor_sync(0xffffffffu, amax, 4));
+                amax = fmaxf(amax, __shfl_xor_sync(0xffffffffu, amax, 2));
+                amax = fmaxf(amax, __shfl_xor_sync(0xffffffffu, amax, 1));
+                const float sc = __fdiv_rn(fmaxf(amax, 0x1p-30f), 7.0f);
+                const float inv = __fdiv_rn(1.0f, sc);
+                if (on) {
+                    uint8_t* qp = sQH + (h * kMp + m) * vrow + li * (e >> 1);
+                    const bool dbg_out = kDbg && blockIdx.x == 0;
+                    for (int i = 0; i < e; i += 2) {
+                        int q0 = __float2int_rn(__fmul_rn(hp[i], inv)), q1 = __float2int_rn(__fmul_rn(hp[i + 1], inv));
+                        q0 = max(-7, min(7, q0));
+                        q1 = max(-7, min(7, q1));
+                        qp[i >> 1] = static_cast<uint8_t>((q0 & 0xF) | ((q1 & 0xF) << 4));       // low nibble = even index
+                        if (dbg_out) {
+                            const size_t o = static_cast<size_t>(m) * r + h * p.gr + li * e + i;
+                            if (p.dbgQH != nullptr) { p.dbgQH[o] = static_cast<int8_t>(q0); p.dbgQH[o + 1] = static_cast<int8_t>(q1); }
+                            if (p.dbgH != nullptr) { p.dbgH[o] = hp[i]; p.dbgH[o + 1] = hp[i + 1]; }
+                        }
+                    }
+                    if (li == 0) {
+                        sSH[h * kMp + m] = sc * 0x1p-8f;                 // both MMA operands are 16*code
+                        if (dbg_out && p.dbgSH != nullptr) p.dbgSH[static_cast<size_t>(m) * p.nh + h] = sc;
+                    }
+                }
             }
             named_bar_sync(1, nlr);
         }
         TWQ_DSTAMP(9);
         // ---- stage 2: Ylr[m, n] = sum_j H[m,j] * L2T[n,j] for this CTA's tiles
         for (int t = lw; t < ntile; t += lrw) {
-            if (t != lw) load_l2(t);
+            if (t != lw) {
+                if constexpr (kL4) load_v(t);
+                else load_l2(t);
+            }
             float d2[MT][4];
 #pragma unroll
             for (int mt = 0; mt < MT; ++mt)
 #pragma unroll
                 for (int e = 0; e < 4; ++e) d2[mt][e] = 0.0f;
+            if constexpr (kL4) {
+                // ---- q4lr stage 2: Ylr = sum_h s_H * sv * (Q_H . qv), int8 MMAs on 16*code (K order: word w of a thread's
+                // grs/8 bytes in K-step w, for Q_H and V alike)
+#pragma unroll
+                for (int h = 0; h < 2; ++h) {
+                    if (h < p.nh) {                              // warp-uniform
+                        const float2 sv2 = __half22float2(*reinterpret_cast<const __half2*>(&svh[h]));
+#pragma unroll
+                        for (int mt = 0; mt < MT; ++mt) {
+                            const uint32_t arow = smem_u32(sQH) + ((h * kMp + mt * 16 + gid) * vrow) + tid4 * (kWr * 4);
+                            uint32_t x0[4] = {0u, 0u, 0u, 0u}, x1[4] = {0u, 0u, 0u, 0u};
+                            if (kWr == 4) {
+                                lds_words<4>(x0, arow);
+                                lds_words<4>(x1, arow + 8 * vrow);
+                            } else {
+#pragma unroll
+                                for (int w = 0; w < 3; ++w)
+                                    if (w < kWr) { x0[w] = lds_u32(arow + w * 4); x1[w] = lds_u32(arow + 8 * vrow + w * 4); }
+                            }
+                            int dd[4] = {0, 0, 0, 0};
+#pragma unroll
+                            for (int w = 0; w < 4; ++w)
+                                if (w < kWr)
+                                    imma_16832(dd, d_lo16(x0[w]), d_lo16(x1[w]), d_hi16(x0[w]), d_hi16(x1[w]), d_lo16(vv[h][w]), d_hi16(vv[h][w]));
+                            const float s0 = sSH[h * kMp + mt * 16 + gid], s1 = sSH[h * kMp + mt * 16 + gid + 8];
+                            d2[mt][0] = fmaf(static_cast<float>(dd[0]) * sv2.x, s0, d2[mt][0]);
+                            d2[mt][1] = fmaf(static_cast<float>(dd[1]) * sv2.y, s0, d2[mt][1]);
+                            d2[mt][2] = fmaf(static_cast<float>(dd[2]) * sv2.x, s1, d2[mt][2]);
+                            d2[mt][3] = fmaf(static_cast<float>(dd[3]) * sv2.y, s1, d2[mt][3]);
+                        }
+                    }
+                }
+            } else {
 #pragma unroll
             for (int js = 0; js < kL2; ++js) {
                 if (js * 32 < r) {                               // warp-uniform
@@ -502,6 +720,7 @@ decode_dual_linear_kernel(const __grid_constant__ CUtensorMap tmXq, const __grid
                         hmma_16816(d2[mt], a.z, b.z, a.w, b.w, l2v[js].z, l2v[js].w);
                     }
                 }
+            }
             }
             const int nl = t * 8 + tid4 * 2;
 #pragma unroll
@@ -589,6 +808,7 @@ decode_dual_linear_kernel(const __grid_constant__ CUtensorMap tmXq, const __grid
                 }
             }
             named_bar_sync(2, nrw * 32);                         // this CTA's share is stored (everywhere)
+            if constexpr (kL4) asm volatile("bar.arrive 4, %0;" ::"r"((nrw + lrw) * 32) : "memory");   // q4lr stage 1 may read it
             if (cs > 1) {
                 if (rw == 0 && lane < cs) mbar_arrive_remote(mapa_u32(DBAR(D_XQ), static_cast<uint32_t>(lane)));
                 mbar_wait_cluster_a(DBAR(D_XQ), 0);              // every rank's share has arrived here
@@ -878,9 +1098,9 @@ namespace {
 
 constexpr int kMaxDevices = 64;
 
-template <int G, int MT, bool kDbg, bool kQ>
+template <int G, int MT, bool kDbg, int kMode>
 cudaError_t decode_launch_inst(const CUtensorMap& tmXq, const DecodeParams& p, cudaStream_t stream) {
-    auto kern = decode_dual_linear_kernel<G, MT, kDbg, kQ>;
+    auto kern = decode_dual_linear_kernel<G, MT, kDbg, kMode>;
     static bool attr_done[kMaxDevices] = {};       // function attributes are per device
     int dev = 0;
     cudaError_t e = cudaGetDevice(&dev);
@@ -924,7 +1144,7 @@ int decode_cluster_capacity(int cs, int num_sms) {
     if (cache[dev][cs] > 0) return cache[dev][cs];
     int n = 0;
     if (have_dev) {
-        auto kern = decode_dual_linear_kernel<128, 1, false, false>;
+        auto kern = decode_dual_linear_kernel<128, 1, false, 0>;
         if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, kDecSmemMax) == cudaSuccess &&
             cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1) == cudaSuccess) {
             cudaLaunchConfig_t cfg = {};
@@ -954,9 +1174,12 @@ int round_up_i(int x, int a) { return (x + a - 1) / a * a; }
 }  // namespace
 
 // Fills the decode plan; false when the shape is outside this kernel's domain (the tcgen05 kernel takes it).
-bool decode_make_plan(int M, int N, int K, int r, int G, int num_sms, bool quant, DecodeParams* out) {
+// quant: 0 = codes and scales come from twq_quantize_act, 1 = in-kernel quantizer, 2 = in-kernel quantizer + 4-bit low-rank branch
+bool decode_make_plan(int M, int N, int K, int r, int G, int num_sms, int quant, DecodeParams* out) {
     if (M < 1 || M > kDecodeMaxM || (G != 64 && G != 128) || K % G != 0 || N % 16 != 0 || r % 16 != 0 || r > 256) return false;
-    if (plan_flags() & kPlanNoDecode) return false;
+    const bool lr4 = quant == 2;
+    if (lr4 && (r == 0 || (r > 128 && r != 256))) return false;   // groups of H along r: r itself up to 128, else 128
+    if ((plan_flags() & kPlanNoDecode) && !lr4) return false;
     DecodeParams p = {};
     p.M = M; p.N = N; p.K = K; p.r = r; p.ng = K / G;
     p.n_tiles = N / 8;
@@ -967,7 +1190,10 @@ bool decode_make_plan(int M, int N, int K, int r, int G, int num_sms, bool quant
     // cluster size: H is shared by the cluster and every cluster streams all of L1 (K*r*2 bytes) from L2, so the
     // largest cluster that still covers 70 % of the SMs wins; otherwise the size covering the most SMs
     p.cs = 1;
-    p.quant = quant ? 1 : 0;
+    p.quant = quant;
+    p.gr = lr4 ? (r <= 128 ? r : 128) : 0;
+    p.grs = (p.gr + 31) / 32 * 32;
+    p.nh = lr4 ? r / p.gr : 0;
     int cap = num_sms;
     if (r > 0 || quant) {                                     // the in-kernel quantizer shares its work across the cluster too
         int best = 0;
@@ -994,9 +1220,10 @@ bool decode_make_plan(int M, int N, int K, int r, int G, int num_sms, bool quant
     if (p.tmax > kTPWh * nrw) return false;
     // ---- shared-memory plan
     const int kBlk = 4 * G;
-    p.nu_max = r > 0 ? ((K >> 5) + p.cs - 1) / p.cs : 0;
+    p.nu_max = r > 0 ? ((lr4 ? p.ng : (K >> 5)) + p.cs - 1) / p.cs : 0;   // stage-1 units: 32-wide slabs of L1, or K-groups of U
     // X slice rows: a pitch of 64 bytes mod 128, so that the 16-byte fragment reads of two adjacent tokens hit disjoint banks
-    p.xs_stride = p.nu_max * 32 + ((p.nu_max & 1) ? 0 : 32);
+    p.xs_stride = lr4 ? 0 : p.nu_max * 32 + ((p.nu_max & 1) ? 0 : 32);
+    const int slab_bytes = lr4 ? r * (G / 2) + r * 2 : r * 64;
     int o = 0;
     p.off_bar = o; o += round_up_i(D_COUNT * 8, 128);
     p.off_sw = o; o += round_up_i(p.tmax * p.ng * 16, 128);
@@ -1004,19 +1231,21 @@ bool decode_make_plan(int M, int N, int K, int r, int G, int num_sms, bool quant
     p.off_xq = o; o += quant ? round_up_i(p.ng * p.mp * (G / 2), 128) : 0;   // resident codes [g][token][G/2] of the in-kernel quantizer
     p.off_ylr = o; o += r > 0 ? round_up_i(p.mp * p.tmax * 8 * 4, 128) : 0;
     p.off_hpart = o; o += r > 0 ? round_up_i(p.mp * r * 4, 128) : 0;
-    p.off_h = o; o += r > 0 ? round_up_i(p.mp * (r + 8) * 2, 128) : 0;
+    p.off_h = o; o += r > 0 ? round_up_i(lr4 ? p.mp * r * 4 : p.mp * (r + 8) * 2, 128) : 0;
+    p.off_qh = o; o += lr4 ? round_up_i(p.nh * p.mp * (p.grs / 2), 128) : 0;
+    p.off_sh = o; o += lr4 ? round_up_i(p.nh * p.mp * 4, 128) : 0;
     p.xrows = M <= 8 ? 8 : p.mp;                              // token rows of the staged X slice
-    p.off_xs = o; o += r > 0 ? round_up_i(p.xrows * p.xs_stride * 2, 128) : 0;
+    p.off_xs = o; o += (r > 0 && !lr4) ? round_up_i(p.xrows * p.xs_stride * 2, 128) : 0;
     // stage-1 ring: chunks of ~16 KB of L1 slabs
     p.sc = 1; p.l1_slots = 1;
     if (r > 0) {
-        p.sc = (16 * 1024) / (r * 64);
+        p.sc = (16 * 1024) / slab_bytes;
         if (p.sc < 1) p.sc = 1;
         if (p.sc > p.nu_max) p.sc = p.nu_max > 0 ? p.nu_max : 1;
         const int chunks = (p.nu_max + p.sc - 1) / p.sc;
         const int max_l1 = p.mt == 4 ? 2 : kMaxL1Slots;       // 64 tokens: the X slice and the H partial take the room
         p.l1_slots = chunks < max_l1 ? (chunks > 0 ? chunks : 1) : max_l1;
-        p.off_l1 = o; o += p.l1_slots * p.sc * r * 64;
+        p.off_l1 = o; o += p.l1_slots * p.sc * slab_bytes;
     } else {
         p.off_l1 = o;
     }
@@ -1052,11 +1281,12 @@ bool decode_make_plan(int M, int N, int K, int r, int G, int num_sms, bool quant
 }
 
 cudaError_t launch_decode(const CUtensorMap& tmXq, const DecodeParams& p, int G, cudaStream_t stream) {
-    const bool dbg = p.dbgP != nullptr;
+    const bool dbg = p.dbgP != nullptr || p.dbgH != nullptr || p.dbgQH != nullptr || p.dbgSH != nullptr;
 #define TWQ_DCASE(g, m)                                                                   \
     if (G == g && p.mt == m) {                                                            \
-        if (p.quant) return dbg ? decode_launch_inst<g, m, true, true>(tmXq, p, stream) : decode_launch_inst<g, m, false, true>(tmXq, p, stream); \
-        return dbg ? decode_launch_inst<g, m, true, false>(tmXq, p, stream) : decode_launch_inst<g, m, false, false>(tmXq, p, stream);        \
+        if (p.quant == 2) return dbg ? decode_launch_inst<g, m, true, 2>(tmXq, p, stream) : decode_launch_inst<g, m, false, 2>(tmXq, p, stream); \
+        if (p.quant == 1) return dbg ? decode_launch_inst<g, m, true, 1>(tmXq, p, stream) : decode_launch_inst<g, m, false, 1>(tmXq, p, stream); \
+        return dbg ? decode_launch_inst<g, m, true, 0>(tmXq, p, stream) : decode_launch_inst<g, m, false, 0>(tmXq, p, stream);        \
     }
     TWQ_DCASE(128, 1) TWQ_DCASE(128, 2) TWQ_DCASE(128, 4) TWQ_DCASE(64, 1) TWQ_DCASE(64, 2) TWQ_DCASE(64, 4)
 #undef TWQ_DCASE

@@ -62,7 +62,15 @@ struct DecodeParams {
     int xs_stride;           // halves per token row of the staged FP16 X slice
     int xrows;               // token rows staged (8 when M <= 8, else mp)
     int off_ring, off_l1, off_sw, off_xs, off_hpart, off_h, off_ylr, off_sx, off_xq, off_res, off_bar, smem_bytes;
-    int quant;               // 1: the activation quantizer runs inside the kernel (twq_dual_linear_x)
+    int quant;               // 1: the activation quantizer runs inside the kernel (twq_dual_linear_x);
+                             // 2: the same with the 4-bit low-rank branch (twq_dual_linear_q4lr_x): then L1D / L2T point to the
+                             //    U / V sections of a q4lr blob, "slab" means one K-group of U, and off_h holds FP32 H
+    int gr, grs, nh;         // q4lr: group of the re-quantized H along r, its stored size (rounded up to 32 codes), r / gr
+    int off_qh, off_sh;      // q4lr: packed Q_H [nh][mp][grs/2], scales s_H * 2^-8 [nh][mp]
+    const __half* sv16;      // q4lr: [N/8][nh][8]
+    float* dbgH;             // q4lr: NULL, or [M][r] FP32 H before re-quantization (parity evidence)
+    int8_t* dbgQH;           // q4lr: NULL, or [M][r] codes of the re-quantized H
+    float* dbgSH;            // q4lr: NULL, or [M][nh] scales s_H
     const float* tinv;       // quant: [K] diagonal transform or NULL
     uint8_t* xq_out;         // quant: NULL, or [M][K/2] copy of the codes (parity evidence)
     float* sx_out;           // quant: NULL, or [M][K/G] copy of the scales
@@ -76,7 +84,7 @@ struct DecodeParams {
     int32_t* dbgP;
     unsigned long long* trace;   // NULL, or the timeline buffer of a -DTWQ_TRACE build (trace.cuh)
 };
-bool decode_make_plan(int M, int N, int K, int r, int G, int num_sms, bool quant, DecodeParams* out);
+bool decode_make_plan(int M, int N, int K, int r, int G, int num_sms, int quant, DecodeParams* out);
 cudaError_t launch_decode(const CUtensorMap& tmXq, const DecodeParams& p, int G, cudaStream_t stream);
 
 // Planner overrides for tests (include/twq_testing.h, twq_testing_set_plan_flags): a process-wide word, never the
@@ -103,5 +111,8 @@ cudaError_t launch_quantize_act(const void* X, int M, int K, int ldx, const floa
                                 float* sx, cudaStream_t stream);
 cudaError_t launch_pack_weights(const int8_t* Rq, const void* sw, const void* L1, const void* L2, int N, int K, int r,
                                 int G, void* packed, cudaStream_t stream, int* launches);
+cudaError_t launch_pack_weights_q4lr(const int8_t* Rq, const void* sw, const int8_t* Uq, const void* su, const int8_t* Vq,
+                                     const void* sv, int N, int K, int r, int G, void* packed, cudaStream_t stream,
+                                     int* launches);
 
 }  // namespace twq

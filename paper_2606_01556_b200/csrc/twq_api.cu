@@ -92,14 +92,15 @@ size_t ctr_bytes(const twq::FusedPlan& pl) {
 struct CallPlan {
     int dev, M, N, K, r, G;
     unsigned flags;
-    bool quant;                // planned for twq_dual_linear_x (in-kernel quantizer): only small-batch plans exist
+    int quant;                 // 1: planned for twq_dual_linear_x (in-kernel quantizer), 2: for twq_dual_linear_q4lr_x; only
+                               // small-batch plans exist for these
     bool valid, decode;
     twq::DecodeParams dp;      // decode == true
     twq::FusedPlan fp;         // decode == false
     size_t ws_bytes;
 };
 
-const CallPlan* get_plan(int M, int N, int K, int r, int G, bool quant = false) {
+const CallPlan* get_plan(int M, int N, int K, int r, int G, int quant = 0) {
     constexpr int kSlots = 16;
     thread_local CallPlan cache[kSlots];
     thread_local unsigned next = 0;
@@ -400,7 +401,7 @@ twq_status twq_dual_linear(const void* X, int ldx, const uint8_t* Xq, const floa
 // (codes, scales; each 256-byte aligned) in front of what twq_dual_linear itself needs.
 size_t twq_workspace_bytes_x(int M, int N, int K, int r, int G) {
     if (!shape_ok(M, N, K, r, G)) return 0;
-    if (get_plan(M, N, K, r, G, true)) return 0;
+    if (get_plan(M, N, K, r, G, 1)) return 0;
     return twq::align256(static_cast<size_t>(M) * (K / 2)) + twq::align256(static_cast<size_t>(M) * (K / G) * sizeof(float)) +
            twq_workspace_bytes(M, N, K, r, G);
 }
@@ -420,7 +421,7 @@ twq_status twq_dual_linear_x(const void* X, int ldx, const float* tinv, const vo
     if (need > 0 && (!ws || ws_bytes < need)) return TWQ_ERR_WORKSPACE;
     if (need > 0 && (reinterpret_cast<uintptr_t>(ws) & 255u)) return TWQ_ERR_INVALID_ARG;
     if (!device_is_sm100()) return TWQ_ERR_UNSUPPORTED;
-    if (const CallPlan* cp = get_plan(M, N, K, r, G, true)) {
+    if (const CallPlan* cp = get_plan(M, N, K, r, G, 1)) {
         // small batches: quantizer, both branches and the epilogue in ONE launch
         const twq::PackedLayout lay = twq::packed_layout(N, K, r, G);
         const uint8_t* base = static_cast<const uint8_t*>(packed);
@@ -451,6 +452,87 @@ twq_status twq_dual_linear_x(const void* X, int ldx, const float* tinv, const vo
     st = twq_dual_linear(X, ldx, xq, sx, packed, M, N, K, r, G, Y, ydt, ldy, w, ws_bytes - used, dbg_P, stream);
     if (st != TWQ_OK) return st;
     g_last_launches = 2;
+    return TWQ_OK;
+}
+
+// ------------------------------------------------------------------ the paper's 4-bit low-rank branch
+static bool q4lr_rank_ok(int r) { return r >= 0 && r % 16 == 0 && (r <= 128 || r == 256); }
+
+size_t twq_packed_bytes_q4lr(int N, int K, int r, int G) {
+    if (!shape_ok(1, N, K, r, G) || !q4lr_rank_ok(r)) return 0;
+    return twq::packed_layout_q4lr(N, K, r, G).total;
+}
+
+twq_status twq_pack_weights_q4lr(const int8_t* Rq, const void* sw, const int8_t* Uq, const void* su, const int8_t* Vq,
+                                 const void* sv, int N, int K, int r, int G, void* packed, size_t packed_bytes,
+                                 void* stream) {
+    g_last_launches = 0;
+    if (!shape_ok(1, N, K, r, G) || !q4lr_rank_ok(r) || r == 0) return TWQ_ERR_INVALID_ARG;
+    if (!Rq || !sw || !Uq || !su || !Vq || !sv || !packed) return TWQ_ERR_INVALID_ARG;
+    if (!aligned16(Rq) || (reinterpret_cast<uintptr_t>(packed) & 255u)) return TWQ_ERR_INVALID_ARG;
+    if (packed_bytes < twq::packed_layout_q4lr(N, K, r, G).total) return TWQ_ERR_INVALID_ARG;
+    if (!device_is_sm100()) return TWQ_ERR_UNSUPPORTED;
+    int n = 0;
+    if (twq::launch_pack_weights_q4lr(Rq, sw, Uq, su, Vq, sv, N, K, r, G, packed, static_cast<cudaStream_t>(stream), &n) !=
+        cudaSuccess)
+        return TWQ_ERR_CUDA;
+    g_last_launches = n;
+    return TWQ_OK;
+}
+
+twq_status twq_dual_linear_q4lr_x(const void* X, int ldx, const float* tinv, const void* packed, int M, int N, int K,
+                                  int r, int G, void* Y, twq_out_dtype ydt, int ldy, uint8_t* Xq_out, float* sx_out,
+                                  int32_t* dbg_P, float* dbg_H, int8_t* dbg_QH, float* dbg_sH, void* stream) {
+    g_last_launches = 0;
+    if (!shape_ok(M, N, K, r, G) || !q4lr_rank_ok(r) || r == 0) return TWQ_ERR_INVALID_ARG;
+    if (!X || !packed || !Y) return TWQ_ERR_INVALID_ARG;
+    if (ydt != TWQ_OUT_BF16 && ydt != TWQ_OUT_FP16 && ydt != TWQ_OUT_FP32) return TWQ_ERR_INVALID_ARG;
+    if (ldy < N || ldx < K || ldx % 8 != 0) return TWQ_ERR_INVALID_ARG;
+    if (!aligned16(X) || !aligned16(Y) || (tinv && !aligned16(tinv)) || (Xq_out && !aligned16(Xq_out)) ||
+        (sx_out && !aligned16(sx_out)) || (reinterpret_cast<uintptr_t>(packed) & 255u))
+        return TWQ_ERR_INVALID_ARG;
+    // row slabs of at most 64 tokens (a slab start keeps every pointer 16-byte aligned: 64 rows of >= 16 bytes each)
+    // (64 where the resident activation tile of 64 tokens fits in shared memory, else 32, else 16)
+    int slab = 0;
+    for (int s = twq::kDecodeMaxM; s >= 16 && slab == 0; s >>= 1)
+        if (get_plan(M < s ? M : s, N, K, r, G, 2)) slab = s;
+    if (slab == 0) return TWQ_ERR_UNSUPPORTED;
+    for (int m0 = 0; m0 < M; m0 += slab)
+        if (!get_plan(M - m0 < slab ? M - m0 : slab, N, K, r, G, 2)) return TWQ_ERR_UNSUPPORTED;
+    if (!device_is_sm100()) return TWQ_ERR_UNSUPPORTED;
+    const twq::PackedLayoutQ4 lay = twq::packed_layout_q4lr(N, K, r, G);
+    const uint8_t* base = static_cast<const uint8_t*>(packed);
+    const int ng = K / G;
+    const size_t ybytes = ydt == TWQ_OUT_FP32 ? 4 : 2;
+    CUtensorMap none;
+    memset(&none, 0, sizeof(none));                           // the one-launch kernel issues no tensor-map copy
+    int launches = 0;
+    for (int m0 = 0; m0 < M; m0 += slab) {
+        const int ms = M - m0 < slab ? M - m0 : slab;
+        const CallPlan* cp = get_plan(ms, N, K, r, G, 2);
+        if (!cp) return TWQ_ERR_UNSUPPORTED;
+        twq::DecodeParams dp = cp->dp;
+        dp.ldx = ldx; dp.ldy = ldy; dp.ydt = static_cast<int>(ydt);
+        dp.R4 = base + lay.off_r4;
+        dp.sw16 = reinterpret_cast<const __half*>(base + lay.off_sw16);
+        dp.L1D = base + lay.off_u;
+        dp.L2T = base + lay.off_v;
+        dp.sv16 = reinterpret_cast<const __half*>(base + lay.off_sv16);
+        dp.X = static_cast<const uint8_t*>(X) + static_cast<size_t>(m0) * ldx * 2;
+        dp.sx = nullptr;
+        dp.Y = static_cast<uint8_t*>(Y) + static_cast<size_t>(m0) * ldy * ybytes;
+        dp.dbgP = dbg_P ? dbg_P + static_cast<size_t>(m0) * ng * N : nullptr;
+        dp.dbgH = dbg_H ? dbg_H + static_cast<size_t>(m0) * r : nullptr;
+        dp.dbgQH = dbg_QH ? dbg_QH + static_cast<size_t>(m0) * r : nullptr;
+        dp.dbgSH = dbg_sH ? dbg_sH + static_cast<size_t>(m0) * lay.nh : nullptr;
+        dp.tinv = tinv;
+        dp.xq_out = Xq_out ? Xq_out + static_cast<size_t>(m0) * (K / 2) : nullptr;
+        dp.sx_out = sx_out ? sx_out + static_cast<size_t>(m0) * ng : nullptr;
+        dp.trace = twq::trace_buffer();
+        if (twq::launch_decode(none, dp, G, static_cast<cudaStream_t>(stream)) != cudaSuccess) return TWQ_ERR_CUDA;
+        ++launches;
+    }
+    g_last_launches = launches;
     return TWQ_OK;
 }
 

@@ -18,9 +18,10 @@ def lib():
 def test_header_symbols_exported(lib):
     hdr = open(os.path.join(ROOT, "include", "twq.h")).read()
     hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
-    names = set(re.findall(r"\b(twq_[a-z_]+)\s*\(", hdr))
+    names = set(re.findall(r"\b(twq_[a-z0-9_]+)\s*\(", hdr))
     assert {"twq_quantize_act", "twq_pack_weights", "twq_dual_linear", "twq_packed_bytes", "twq_dual_linear_x",
-            "twq_workspace_bytes", "twq_workspace_bytes_x", "twq_status_string", "twq_last_launch_count"} <= names
+            "twq_workspace_bytes", "twq_workspace_bytes_x", "twq_status_string", "twq_last_launch_count",
+            "twq_packed_bytes_q4lr", "twq_pack_weights_q4lr", "twq_dual_linear_q4lr_x"} <= names
     for n in names:
         assert getattr(lib, n) is not None, n
     from paper_2606_01556_b200.binding import EXPORTS
