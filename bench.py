@@ -312,6 +312,73 @@ def measure_workload(name, twq, torch, steps, warmup, peaks, with_e2e=False, wit
     return out, gl, L
 
 
+def measure_q4lr(name, twq, torch, steps, warmup, peaks, with_oracle=False):
+    """the same layer shape with the paper's 4-bit low-rank branch (twq_dual_linear_q4lr_x: quantizer,
+    both 4-bit branches, re-quantization of H and the epilogue in one launch), timed like the main path: a CUDA graph of
+    `steps` calls over rotating blobs (> 2 x L2 per lap), median / min of 20 replays."""
+    L = make_layer(name)
+    Uq, su, Vq, sv = gen.make_q4_lowrank(L.K, L.N, L.r, L.G, seed=4242)
+    dev = torch.device("cuda", torch.cuda.current_device())
+    t = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(dev)
+    first = twq.pack_weights_q4lr(t(L.Rq), t(L.sw), t(Uq), t(su), t(Vq), t(sv), L.G)
+    per_copy = first.blob.numel() + 2 * L.M * L.K + 2 * L.M * L.N
+    ncopies = int(min(32, max(2, -(-2 * L2_BYTES // per_copy))))
+    packed = [first] + [twq.PackedLayer(first.blob.clone(), first.N, first.K, first.r, first.G) for _ in range(ncopies - 1)]
+    Xh = torch.from_numpy(L.X.view(np.int16)).view(torch.bfloat16)
+    X = [Xh.to(dev) for _ in range(ncopies)]
+    Y = [torch.empty((L.M, L.N), dtype=torch.bfloat16, device=dev) for _ in range(ncopies)]
+
+    def step(i):
+        c = i % ncopies
+        twq.dual_linear_q4lr_x(X[c], packed[c], None, twq.OUT_BF16, Y=Y[c])
+
+    s = torch.cuda.Stream()
+    s.wait_stream(torch.cuda.current_stream())
+    with torch.cuda.stream(s):
+        for i in range(max(warmup, ncopies)):
+            step(i)
+        launches = twq.last_launch_count()
+        s.synchronize()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=s):
+            for i in range(steps):
+                step(i)
+        g.replay()
+        s.synchronize()
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(20)]
+        for e0, e1 in ev:
+            e0.record(s)
+            g.replay()
+            e1.record(s)
+        s.synchronize()
+    torch.cuda.current_stream().wait_stream(s)
+    us = sorted(e0.elapsed_time(e1) * 1e3 / steps for e0, e1 in ev)
+    med = float(np.median(us))
+    by = twq.algorithmic_bytes_q4lr(L.M, L.N, L.K, L.r, L.G)
+    ach = by / (med * 1e-6) / 1e9
+    out = dict(workload=name + "_q4lr", M=L.M, N=L.N, K=L.K, r=L.r, G=L.G, us_step=round(med, 3), us_min=round(us[0], 3),
+               launches_per_step=launches, weight_copies=ncopies,
+               roofline=dict(bound="hbm", achieved=round(ach, 1), peak=peaks["hbm_gbs"], unit="GB/s",
+                             frac=round(ach / peaks["hbm_gbs"], 4), traffic=None, kernel="decode_dual_linear_kernel<mode 2>",
+                             us=round(med, 3), algorithmic_bytes=by, peak_source=peaks["source"]))
+    if with_oracle:
+        from oracle import oracle
+        oracle.build()
+        rows = list(range(min(L.M, 4)))
+        t0 = time.perf_counter()
+        n = 0
+        while time.perf_counter() - t0 < 4.0:
+            oracle.forward_q4lr(L.X, L.Rq, L.sw, Uq, su, Vq, sv, L.G, rows=rows)
+            n += 1
+        dt = (time.perf_counter() - t0) / n
+        out["cpu_baseline"] = dict(value=round(dt * 1e6 * L.M / len(rows), 1), unit="us/call", cores=oracle.num_threads(),
+                                   kind="oracle", sample="oracle.forward_q4lr on %d of %d token rows, %d repeats in 4 s, "
+                                   "scaled to the full call" % (len(rows), L.M, n))
+    del packed, X, Y
+    torch.cuda.empty_cache()
+    return out
+
+
 # ----------------------------------------------------------------------------- CPU oracle arm
 def time_oracle(L, budget_s=12.0, max_calls=10000):
     """The oracle as it stands (quantize + pack + forward), all host cores; bounded by ~budget_s of work."""
@@ -450,6 +517,12 @@ def main():
         by_name = {r["workload"]: r for r in sweep}
         by_name.setdefault(args.workload, main_res)
 
+    next1 = None
+    if rank == 0 and not args.no_sweep:
+        next1 = [measure_q4lr(n, twq, torch, max(20, min(args.steps, 100)), args.warmup, peaks,
+                              with_oracle=(n == "c2_qproj_m16" and not args.no_cpu_baseline))
+                 for n in ("c2_qproj_m1", "c2_qproj_m16", "c2_qproj_m64")]
+
     if rank == 0:
         cpu = None if args.no_cpu_baseline else time_oracle(L)
         # whole-job figure: N replicas each finish K calls in the max-over-ranks time
@@ -483,6 +556,9 @@ def main():
                     eff_tops=main_res["eff_tops"], gbs=main_res["gbs"],
                     cublas_bf16_gemm_us=main_res.get("us_cublas_bf16_gemm"),
                     paper_context="paper: up to 1.8x over FP16 TensorRT-LLM end to end on RTX 4090 / L20 (PAPER.md L232)",
+                    # the paper's 4-bit low-rank branch on the same shapes (whole path, one launch);
+                    # compare with us_step_dual_linear_x of the matching sweep entry (FP16 low-rank branch, one launch)
+                    next1_q4lr=next1,
                     sweep=sweep)
         print(json.dumps(line))
     if dist is not None:

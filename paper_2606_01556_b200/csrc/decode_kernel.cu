@@ -146,6 +146,133 @@ __device__ __forceinline__ void lds_words(uint32_t (&dst)[kW], uint32_t a) {
 
 }  // namespace
 
+// The in-kernel activation quantizer and its all-gather (kMode >= 1), run by the residual warps.
+template <int G, int MT, bool kL4>
+__device__ __forceinline__ void decode_quantize_share(const DecodeParams& p, uint8_t* dsm, int rank, int rw, int lane, int nrw, int lrw,
+                                                   bool xq_bulk) {
+    constexpr int kMp = 16 * MT;
+    const int ng = p.ng, cs = p.cs;
+    float* sSx = reinterpret_cast<float*>(dsm + p.off_sx);
+    const uint32_t bar0 = smem_u32(dsm + p.off_bar);
+#define DBAR(i) (bar0 + 8u * static_cast<uint32_t>(i))
+    // ---- steps a1-a2 inside the kernel (Eq. 1; the FP32 operation order of
+    // include/twq.h, bit for bit the codes and scales twq_quantize_act writes).  Cluster rank q quantizes the
+    // K-groups [ng*q/cs, ng*(q+1)/cs) of every token and stores codes and scales into EVERY peer's shared memory
+    // ([g][token][G/2], the layout the MMA fragments read without bank conflicts): the activation tile is
+    // quantized once per cluster and reused by all its CTAs and tiles (L179).
+    uint8_t* sXq = dsm + p.off_xq;
+    constexpr int kLPI = G / 8;                          // lanes per (token, group): 8 elements each
+    constexpr int kIPW = 32 / kLPI;                      // (token, group) items per warp pass
+    // Rows beyond M are written by nobody and stay whatever the shared memory held: row m of the MMA's activation
+    // operand only reaches row m of its result, and no result row >= M is ever read (clearing the 32 KB tile cost
+    // 1.1 us at the head of the critical path; in-kernel timeline, r02).
+    const int gq0 = static_cast<int>(static_cast<unsigned>(ng) * rank / cs);
+    const int ngq = static_cast<int>(static_cast<unsigned>(ng) * (rank + 1) / cs) - gq0;
+    const int items = p.M * ngq;
+    const int li = lane % kLPI, sub = lane / kLPI;
+    const uint16_t* X = static_cast<const uint16_t*>(p.X);
+    TWQ_DSTAMP(21);
+    // This loop heads the critical path of the call and is one dependent chain per warp: every instruction in it is paid in
+    // full (a software prefetch of four passes with its index divisions cost 0.6 us at M = 1; measured, r02).
+    bool waited = cs <= 1;
+    TWQ_DCLK(4);
+#pragma unroll 1
+    for (int base0 = rw * kIPW; base0 < items; base0 += nrw * kIPW) {
+    {
+        const int it = base0 + sub;
+        const bool on = it < items;                      // whole items are on or off: the shuffles below stay inside one
+        int m = 0, gi = 0;
+        if (on) {
+            if (ngq == 1) { m = it; }
+            else if (ngq == 2) { m = it >> 1; gi = it & 1; }
+            else { m = it / ngq; gi = it - m * ngq; }
+        }
+        const int g = gq0 + gi;
+        const uint4 vld = on ? ldg_v4(X + static_cast<size_t>(m) * p.ldx + g * G + li * 8) : make_uint4(0u, 0u, 0u, 0u);
+        if (!waited) {                                   // warp-uniform; after the load is in flight
+            cluster_wait();                              // every CTA of the cluster is running (its barriers exist)
+            waited = true;
+        }
+        float x[8];
+#pragma unroll
+        for (int i = 0; i < 8; ++i) x[i] = 0.0f;
+        if (on) {
+            const uint4 v = vld;
+            const uint32_t w[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                x[2 * i] = __uint_as_float(w[i] << 16);              // BF16 -> FP32, exact
+                x[2 * i + 1] = __uint_as_float(w[i] & 0xFFFF0000u);
+            }
+            if (p.tinv != nullptr) {
+                const float4 t0 = __ldg(reinterpret_cast<const float4*>(p.tinv + g * G + li * 8));
+                const float4 t1 = __ldg(reinterpret_cast<const float4*>(p.tinv + g * G + li * 8) + 1);
+                x[0] = __fmul_rn(x[0], t0.x); x[1] = __fmul_rn(x[1], t0.y); x[2] = __fmul_rn(x[2], t0.z); x[3] = __fmul_rn(x[3], t0.w);
+                x[4] = __fmul_rn(x[4], t1.x); x[5] = __fmul_rn(x[5], t1.y); x[6] = __fmul_rn(x[6], t1.z); x[7] = __fmul_rn(x[7], t1.w);
+            }
+        }
+        float amax = 0.0f;
+#pragma unroll
+        for (int i = 0; i < 8; ++i) amax = fmaxf(amax, fabsf(x[i]));
+#pragma unroll
+        for (int d = kLPI / 2; d >= 1; d >>= 1) amax = fmaxf(amax, __shfl_xor_sync(0xffffffffu, amax, d));
+        const float sc = __fdiv_rn(fmaxf(amax, 0x1p-30f), 7.0f);
+        const float inv = __fdiv_rn(1.0f, sc);
+        uint32_t pk = 0u;
+#pragma unroll
+        for (int i = 0; i < 8; ++i) {
+            int q = __float2int_rn(__fmul_rn(x[i], inv));            // round-half-to-even
+            q = max(-7, min(7, q));
+            pk |= (static_cast<uint32_t>(q) & 0xFu) << (4 * i);      // low nibble = even k
+        }
+        if (on) {
+            uint32_t* qd = reinterpret_cast<uint32_t*>(sXq + (g * kMp + m) * (G / 2) + li * 4);
+            if (xq_bulk) {
+                *qd = pk;
+            } else {
+                const uint32_t qa = smem_u32(qd);
+                for (int pr = 0; pr < cs; ++pr) st_dsmem_u32(mapa_u32(qa, pr), pk);
+            }
+            if (li == 0) {
+                const float s8 = sc * 0x1p-8f;                       // MMA operands are 16*code
+                if (xq_bulk) {
+                    sSx[g * kMp + m] = s8;
+                } else {
+                    const uint32_t sa = smem_u32(sSx + g * kMp + m);
+                    for (int pr = 0; pr < cs; ++pr) st_dsmem_u32(mapa_u32(sa, pr), __float_as_uint(s8));
+                }
+                if (p.sx_out != nullptr) p.sx_out[static_cast<size_t>(m) * ng + g] = sc;
+            }
+            if (p.xq_out != nullptr)
+                *reinterpret_cast<uint32_t*>(p.xq_out + static_cast<size_t>(m) * (p.K >> 1) + g * (G / 2) + li * 4) = pk;
+        }
+    }
+    }
+    if (!waited) cluster_wait();                         // warps without an item
+    TWQ_DCLK(5);
+    TWQ_DSTAMP(22);
+    if (xq_bulk) fence_proxy_async_smem();               // the bulk copies below read what this thread stored
+    named_bar_sync(2, nrw * 32);                         // this CTA's share is stored (in bulk mode: in its own shared memory)
+    TWQ_DSTAMP(23);
+    if constexpr (kL4) asm volatile("bar.arrive 4, %0;" ::"r"((nrw + lrw) * 32) : "memory");   // q4lr stage 1 may read it
+    if (xq_bulk) {
+        // All-gather: this rank's K-groups (contiguous in [g][token][G/2] and [g][token]) go to every peer as two bulk
+        // copies through distributed shared memory, completing on the peer's barrier.  Per-lane remote stores were 450
+        // remote operations per pass and 1.8 us at M = 16 (in-kernel timeline, r02).
+        if (rw == 0 && lane < cs && lane != rank && ngq > 0) {
+            const uint32_t cs_a = smem_u32(sXq + gq0 * kMp * (G / 2)), ss_a = smem_u32(sSx + gq0 * kMp);
+            const uint32_t rb = mapa_u32(DBAR(D_XQ), static_cast<uint32_t>(lane));
+            bulk_copy_to_peer(mapa_u32(cs_a, lane), cs_a, static_cast<uint32_t>(ngq) * kMp * (G / 2), rb);
+            bulk_copy_to_peer(mapa_u32(ss_a, lane), ss_a, static_cast<uint32_t>(ngq) * kMp * 4, rb);
+        }
+        mbar_wait_a(DBAR(D_XQ), 0);                      // every peer's share has arrived here
+    } else if (cs > 1) {
+        if (rw == 0 && lane < cs) mbar_arrive_remote(mapa_u32(DBAR(D_XQ), static_cast<uint32_t>(lane)));
+        mbar_wait_cluster_a(DBAR(D_XQ), 0);              // every rank's share has arrived here
+    }
+#undef DBAR
+}
+
 // kMode >= 1 (kQ): the activation quantizer (steps a1-a2) runs inside this kernel: every cluster rank quantizes 1/cs of the
 // K-groups of all tokens and the cluster all-gathers codes and scales through distributed shared memory (twq_dual_linear_x).
 // kMode == 2 (kL4): in addition the low-rank branch is the paper's own 4-bit pipeline (R18-R22):
@@ -204,6 +331,9 @@ decode_dual_linear_kernel(const __grid_constant__ CUtensorMap tmXq, const __grid
     const int nloc = p.tmax * 8;
     const int hstride = r + 8;
 
+    // The in-kernel quantizer's all-gather: per-lane remote stores for a handful of tokens (lowest latency), bulk copies through
+    // distributed shared memory above that (one remote transaction per warp and peer does not scale with M).
+    const bool xq_bulk = kQ && cs > 1 && p.M > 4;
     TWQ_DSTAMP(0);
     const uint32_t bar0 = smem_u32(dsm + p.off_bar);
 #define DBAR(i) (bar0 + 8u * static_cast<uint32_t>(i))
@@ -213,8 +343,14 @@ decode_dual_linear_kernel(const __grid_constant__ CUtensorMap tmXq, const __grid
         for (int i = 0; i < kMaxL1Slots; ++i) { mbar_init(&bars[D_L1FULL + i], 1); mbar_init(&bars[D_L1EMPTY + i], lrw > 0 ? lrw : 1); }
         mbar_init(&bars[D_X1], cs);
         mbar_init(&bars[D_X2], cs);
-        mbar_init(&bars[D_XQ], cs);
+        mbar_init(&bars[D_XQ], xq_bulk ? 1 : cs);
         fence_mbar_init();
+        if (xq_bulk) {
+            // the in-kernel quantizer's all-gather arrives as bulk copies from the cs - 1 peers: every K-group this rank does
+            // not quantize itself, all kMp token rows of codes and scales
+            const int own = static_cast<int>(static_cast<unsigned>(ng) * (rank + 1) / cs) - static_cast<int>(static_cast<unsigned>(ng) * rank / cs);
+            mbar_arrive_expect_tx_a(DBAR(D_XQ), static_cast<uint32_t>(ng - own) * (kMp * (G / 2) + kMp * 4));
+        }
     }
     __syncthreads();
     // split cluster barrier: "my mbarriers exist".  The low-rank warps wait for it before their first remote arrive,
@@ -466,9 +602,11 @@ decode_dual_linear_kernel(const __grid_constant__ CUtensorMap tmXq, const __grid
             const uint32_t chunk_bytes = static_cast<uint32_t>(p.sc) * slab_bytes;
             int slot = 0, lap = 0;
             uint32_t slot_a = 0;
+            TWQ_DCLK(0);
 #pragma unroll 1
             for (int i = 0; i < nl1; ++i) {
                 mbar_wait_a(DBAR(D_L1FULL + slot), lap & 1);
+                if (i == 0) TWQ_DCLK(1);
                 const int cnt = min(p.sc, nu - i * p.sc);
                 uint32_t la = slot_a;
 #pragma unroll 1
@@ -516,6 +654,7 @@ decode_dual_linear_kernel(const __grid_constant__ CUtensorMap tmXq, const __grid
                 slot_a += chunk_bytes;
                 if (++slot == p.l1_slots) { slot = 0; slot_a = 0; ++lap; }
             }
+            TWQ_DCLK(2);
             TWQ_DSTAMP(4);
 #pragma unroll
             for (int q = 0; q < NQ; ++q) {
@@ -621,40 +760,91 @@ decode_dual_linear_kernel(const __grid_constant__ CUtensorMap tmXq, const __grid
             named_bar_sync(1, nlr);
         }
         if constexpr (kL4) {
-            // ---- re-quantization of H on the fly (Eq. 1 L43-47 on the FP32 H, R18 / R19): eight lanes
-            // per (token, r-group), gr/8 consecutive elements each; every CTA does this for all of H (2 K elements at most)
-            const int e = p.gr >> 3, items = p.M * p.nh;
-            const int li = lane & 7, sub = lane >> 3;
-            for (int base = lw * 4; base < items; base += lrw * 4) {
-                const int it = base + sub;
-                const bool on = it < items;
-                const int m = on ? it / p.nh : 0, h = on ? it - m * p.nh : 0;
-                const float* hp = sH32 + m * r + h * p.gr + li * e;
-                float amax = 0.0f;
-                if (on)
-                    for (int i = 0; i < e; ++i) amax = fmaxf(amax, fabsf(hp[i]));
-                amax = fmaxf(amax, __shfl_xor_sync(0xffffffffu, amax, 4));
-                amax = fmaxf(amax, __shfl_xor_sync(0xffffffffu, amax, 2));
-                amax = fmaxf(amax, __shfl_xor_sync(0xffffffffu, amax, 1));
-                const float sc = __fdiv_rn(fmaxf(amax, 0x1p-30f), 7.0f);
-                const float inv = __fdiv_rn(1.0f, sc);
-                if (on) {
-                    uint8_t* qp = sQH + (h * kMp + m) * vrow + li * (e >> 1);
-                    const bool dbg_out = kDbg && blockIdx.x == 0;
-                    for (int i = 0; i < e; i += 2) {
-                        int q0 = __float2int_rn(__fmul_rn(hp[i], inv)), q1 = __float2int_rn(__fmul_rn(hp[i + 1], inv));
-                        q0 = max(-7, min(7, q0));
-                        q1 = max(-7, min(7, q1));
-                        qp[i >> 1] = static_cast<uint8_t>((q0 & 0xF) | ((q1 & 0xF) << 4));       // low nibble = even index
-                        if (dbg_out) {
-                            const size_t o = static_cast<size_t>(m) * r + h * p.gr + li * e + i;
-                            if (p.dbgQH != nullptr) { p.dbgQH[o] = static_cast<int8_t>(q0); p.dbgQH[o + 1] = static_cast<int8_t>(q1); }
-                            if (p.dbgH != nullptr) { p.dbgH[o] = hp[i]; p.dbgH[o + 1] = hp[i + 1]; }
+            // ---- re-quantization of H on the fly (Eq. 1 L43-47 on the FP32 H, R18 / R19).  Every CTA
+            // does this for all of H (a few K elements).  An item = one (token, r-group): lpi lanes, gr / lpi consecutive elements
+            // each.  The chain max -> shuffles -> two divisions -> round is ~100 dependent instructions, so for the common group
+            // sizes (gr = 128 / 64: four elements per lane) a warp works on kIB items at once (one item at a time took 650 ns per
+            // pass on the critical path; in-kernel timeline, r02).
+            const int lpi = p.gr == 128 ? 32 : (p.gr == 64 ? 16 : 8), ipw = 32 / lpi;
+            const int e = p.gr / lpi, items = p.M * p.nh;
+            const int li = lane & (lpi - 1), sub = lane / lpi;
+            const bool dbg_out = kDbg && blockIdx.x == 0;
+            if (e == 4) {
+                constexpr int kIB = 4;
+                for (int base = lw * ipw * kIB; base < items; base += lrw * ipw * kIB) {
+                    float4 v[kIB];
+                    float amax[kIB];
+                    int mm[kIB], hh[kIB];
+                    bool on[kIB];
+#pragma unroll
+                    for (int b = 0; b < kIB; ++b) {
+                        const int it = base + b * ipw + sub;
+                        on[b] = it < items;
+                        mm[b] = on[b] ? (p.nh == 2 ? it >> 1 : it) : 0;
+                        hh[b] = on[b] && p.nh == 2 ? (it & 1) : 0;
+                        v[b] = on[b] ? *reinterpret_cast<const float4*>(sH32 + mm[b] * r + hh[b] * p.gr + li * 4)
+                                     : make_float4(0.f, 0.f, 0.f, 0.f);
+                        amax[b] = fmaxf(fmaxf(fabsf(v[b].x), fabsf(v[b].y)), fmaxf(fabsf(v[b].z), fabsf(v[b].w)));
+                    }
+                    for (int d = lpi >> 1; d >= 1; d >>= 1)
+#pragma unroll
+                        for (int b = 0; b < kIB; ++b) amax[b] = fmaxf(amax[b], __shfl_xor_sync(0xffffffffu, amax[b], d));
+#pragma unroll
+                    for (int b = 0; b < kIB; ++b) {
+                        const float sc = __fdiv_rn(fmaxf(amax[b], 0x1p-30f), 7.0f);
+                        const float inv = __fdiv_rn(1.0f, sc);
+                        int q[4] = {__float2int_rn(__fmul_rn(v[b].x, inv)), __float2int_rn(__fmul_rn(v[b].y, inv)),
+                                    __float2int_rn(__fmul_rn(v[b].z, inv)), __float2int_rn(__fmul_rn(v[b].w, inv))};
+                        uint32_t pk = 0u;
+#pragma unroll
+                        for (int i = 0; i < 4; ++i) {
+                            q[i] = max(-7, min(7, q[i]));
+                            pk |= (static_cast<uint32_t>(q[i]) & 0xFu) << (4 * i);               // low nibble = even index
+                        }
+                        if (on[b]) {
+                            *reinterpret_cast<uint16_t*>(sQH + (hh[b] * kMp + mm[b]) * vrow + li * 2) = static_cast<uint16_t>(pk);
+                            if (li == 0) sSH[hh[b] * kMp + mm[b]] = sc * 0x1p-8f;                 // both MMA operands are 16*code
+                            if (dbg_out) {
+                                const size_t o = static_cast<size_t>(mm[b]) * r + hh[b] * p.gr + li * 4;
+                                const float hv[4] = {v[b].x, v[b].y, v[b].z, v[b].w};
+                                for (int i = 0; i < 4; ++i) {
+                                    if (p.dbgQH != nullptr) p.dbgQH[o + i] = static_cast<int8_t>(q[i]);
+                                    if (p.dbgH != nullptr) p.dbgH[o + i] = hv[i];
+                                }
+                                if (li == 0 && p.dbgSH != nullptr) p.dbgSH[static_cast<size_t>(mm[b]) * p.nh + hh[b]] = sc;
+                            }
                         }
                     }
-                    if (li == 0) {
-                        sSH[h * kMp + m] = sc * 0x1p-8f;                 // both MMA operands are 16*code
-                        if (dbg_out && p.dbgSH != nullptr) p.dbgSH[static_cast<size_t>(m) * p.nh + h] = sc;
+                }
+            } else {
+                for (int base = lw * ipw; base < items; base += lrw * ipw) {
+                    const int it = base + sub;
+                    const bool on = it < items;
+                    const int m = on ? it / p.nh : 0, h = on ? it - m * p.nh : 0;
+                    const float* hp = sH32 + m * r + h * p.gr + li * e;
+                    float amax = 0.0f;
+                    if (on)
+                        for (int i = 0; i < e; ++i) amax = fmaxf(amax, fabsf(hp[i]));
+                    for (int d = lpi >> 1; d >= 1; d >>= 1) amax = fmaxf(amax, __shfl_xor_sync(0xffffffffu, amax, d));
+                    const float sc = __fdiv_rn(fmaxf(amax, 0x1p-30f), 7.0f);
+                    const float inv = __fdiv_rn(1.0f, sc);
+                    if (on) {
+                        uint8_t* qp = sQH + (h * kMp + m) * vrow + li * (e >> 1);
+                        for (int i = 0; i < e; i += 2) {
+                            int q0 = __float2int_rn(__fmul_rn(hp[i], inv)), q1 = __float2int_rn(__fmul_rn(hp[i + 1], inv));
+                            q0 = max(-7, min(7, q0));
+                            q1 = max(-7, min(7, q1));
+                            qp[i >> 1] = static_cast<uint8_t>((q0 & 0xF) | ((q1 & 0xF) << 4));   // low nibble = even index
+                            if (dbg_out) {
+                                const size_t o = static_cast<size_t>(m) * r + h * p.gr + li * e + i;
+                                if (p.dbgQH != nullptr) { p.dbgQH[o] = static_cast<int8_t>(q0); p.dbgQH[o + 1] = static_cast<int8_t>(q1); }
+                                if (p.dbgH != nullptr) { p.dbgH[o] = hp[i]; p.dbgH[o + 1] = hp[i + 1]; }
+                            }
+                        }
+                        if (li == 0) {
+                            sSH[h * kMp + m] = sc * 0x1p-8f;             // both MMA operands are 16*code
+                            if (dbg_out && p.dbgSH != nullptr) p.dbgSH[static_cast<size_t>(m) * p.nh + h] = sc;
+                        }
                     }
                 }
             }
@@ -739,80 +929,7 @@ decode_dual_linear_kernel(const __grid_constant__ CUtensorMap tmXq, const __grid
         pdl_wait();                                              // sx (or X) comes from the previous kernel of the stream
         TWQ_DSTAMP(2);
         if constexpr (kQ) {
-            // ---- steps a1-a2 inside the kernel (Eq. 1; the FP32 operation order of
-            // include/twq.h, bit for bit the codes and scales twq_quantize_act writes).  Cluster rank q quantizes the
-            // K-groups [ng*q/cs, ng*(q+1)/cs) of every token and stores codes and scales into EVERY peer's shared memory
-            // ([g][token][G/2], the layout the MMA fragments read without bank conflicts): the activation tile is
-            // quantized once per cluster and reused by all its CTAs and tiles (L179).
-            uint8_t* sXq = dsm + p.off_xq;
-            constexpr int kLPI = G / 8;                          // lanes per (token, group): 8 elements each
-            constexpr int kIPW = 32 / kLPI;                      // (token, group) items per warp pass
-            // rows beyond M are written by nobody: codes 0, scale 0
-            for (int i = rw * 32 + lane; i < ng * kMp * (G / 8); i += nrw * 32)
-                if ((i / (G / 8)) % kMp >= p.M) reinterpret_cast<uint32_t*>(sXq)[i] = 0u;
-            for (int i = rw * 32 + lane; i < ng * kMp; i += nrw * 32)
-                if (i % kMp >= p.M) sSx[i] = 0.0f;
-            const int gq0 = static_cast<int>(static_cast<unsigned>(ng) * rank / cs);
-            const int ngq = static_cast<int>(static_cast<unsigned>(ng) * (rank + 1) / cs) - gq0;
-            const int items = p.M * ngq;
-            const int li = lane % kLPI, sub = lane / kLPI;
-            const uint16_t* X = static_cast<const uint16_t*>(p.X);
-            if (cs > 1) cluster_wait();                          // every CTA of the cluster is running (its shared memory exists)
-            for (int base = rw * kIPW; base < items; base += nrw * kIPW) {
-                const int it = base + sub;
-                const bool on = it < items;                      // whole items are on or off: the shuffles below stay inside one
-                const int m = on ? it / ngq : 0, g = gq0 + (on ? it - (it / ngq) * ngq : 0);
-                float x[8];
-#pragma unroll
-                for (int i = 0; i < 8; ++i) x[i] = 0.0f;
-                if (on) {
-                    const uint4 v = ldg_v4(X + static_cast<size_t>(m) * p.ldx + g * G + li * 8);
-                    const uint32_t w[4] = {v.x, v.y, v.z, v.w};
-#pragma unroll
-                    for (int i = 0; i < 4; ++i) {
-                        x[2 * i] = __uint_as_float(w[i] << 16);              // BF16 -> FP32, exact
-                        x[2 * i + 1] = __uint_as_float(w[i] & 0xFFFF0000u);
-                    }
-                    if (p.tinv != nullptr) {
-                        const float4 t0 = __ldg(reinterpret_cast<const float4*>(p.tinv + g * G + li * 8));
-                        const float4 t1 = __ldg(reinterpret_cast<const float4*>(p.tinv + g * G + li * 8) + 1);
-                        x[0] = __fmul_rn(x[0], t0.x); x[1] = __fmul_rn(x[1], t0.y); x[2] = __fmul_rn(x[2], t0.z); x[3] = __fmul_rn(x[3], t0.w);
-                        x[4] = __fmul_rn(x[4], t1.x); x[5] = __fmul_rn(x[5], t1.y); x[6] = __fmul_rn(x[6], t1.z); x[7] = __fmul_rn(x[7], t1.w);
-                    }
-                }
-                float amax = 0.0f;
-#pragma unroll
-                for (int i = 0; i < 8; ++i) amax = fmaxf(amax, fabsf(x[i]));
-#pragma unroll
-                for (int d = kLPI / 2; d >= 1; d >>= 1) amax = fmaxf(amax, __shfl_xor_sync(0xffffffffu, amax, d));
-                const float sc = __fdiv_rn(fmaxf(amax, 0x1p-30f), 7.0f);
-                const float inv = __fdiv_rn(1.0f, sc);
-                uint32_t pk = 0u;
-#pragma unroll
-                for (int i = 0; i < 8; ++i) {
-                    int q = __float2int_rn(__fmul_rn(x[i], inv));            // round-half-to-even
-                    q = max(-7, min(7, q));
-                    pk |= (static_cast<uint32_t>(q) & 0xFu) << (4 * i);      // low nibble = even k
-                }
-                if (on) {
-                    const uint32_t qa = smem_u32(sXq + (g * kMp + m) * (G / 2) + li * 4);
-                    for (int pr = 0; pr < cs; ++pr) st_dsmem_u32(mapa_u32(qa, pr), pk);
-                    if (li == 0) {
-                        const uint32_t sa = smem_u32(sSx + g * kMp + m);
-                        const uint32_t sv = __float_as_uint(sc * 0x1p-8f);   // MMA operands are 16*code
-                        for (int pr = 0; pr < cs; ++pr) st_dsmem_u32(mapa_u32(sa, pr), sv);
-                        if (p.sx_out != nullptr) p.sx_out[static_cast<size_t>(m) * ng + g] = sc;
-                    }
-                    if (p.xq_out != nullptr)
-                        *reinterpret_cast<uint32_t*>(p.xq_out + static_cast<size_t>(m) * (p.K >> 1) + g * (G / 2) + li * 4) = pk;
-                }
-            }
-            named_bar_sync(2, nrw * 32);                         // this CTA's share is stored (everywhere)
-            if constexpr (kL4) asm volatile("bar.arrive 4, %0;" ::"r"((nrw + lrw) * 32) : "memory");   // q4lr stage 1 may read it
-            if (cs > 1) {
-                if (rw == 0 && lane < cs) mbar_arrive_remote(mapa_u32(DBAR(D_XQ), static_cast<uint32_t>(lane)));
-                mbar_wait_cluster_a(DBAR(D_XQ), 0);              // every rank's share has arrived here
-            }
+            decode_quantize_share<G, MT, kL4>(p, dsm, rank, rw, lane, nrw, lrw, xq_bulk);
         } else {
             for (int i = rw * 32 + lane; i < kMp * ng; i += nrw * 32) {
                 const int g = i / kMp, m = i - g * kMp;
@@ -1090,6 +1207,13 @@ decode_dual_linear_kernel(const __grid_constant__ CUtensorMap tmXq, const __grid
     }
     TWQ_DSTAMP(29);
     if (cs > 1 && !is_lr && !(kQ && warp < nrw)) cluster_wait();   // completes this thread's half of the split barrier (long since released)
+    if (xq_bulk) {
+        // The all-gather's bulk copies read the SENDER's shared memory: no CTA may exit (and hand its shared memory to another
+        // block) before every peer has received its share.  Every CTA gets here after its own share arrived in full, so one
+        // more cluster barrier is enough; the kernel ends with its slowest CTA either way.
+        cluster_arrive_relaxed();
+        cluster_wait();
+    }
 #undef DBAR
 }
 

@@ -206,6 +206,14 @@ __device__ __forceinline__ void bulk_load_1d_a(uint32_t smem_dst, const void* gs
         ::"r"(smem_dst), "l"(gsrc), "r"(bytes), "r"(bar), "l"(policy)
         : "memory");
 }
+// 1-D bulk copy from this CTA's shared memory into a peer CTA's (distributed shared memory): `bytes` a multiple of 16,
+// addresses 16-byte aligned; destination and mbarrier are shared::cluster addresses of the SAME peer (mapa); completes
+// `bytes` on that peer's mbarrier.  The source must have been made visible to the async proxy (fence.proxy.async).
+__device__ __forceinline__ void bulk_copy_to_peer(uint32_t dst_cluster, uint32_t src_cta, uint32_t bytes, uint32_t bar_cluster) {
+    asm volatile("cp.async.bulk.shared::cluster.shared::cta.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(dst_cluster), "r"(src_cta), "r"(bytes), "r"(bar_cluster)
+                 : "memory");
+}
 // pull a global range into L2 (no destination)
 __device__ __forceinline__ void bulk_prefetch_l2(const void* gsrc, uint32_t bytes) {
     asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(gsrc), "r"(bytes) : "memory");
