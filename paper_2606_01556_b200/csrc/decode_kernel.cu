@@ -337,7 +337,21 @@ decode_dual_linear_kernel(const __grid_constant__ CUtensorMap tmXq, const __grid
     TWQ_DSTAMP(0);
     const uint32_t bar0 = smem_u32(dsm + p.off_bar);
 #define DBAR(i) (bar0 + 8u * static_cast<uint32_t>(i))
-    if (threadIdx.x == 0) {
+    // Barrier initialisation.  The kernel runs at its register limit (96 per thread with 20 warps) and ptxas' allocation there
+    // is brittle: with the one-thread-per-barrier form below, the instantiations that contain the in-kernel quantizer spill
+    // three preamble values (tile0, rank, ...) and lose 0.5 us at M = 1; with the serial form the two-call instantiation
+    // spills instead and loses 0.1-0.3 us (A/B of both builds in one run, r02).  Each instantiation keeps the form it is
+    // spill-free with; `ptxas -v` must show 0 spill bytes for MT = 1 after any change to this kernel.
+    if (!kQ && threadIdx.x < D_COUNT) {
+        const int i = threadIdx.x;
+        int count = 1;                                                        // D_FULL, D_L1FULL: the producer's expect_tx
+        if (i >= D_EMPTY && i < D_EMPTY + kMaxSlots) count = nrw;
+        else if (i >= D_L1EMPTY && i < D_L1EMPTY + kMaxL1Slots) count = lrw > 0 ? lrw : 1;
+        else if (i == D_X1 || i == D_X2 || i == D_XQ) count = cs;
+        mbar_init(reinterpret_cast<uint64_t*>(dsm + p.off_bar) + i, count);
+        fence_mbar_init();
+    }
+    if (kQ && threadIdx.x == 0) {
         uint64_t* bars = reinterpret_cast<uint64_t*>(dsm + p.off_bar);
         for (int i = 0; i < kMaxSlots; ++i) { mbar_init(&bars[D_FULL + i], 1); mbar_init(&bars[D_EMPTY + i], nrw); }
         for (int i = 0; i < kMaxL1Slots; ++i) { mbar_init(&bars[D_L1FULL + i], 1); mbar_init(&bars[D_L1EMPTY + i], lrw > 0 ? lrw : 1); }
