@@ -76,7 +76,7 @@ def config_for(name):
     """The `config` object of the JSON line: identical for the GPU arm and the reference (oracle) arm."""
     return dict(workload=name, desc=WORKLOADS[name][2],
                 l2="inputs larger than L2: weights and activations rotate through copies, one lap >= 2x the 126 MB L2",
-                launch="CUDA graph of K steps; step = twq_quantize_act + twq_dual_linear",
+                launch="CUDA graph of K steps; step = the whole hot path (quantizer, both branches, epilogue) through twq_dual_linear_x",
                 multi_gpu="replicas only")
 
 
@@ -155,6 +155,8 @@ class GpuLayer:
         need_x = twq.workspace_bytes_x(L.M, L.N, L.K, L.r, L.G)
         self.ws_x = torch.zeros(max(need_x, 256), dtype=torch.uint8, device=dev) if need_x else None
         self.Yh = torch.empty((L.M, L.N), dtype=torch.bfloat16).pin_memory()
+        # the whole hot path is ONE launch (twq_dual_linear_x with the in-kernel quantizer) where the small-batch plan exists
+        self.one_launch = L.M <= 64 and need_x == 0
         self.lap_bytes = per_copy * self.ncopies
         del Rq, sw, L1, L2
         torch.cuda.synchronize()
@@ -175,7 +177,7 @@ class GpuLayer:
     def e2e_step(self, i):
         c = i % self.ncopies
         self.X[c].copy_(self.Xh, non_blocking=True)
-        self.step(i)
+        self.step_x(i)
         self.Yh.copy_(self.Y[c], non_blocking=True)
 
     def time_graph(self, steps, warmup, quant=True, dual=True, replays=20, fused=False):
@@ -210,17 +212,17 @@ class GpuLayer:
         return float(np.median(us)), us[0]                        # us per step: median, min
 
     def time_host(self, calls=2000):
-        """Host time of one twq_dual_linear call through the binding (plan + descriptor caches warm), no device
+        """Host time of one twq_dual_linear_x call through the binding (plan + descriptor caches warm), no device
         synchronisation inside the loop; the queue is drained every 100 calls so that it never back-pressures."""
         torch = self.torch
         for i in range(max(20, self.ncopies)):                   # every rotating copy has its descriptors cached
-            self.step(i, False, True)
+            self.step_x(i)
         torch.cuda.synchronize()
         t = 0.0
         for base in range(0, calls, 100):
             t0 = time.perf_counter()
             for i in range(base, base + 100):
-                self.step(i, False, True)
+                self.step_x(i)
             t += time.perf_counter() - t0
             torch.cuda.synchronize()
         return t / calls * 1e6
@@ -239,8 +241,9 @@ class GpuLayer:
         return e0.elapsed_time(e1) * 1e3 / steps
 
 
-def roofline_for(L, twq, us_dual, peaks, traffic=None, traffic_src=None):
-    by = twq.algorithmic_bytes(L.M, L.N, L.K, L.r, L.G)
+def roofline_for(L, twq, us_dual, peaks, traffic=None, traffic_src=None, one_launch=False):
+    """Roofline of the dominant kernel: twq_dual_linear's kernel, or (one_launch) the single kernel of twq_dual_linear_x."""
+    by = (twq.algorithmic_bytes_x if one_launch else twq.algorithmic_bytes)(L.M, L.N, L.K, L.r, L.G)
     ops_i8, fl_lr = twq.flops(L.M, L.N, L.K, L.r)
     p_i8 = 2.0 * peaks["bf16_tflops"] * 1e12        # int8 dense = 2x bf16 (guide's nominal ratio) x measured bf16
     p_f16 = peaks["bf16_tflops"] * 1e12
@@ -251,7 +254,9 @@ def roofline_for(L, twq, us_dual, peaks, traffic=None, traffic_src=None):
         ach = by / t / 1e9
         return dict(bound="hbm", achieved=round(ach, 1), peak=peaks["hbm_gbs"], unit="GB/s",
                     frac=round(ach / peaks["hbm_gbs"], 4), traffic=traffic, traffic_source=traffic_src,
-                    peak_source=peaks["source"], kernel=kernel_name(L), us=round(us_dual, 3), algorithmic_bytes=by)
+                    peak_source=peaks["source"],
+                    kernel=kernel_name(L) + ("<in-kernel quantizer> (the whole step)" if one_launch else ""),
+                    us=round(us_dual, 3), algorithmic_bytes=by)
     eq_ops = ops_i8 + 2.0 * fl_lr                    # low-rank flops run at half the int8 rate
     ach = eq_ops / t / 1e12
     return dict(bound="tensor", achieved=round(ach, 1), peak=round(p_i8 / 1e12, 1), unit="TFLOP/s",
@@ -260,13 +265,13 @@ def roofline_for(L, twq, us_dual, peaks, traffic=None, traffic_src=None):
                 kernel=kernel_name(L), us=round(us_dual, 3), int8_equivalent_ops=eq_ops)
 
 
-def load_traffic(name):
+def load_traffic(name, one_launch=False):
     """dram__bytes_read.sum + dram__bytes_write.sum per launch of the dual-linear kernel, from the `ncu --set full`
     captures summarised under profiles/ (profiles/traffic.json names capture file and commit per workload)."""
     path = os.path.join(ROOT, "profiles", "traffic.json")
     if not os.path.exists(path):
         return None, None
-    ent = json.load(open(path)).get(name)
+    ent = json.load(open(path)).get(name + ("_x" if one_launch else ""))
     if not ent:
         return None, None
     return int(ent["dram_bytes"]), "%s @ %s" % (ent["capture"], ent["commit"])
@@ -279,20 +284,25 @@ def kernel_name(L):
 def measure_workload(name, twq, torch, steps, warmup, peaks, with_e2e=False, with_cublas=False):
     L = make_layer(name)
     gl = GpuLayer(L, twq, torch)
-    us_step, us_step_min = gl.time_graph(steps, warmup, True, True)
+    # The step = the whole hot path through the public call twq_dual_linear_x: ONE launch for M <= 64 (in-kernel quantizer),
+    # twq_quantize_act + twq_dual_linear otherwise.  The two-call step and its two kernels are timed beside it.
+    us_x, us_x_min = gl.time_graph(steps, warmup, fused=True)
+    us_two, us_two_min = gl.time_graph(steps, warmup, True, True)
     us_dual, us_dual_min = gl.time_graph(steps, warmup, False, True)
     us_quant, us_quant_min = gl.time_graph(steps, warmup, True, False)
-    us_x, us_x_min = gl.time_graph(steps, warmup, fused=True)   # the same step through twq_dual_linear_x
     ops_i8, fl_lr = twq.flops(L.M, L.N, L.K, L.r)
-    traffic, traffic_src = load_traffic(name)
-    out = dict(workload=name, M=L.M, N=L.N, K=L.K, r=L.r, G=L.G, us_step=round(us_step, 3),
-               us_dual_linear=round(us_dual, 3), us_quantize_act=round(us_quant, 3), us_step_dual_linear_x=round(us_x, 3),
-               us_min=dict(step=round(us_step_min, 3), step_dual_linear_x=round(us_x_min, 3), dual_linear=round(us_dual_min, 3), quantize_act=round(us_quant_min, 3)),
+    one = gl.one_launch
+    us_kernel = us_x if one else us_dual                       # the dominant kernel: the single one, or twq_dual_linear's
+    traffic, traffic_src = load_traffic(name, one)
+    out = dict(workload=name, M=L.M, N=L.N, K=L.K, r=L.r, G=L.G, us_step=round(us_x, 3),
+               launches_per_step=1 if one else 2,
+               us_step_two_call=round(us_two, 3), us_dual_linear=round(us_dual, 3), us_quantize_act=round(us_quant, 3),
+               us_min=dict(step=round(us_x_min, 3), step_two_call=round(us_two_min, 3), dual_linear=round(us_dual_min, 3), quantize_act=round(us_quant_min, 3)),
                timing="median of 20 replays of a CUDA graph of %d steps (min alongside)" % steps,
-               eff_tops=round((ops_i8 + fl_lr) / (us_dual * 1e-6) / 1e12, 2),
-               gbs=round(twq.algorithmic_bytes(L.M, L.N, L.K, L.r, L.G) / (us_dual * 1e-6) / 1e9, 1),
+               eff_tops=round((ops_i8 + fl_lr) / (us_kernel * 1e-6) / 1e12, 2),
+               gbs=round((twq.algorithmic_bytes_x if one else twq.algorithmic_bytes)(L.M, L.N, L.K, L.r, L.G) / (us_kernel * 1e-6) / 1e9, 1),
                weight_copies=gl.ncopies, lap_mb=round(gl.lap_bytes / 2 ** 20, 1),
-               roofline=roofline_for(L, twq, us_dual, peaks, traffic, traffic_src))
+               roofline=roofline_for(L, twq, us_kernel, peaks, traffic, traffic_src, one))
     if with_e2e:
         out["us_e2e"] = round(gl.time_e2e(steps, warmup), 3)
         out["us_host_per_call"] = round(gl.time_host(), 3)
@@ -457,6 +467,8 @@ def main():
     ap.add_argument("--impl", default="twq", choices=["twq", "reference"])
     ap.add_argument("--no-sweep", action="store_true", help="time only --workload")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--q4lr", action="store_true",
+                    help="time only the 4-bit low-rank variant (twq_dual_linear_q4lr_x, SURVEY 8f NEXT-1) of --workload")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3)
 
@@ -480,6 +492,14 @@ def main():
         dist.init_process_group("nccl")
 
     peaks = load_peaks()
+    if args.q4lr:
+        if rank == 0:
+            print(json.dumps(measure_q4lr(args.workload, twq, torch, args.steps, args.warmup, peaks,
+                                          with_oracle=not args.no_cpu_baseline)))
+        if dist is not None:
+            dist.barrier()
+            dist.destroy_process_group()
+        return
     sampler = ClockSampler(local) if rank == 0 else None
 
     def barrier():
@@ -537,7 +557,7 @@ def main():
                     clocks=clocks,
                     e2e=dict(value=round(whole_job_us_per_call(us_e2e, world), 3), unit="us/call", h2d_bytes_per_step=2 * L.M * L.K,
                              d2h_bytes_per_step=2 * L.M * L.N),
-                    gpu_launches=2 * args.steps,
+                    gpu_launches=main_res["launches_per_step"] * args.steps,
                     roofline=main_res["roofline"],
                     # the two graded shapes (north_star: ">= 60 % of roofline at M = 1 and M = 2048"), lifted out of `sweep`
                     roofline_m1=by_name.get("c2_qproj_m1", {}).get("roofline"),
@@ -549,15 +569,16 @@ def main():
                                        "(csrc/peak_i8.cu); the roofline denominator stays 2 x measured cuBLAS BF16 burst"),
                     us_host_per_call=main_res.get("us_host_per_call"),
                     cpu_baseline=cpu,
+                    # `value` = the whole hot path through twq_dual_linear_x (one launch for M <= 64); beside it the same step as
+                    # twq_quantize_act + twq_dual_linear (two launches) and those two kernels alone
+                    api="twq_dual_linear_x", launches_per_step=main_res["launches_per_step"],
+                    us_step_two_call=main_res["us_step_two_call"],
                     us_dual_linear=main_res["us_dual_linear"], us_quantize_act=main_res["us_quantize_act"],
-                    # the same step through twq_dual_linear_x (one launch for M <= 64): reported beside `value`, which stays the
-                    # two-call step that BASELINE.json's subsystems name (twq_quantize_act + twq_dual_linear)
-                    us_step_dual_linear_x=main_res["us_step_dual_linear_x"],
                     eff_tops=main_res["eff_tops"], gbs=main_res["gbs"],
                     cublas_bf16_gemm_us=main_res.get("us_cublas_bf16_gemm"),
                     paper_context="paper: up to 1.8x over FP16 TensorRT-LLM end to end on RTX 4090 / L20 (PAPER.md L232)",
                     # the paper's 4-bit low-rank branch on the same shapes (whole path, one launch);
-                    # compare with us_step_dual_linear_x of the matching sweep entry (FP16 low-rank branch, one launch)
+                    # compare with us_step of the matching sweep entry (FP16 low-rank branch, also one launch)
                     next1_q4lr=next1,
                     sweep=sweep)
         print(json.dumps(line))

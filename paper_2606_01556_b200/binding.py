@@ -311,6 +311,13 @@ def algorithmic_bytes(M: int, N: int, K: int, r: int, G: int, with_quantizer: bo
     return w + a + q
 
 
+def algorithmic_bytes_x(M: int, N: int, K: int, r: int, G: int, out_bytes: int = 2) -> int:
+    """Bytes one ONE-LAUNCH twq_dual_linear_x call (M <= 64) must move: the weights as in algorithmic_bytes, X read
+    once, Y written once (codes and scales never leave the chip)."""
+    ng = K // G
+    return N * K // 2 + 2 * N * ng + 2 * K * r + 2 * r * N + 2 * M * K + out_bytes * M * N
+
+
 def flops(M: int, N: int, K: int, r: int):
     """(int8 residual ops, 16-bit low-rank flops) of one call."""
     return 2 * M * K * N, 2 * M * r * (K + N)
