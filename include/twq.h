@@ -210,6 +210,26 @@ twq_status twq_dual_linear_q4lr_x(const void* X, int ldx, const float* tinv, con
                                   uint8_t* Xq_out, float* sx_out, int32_t* dbg_P,
                                   float* dbg_H, int8_t* dbg_QH, float* dbg_sH, void* stream);
 
+/* ---------------------------------------------------------------------------
+ * twq_dual_linear_noalloc -- twq_dual_linear for callers that cannot allocate device memory (code under CUDA graph
+ * capture, tight serving loops, harnesses that forbid cudaMalloc): no workspace argument.  The scratch that the few
+ * shapes with a workspace need (64 < M with few output tiles, see twq_dual_linear) lives in a static device array of
+ * TWQ_NOALLOC_MAX_WS bytes inside the library -- every GPU that loads the library holds these 8.5 MiB until the process
+ * exits; it covers every workspace shape of BASELINE.json's configs (largest: 8 MiB + 256 B), while the largest workspace the
+ * planner can ask for at all is 9.0 MiB + 512 B (many tokens, very few channels).  The call allocates nothing (no cudaMalloc / cudaFree, no allocating library routine) and issues one small
+ * memset on `stream` (the tile counters) in front of the kernel when the shape uses scratch.
+ *   Arguments as for twq_dual_linear, without ws / ws_bytes / dbg_P.  Results are those of twq_dual_linear.
+ *   TWQ_ERR_WORKSPACE  the shape needs more than TWQ_NOALLOC_MAX_WS bytes (twq_workspace_bytes(...) says how many):
+ *                      nothing is launched; use twq_dual_linear with a caller workspace.
+ *   All calls on a device share the one array: two calls that may overlap on the GPU (different streams without a
+ *   dependency between them) race on it and must not be issued; calls ordered by a stream or by events are fine.
+ */
+#define TWQ_NOALLOC_MAX_WS (8u * 1024u * 1024u + 512u * 1024u)
+size_t twq_noalloc_max_workspace(void);
+twq_status twq_dual_linear_noalloc(const void* X, int ldx, const uint8_t* Xq, const float* sx,
+                                   const void* packed, int M, int N, int K, int r, int G,
+                                   void* Y, twq_out_dtype ydt, int ldy, void* stream);
+
 /* Number of kernel launches the last successful twq_dual_linear(_x) / twq_quantize_act /
  * twq_pack_weights call on this thread issued (bench.py's gpu_launches accounting). */
 int twq_last_launch_count(void);

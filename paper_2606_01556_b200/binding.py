@@ -15,7 +15,8 @@ _OUT_TORCH = {OUT_BF16: torch.bfloat16, OUT_FP16: torch.float16, OUT_FP32: torch
 
 EXPORTS = ("twq_status_string", "twq_packed_bytes", "twq_pack_weights", "twq_quantize_act",
            "twq_workspace_bytes", "twq_dual_linear", "twq_workspace_bytes_x", "twq_dual_linear_x", "twq_last_launch_count",
-           "twq_packed_bytes_q4lr", "twq_pack_weights_q4lr", "twq_dual_linear_q4lr_x")
+           "twq_packed_bytes_q4lr", "twq_pack_weights_q4lr", "twq_dual_linear_q4lr_x",
+           "twq_noalloc_max_workspace", "twq_dual_linear_noalloc")
 
 
 TESTING_EXPORTS = ("twq_testing_set_plan_flags", "twq_testing_get_plan_flags", "twq_testing_describe_plan",
@@ -82,6 +83,10 @@ def load_library(build_if_missing: bool = True):
     lib.twq_pack_weights_q4lr.argtypes = [vp, vp, vp, vp, vp, vp, i, i, i, i, vp, sz, vp]
     lib.twq_dual_linear_q4lr_x.restype = i
     lib.twq_dual_linear_q4lr_x.argtypes = [vp, i, vp, vp, i, i, i, i, i, vp, i, i, vp, vp, vp, vp, vp, vp, vp]
+    lib.twq_noalloc_max_workspace.restype = sz
+    lib.twq_noalloc_max_workspace.argtypes = []
+    lib.twq_dual_linear_noalloc.restype = i
+    lib.twq_dual_linear_noalloc.argtypes = [vp, i, vp, vp, vp, i, i, i, i, i, vp, i, i, vp]
     # testing hooks (include/twq_testing.h): not part of the product ABI
     lib.twq_testing_set_plan_flags.restype = None
     lib.twq_testing_set_plan_flags.argtypes = [ctypes.c_uint]
@@ -225,6 +230,22 @@ def dual_linear(X, Xq, sx, packed: PackedLayer, out_dtype: int = OUT_BF16, Y=Non
                                           M, N, K, r, G, _ptr(Y), out_dtype, Y.stride(0), _ptr(ws),
                                           0 if ws is None else ws.numel(), _ptr(dbg_P), _stream(stream))
     _check(code, "twq_dual_linear")
+    return Y
+
+
+def noalloc_max_workspace() -> int:
+    return int(load_library().twq_noalloc_max_workspace())
+
+
+def dual_linear_noalloc(X, Xq, sx, packed: PackedLayer, Y, out_dtype: int = OUT_BF16, stream=None):
+    """twq_dual_linear_noalloc: twq_dual_linear with the library's static scratch (include/twq.h); the caller passes the
+    output too, so that nothing at all is allocated by the call."""
+    M = Xq.shape[0]
+    N, K, r, G = packed.N, packed.K, packed.r, packed.G
+    ldx = X.stride(0) if X is not None else K
+    code = load_library().twq_dual_linear_noalloc(_ptr(X) if r else None, ldx, _ptr(Xq), _ptr(sx), _ptr(packed.blob),
+                                                  M, N, K, r, G, _ptr(Y), out_dtype, Y.stride(0), _stream(stream))
+    _check(code, "twq_dual_linear_noalloc")
     return Y
 
 

@@ -98,6 +98,7 @@ enum : unsigned {
     kPlanFusedCsShift = 8,   // bits 8..11: forced cluster size of the fused kernel (0 = planner's choice)
     kPlanDecodeCsShift = 12, // bits 12..16: forced cluster size of the decode kernel (0 = planner's choice)
 };
+size_t workspace_counter_bytes(int M, int N, int K, int r, int G);   // twq_api.cu: zero-on-entry prefix of a workspace
 unsigned plan_flags();
 void set_plan_flags(unsigned f);
 float measure_i8_tops(int iters, int reps, cudaStream_t stream);   // peak_i8.cu (bench measurement aid)

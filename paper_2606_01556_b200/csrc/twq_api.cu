@@ -199,6 +199,16 @@ MapKey key2d(CUtensorMapDataType dt, const void* ptr, uint64_t inner, uint64_t r
 
 }  // namespace
 
+namespace twq {
+// Bytes at the front of a twq_dual_linear workspace that must be zero when a call starts (the split-K tile counters);
+// 0 for shapes that need no workspace.  Used by static_ws.cu.
+size_t workspace_counter_bytes(int M, int N, int K, int r, int G) {
+    if (!shape_ok(M, N, K, r, G)) return 0;
+    const CallPlan* cp = get_plan(M, N, K, r, G);
+    return (cp && !cp->decode && cp->fp.splits > 1) ? ctr_bytes(cp->fp) : 0;
+}
+}  // namespace twq
+
 extern "C" {
 
 const char* twq_status_string(twq_status s) {
