@@ -48,6 +48,9 @@ WORKLOADS = {
     "c1_tiny": ("config1_tiny", dict(), "tiny M=8 K=256 N=512 r=16 G=64"),
     # rank 0 (plain W4A4): what the residual stream alone costs
     "c2_qproj_m1_r0": ("config2_qproj", dict(M=1, r=0), "LLaMA3-8B q_proj K=4096 N=4096 r=0 G=128 M=1"),
+    "c2_qproj_m128_r0": ("config2_qproj", dict(M=128, r=0), "LLaMA3-8B q_proj K=4096 N=4096 r=0 G=128 M=128"),
+    "c2_qproj_m256": ("config2_qproj", dict(M=256), "LLaMA3-8B q_proj K=4096 N=4096 r=128 G=128 M=256"),
+    "c2_qproj_m512": ("config2_qproj", dict(M=512), "LLaMA3-8B q_proj K=4096 N=4096 r=128 G=128 M=512"),
     "c2_qproj_m16_r0": ("config2_qproj", dict(M=16, r=0), "LLaMA3-8B q_proj K=4096 N=4096 r=0 G=128 M=16"),
     # configs 4 / 5 (rank 256): not in the default sweep; DESIGN.md section 10 quotes them
     "c4_gateup_m4096": ("config4_qwen", dict(which="gate_up", M=4096), "Qwen3-32B gate/up K=5120 N=25600 r=256 M=4096"),

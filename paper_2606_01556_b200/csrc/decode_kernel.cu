@@ -161,97 +161,115 @@ __device__ __forceinline__ void decode_quantize_share(const DecodeParams& p, uin
     // ([g][token][G/2], the layout the MMA fragments read without bank conflicts): the activation tile is
     // quantized once per cluster and reused by all its CTAs and tiles (L179).
     uint8_t* sXq = dsm + p.off_xq;
-    constexpr int kLPI = G / 8;                          // lanes per (token, group): 8 elements each
-    constexpr int kIPW = 32 / kLPI;                      // (token, group) items per warp pass
     // Rows beyond M are written by nobody and stay whatever the shared memory held: row m of the MMA's activation
     // operand only reaches row m of its result, and no result row >= M is ever read (clearing the 32 KB tile cost
     // 1.1 us at the head of the critical path; in-kernel timeline, r02).
     const int gq0 = static_cast<int>(static_cast<unsigned>(ng) * rank / cs);
     const int ngq = static_cast<int>(static_cast<unsigned>(ng) * (rank + 1) / cs) - gq0;
     const int items = p.M * ngq;
-    const int li = lane % kLPI, sub = lane / kLPI;
     const uint16_t* X = static_cast<const uint16_t*>(p.X);
     TWQ_DSTAMP(21);
     // This loop heads the critical path of the call and is one dependent chain per warp: every instruction in it is paid in
     // full (a software prefetch of four passes with its index divisions cost 0.6 us at M = 1; measured, r02).
     bool waited = cs <= 1;
     TWQ_DCLK(4);
+    // One pass of the residual warps covers nrw * 32 / (G/8) items with 8 elements per lane.  Where that is not enough
+    // (M >= 16 at 16 ranks) a lane takes 16 elements instead: one pass where there were two, and every pass is a DRAM round
+    // trip plus ~150 dependent instructions at the head of the critical path (M = 16: 3.0 -> 1.9 us; in-kernel timeline, r02).
+    auto pass = [&](auto epl_c) {
+        constexpr int EPL = decltype(epl_c)::value;          // elements per lane: 8 or 16
+        constexpr int kLPI = G / EPL;                        // lanes per (token, group)
+        constexpr int kIPW = 32 / kLPI;                      // (token, group) items per warp pass
+        constexpr int kV = EPL / 8;                          // 16-byte loads per lane
+        const int li = lane % kLPI, sub = lane / kLPI;
 #pragma unroll 1
-    for (int base0 = rw * kIPW; base0 < items; base0 += nrw * kIPW) {
-    {
-        const int it = base0 + sub;
-        const bool on = it < items;                      // whole items are on or off: the shuffles below stay inside one
-        int m = 0, gi = 0;
-        if (on) {
-            if (ngq == 1) { m = it; }
-            else if (ngq == 2) { m = it >> 1; gi = it & 1; }
-            else { m = it / ngq; gi = it - m * ngq; }
-        }
-        const int g = gq0 + gi;
-        const uint4 vld = on ? ldg_v4(X + static_cast<size_t>(m) * p.ldx + g * G + li * 8) : make_uint4(0u, 0u, 0u, 0u);
-        if (!waited) {                                   // warp-uniform; after the load is in flight
-            cluster_wait();                              // every CTA of the cluster is running (its barriers exist)
-            waited = true;
-        }
-        float x[8];
-#pragma unroll
-        for (int i = 0; i < 8; ++i) x[i] = 0.0f;
-        if (on) {
-            const uint4 v = vld;
-            const uint32_t w[4] = {v.x, v.y, v.z, v.w};
-#pragma unroll
-            for (int i = 0; i < 4; ++i) {
-                x[2 * i] = __uint_as_float(w[i] << 16);              // BF16 -> FP32, exact
-                x[2 * i + 1] = __uint_as_float(w[i] & 0xFFFF0000u);
+        for (int base0 = rw * kIPW; base0 < items; base0 += nrw * kIPW) {
+            const int it = base0 + sub;
+            const bool on = it < items;                      // whole items are on or off: the shuffles below stay inside one
+            int m = 0, gi = 0;
+            if (on) {
+                if (ngq == 1) { m = it; }
+                else if (ngq == 2) { m = it >> 1; gi = it & 1; }
+                else { m = it / ngq; gi = it - m * ngq; }
             }
-            if (p.tinv != nullptr) {
-                const float4 t0 = __ldg(reinterpret_cast<const float4*>(p.tinv + g * G + li * 8));
-                const float4 t1 = __ldg(reinterpret_cast<const float4*>(p.tinv + g * G + li * 8) + 1);
-                x[0] = __fmul_rn(x[0], t0.x); x[1] = __fmul_rn(x[1], t0.y); x[2] = __fmul_rn(x[2], t0.z); x[3] = __fmul_rn(x[3], t0.w);
-                x[4] = __fmul_rn(x[4], t1.x); x[5] = __fmul_rn(x[5], t1.y); x[6] = __fmul_rn(x[6], t1.z); x[7] = __fmul_rn(x[7], t1.w);
+            const int g = gq0 + gi;
+            uint4 vld[kV];
+#pragma unroll
+            for (int v = 0; v < kV; ++v)
+                vld[v] = on ? ldg_v4(X + static_cast<size_t>(m) * p.ldx + g * G + li * EPL + v * 8) : make_uint4(0u, 0u, 0u, 0u);
+            if (!waited) {                                   // warp-uniform; after the loads are in flight
+                cluster_wait();                              // every CTA of the cluster is running (its barriers exist)
+                waited = true;
             }
-        }
-        float amax = 0.0f;
+            float x[EPL];
 #pragma unroll
-        for (int i = 0; i < 8; ++i) amax = fmaxf(amax, fabsf(x[i]));
+            for (int v = 0; v < kV; ++v) {
+                const uint32_t w[4] = {vld[v].x, vld[v].y, vld[v].z, vld[v].w};
 #pragma unroll
-        for (int d = kLPI / 2; d >= 1; d >>= 1) amax = fmaxf(amax, __shfl_xor_sync(0xffffffffu, amax, d));
-        const float sc = __fdiv_rn(fmaxf(amax, 0x1p-30f), 7.0f);
-        const float inv = __fdiv_rn(1.0f, sc);
-        uint32_t pk = 0u;
-#pragma unroll
-        for (int i = 0; i < 8; ++i) {
-            int q = __float2int_rn(__fmul_rn(x[i], inv));            // round-half-to-even
-            q = max(-7, min(7, q));
-            pk |= (static_cast<uint32_t>(q) & 0xFu) << (4 * i);      // low nibble = even k
-        }
-        if (on) {
-            uint32_t* qd = reinterpret_cast<uint32_t*>(sXq + (g * kMp + m) * (G / 2) + li * 4);
-            if (xq_bulk) {
-                *qd = pk;
-            } else {
-                const uint32_t qa = smem_u32(qd);
-                for (int pr = 0; pr < cs; ++pr) st_dsmem_u32(mapa_u32(qa, pr), pk);
-            }
-            if (li == 0) {
-                const float s8 = sc * 0x1p-8f;                       // MMA operands are 16*code
-                if (xq_bulk) {
-                    sSx[g * kMp + m] = s8;
-                } else {
-                    const uint32_t sa = smem_u32(sSx + g * kMp + m);
-                    for (int pr = 0; pr < cs; ++pr) st_dsmem_u32(mapa_u32(sa, pr), __float_as_uint(s8));
+                for (int i = 0; i < 4; ++i) {
+                    x[v * 8 + 2 * i] = __uint_as_float(w[i] << 16);              // BF16 -> FP32, exact (0 when off)
+                    x[v * 8 + 2 * i + 1] = __uint_as_float(w[i] & 0xFFFF0000u);
                 }
-                if (p.sx_out != nullptr) p.sx_out[static_cast<size_t>(m) * ng + g] = sc;
             }
-            if (p.xq_out != nullptr)
-                *reinterpret_cast<uint32_t*>(p.xq_out + static_cast<size_t>(m) * (p.K >> 1) + g * (G / 2) + li * 4) = pk;
+            if (on && p.tinv != nullptr) {
+#pragma unroll
+                for (int v = 0; v < EPL / 4; ++v) {
+                    const float4 t = __ldg(reinterpret_cast<const float4*>(p.tinv + g * G + li * EPL) + v);
+                    x[4 * v] = __fmul_rn(x[4 * v], t.x); x[4 * v + 1] = __fmul_rn(x[4 * v + 1], t.y);
+                    x[4 * v + 2] = __fmul_rn(x[4 * v + 2], t.z); x[4 * v + 3] = __fmul_rn(x[4 * v + 3], t.w);
+                }
+            }
+            float amax = 0.0f;
+#pragma unroll
+            for (int i = 0; i < EPL; ++i) amax = fmaxf(amax, fabsf(x[i]));
+#pragma unroll
+            for (int d = kLPI / 2; d >= 1; d >>= 1) amax = fmaxf(amax, __shfl_xor_sync(0xffffffffu, amax, d));
+            const float sc = __fdiv_rn(fmaxf(amax, 0x1p-30f), 7.0f);
+            const float inv = __fdiv_rn(1.0f, sc);
+            uint32_t pk[kV];
+#pragma unroll
+            for (int v = 0; v < kV; ++v) {
+                pk[v] = 0u;
+#pragma unroll
+                for (int i = 0; i < 8; ++i) {
+                    int q = __float2int_rn(__fmul_rn(x[v * 8 + i], inv));        // round-half-to-even
+                    q = max(-7, min(7, q));
+                    pk[v] |= (static_cast<uint32_t>(q) & 0xFu) << (4 * i);       // low nibble = even k
+                }
+            }
+            if (on) {
+                uint32_t* qd = reinterpret_cast<uint32_t*>(sXq + (g * kMp + m) * (G / 2) + li * (EPL / 2));
+#pragma unroll
+                for (int v = 0; v < kV; ++v) {
+                    if (xq_bulk) {
+                        qd[v] = pk[v];
+                    } else {
+                        const uint32_t qa = smem_u32(qd + v);
+                        for (int pr = 0; pr < cs; ++pr) st_dsmem_u32(mapa_u32(qa, pr), pk[v]);
+                    }
+                    if (p.xq_out != nullptr)
+                        *reinterpret_cast<uint32_t*>(p.xq_out + static_cast<size_t>(m) * (p.K >> 1) + g * (G / 2) + li * (EPL / 2) + v * 4) = pk[v];
+                }
+                if (li == 0) {
+                    const float s8 = sc * 0x1p-8f;                   // MMA operands are 16*code
+                    if (xq_bulk) {
+                        sSx[g * kMp + m] = s8;
+                    } else {
+                        const uint32_t sa = smem_u32(sSx + g * kMp + m);
+                        for (int pr = 0; pr < cs; ++pr) st_dsmem_u32(mapa_u32(sa, pr), __float_as_uint(s8));
+                    }
+                    if (p.sx_out != nullptr) p.sx_out[static_cast<size_t>(m) * ng + g] = sc;
+                }
+            }
         }
-    }
-    }
+    };
+    if (items > nrw * (32 / (G / 8))) pass(std::integral_constant<int, 16>{});
+    else pass(std::integral_constant<int, 8>{});
     if (!waited) cluster_wait();                         // warps without an item
     TWQ_DCLK(5);
     TWQ_DSTAMP(22);
     if (xq_bulk) fence_proxy_async_smem();               // the bulk copies below read what this thread stored
+    TWQ_DSTAMP(24);
     named_bar_sync(2, nrw * 32);                         // this CTA's share is stored (in bulk mode: in its own shared memory)
     TWQ_DSTAMP(23);
     if constexpr (kL4) asm volatile("bar.arrive 4, %0;" ::"r"((nrw + lrw) * 32) : "memory");   // q4lr stage 1 may read it
@@ -1156,7 +1174,9 @@ decode_dual_linear_kernel(const __grid_constant__ CUtensorMap tmXq, const __grid
             }
             // this warp's partial tiles: [tile * P + part][token][8 channels], parked in the ring, which every residual
             // warp has finished reading (all chunks have landed and been consumed)
+            TWQ_DSTAMP(25);
             named_bar_sync(2, nrw * 32);
+            TWQ_DSTAMP(26);
 #pragma unroll
             for (int i = 0; i < kTPW; ++i) {
                 if (slot_on(i)) {
