@@ -19,6 +19,7 @@ extern "C" {
 #define TWQ_PLAN_NO_DECODE     16u   /* small batches go to the tcgen05 kernel as well */
 #define TWQ_PLAN_FUSED_CS(c)   (((unsigned)(c) & 15u) << 8)    /* forced cluster size of the tcgen05 kernel */
 #define TWQ_PLAN_DECODE_CS(c)  (((unsigned)(c) & 31u) << 12)   /* forced cluster size of the small-batch kernel */
+#define TWQ_PLAN_FUSED_TN_CAP(c) (((unsigned)(c) & 3u) << 17)   /* tcgen05 kernel token tile: 1 = at most 64, 2 = at most 32 */
 
 void twq_testing_set_plan_flags(unsigned flags);
 unsigned twq_testing_get_plan_flags(void);

@@ -34,6 +34,11 @@ def plan_decode_cs(c: int) -> int:
     return (c & 31) << 12
 
 
+def plan_fused_tn_cap(c: int) -> int:
+    """TWQ_PLAN_FUSED_TN_CAP: 1 = token tile of the tcgen05 kernel at most 64, 2 = at most 32."""
+    return (c & 3) << 17
+
+
 class TwqError(RuntimeError):
     def __init__(self, code: int, where: str):
         super().__init__(f"{where}: {_STATUS.get(code, code)}")

@@ -191,7 +191,11 @@ static bool make_plan_tn(int TN, int M, int N, int K, int r, int G, int num_sms,
 
 bool fused_make_plan(int M, int N, int K, int r, int G, int num_sms, FusedPlan* out) {
     // a smaller token tile is the fallback when rank-256 buffers do not fit beside a 128-token tile
-    for (int TN = pick_tn(M); TN >= 16; TN >>= 1)
+    int tn0 = pick_tn(M);
+    const unsigned cap = (plan_flags() >> kPlanFusedTnShift) & 3u;       // test / measurement override
+    if (cap == 1 && tn0 > 64) tn0 = 64;
+    if (cap == 2 && tn0 > 32) tn0 = 32;
+    for (int TN = tn0; TN >= 16; TN >>= 1)
         if (make_plan_tn(TN, M, N, K, r, G, num_sms, out)) return true;
     return false;
 }

@@ -97,6 +97,7 @@ enum : unsigned {
     kPlanNoDecode = 16u,     // small-batch calls go to the tcgen05 kernel too
     kPlanFusedCsShift = 8,   // bits 8..11: forced cluster size of the fused kernel (0 = planner's choice)
     kPlanDecodeCsShift = 12, // bits 12..16: forced cluster size of the decode kernel (0 = planner's choice)
+    kPlanFusedTnShift = 17,  // bits 17..18: token tile of the fused kernel: 0 = planner's choice, 1 = at most 64, 2 = at most 32
 };
 size_t workspace_counter_bytes(int M, int N, int K, int r, int G);   // twq_api.cu: zero-on-entry prefix of a workspace
 unsigned plan_flags();

@@ -175,6 +175,22 @@ def test_fused_kernel_cta_pairs(twq, oracle, plan_flags, M, K, N, r, G):
     _check_layer(twq, oracle, gen.make_layer(M, K, N, r, G, seed=3000 + M, with_tinv=(M % 2 == 0)), rows=rows)
 
 
+@pytest.mark.parametrize("cap,tn,M,K,N,r,G", [
+    (1, 64, 256, 1024, 2048, 128, 128),    # 4 token tiles of 64, several per cluster
+    (2, 32, 128, 2048, 4096, 128, 128),    # the mid-M measurement of DESIGN.md 6.3: 4 x 32 tokens, no K split, no workspace
+    (2, 32, 100, 512, 1040, 64, 64),       # ragged token tile and channel tile, G = 64
+    (1, 64, 200, 1024, 1024, 256, 128),    # rank 256 beside a 64-token tile
+])
+def test_fused_kernel_small_token_tiles_unsplit(twq, oracle, plan_flags, cap, tn, M, K, N, r, G):
+    """M > 64 with the token tile capped (TWQ_PLAN_FUSED_TN_CAP): the 32- / 64-token instantiations of the tcgen05 kernel
+    walking several token tiles, which production shapes only reach through the rank-256 fallback; same bar."""
+    plan_flags(twq.plan_fused_tn_cap(cap) | twq.PLAN_NO_SPLIT)
+    plan = twq.testing_describe_plan(M, N, K, r, G)
+    assert plan["kernel"] == "tcgen05" and plan["tile_tokens"] == tn and plan["splits"] == 1
+    assert twq.workspace_bytes(M, N, K, r, G) == 0
+    _check_layer(twq, oracle, gen.make_layer(M, K, N, r, G, seed=3300 + M, with_tinv=(M % 2 == 0)))
+
+
 @pytest.mark.parametrize("pad", [0, 8, 2, 1])
 @pytest.mark.parametrize("split,N", [(False, 1232), (False, 1200), (True, 1232)])
 def test_fused_kernel_store_paths(twq, oracle, plan_flags, pad, split, N):
