@@ -46,9 +46,14 @@ namespace twq {
 
 namespace {
 
-constexpr int kDecWarps = 18;                       // compute warps (registers are allotted to warps in fours: 20 warps
-                                                    // cost the same 96 registers per thread as 18 would)
-constexpr int kDecThreads = (kDecWarps + 2) * 32;   // + the producer warp and a spare
+// Compute warps per CTA, + the producer warp and the activation-side producer.  Up to two token tiles (M <= 32): 14 + 2 =
+// 16 warps, which is the largest CTA that gets 128 registers per thread -- the MT = 1 instantiations need 116 and were at
+// the 96-register limit of a 20-warp CTA, where ptxas' allocation decided the result (lesson 16):
+// M = 1 / 16 / 32 went 8.9 / 9.9 / 14.8 -> 8.6 / 9.5 / 14.1 us.  Four token tiles (M <= 64) keep 18 + 2 warps at 96
+// registers: there the extra warps are worth more than the spills they cause (M = 64: 22.1 vs 22.5 us; r = 256: 34.7 vs 38.5).
+// (The 4-bit low-rank mode is better off with 16 warps at four token tiles too: 28.8 vs 34.0 us.)
+__host__ __device__ constexpr int dec_warps(int mt, bool lr4) { return (mt == 4 && !lr4) ? 18 : 14; }
+__host__ __device__ constexpr int dec_threads(int mt, bool lr4) { return (dec_warps(mt, lr4) + 2) * 32; }
 constexpr int kMaxSlots = 8, kMaxL1Slots = 4;
 constexpr int kTB = 3;                              // tiles whose MMA chains a residual warp interleaves
 constexpr int kJT = 8;                              // 8-wide j tiles of H one low-rank warp can own
@@ -301,9 +306,10 @@ __device__ __forceinline__ void decode_quantize_share(const DecodeParams& p, uin
 //             Q_H in shared memory, in the activation quantizer's FP32 operation order;
 //   stage 2   Ylr = sum_h s_H*sv*(Q_H . qv): a second int8 MMA against the V section, folded into the same epilogue.
 template <int G, int MT, bool kDbg, int kMode>
-__global__ void __launch_bounds__(kDecThreads, 1)
+__global__ void __launch_bounds__(dec_threads(MT, kMode == 2), 1)
 decode_dual_linear_kernel(const __grid_constant__ CUtensorMap tmXq, const __grid_constant__ DecodeParams p) {
     constexpr bool kQ = kMode >= 1, kL4 = kMode == 2;
+    constexpr int kDecWarps = dec_warps(MT, kL4);
     extern __shared__ uint8_t dsm_raw[];
     // 1024-byte aligned base; the same offset in every CTA of the cluster (DSMEM addresses are formed from local ones)
     uint8_t* dsm = dsm_raw + ((1024u - (smem_u32(dsm_raw) & 1023u)) & 1023u);
@@ -1272,7 +1278,7 @@ cudaError_t decode_launch_inst(const CUtensorMap& tmXq, const DecodeParams& p, c
     }
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(static_cast<unsigned>(p.grid));
-    cfg.blockDim = dim3(kDecThreads);
+    cfg.blockDim = dim3(dec_threads(MT, kMode == 2));
     cfg.dynamicSmemBytes = static_cast<size_t>(p.smem_bytes);
     cfg.stream = stream;
     cudaLaunchAttribute attrs[2];
@@ -1307,7 +1313,7 @@ int decode_cluster_capacity(int cs, int num_sms) {
             cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1) == cudaSuccess) {
             cudaLaunchConfig_t cfg = {};
             cfg.gridDim = dim3(static_cast<unsigned>(num_sms / cs * cs));
-            cfg.blockDim = dim3(kDecThreads);
+            cfg.blockDim = dim3(dec_threads(4, false));
             cfg.dynamicSmemBytes = 200 * 1024;
             cudaLaunchAttribute attr;
             attr.id = cudaLaunchAttributeClusterDimension;
@@ -1344,7 +1350,7 @@ bool decode_make_plan(int M, int N, int K, int r, int G, int num_sms, int quant,
     p.mt = M <= 16 ? 1 : (M <= 32 ? 2 : 4);
     p.mp = 16 * p.mt;
     p.lrw = r > 0 ? (p.mt == 4 ? 8 : 4) : 0;              // more token tiles: stage 1 / stage 2 over eight warps
-    const int nrw = kDecWarps - p.lrw;
+    const int nrw = dec_warps(p.mt, lr4) - p.lrw;
     // cluster size: H is shared by the cluster and every cluster streams all of L1 (K*r*2 bytes) from L2, so the
     // largest cluster that still covers 70 % of the SMs wins; otherwise the size covering the most SMs
     p.cs = 1;
