@@ -153,10 +153,13 @@ __device__ __forceinline__ void lds_words(uint32_t (&dst)[kW], uint32_t a) {
 
 // The in-kernel activation quantizer and its all-gather (kMode >= 1), run by the residual warps.
 template <int G, int MT, bool kL4>
-__device__ __forceinline__ void decode_quantize_share(const DecodeParams& p, uint8_t* dsm, int rank, int rw, int lane, int nrw, int lrw,
-                                                   bool xq_bulk) {
+__device__ __forceinline__ void decode_quantize_share(const DecodeParams& p, uint8_t* dsm, int rank, int cs, int rw, int lane, int nrw,
+                                                   int lrw, bool xq_bulk) {
+    // (rank, cs) = the cluster rank and size, or (0, 1) in local mode: one or two tokens, where every CTA quantizes the whole
+    // row block itself (M x K elements, L2-resident after the first cluster) and nothing is exchanged -- the all-gather's skew
+    // and remote latency (~1 us) cost more than the extra items.  Local mode runs the bulk branch with no peer to copy to.
     constexpr int kMp = 16 * MT;
-    const int ng = p.ng, cs = p.cs;
+    const int ng = p.ng;
     float* sSx = reinterpret_cast<float*>(dsm + p.off_sx);
     const uint32_t bar0 = smem_u32(dsm + p.off_bar);
 #define DBAR(i) (bar0 + 8u * static_cast<uint32_t>(i))
@@ -357,7 +360,10 @@ decode_dual_linear_kernel(const __grid_constant__ CUtensorMap tmXq, const __grid
 
     // The in-kernel quantizer's all-gather: per-lane remote stores for a handful of tokens (lowest latency), bulk copies through
     // distributed shared memory above that (one remote transaction per warp and peer does not scale with M).
-    const bool xq_bulk = kQ && cs > 1 && p.M > 4;
+    // (only where the low-rank chain waits for the quantized tile too: in the FP16 mode the all-gather is off the critical
+    // path at these M and the local mode measured 0.3 us slower)
+    const bool xq_local = kL4 && cs > 1 && p.M <= 2;
+    const bool xq_bulk = kQ && cs > 1 && (p.M > 4 || xq_local);
     TWQ_DSTAMP(0);
     const uint32_t bar0 = smem_u32(dsm + p.off_bar);
 #define DBAR(i) (bar0 + 8u * static_cast<uint32_t>(i))
@@ -387,7 +393,7 @@ decode_dual_linear_kernel(const __grid_constant__ CUtensorMap tmXq, const __grid
             // the in-kernel quantizer's all-gather arrives as bulk copies from the cs - 1 peers: every K-group this rank does
             // not quantize itself, all kMp token rows of codes and scales
             const int own = static_cast<int>(static_cast<unsigned>(ng) * (rank + 1) / cs) - static_cast<int>(static_cast<unsigned>(ng) * rank / cs);
-            mbar_arrive_expect_tx_a(DBAR(D_XQ), static_cast<uint32_t>(ng - own) * (kMp * (G / 2) + kMp * 4));
+            mbar_arrive_expect_tx_a(DBAR(D_XQ), xq_local ? 0u : static_cast<uint32_t>(ng - own) * (kMp * (G / 2) + kMp * 4));
         }
     }
     __syncthreads();
@@ -967,7 +973,7 @@ decode_dual_linear_kernel(const __grid_constant__ CUtensorMap tmXq, const __grid
         pdl_wait();                                              // sx (or X) comes from the previous kernel of the stream
         TWQ_DSTAMP(2);
         if constexpr (kQ) {
-            decode_quantize_share<G, MT, kL4>(p, dsm, rank, rw, lane, nrw, lrw, xq_bulk);
+            decode_quantize_share<G, MT, kL4>(p, dsm, xq_local ? 0 : rank, xq_local ? 1 : cs, rw, lane, nrw, lrw, xq_bulk);
         } else {
             for (int i = rw * 32 + lane; i < kMp * ng; i += nrw * 32) {
                 const int g = i / kMp, m = i - g * kMp;
@@ -1246,8 +1252,8 @@ decode_dual_linear_kernel(const __grid_constant__ CUtensorMap tmXq, const __grid
         }
     }
     TWQ_DSTAMP(29);
-    if (cs > 1 && !is_lr && !(kQ && warp < nrw)) cluster_wait();   // completes this thread's half of the split barrier (long since released)
-    if (xq_bulk) {
+    if (cs > 1 && !is_lr && !(kQ && warp < nrw && !xq_local)) cluster_wait();   // completes this thread's half of the split barrier (long since released)
+    if (xq_bulk && !xq_local) {
         // The all-gather's bulk copies read the SENDER's shared memory: no CTA may exit (and hand its shared memory to another
         // block) before every peer has received its share.  Every CTA gets here after its own share arrived in full, so one
         // more cluster barrier is enough; the kernel ends with its slowest CTA either way.
