@@ -367,11 +367,10 @@ decode_dual_linear_kernel(const __grid_constant__ CUtensorMap tmXq, const __grid
     TWQ_DSTAMP(0);
     const uint32_t bar0 = smem_u32(dsm + p.off_bar);
 #define DBAR(i) (bar0 + 8u * static_cast<uint32_t>(i))
-    // Barrier initialisation.  The kernel runs at its register limit (96 per thread with 20 warps) and ptxas' allocation there
-    // is brittle: with the one-thread-per-barrier form below, the instantiations that contain the in-kernel quantizer spill
-    // three preamble values (tile0, rank, ...) and lose 0.5 us at M = 1; with the serial form the two-call instantiation
-    // spills instead and loses 0.1-0.3 us (A/B of both builds in one run, r02).  Each instantiation keeps the form it is
-    // spill-free with; `ptxas -v` must show 0 spill bytes for MT = 1 after any change to this kernel.
+    // Barrier initialisation: one thread per barrier without the in-kernel quantizer, serial with it.  Measured, not
+    // reasoned: at the 96-register limit of the former 20-warp CTA the parallel form made the quantizer instantiations spill
+    // (-0.5 us at M = 1) and the serial form the other one; with 16-warp CTAs at 128 registers nothing spills any more, and
+    // the parallel form is still 0.15 us slower in the quantizer instantiations (A/B of both libraries in one run, r02).
     if (!kQ && threadIdx.x < D_COUNT) {
         const int i = threadIdx.x;
         int count = 1;                                                        // D_FULL, D_L1FULL: the producer's expect_tx
