@@ -73,6 +73,14 @@ __device__ __forceinline__ void imma_16832(int (&d)[4], uint32_t a0, uint32_t a1
         : "+r"(d[0]), "+r"(d[1]), "+r"(d[2]), "+r"(d[3])
         : "r"(a0), "r"(a1), "r"(a2), "r"(a3), "r"(b0), "r"(b1));
 }
+// D[16x8] (s32) = A * B (zero accumulator: the first K-step of a chain; saves the four moves that clear D)
+__device__ __forceinline__ void imma_16832_z(int (&d)[4], uint32_t a0, uint32_t a1, uint32_t a2, uint32_t a3,
+                                             uint32_t b0, uint32_t b1) {
+    asm volatile(
+        "mma.sync.aligned.m16n8k32.row.col.s32.s8.s8.s32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%10,%10,%10,%10};"
+        : "=r"(d[0]), "=r"(d[1]), "=r"(d[2]), "=r"(d[3])
+        : "r"(a0), "r"(a1), "r"(a2), "r"(a3), "r"(b0), "r"(b1), "r"(0));
+}
 // D[16x8] (f32) += A[16x16] (f16, row) * B[16x8] (f16, col)
 __device__ __forceinline__ void hmma_16816(float (&d)[4], uint32_t a0, uint32_t a1, uint32_t a2, uint32_t a3,
                                            uint32_t b0, uint32_t b1) {
@@ -1121,10 +1129,6 @@ decode_dual_linear_kernel(const __grid_constant__ CUtensorMap tmXq, const __grid
                                         lds_words<kW>(wt[b], wa + toff[ib + b]);
                                         swh[b] = lds_u32(swp + swoff[ib + b]);
                                     }
-#pragma unroll
-                                    for (int mt = 0; mt < MT; ++mt)
-#pragma unroll
-                                        for (int e = 0; e < 4; ++e) dd[b][mt][e] = 0;
                                 }
 #pragma unroll
                                 for (int w = 0; w < kW; ++w) {   // one K-step of 32 codes per packed word
@@ -1134,7 +1138,8 @@ decode_dual_linear_kernel(const __grid_constant__ CUtensorMap tmXq, const __grid
                                             const uint32_t b0 = d_lo16(wt[b][w]), b1 = d_hi16(wt[b][w]);
 #pragma unroll
                                             for (int mt = 0; mt < MT; ++mt)
-                                                imma_16832(dd[b][mt], ax[mt][w][0], ax[mt][w][1], ax[mt][w][2], ax[mt][w][3], b0, b1);
+                                                if (w == 0) imma_16832_z(dd[b][mt], ax[mt][w][0], ax[mt][w][1], ax[mt][w][2], ax[mt][w][3], b0, b1);
+                                                else imma_16832(dd[b][mt], ax[mt][w][0], ax[mt][w][1], ax[mt][w][2], ax[mt][w][3], b0, b1);
                                         }
                                     }
                                 }
