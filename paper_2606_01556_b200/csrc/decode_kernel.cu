@@ -335,7 +335,9 @@ decode_dual_linear_kernel(const __grid_constant__ CUtensorMap tmXq, const __grid
     float* sRes = reinterpret_cast<float*>(dsm + p.off_res);       // [tile * P + part][kMp][8]
     __half* sXs = reinterpret_cast<__half*>(dsm + p.off_xs);       // [kMp][xs_stride] FP16 copy of the X slice
 
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    // the warp index through a shuffle: the compiler then knows it is warp-uniform, and with it every role branch and loop bound
+    // derived from it (otherwise each mma.sync in those loops is preceded by a WARPSYNC)
+    const int warp = __shfl_sync(0xffffffffu, static_cast<int>(threadIdx.x >> 5), 0), lane = threadIdx.x & 31;
     const int gid = lane >> 2, tid4 = lane & 3;
     const int r = p.r, ng = p.ng, cs = p.cs, lrw = p.lrw;
     const int nrw = kDecWarps - lrw;
