@@ -193,7 +193,8 @@ fused_dual_linear_kernel(const __grid_constant__ CUtensorMap tmW, const __grid_c
     uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(bars + B_COUNT);
 
     TWQ_TG(0);
-    const int warp = threadIdx.x >> 5;
+    // through a shuffle: the compiler then knows the warp index, the role branches and their loop bounds are warp-uniform
+    const int warp = __shfl_sync(0xffffffffu, static_cast<int>(threadIdx.x >> 5), 0);
     const int lane = threadIdx.x & 31;
     const int r = p.r;
     const int nrb = (r + 127) >> 7;          // 128-row blocks of L1T / H^T
