@@ -9,21 +9,23 @@
 // Everything that does not depend on the activations is therefore in flight from the first instruction, as
 // asynchronous bulk copies (TMA, cp.async.bulk) into shared memory that complete on mbarriers:
 //
-//   warp 18      residual producer.  The CTA owns `ntile` consecutive 8-channel tiles; R4 is stored tile-major
-//                ([N/8][K/G][8][G/2]), so the K-groups [c*gc, (c+1)*gc) of a tile are one contiguous range.  Chunk c
-//                of the ring = those ranges of all tiles (1-D bulk copies, issued BEFORE griddepcontrol.wait: weights
-//                do not depend on the previous kernel) + the same groups of Xq for all tokens (one 3-D tensor-map box,
-//                after the wait; rows beyond M are zero-filled by the TMA unit).
-//   warp 19      stage-1 producer: this cluster rank's K slice of L1 (slab layout [K/32][r][32]: one contiguous
-//                range) through its own ring; also pulls the CTA's rows of L2T into L2.
-//   warps 0..lrw-1   the low-rank chain: X slice -> FP16 shared memory, H partial (FP16 warp MMA, FP32 accumulate),
+//   W compute warps (14 up to two token tiles, 18 for four) + two producer warps; warp ids in this order:
+//   residual     (W - lrw warps) per ring chunk, INT4 -> int8 (each code c becomes the byte 16*c: one shift / and per word,
+//                sign for free), warp-level int8 MMAs (activations are the 16-row operand, so a tile is 8 channels),
+//                int32 = 256*P folded with both group scales in FP32.  When the CTA has fewer tiles than residual warps
+//                the K-groups of a tile are dealt round-robin to P warps and summed in fixed order.
+//   warp W       activation-side producer: the Xq boxes of the ring's first lap (one 3-D tensor-map box per chunk = the
+//                chunk's K-groups of all tokens, rows beyond M zero-filled by the TMA unit), right after
+//                griddepcontrol.wait; idle when the quantizer runs inside the kernel.
+//   warp W + 1   producer of everything that does not depend on the activations, issued BEFORE griddepcontrol.wait: first
+//                this cluster rank's K slice of L1 (slab layout [K/32][r][32]: one contiguous range) through its own
+//                ring, then the residual ring -- the CTA owns `ntile` consecutive 8-channel tiles and R4 is stored
+//                tile-major ([N/8][K/G][8][G/2]), so the K-groups [c*gc, (c+1)*gc) of a tile are one contiguous range and
+//                chunk c = those ranges of all tiles (1-D bulk copies); also pulls the CTA's rows of L2T into L2.
+//   lrw warps    the low-rank chain: X slice -> FP16 shared memory, H partial (FP16 warp MMA, FP32 accumulate),
 //                reduce-scatter of the FP32 partials and all-gather of the FP16 result through distributed shared
 //                memory (fixed order; mbarriers with cluster-scope release / acquire), then Ylr = H * L2T rows.
 //                H never leaves the chip (L177-179).
-//   warps lrw..17    the residual: per ring chunk, INT4 -> int8 (each code c becomes the byte 16*c: one shift / and
-//                per word, sign for free), warp-level int8 MMAs (activations are the 16-row operand, so a tile is 8
-//                channels), int32 = 256*P folded with both group scales in FP32.  When the CTA has fewer tiles than
-//                residual warps the K-groups of a tile are dealt round-robin to P warps and summed in fixed order.
 //   all          single epilogue: sum of the K-parts + Ylr, one rounding, one store (L181).
 //
 // The two branches only meet in the epilogue, so the weight stream, the low-rank chain and the cluster exchange
