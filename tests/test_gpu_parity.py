@@ -438,6 +438,29 @@ def test_dual_linear_x_one_launch(twq, oracle, M, K, N, r, G, with_tinv):
         assert (Y2 - Y32).abs().max().item() <= 1e-5 * float(np.abs(ref["Y"]).max())
 
 
+@pytest.mark.parametrize("M,K,N,r,G", [(1, 4096, 4096, 128, 128), (5, 2048, 1040, 64, 64), (16, 4096, 4096, 128, 128),
+                                       (33, 2048, 2064, 128, 128), (64, 1024, 4096, 256, 128)])
+def test_dual_linear_x_is_deterministic_under_repetition(twq, M, K, N, r, G):
+    """The one-launch kernel hands data between CTAs of a cluster three times (quantized tile, H partials, H) through
+    distributed shared memory, by per-lane stores or bulk copies, ordered by mbarriers only.  A missing fence or an early exit
+    shows up as a run-to-run difference: 60 back-to-back calls on rotating outputs must be bit-identical, codes included."""
+    import torch
+    L = gen.make_layer(M, K, N, r, G, seed=7200 + M, with_tinv=True)
+    X, packed, tinv = _upload(twq, L)
+    Ys = [torch.empty((M, N), dtype=torch.float32, device="cuda") for _ in range(4)]
+    Xqs = [torch.empty((M, K // 2), dtype=torch.uint8, device="cuda") for _ in range(4)]
+    Y0 = twq.dual_linear_x(X, packed, tinv, twq.OUT_FP32).clone()
+    Xq0, _ = twq.quantize_act(X, G, tinv)
+    for i in range(60):
+        twq.dual_linear_x(X, packed, tinv, twq.OUT_FP32, Y=Ys[i % 4], Xq_out=Xqs[i % 4] if i % 3 == 0 else None)
+        if i % 4 == 3:
+            for Y in Ys:
+                assert torch.equal(Y, Y0), i
+    torch.cuda.synchronize()
+    for Xq in Xqs:
+        assert torch.equal(Xq, Xq0)
+
+
 @pytest.mark.parametrize("M,K,N,r,G", [(80, 512, 384, 32, 128), (300, 1024, 1024, 128, 128)])
 def test_dual_linear_x_larger_batches_use_the_workspace(twq, oracle, M, K, N, r, G):
     """Beyond the small-batch kernel twq_dual_linear_x runs the stand-alone quantizer into the workspace, then the fused

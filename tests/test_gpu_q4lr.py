@@ -141,6 +141,30 @@ def test_q4lr_every_cluster_size(twq, oracle, plan_flags, cs, M, K, N, r, G):
     _check(twq, oracle, M, K, N, r, G, False, seed=cs + M)
 
 
+@pytest.mark.parametrize("M,K,N,r,G", [(1, 4096, 4096, 128, 128), (2, 1024, 528, 32, 64), (16, 4096, 4096, 128, 128),
+                                       (40, 2048, 1040, 256, 128)])
+def test_q4lr_is_deterministic_under_repetition(twq, M, K, N, r, G):
+    """Four hand-offs between the CTAs of a cluster (quantized tile -- local for one or two tokens --, H partials, H) ordered
+    by mbarriers only: 60 back-to-back calls must be bit-identical, the re-quantized codes included."""
+    import torch
+    L = gen.make_layer(M, K, N, 0, G, seed=8300 + M, with_tinv=True)
+    Uq, su, Vq, sv = gen.make_q4_lowrank(K, N, r, G, seed=9300 + M)
+    X = _dev(L.X.view(np.int16), torch.bfloat16)
+    tinv = _dev(L.tinv)
+    packed = twq.pack_weights_q4lr(_dev(L.Rq), _dev(L.sw), _dev(Uq), _dev(su), _dev(Vq), _dev(sv), G)
+    Y0 = twq.dual_linear_q4lr_x(X, packed, tinv, twq.OUT_FP32).clone()
+    Q0 = torch.empty((M, r), dtype=torch.int8, device="cuda")
+    twq.dual_linear_q4lr_x(X, packed, tinv, twq.OUT_FP32, dbg_QH=Q0)
+    Ys = [torch.empty((M, N), dtype=torch.float32, device="cuda") for _ in range(4)]
+    Q = torch.empty((M, r), dtype=torch.int8, device="cuda")
+    for i in range(60):
+        twq.dual_linear_q4lr_x(X, packed, tinv, twq.OUT_FP32, Y=Ys[i % 4], dbg_QH=Q if i % 5 == 0 else None)
+        if i % 4 == 3:
+            for Y in Ys:
+                assert torch.equal(Y, Y0), i
+            assert torch.equal(Q, Q0)
+
+
 def test_q4lr_zero_factor_is_the_plain_residual(twq, oracle):
     """U = 0: H = 0, s_H = 2^-30 / 7, Q_H = 0, and Y is the rank-0 layer (north_star's r = 0 reduction)."""
     import torch
