@@ -197,7 +197,9 @@ twq_status twq_dual_linear_x(const void* X, int ldx, const float* tinv, const vo
  *   dbg_H  [M,r] fp32       NULL, or receives H as the re-quantizer saw it
  *   dbg_QH [M,r] int8       NULL, or receives the codes Q_H;  dbg_sH [M,r/gr] fp32: NULL, or receives s_H
  *                           (parity evidence taken from the path that feeds Y; slows the call)
- * Returns TWQ_ERR_UNSUPPORTED when even a 16-token slab's shared-memory plan does not fit (K / G > ~200 groups).
+ * Returns TWQ_ERR_UNSUPPORTED when even a 16-token slab's shared-memory plan does not fit: the resident quantized tile
+ * (16 tokens x K/2 bytes), the FP32 H and the weight rings share 227 KB, which excludes e.g. K = 25600 at r = 256 and
+ * K = 8192 with N = 28672 at r = 256 (32 channel tiles per CTA).  Nothing is launched in that case.
  * Stream ordering and the other errors as for twq_dual_linear.
  */
 size_t twq_packed_bytes_q4lr(int N, int K, int r, int G);

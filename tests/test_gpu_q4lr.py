@@ -122,6 +122,39 @@ def test_q4lr_one_launch(twq, oracle, M, K, N, r, G, with_tinv):
     _check(twq, oracle, M, K, N, r, G, with_tinv, seed=M + N + r, expect_launches=1)
 
 
+@pytest.mark.parametrize("M,K,N,r,G", [
+    (16, 4096, 14336, 128, 128),     # configs[2] gate/up
+    (8, 14336, 4096, 128, 128),      # configs[2] down: 112 K-groups
+    (16, 4096, 14336, 256, 128),     # configs[2] at r = 256
+    (16, 8192, 8192, 256, 128),      # configs[4] q / o
+    (4, 5120, 25600, 256, 128),      # configs[3] gate/up
+])
+def test_q4lr_config_shapes_small_batches(twq, oracle, M, K, N, r, G):
+    """The layer shapes of BASELINE.json's configs 3-5 at decode-sized M through the 4-bit low-rank path."""
+    _check(twq, oracle, M, K, N, r, G, False, seed=M + N // 7 + r, expect_launches=1)
+
+
+@pytest.mark.parametrize("M,K,N,r,G", [
+    (4, 25600, 5120, 256, 128),      # configs[3] down: 200 K-groups
+    (1, 8192, 28672, 256, 128),      # configs[4] gate/up: 32 channel tiles per CTA beside a 64 KB resident activation tile
+])
+def test_q4lr_shapes_beyond_shared_memory_are_refused_not_wrong(twq, M, K, N, r, G):
+    """Where the resident quantized tile, the FP32 H and the rings do not fit in shared memory even for a 16-token slab the call
+    returns TWQ_ERR_UNSUPPORTED (include/twq.h) and launches nothing."""
+    import torch
+    L = gen.make_layer(M, K, 64, 0, G, seed=8400)
+    X = _dev(L.X.view(np.int16), torch.bfloat16)
+    nbytes = int(twq.load_library().twq_packed_bytes_q4lr(N, K, r, G))
+    assert nbytes > 0
+    packed = twq.PackedLayer(torch.zeros(nbytes, dtype=torch.uint8, device="cuda"), N, K, r, G)
+    Y = torch.full((M, N), 3.0, dtype=torch.float32, device="cuda")
+    with pytest.raises(twq.TwqError) as e:
+        twq.dual_linear_q4lr_x(X, packed, None, twq.OUT_FP32, Y=Y)
+    assert e.value.code == 2
+    torch.cuda.synchronize()
+    assert (Y == 3.0).all()
+
+
 def test_q4lr_long_K_takes_smaller_slabs(twq, oracle):
     """configs[3] q shape at M = 64: the quantized tile of 64 (or 32) tokens, the FP32 H and its partial do not fit beside
     the rings at r = 256, so the call runs as four slabs of 16 tokens."""
