@@ -48,14 +48,15 @@ namespace twq {
 
 namespace {
 
-// Compute warps per CTA, + the producer warp and the activation-side producer.  Up to two token tiles (M <= 32): 14 + 2 =
-// 16 warps, which is the largest CTA that gets 128 registers per thread -- the MT = 1 instantiations need 116 and were at
-// the 96-register limit of a 20-warp CTA, where ptxas' allocation decided the result (lesson 16):
-// M = 1 / 16 / 32 went 8.9 / 9.9 / 14.8 -> 8.6 / 9.5 / 14.1 us.  Four token tiles (M <= 64) keep 18 + 2 warps at 96
-// registers: there the extra warps are worth more than the spills they cause (M = 64: 22.1 vs 22.5 us; r = 256: 34.7 vs 38.5).
-// (The 4-bit low-rank mode is better off with 16 warps at four token tiles too: 28.8 vs 34.0 us.)
-__host__ __device__ constexpr int dec_warps(int mt, bool lr4) { return (mt == 4 && !lr4) ? 18 : 14; }
-__host__ __device__ constexpr int dec_threads(int mt, bool lr4) { return (dec_warps(mt, lr4) + 2) * 32; }
+// Compute warps per CTA, + the producer warp and the activation-side producer: 14 + 2 = 16 warps, the largest CTA that gets
+// 128 registers per thread -- the MT = 1 instantiations need 109-116 and were at the 96-register limit of the 20-warp CTA
+// this kernel started with, where ptxas' allocation decided the result (lessons 16 and 20):
+// M = 1 / 16 / 32 went 8.9 / 9.9 / 14.8 -> 8.6 / 9.5 / 14.1 us.  The wide variant (18 + 2 warps, 96 registers) remains for
+// four token tiles at r > 128, where eight low-rank warps would leave six residual warps (M = 64, r = 256: 33.1 vs 35.0 us;
+// at r = 128 the narrow CTA wins, 20.4 vs 21.0 us, and so it does in the 4-bit low-rank mode, 28.1 vs 34.0 us).
+__host__ __device__ constexpr int dec_warps(bool wide) { return wide ? 18 : 14; }
+__host__ __device__ constexpr int dec_threads(bool wide) { return (dec_warps(wide) + 2) * 32; }
+inline bool dec_is_wide(int mt, int r, int quant) { return mt == 4 && r > 128 && quant != 2; }
 constexpr int kMaxSlots = 8, kMaxL1Slots = 4;
 constexpr int kTB = 3;                              // tiles whose MMA chains a residual warp interleaves
 constexpr int kJT = 8;                              // 8-wide j tiles of H one low-rank warp can own
@@ -318,11 +319,11 @@ __device__ __forceinline__ void decode_quantize_share(const DecodeParams& p, uin
 //   re-quantization on the fly (L181): per token and group of gr rank indices, s_H = max(amax, 2^-30)/7 and packed 4-bit
 //             Q_H in shared memory, in the activation quantizer's FP32 operation order;
 //   stage 2   Ylr = sum_h s_H*sv*(Q_H . qv): a second int8 MMA against the V section, folded into the same epilogue.
-template <int G, int MT, bool kDbg, int kMode>
-__global__ void __launch_bounds__(dec_threads(MT, kMode == 2), 1)
+template <int G, int MT, bool kDbg, int kMode, bool kWide>
+__global__ void __launch_bounds__(dec_threads(kWide), 1)
 decode_dual_linear_kernel(const __grid_constant__ CUtensorMap tmXq, const __grid_constant__ DecodeParams p) {
     constexpr bool kQ = kMode >= 1, kL4 = kMode == 2;
-    constexpr int kDecWarps = dec_warps(MT, kL4);
+    constexpr int kDecWarps = dec_warps(kWide);
     extern __shared__ uint8_t dsm_raw[];
     // 1024-byte aligned base; the same offset in every CTA of the cluster (DSMEM addresses are formed from local ones)
     uint8_t* dsm = dsm_raw + ((1024u - (smem_u32(dsm_raw) & 1023u)) & 1023u);
@@ -1276,9 +1277,9 @@ namespace {
 
 constexpr int kMaxDevices = 64;
 
-template <int G, int MT, bool kDbg, int kMode>
+template <int G, int MT, bool kDbg, int kMode, bool kWide = false>
 cudaError_t decode_launch_inst(const CUtensorMap& tmXq, const DecodeParams& p, cudaStream_t stream) {
-    auto kern = decode_dual_linear_kernel<G, MT, kDbg, kMode>;
+    auto kern = decode_dual_linear_kernel<G, MT, kDbg, kMode, kWide>;
     static bool attr_done[kMaxDevices] = {};       // function attributes are per device
     int dev = 0;
     cudaError_t e = cudaGetDevice(&dev);
@@ -1292,7 +1293,7 @@ cudaError_t decode_launch_inst(const CUtensorMap& tmXq, const DecodeParams& p, c
     }
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(static_cast<unsigned>(p.grid));
-    cfg.blockDim = dim3(dec_threads(MT, kMode == 2));
+    cfg.blockDim = dim3(dec_threads(kWide));
     cfg.dynamicSmemBytes = static_cast<size_t>(p.smem_bytes);
     cfg.stream = stream;
     cudaLaunchAttribute attrs[2];
@@ -1322,12 +1323,12 @@ int decode_cluster_capacity(int cs, int num_sms) {
     if (cache[dev][cs] > 0) return cache[dev][cs];
     int n = 0;
     if (have_dev) {
-        auto kern = decode_dual_linear_kernel<128, 1, false, 0>;
+        auto kern = decode_dual_linear_kernel<128, 4, false, 0, true>;
         if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, kDecSmemMax) == cudaSuccess &&
             cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1) == cudaSuccess) {
             cudaLaunchConfig_t cfg = {};
             cfg.gridDim = dim3(static_cast<unsigned>(num_sms / cs * cs));
-            cfg.blockDim = dim3(dec_threads(4, false));
+            cfg.blockDim = dim3(dec_threads(true));
             cfg.dynamicSmemBytes = 200 * 1024;
             cudaLaunchAttribute attr;
             attr.id = cudaLaunchAttributeClusterDimension;
@@ -1364,7 +1365,7 @@ bool decode_make_plan(int M, int N, int K, int r, int G, int num_sms, int quant,
     p.mt = M <= 16 ? 1 : (M <= 32 ? 2 : 4);
     p.mp = 16 * p.mt;
     p.lrw = r > 0 ? (p.mt == 4 ? 8 : 4) : 0;              // more token tiles: stage 1 / stage 2 over eight warps
-    const int nrw = dec_warps(p.mt, lr4) - p.lrw;
+    const int nrw = dec_warps(dec_is_wide(p.mt, r, quant)) - p.lrw;
     // cluster size: H is shared by the cluster and every cluster streams all of L1 (K*r*2 bytes) from L2, so the
     // largest cluster that still covers 70 % of the SMs wins; otherwise the size covering the most SMs
     p.cs = 1;
@@ -1460,6 +1461,14 @@ bool decode_make_plan(int M, int N, int K, int r, int G, int num_sms, int quant,
 
 cudaError_t launch_decode(const CUtensorMap& tmXq, const DecodeParams& p, int G, cudaStream_t stream) {
     const bool dbg = p.dbgP != nullptr || p.dbgH != nullptr || p.dbgQH != nullptr || p.dbgSH != nullptr;
+    if (dec_is_wide(p.mt, p.r, p.quant)) {              // four token tiles, r > 128: the 20-warp CTA
+        if (G == 128) {
+            if (p.quant == 1) return dbg ? decode_launch_inst<128, 4, true, 1, true>(tmXq, p, stream) : decode_launch_inst<128, 4, false, 1, true>(tmXq, p, stream);
+            return dbg ? decode_launch_inst<128, 4, true, 0, true>(tmXq, p, stream) : decode_launch_inst<128, 4, false, 0, true>(tmXq, p, stream);
+        }
+        if (p.quant == 1) return dbg ? decode_launch_inst<64, 4, true, 1, true>(tmXq, p, stream) : decode_launch_inst<64, 4, false, 1, true>(tmXq, p, stream);
+        return dbg ? decode_launch_inst<64, 4, true, 0, true>(tmXq, p, stream) : decode_launch_inst<64, 4, false, 0, true>(tmXq, p, stream);
+    }
 #define TWQ_DCASE(g, m)                                                                   \
     if (G == g && p.mt == m) {                                                            \
         if (p.quant == 2) return dbg ? decode_launch_inst<g, m, true, 2>(tmXq, p, stream) : decode_launch_inst<g, m, false, 2>(tmXq, p, stream); \
