@@ -62,8 +62,8 @@ WORKLOADS = {
     "c5_qproj_m16": ("config5_llama70b", dict(which="q", M=16), "LLaMA3-70B q_proj K=8192 N=8192 r=256 M=16"),
 }
 DEFAULT_WORKLOAD = "c2_qproj_m16"
-DEFAULT_SWEEP = ["c2_qproj_m1", "c2_qproj_m16", "c2_qproj_m128", "c3_gateup_m2048", "c3_down_m2048",
-                 "c3_gateup_m2048_r256"]
+DEFAULT_SWEEP = ["c2_qproj_m1", "c2_qproj_m16", "c2_qproj_m32", "c2_qproj_m64", "c2_qproj_m128", "c3_gateup_m2048",
+                 "c3_down_m2048", "c3_gateup_m2048_r256"]
 
 
 def load_peaks():
@@ -372,7 +372,8 @@ def measure_q4lr(name, twq, torch, steps, warmup, peaks, with_oracle=False):
     out = dict(workload=name + "_q4lr", M=L.M, N=L.N, K=L.K, r=L.r, G=L.G, us_step=round(med, 3), us_min=round(us[0], 3),
                launches_per_step=launches, weight_copies=ncopies,
                roofline=dict(bound="hbm", achieved=round(ach, 1), peak=peaks["hbm_gbs"], unit="GB/s",
-                             frac=round(ach / peaks["hbm_gbs"], 4), traffic=None, kernel="decode_dual_linear_kernel<mode 2>",
+                             frac=round(ach / peaks["hbm_gbs"], 4), traffic=load_traffic(name + "_q4lr")[0],
+                             traffic_source=load_traffic(name + "_q4lr")[1], kernel="decode_dual_linear_kernel<mode 2>",
                              us=round(med, 3), algorithmic_bytes=by, peak_source=peaks["source"]))
     if with_oracle:
         from oracle import oracle
