@@ -135,6 +135,7 @@ def last_launch_count() -> int:
 
 def testing_set_plan_flags(flags: int) -> None:
     """include/twq_testing.h: process-wide planner overrides (0 = production)."""
+    _wsx_cache.clear()
     load_library().twq_testing_set_plan_flags(flags)
 
 
@@ -254,8 +255,18 @@ def dual_linear_noalloc(X, Xq, sx, packed: PackedLayer, Y, out_dtype: int = OUT_
     return Y
 
 
+_wsx_cache = {}
+
+
 def workspace_bytes_x(M: int, N: int, K: int, r: int, G: int) -> int:
-    return int(load_library().twq_workspace_bytes_x(M, N, K, r, G))
+    """twq_workspace_bytes_x, remembered per shape (a pure function of the shape and the planner flags; the cache is cleared
+    by testing_set_plan_flags): saves a library call per twq_dual_linear_x call on the host."""
+    key = (M, N, K, r, G)
+    v = _wsx_cache.get(key)
+    if v is None:
+        v = int(load_library().twq_workspace_bytes_x(M, N, K, r, G))
+        _wsx_cache[key] = v
+    return v
 
 
 def dual_linear_x(X, packed: PackedLayer, tinv=None, out_dtype: int = OUT_BF16, Y=None, ws=None, Xq_out=None,
