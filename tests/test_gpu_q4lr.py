@@ -198,6 +198,33 @@ def test_q4lr_is_deterministic_under_repetition(twq, M, K, N, r, G):
             assert torch.equal(Q, Q0)
 
 
+@pytest.mark.parametrize("M,out", [(7, "fp16"), (70, "bf16")])
+def test_q4lr_row_strides_and_16_bit_outputs(twq, oracle, M, out):
+    """ldx > K, ldy > N (a pitch that is not a multiple of 16 bytes for the second slab's start to matter), FP16 / BF16
+    outputs, two slabs: outputs equal the rounding of the FP32 output, padding columns of Y untouched."""
+    import torch
+    K, N, r, G = 1024, 528, 64, 128
+    L = gen.make_layer(M, K, N, 0, G, seed=8500 + M, with_tinv=True)
+    Uq, su, Vq, sv = gen.make_q4_lowrank(K, N, r, G, seed=9500 + M)
+    buf = np.zeros((M, K + 72), np.uint16)
+    buf[:, :K] = L.X
+    X = _dev(buf.view(np.int16), torch.bfloat16)[:, :K]
+    assert X.stride(0) == K + 72
+    tinv = _dev(L.tinv)
+    packed = twq.pack_weights_q4lr(_dev(L.Rq), _dev(L.sw), _dev(Uq), _dev(su), _dev(Vq), _dev(sv), G)
+    Y32 = twq.dual_linear_q4lr_x(X, packed, tinv, twq.OUT_FP32)
+    dt, code = (torch.float16, twq.OUT_FP16) if out == "fp16" else (torch.bfloat16, twq.OUT_BF16)
+    Ybuf = torch.full((M, N + 6), 5.0, dtype=dt, device="cuda")
+    Y = Ybuf[:, :N]
+    assert Y.stride(0) == N + 6
+    twq.dual_linear_q4lr_x(X, packed, tinv, code, Y=Y)
+    torch.cuda.synchronize()
+    assert torch.equal(Y.contiguous().view(torch.int16), Y32.to(dt).view(torch.int16))
+    assert (Ybuf[:, N:] == 5.0).all()
+    ref = oracle.forward_q4lr(L.X, L.Rq, L.sw, Uq, su, Vq, sv, G, tinv=L.tinv)["Y"]
+    assert np.abs(Y32.cpu().numpy().astype(np.float64) - ref).max() / np.abs(ref).max() <= TOL
+
+
 def test_q4lr_zero_factor_is_the_plain_residual(twq, oracle):
     """U = 0: H = 0, s_H = 2^-30 / 7, Q_H = 0, and Y is the rank-0 layer (north_star's r = 0 reduction)."""
     import torch
