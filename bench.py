@@ -48,6 +48,9 @@ WORKLOADS = {
     "c1_tiny": ("config1_tiny", dict(), "tiny M=8 K=256 N=512 r=16 G=64"),
     # rank 0 (plain W4A4): what the residual stream alone costs
     "c2_qproj_m1_r0": ("config2_qproj", dict(M=1, r=0), "LLaMA3-8B q_proj K=4096 N=4096 r=0 G=128 M=1"),
+    "c2_qproj_m384": ("config2_qproj", dict(M=384), "LLaMA3-8B q_proj K=4096 N=4096 r=128 G=128 M=384"),
+    "c2_qproj_m96": ("config2_qproj", dict(M=96), "LLaMA3-8B q_proj K=4096 N=4096 r=128 G=128 M=96"),
+    "c2_qproj_m192": ("config2_qproj", dict(M=192), "LLaMA3-8B q_proj K=4096 N=4096 r=128 G=128 M=192"),
     "c2_qproj_m128_r0": ("config2_qproj", dict(M=128, r=0), "LLaMA3-8B q_proj K=4096 N=4096 r=0 G=128 M=128"),
     "c2_qproj_m256": ("config2_qproj", dict(M=256), "LLaMA3-8B q_proj K=4096 N=4096 r=128 G=128 M=256"),
     "c2_qproj_m512": ("config2_qproj", dict(M=512), "LLaMA3-8B q_proj K=4096 N=4096 r=128 G=128 M=512"),

@@ -129,7 +129,7 @@ size_t twq_workspace_bytes(int M, int N, int K, int r, int G);
  *   Y      [M,ldy]          out, dtype ydt (ldy >= N elements)
  *   ws, ws_bytes            scratch of at least twq_workspace_bytes(...) bytes, 256-byte aligned (may be
  *                           NULL when that is 0).  Only calls with few output tiles beyond the small-batch
- *                           kernel (64 < M, roughly M*N < 1.5 M outputs) need it: split-K partial sums of Y
+ *                           kernel (64 < M, roughly M*N < 0.5 M outputs) need it: split-K partial sums of Y
  *                           and tile counters.  Small batches (M <= 64) and prefill-shaped calls need none,
  *                           and the on-chip intermediate H never passes through it.  The caller zero-fills it
  *                           ONCE after allocation; every call leaves the counters zero again, so it can be
@@ -218,8 +218,9 @@ twq_status twq_dual_linear_q4lr_x(const void* X, int ldx, const float* tinv, con
  * shapes with a workspace need (64 < M with few output tiles, see twq_dual_linear) lives in a static device array of
  * TWQ_NOALLOC_MAX_WS bytes inside the library -- every GPU that loads the library holds these 8.5 MiB until the process
  * exits; it covers every workspace shape of BASELINE.json's configs (largest: 8 MiB + 256 B), while the largest workspace the
- * planner can ask for at all is 9.0 MiB + 512 B (many tokens, very few channels).  The call allocates nothing (no cudaMalloc / cudaFree, no allocating library routine) and issues one small
- * memset on `stream` (the tile counters) in front of the kernel when the shape uses scratch.
+ * planner can ask for at all is about 9.5 MB (a few hundred tokens, few channels).  The call allocates nothing (no
+ * cudaMalloc / cudaFree, no allocating library routine) and issues one small memset on `stream` (the tile counters) in
+ * front of the kernel when the shape uses scratch.
  *   Arguments as for twq_dual_linear, without ws / ws_bytes / dbg_P.  Results are those of twq_dual_linear.
  *   TWQ_ERR_WORKSPACE  the shape needs more than TWQ_NOALLOC_MAX_WS bytes (twq_workspace_bytes(...) says how many):
  *                      nothing is launched; use twq_dual_linear with a caller workspace.

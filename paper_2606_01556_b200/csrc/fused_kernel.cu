@@ -195,6 +195,23 @@ bool fused_make_plan(int M, int N, int K, int r, int G, int num_sms, FusedPlan* 
     const unsigned cap = (plan_flags() >> kPlanFusedTnShift) & 3u;       // test / measurement override
     if (cap == 1 && tn0 > 64) tn0 = 64;
     if (cap == 2 && tn0 > 32) tn0 = 32;
+    // Mid-size M: where 128-token tiles alone cannot fill the machine (the plan would split K: partial tiles through L2 and a
+    // fix-up pass that move as many bytes as the weights), a smaller token tile WITHOUT a K split wins as soon as it yields
+    // enough tiles -- measured on q_proj (4096 x 4096, r = 128): M = 128 as 4 x 32 tokens 24.1 vs 27.5 us, M = 192 as 6 x 32
+    // 32.6 vs 36.0, M = 256 as 4 x 64 33.9 vs 36.3; with only 96 tiles (M = 96 as 3 x 32, M = 192 as 3 x 64) it loses.  The largest
+    // tile that reaches 85 % of the SMs is taken; no workspace is needed then.
+    if (tn0 == 128 && cap == 0 && !(plan_flags() & kPlanNoSplit)) {
+        const long long n_tiles = (N + kTileN - 1) / kTileN;
+        if (((M + 127) / 128) * n_tiles < (3 * num_sms) / 4) {
+            for (int TN = 64; TN >= 32; TN >>= 1) {
+                const long long tiles = ((M + TN - 1) / TN) * n_tiles;
+                if (tiles * 100 < static_cast<long long>(num_sms) * 85) continue;
+                FusedPlan q;
+                if (make_plan_tn(TN, M, N, K, r, G, num_sms, &q) && q.splits == 1) { *out = q; return true; }
+                break;
+            }
+        }
+    }
     for (int TN = tn0; TN >= 16; TN >>= 1)
         if (make_plan_tn(TN, M, N, K, r, G, num_sms, out)) return true;
     return false;

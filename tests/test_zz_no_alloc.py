@@ -42,7 +42,7 @@ def _layer(twq, M, K, N, r, G, seed):
 
 
 @pytest.mark.parametrize("M,K,N,r,G", [
-    (128, 4096, 4096, 128, 128),      # configs[1] at M = 128: the split-K shape with the largest scratch of the configs
+    (128, 4096, 2048, 128, 128),      # 16 channel tiles x 8 K splits: 8 MiB + 256 B of scratch, the largest of the config-shaped calls
     (80, 512, 384, 32, 128),          # three splits, ragged token tile
     (300, 1024, 1024, 128, 128),      # several token tiles, four splits
 ])
@@ -97,9 +97,9 @@ def test_noalloc_shapes_without_scratch(twq, oracle, M, K, N, r, G):
 
 
 def test_noalloc_rejects_a_shape_beyond_the_static_scratch(twq):
-    """Many tokens x very few channels with a long K: 9.3 MB of split-K scratch > 8.5 MiB -> TWQ_ERR_WORKSPACE, nothing runs."""
+    """A few hundred tokens x few channels: 9.5 MB of split-K scratch > 8.5 MiB -> TWQ_ERR_WORKSPACE, nothing runs."""
     import torch
-    M, N, K, r, G = 1009, 768, 14336, 0, 128
+    M, N, K, r, G = 377, 896, 4096, 0, 128
     assert twq.workspace_bytes(M, N, K, r, G) > twq.noalloc_max_workspace()
     Xq = torch.zeros((M, K // 2), dtype=torch.uint8, device="cuda")
     sx = torch.ones((M, K // G), dtype=torch.float32, device="cuda")
