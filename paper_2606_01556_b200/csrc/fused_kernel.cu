@@ -199,8 +199,10 @@ bool fused_make_plan(int M, int N, int K, int r, int G, int num_sms, FusedPlan* 
     // fix-up pass that move as many bytes as the weights), a smaller token tile WITHOUT a K split wins as soon as it yields
     // enough tiles -- measured on q_proj (4096 x 4096, r = 128): M = 128 as 4 x 32 tokens 24.1 vs 27.5 us, M = 192 as 6 x 32
     // 32.6 vs 36.0, M = 256 as 4 x 64 33.9 vs 36.3; with only 96 tiles (M = 96 as 3 x 32, M = 192 as 3 x 64) it loses.  The largest
-    // tile that reaches 85 % of the SMs is taken; no workspace is needed then.
-    if (tn0 == 128 && cap == 0 && !(plan_flags() & kPlanNoSplit)) {
+    // tile that reaches 85 % of the SMs is taken; no workspace is needed then.  Only for short K and rank <= 128: an unsplit CTA
+    // walks all K-groups in series, and on longer layers the K split wins again (down, K = 14336: M = 128 / 256 62.6 / 91.5 us
+    // unsplit against 47.3 / 75.5 us split; Qwen3 attention, K = 5120, r = 256, M = 128: 53.5 against 46.1 us).
+    if (tn0 == 128 && cap == 0 && !(plan_flags() & kPlanNoSplit) && K / G <= 32 && r <= 128) {
         const long long n_tiles = (N + kTileN - 1) / kTileN;
         if (((M + 127) / 128) * n_tiles < (3 * num_sms) / 4) {
             for (int TN = 64; TN >= 32; TN >>= 1) {
