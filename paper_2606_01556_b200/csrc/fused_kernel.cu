@@ -43,7 +43,10 @@ static bool make_plan_tn(int TN, int M, int N, int K, int r, int G, int num_sms,
     pl.cs = 1;
     if (r > 0) {
         const long long tiles0 = static_cast<long long>(pl.n_tiles) * pl.m_tiles;
-        if (tiles0 < (3 * num_sms) / 4) {
+        // (a K split needs room for at least two splits per tile; between num_sms / 2 and 3/4 num_sms tiles the call runs unsplit
+        // on fewer SMs, and the cost model below picks the cluster: Qwen3 attention, 80 tiles at M = 128: 46.1 us with clusters
+        // of 2, 40.7 / 41.9 us with 4 / 8)
+        if (tiles0 < (3 * num_sms) / 4 && 2 * tiles0 <= num_sms) {
             // few tiles (K will be split): the size that keeps the most SMs busy; ties go to the larger cluster
             int best = 0;
             for (int c = 8; c >= 1; c >>= 1) {
