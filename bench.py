@@ -49,6 +49,9 @@ WORKLOADS = {
     # rank 0 (plain W4A4): what the residual stream alone costs
     "c2_qproj_m1_r0": ("config2_qproj", dict(M=1, r=0), "LLaMA3-8B q_proj K=4096 N=4096 r=0 G=128 M=1"),
     "c2_qproj_m384": ("config2_qproj", dict(M=384), "LLaMA3-8B q_proj K=4096 N=4096 r=128 G=128 M=384"),
+    "c3_gateup_m128": ("config3_mlp", dict(which="gate_up", M=128), "LLaMA3-8B gate/up K=4096 N=14336 r=128 G=128 M=128"),
+    "c3_gateup_m256": ("config3_mlp", dict(which="gate_up", M=256), "LLaMA3-8B gate/up K=4096 N=14336 r=128 G=128 M=256"),
+    "c3_gateup_m512": ("config3_mlp", dict(which="gate_up", M=512), "LLaMA3-8B gate/up K=4096 N=14336 r=128 G=128 M=512"),
     "c3_down_m128": ("config3_mlp", dict(which="down", M=128), "LLaMA3-8B down K=14336 N=4096 r=128 G=128 M=128"),
     "c3_down_m256": ("config3_mlp", dict(which="down", M=256), "LLaMA3-8B down K=14336 N=4096 r=128 G=128 M=256"),
     "c4_attn_m128": ("config4_qwen", dict(which="attn", M=128), "Qwen3-32B attention K=5120 N=5120 r=256 M=128"),
