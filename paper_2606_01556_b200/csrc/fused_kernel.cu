@@ -116,7 +116,7 @@ static bool make_plan_tn(int TN, int M, int N, int K, int r, int G, int num_sms,
     const int ybytes = TN * kTileN * 2;
     pl.ystage = (TN == 128 && pl.splits == 1 && !(flags & kPlanNoYStage)) ? 1 : 0;
     pl.nsu = kMaxNSU;
-    pl.nsp = pl.pair ? kMaxNSP : (TN <= 32 ? 5 : 4);   // a pair's packed stage is 12 KB: the ring can be twice as deep
+    pl.nsp = pl.pair ? kMaxNSP : (TN <= 32 ? 5 : (TN == 64 ? 3 : 4));   // a pair's packed stage is 12 KB: the ring can be twice as deep
     pl.ns1 = r > 0 ? (TN <= 32 ? 3 : 2) : 0;
     pl.alias = 0;
     auto total = [&](const FusedPlan& q) {
