@@ -83,7 +83,7 @@ constexpr int kRegsCtl = 40, kRegsPrep = 56, kRegsEpi = 160;
 constexpr int kTileN = 128;             // output channels per CTA (MMA M)
 constexpr int kSxSlots = 16;            // per-group activation-scale slots (two blocks of 8 groups)
 constexpr int kNB = 3;                  // P accumulator buffers in rotation
-constexpr int kMaxNS1 = 6, kMaxNSP = 8, kMaxNSU = 4;
+constexpr int kMaxNS1 = 5, kMaxNSP = 8, kMaxNSU = 4;
 constexpr int kL1Chunk = 128 * 128;     // 128 rows x 64 fp16 (one 128B-swizzled tile)
 constexpr uint32_t kMagic = 0x4B400000u;  // bits of 1.5 * 2^23
 constexpr int kMaxDynSmem = 232448 - 64;
