@@ -543,6 +543,19 @@ def main():
             del g2
             torch.cuda.empty_cache()
 
+    cold = None
+    if rank == 0:
+        # csrc/cold_fill.cu: how long a one-shot burst of the q_proj weight share (10.75 MB over the SMs) takes to reach shared memory
+        # from cold HBM, by bulk copies and by plain loads: the floor under the decode-shaped calls that the bytes / bandwidth
+        # roofline does not contain (lesson 24)
+        try:
+            sms = torch.cuda.get_device_properties(local).multi_processor_count
+            per = (10_750_000 // sms + 63) // 64 * 64
+            cold = dict(bulk=twq.testing_cold_fill_us(per, 0, sms), ldg=twq.testing_cold_fill_us(per, 1, sms),
+                        what="us until every SM holds its 1/%d share of 10.75 MB of cold weights in shared memory (one launch, in-kernel "
+                             "%%globaltimer; excludes the launch itself)" % sms)
+        except Exception as e:                      # a measurement aid must not take the bench line down
+            cold = dict(error=str(e))
     i8_tops = None
     if rank == 0:
         # an MMA-only tcgen05 kind::i8 loop on every SM, next to the 2 x BF16 figure the roofline uses
@@ -580,6 +593,7 @@ def main():
                                    roofline_uses_tops=round(2.0 * peaks["bf16_tflops"], 1),
                                    how="tcgen05.mma kind::i8 128x128x32 from shared memory, 4096 x 8 MMAs per SM, best of 5 "
                                        "(csrc/peak_i8.cu); the roofline denominator stays 2 x measured cuBLAS BF16 burst"),
+                    cold_fill=cold,
                     us_host_per_call=main_res.get("us_host_per_call"),
                     cpu_baseline=cpu,
                     # `value` = the whole hot path through twq_dual_linear_x (one launch for M <= 64); beside it the same step as

@@ -7,6 +7,7 @@
 #ifndef TWQ_TESTING_H_
 #define TWQ_TESTING_H_
 
+#include <stddef.h>
 #ifdef __cplusplus
 extern "C" {
 #endif
@@ -47,6 +48,15 @@ int twq_testing_describe_plan(int M, int N, int K, int r, int G, int* out, int n
  * (csrc/peak_i8.cu), best of `reps` launches of iters x 8 MMAs per SM.  SYNCHRONISES the stream.  Negative on failure.
  * bench.py prints it next to the 2 x BF16 figure that the prefill roofline uses. */
 float twq_testing_measure_i8_tops(int iters, int reps, void* stream);
+
+/* Cold-fill probe (csrc/cold_fill.cu): ONE launch of `ctas` CTAs (one per SM), each bringing `bytes` (a multiple of 64, at most
+ * 200 KiB) from src + cta * stride into its shared memory -- mode 0: four bulk copies completing on an mbarrier (the small-batch
+ * kernel's mechanism), mode 1: plain 16-byte loads, eight in flight per thread.  out_ns[cta] (device, ctas x u64) receives the
+ * %globaltimer nanoseconds from the CTA's first instruction to its last byte.  Asynchronous on `stream`.  The caller provides
+ * the buffer (ctas * stride bytes per region) and rotates regions so that nothing is L2-resident: the result is the floor under
+ * any decode-shaped call that streams its weights once, which the bytes / bandwidth roofline ignores.  Returns 0, -1 (bad
+ * argument / no sm_100 device) or -2 (launch failure). */
+int twq_testing_cold_fill(const void* src, size_t stride, int bytes, int mode, int ctas, unsigned long long* out_ns, void* stream);
 
 /* In-kernel timeline (csrc/trace.cuh).  Hands a device buffer of at least 16384 unsigned 64-bit words to the library;
  * NULL switches the timeline off.  Returns 1 if this library was built with the timeline compiled in

@@ -13,7 +13,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libtwq.so")
 TRACE_LIB = os.path.join(HERE, "libtwq_trace.so")      # --trace: the same library with the in-kernel timeline (csrc/trace.cuh)
-SOURCES = ["twq_api.cu", "quantize_act.cu", "pack_weights.cu", "fused_kernel.cu", "decode_kernel.cu", "peak_i8.cu", "static_ws.cu", "fused_inst_tn16.cu",
+SOURCES = ["twq_api.cu", "quantize_act.cu", "pack_weights.cu", "fused_kernel.cu", "decode_kernel.cu", "peak_i8.cu", "cold_fill.cu", "static_ws.cu", "fused_inst_tn16.cu",
            "fused_inst_tn32.cu", "fused_inst_tn64.cu", "fused_inst_tn128.cu", "fused_inst_tn128p.cu"]
 HEADERS = ["sm100_ptx.cuh", "trace.cuh", "fused_kernel.h", "fused_kernel.cuh", "packed_layout.h", os.path.join("..", "..", "include", "twq.h"),
            os.path.join("..", "..", "include", "twq_testing.h")]

@@ -20,7 +20,7 @@ EXPORTS = ("twq_status_string", "twq_packed_bytes", "twq_pack_weights", "twq_qua
 
 
 TESTING_EXPORTS = ("twq_testing_set_plan_flags", "twq_testing_get_plan_flags", "twq_testing_describe_plan",
-                   "twq_testing_set_trace_buffer", "twq_testing_measure_i8_tops")
+                   "twq_testing_set_trace_buffer", "twq_testing_measure_i8_tops", "twq_testing_cold_fill")
 # include/twq_testing.h: planner overrides for tests
 PLAN_NO_SPLIT, PLAN_NO_PAIR, PLAN_NO_YSTAGE, PLAN_NO_ALIAS2, PLAN_NO_DECODE = 1, 2, 4, 8, 16
 _PLAN_FIELDS = ("kernel", "cluster", "grid", "tile_tokens", "splits", "pair", "smem", "ring", "chunks", "s1_ring", "alias")
@@ -103,6 +103,8 @@ def load_library(build_if_missing: bool = True):
     lib.twq_testing_set_trace_buffer.argtypes = [vp]
     lib.twq_testing_measure_i8_tops.restype = ctypes.c_float
     lib.twq_testing_measure_i8_tops.argtypes = [i, i, vp]
+    lib.twq_testing_cold_fill.restype = i
+    lib.twq_testing_cold_fill.argtypes = [vp, sz, i, i, i, vp, vp]
     _lib = lib
     return lib
 
@@ -147,6 +149,31 @@ def testing_set_trace_buffer(buf) -> bool:
 def testing_measure_i8_tops(iters: int = 4096, reps: int = 5) -> float:
     """csrc/peak_i8.cu: measured tcgen05 kind::i8 rate in TOP/s (synchronises)."""
     return float(load_library().twq_testing_measure_i8_tops(iters, reps, _stream()))
+
+
+def testing_cold_fill_us(bytes_per_cta: int, mode: int, ctas: int = 148, reps: int = 12) -> dict:
+    """csrc/cold_fill.cu: microseconds until every one of `ctas` CTAs has `bytes_per_cta` of COLD global memory in its shared
+    memory (mode 0 bulk copies, 1 plain loads).  Regions rotate through > 2 x L2; median over reps of the slowest and of the
+    median CTA.  Synchronises."""
+    lib = load_library()
+    stride = (bytes_per_cta + 255) // 256 * 256
+    region = stride * ctas
+    nreg = max(reps, (2 * 126 * 1024 * 1024) // region + 2)
+    buf = torch.ones(nreg * region, dtype=torch.uint8, device="cuda")
+    out = torch.zeros(ctas, dtype=torch.int64, device="cuda")
+    mx, med = [], []
+    for rep in range(nreg + reps):
+        base = ctypes.c_void_p(buf.data_ptr() + (rep % nreg) * region)
+        code = lib.twq_testing_cold_fill(base, stride, bytes_per_cta, mode, ctas, _ptr(out), _stream())
+        if code != 0:
+            raise TwqError(4 if code == -2 else 1, "twq_testing_cold_fill")
+        torch.cuda.synchronize()
+        if rep >= nreg:                      # the first lap only makes sure every region has left L2 since it was written
+            t = out.sort().values
+            mx.append(int(t[-1])); med.append(int(t[ctas // 2]))
+    mx.sort(); med.sort()
+    return dict(slowest_cta_us=mx[len(mx) // 2] / 1e3, median_cta_us=med[len(med) // 2] / 1e3, bytes_per_cta=bytes_per_cta, ctas=ctas,
+                mode="bulk" if mode == 0 else "ldg")
 
 
 def testing_describe_plan(M: int, N: int, K: int, r: int, G: int) -> dict:

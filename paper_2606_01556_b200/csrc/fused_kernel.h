@@ -103,6 +103,8 @@ size_t workspace_counter_bytes(int M, int N, int K, int r, int G);   // twq_api.
 unsigned plan_flags();
 void set_plan_flags(unsigned f);
 float measure_i8_tops(int iters, int reps, cudaStream_t stream);   // peak_i8.cu (bench measurement aid)
+cudaError_t launch_cold_fill(const void* src, size_t stride, int bytes, int mode, int ctas, unsigned long long* tout,
+                             cudaStream_t stream);          // cold_fill.cu (bench measurement aid)
 unsigned long long* trace_buffer();   // set by twq_testing_set_trace_buffer; only read by -DTWQ_TRACE builds
 
 // Fills `plan` for a shape; returns false if the shape cannot be planned (never for valid ABI shapes).

@@ -240,6 +240,13 @@ float twq_testing_measure_i8_tops(int iters, int reps, void* stream) {
     return twq::measure_i8_tops(iters, reps, static_cast<cudaStream_t>(stream));
 }
 
+int twq_testing_cold_fill(const void* src, size_t stride, int bytes, int mode, int ctas, unsigned long long* out_ns, void* stream) {
+    if (!src || !out_ns || bytes < 64 || bytes > 200 * 1024 || bytes % 64 != 0 || stride < static_cast<size_t>(bytes) || ctas < 1 ||
+        (mode != 0 && mode != 1) || !device_is_sm100())
+        return -1;
+    return twq::launch_cold_fill(src, stride, bytes, mode, ctas, out_ns, static_cast<cudaStream_t>(stream)) == cudaSuccess ? 0 : -2;
+}
+
 int twq_testing_describe_plan(int M, int N, int K, int r, int G, int* out, int n_out) {
     if (!shape_ok(M, N, K, r, G) || !out) return -1;
     const CallPlan* cp = get_plan(M, N, K, r, G);
